@@ -1,0 +1,573 @@
+/*
+ * mm_oracle.c -- plain CPU oracle for the micromagnetic hot path of
+ * arxiv/paper_2606_01114 ("Magnum.np.distributed").
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.  It
+ * shares no code, header, table or constant generator with the CUDA path under
+ * paper_2606_01114_b200/ and neither side imports the other.
+ *
+ * Everything is fp64 (the Newell tensor is evaluated in __float128 and rounded once).
+ * Array layout everywhere: [nx][ny][nz][3], component fastest (the
+ * paper's state tensor state.m[x,y,z,c]).
+ *
+ * What each function follows (PAPER.md = /root/reference/PAPER.md, SURVEY = SURVEY.md):
+ *   O1 orc_newell_*          Newell tensor, PAPER.md:43 (cited, not printed; ref 23) -> SURVEY 8(c) O1
+ *   O2 sign/scale            PAPER.md:45 eq. 4, reading Q2: H = -Ms * sum N(r-r') m(r')
+ *   O3 orc_demag_direct*     eq. 4 written out as the O(n^2) real-space sum (ground truth)
+ *   O4 orc_demag_dft         the zero-padded circular convolution of PAPER.md:47 by literal DFT
+ *   O5 orc_demag_fft*        the same by an own radix-2 FFT, z then y then x
+ *   O6 orc_exchange          PAPER.md:32 eq. 2, 6-point stencil, Neumann boundary (reading Q5)
+ *   O7 orc_anisotropy/zeeman PAPER.md:30 (uniaxial, reading Q7), PAPER.md:140-143 (B/mu0)
+ *   O8 orc_llg_rhs           PAPER.md:25 eq. 1 on unit m (reading Q4)
+ *   O9 orc_rk4_step          classic RK4 + renormalise (reading Q14)
+ *
+ * Pins: tests/test_oracle_*.py (closed forms, survey/mpmath values in tests/golden/,
+ * Gauss-Legendre quadrature of the defining integral, direct-sum vs DFT vs FFT, invariants).
+ * Parity unpinned: none of the functions; the SP4-shaped trajectory of config 2 has no
+ * external truth in the container (SURVEY 8(c) last pin row) and is GPU-vs-oracle only.
+ */
+#define _GNU_SOURCE
+#include <complex.h>
+#include <math.h>
+#include <quadmath.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef __float128 quad;
+
+#define ORC_MU0 (4.0e-7 * M_PI) /* reading Q8: 4 pi 1e-7 T m / A */
+
+enum { ORC_TERM_DEMAG = 1, ORC_TERM_EXCHANGE = 2, ORC_TERM_ANISOTROPY = 4, ORC_TERM_ZEEMAN = 8 };
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------ O1: Newell f, g */
+
+/* f(x,y,z), even in every argument.  A term whose prefactor or denominator is 0 is dropped. */
+static quad newell_f(quad x, quad y, quad z) {
+  x = fabsq(x); y = fabsq(y); z = fabsq(z);
+  const quad x2 = x * x, y2 = y * y, z2 = z * z;
+  const quad R = sqrtq(x2 + y2 + z2);
+  quad r = 0;
+  if (y > 0 && (x2 + z2) > 0) r += (y / 2) * (z2 - x2) * asinhq(y / sqrtq(x2 + z2));
+  if (z > 0 && (x2 + y2) > 0) r += (z / 2) * (y2 - x2) * asinhq(z / sqrtq(x2 + y2));
+  if (x > 0 && y > 0 && z > 0) r -= x * y * z * atanq(y * z / (x * R));
+  r += (2 * x2 - y2 - z2) * R / 6;
+  return r;
+}
+
+/* g(x,y,z), odd in x, odd in y, even in z. */
+static quad newell_g(quad x, quad y, quad z) {
+  const quad sgn = ((x < 0) ? -1 : 1) * ((y < 0) ? -1 : 1);
+  x = fabsq(x); y = fabsq(y); z = fabsq(z);
+  const quad x2 = x * x, y2 = y * y, z2 = z * z;
+  const quad R = sqrtq(x2 + y2 + z2);
+  quad r = 0;
+  if (x > 0 && y > 0) {
+    if (z > 0) r += x * y * z * asinhq(z / sqrtq(x2 + y2));
+    r += (y / 6) * (3 * z2 - y2) * asinhq(x / sqrtq(y2 + z2));
+    r += (x / 6) * (3 * z2 - x2) * asinhq(y / sqrtq(x2 + z2));
+    if (z > 0) {
+      r -= (z * z2 / 6) * atanq(x * y / (z * R));
+      r -= (z * y2 / 2) * atanq(x * z / (y * R));
+      r -= (z * x2 / 2) * atanq(y * z / (x * R));
+    }
+    r -= x * y * R / 3;
+  }
+  return sgn * r;
+}
+
+/* The six generating functions with their argument permutations:
+ * xx f(x,y,z)  yy f(y,z,x)  zz f(z,x,y)  xy g(x,y,z)  xz g(x,z,y)  yz g(y,z,x) */
+static quad newell_F(int comp, quad X, quad Y, quad Z) {
+  switch (comp) {
+    case 0: return newell_f(X, Y, Z);
+    case 1: return newell_f(Y, Z, X);
+    case 2: return newell_f(Z, X, Y);
+    case 3: return newell_g(X, Y, Z);
+    case 4: return newell_g(X, Z, Y);
+    default: return newell_g(Y, Z, X);
+  }
+}
+
+static int structurally_zero(int comp, int i, int j, int k) {
+  if (comp == 3) return i == 0 || j == 0;
+  if (comp == 4) return i == 0 || k == 0;
+  if (comp == 5) return j == 0 || k == 0;
+  return 0;
+}
+
+/* Literal definition at one offset: N = -D[F](X,Y,Z)/(4 pi V), D the 27-point
+ * second-difference with weights (1,-2,1)^3.  out[6] = xx yy zz xy xz yz. */
+void orc_newell_point(double dx, double dy, double dz, int i, int j, int k, double out[6]) {
+  const quad qx = dx, qy = dy, qz = dz;
+  const quad pref = -1 / (4 * M_PIq * qx * qy * qz);
+  static const int w[3] = {1, -2, 1};
+  for (int comp = 0; comp < 6; ++comp) {
+    if (structurally_zero(comp, i, j, k)) { out[comp] = 0.0; continue; }
+    quad s = 0;
+    for (int a = -1; a <= 1; ++a)
+      for (int b = -1; b <= 1; ++b)
+        for (int c = -1; c <= 1; ++c)
+          s += (quad)(w[a + 1] * w[b + 1] * w[c + 1]) *
+               newell_F(comp, (i + a) * qx, (j + b) * qy, (k + c) * qz);
+    out[comp] = (double)(pref * s);
+  }
+}
+
+/* Octant table N[comp][i][j][k], i<nx, j<ny, k<nz, comp in xx yy zz xy xz yz.
+ * Same definition; F is evaluated once per lattice point (-1..n) and D applied to the
+ * stored quad values (the 27-term sum regrouped, still in quad; rounded to fp64 once). */
+int orc_newell_octant(int nx, int ny, int nz, double dx, double dy, double dz, double *N) {
+  if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || !N) return 1;
+  const size_t sx = (size_t)nx + 2, sy = (size_t)ny + 2, sz = (size_t)nz + 2;
+  quad *F = (quad *)malloc(sx * sy * sz * sizeof(quad));
+  if (!F) return 2;
+  const quad qx = dx, qy = dy, qz = dz;
+  const quad pref = -1 / (4 * M_PIq * qx * qy * qz);
+  static const int w[3] = {1, -2, 1};
+  for (int comp = 0; comp < 6; ++comp) {
+#pragma omp parallel for collapse(2) schedule(dynamic, 4)
+    for (int i = -1; i <= nx; ++i)
+      for (int j = -1; j <= ny; ++j)
+        for (int k = -1; k <= nz; ++k)
+          F[((size_t)(i + 1) * sy + (size_t)(j + 1)) * sz + (size_t)(k + 1)] =
+              newell_F(comp, i * qx, j * qy, k * qz);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int i = 0; i < nx; ++i)
+      for (int j = 0; j < ny; ++j)
+        for (int k = 0; k < nz; ++k) {
+          double v = 0.0;
+          if (!structurally_zero(comp, i, j, k)) {
+            quad s = 0;
+            for (int a = 0; a < 3; ++a)
+              for (int b = 0; b < 3; ++b)
+                for (int c = 0; c < 3; ++c)
+                  s += (quad)(w[a] * w[b] * w[c]) *
+                       F[((size_t)(i + a) * sy + (size_t)(j + b)) * sz + (size_t)(k + c)];
+            v = (double)(pref * s);
+          }
+          N[(((size_t)comp * nx + i) * ny + j) * nz + k] = v;
+        }
+  }
+  free(F);
+  return 0;
+}
+
+/* N_rc at a signed offset from the octant table: diagonal even, xy odd in x,y, etc. */
+static const int COMP_OF[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};
+
+static inline double newell_lookup(const double *N, int nx, int ny, int nz, int r, int c, int di,
+                                   int dj, int dk) {
+  const int comp = COMP_OF[r][c];
+  const int ai = di < 0 ? -di : di, aj = dj < 0 ? -dj : dj, ak = dk < 0 ? -dk : dk;
+  double v = N[(((size_t)comp * nx + ai) * ny + aj) * nz + ak];
+  int flip = 0;
+  if (comp == 3) flip = (di < 0) ^ (dj < 0);
+  if (comp == 4) flip = (di < 0) ^ (dk < 0);
+  if (comp == 5) flip = (dj < 0) ^ (dk < 0);
+  return flip ? -v : v;
+}
+
+/* ------------------------------------------------------------------ O3: direct sum */
+
+static void direct_at(int nx, int ny, int nz, const double *N, double Ms, const double *m, int xi,
+                      int yi, int zi, double out[3]) {
+  long double acc[3] = {0, 0, 0};
+  for (int x = 0; x < nx; ++x)
+    for (int y = 0; y < ny; ++y)
+      for (int z = 0; z < nz; ++z) {
+        const double *mj = m + (((size_t)x * ny + y) * nz + z) * 3;
+        for (int r = 0; r < 3; ++r)
+          for (int c = 0; c < 3; ++c)
+            acc[r] += (long double)newell_lookup(N, nx, ny, nz, r, c, xi - x, yi - y, zi - z) *
+                      (long double)mj[c];
+      }
+  for (int r = 0; r < 3; ++r) out[r] = (double)(-(long double)Ms * acc[r]);
+}
+
+/* H(i) = -Ms sum_j N(i-j) m(j) for every cell (O(n^2)). */
+int orc_demag_direct(int nx, int ny, int nz, const double *N, double Ms, const double *m,
+                     double *H) {
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+  for (int x = 0; x < nx; ++x)
+    for (int y = 0; y < ny; ++y)
+      for (int z = 0; z < nz; ++z)
+        direct_at(nx, ny, nz, N, Ms, m, x, y, z, H + (((size_t)x * ny + y) * nz + z) * 3);
+  return 0;
+}
+
+/* The same sum at nsamp chosen cells (flat cell index (x*ny+y)*nz+z); Hs[nsamp][3]. */
+int orc_demag_direct_sampled(int nx, int ny, int nz, const double *N, double Ms, const double *m,
+                             int nsamp, const int64_t *cells, double *Hs) {
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int s = 0; s < nsamp; ++s) {
+    const int64_t c = cells[s];
+    const int z = (int)(c % nz), y = (int)((c / nz) % ny), x = (int)(c / ((int64_t)nz * ny));
+    direct_at(nx, ny, nz, N, Ms, m, x, y, z, Hs + (size_t)s * 3);
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------ padded grids */
+
+static int padded(int n) { return n == 1 ? 1 : 2 * n; } /* reading Q10 */
+
+/* Mirror the octant table onto the padded grid: offset -i sits at index P-i, index n
+ * (distance +-n, never needed) is 0 (reading Q11).  out[Px][Py][Pz] for one component. */
+static void mirror_fill(const double *N, int nx, int ny, int nz, int comp, double complex *out) {
+  const int Px = padded(nx), Py = padded(ny), Pz = padded(nz);
+  for (int a = 0; a < Px; ++a)
+    for (int b = 0; b < Py; ++b)
+      for (int c = 0; c < Pz; ++c) {
+        const int di = a < nx ? a : a - Px, dj = b < ny ? b : b - Py, dk = c < nz ? c : c - Pz;
+        double v = 0.0;
+        if (!(Px > 1 && a == nx) && !(Py > 1 && b == ny) && !(Pz > 1 && c == nz)) {
+          const int r = comp < 3 ? comp : (comp == 5 ? 1 : 0);
+          const int cc = comp < 3 ? comp : (comp == 3 ? 1 : 2);
+          v = newell_lookup(N, nx, ny, nz, r, cc, di, dj, dk);
+        }
+        out[((size_t)a * Py + b) * Pz + c] = v;
+      }
+}
+
+/* ------------------------------------------------------------------ O4: literal DFT */
+
+/* Zero-padded circular convolution by literal 3D DFTs (no FFT algorithm at all).
+ * Only for tiny meshes: cost ~ 9 * (Px Py Pz)^2. */
+int orc_demag_dft(int nx, int ny, int nz, const double *N, double Ms, const double *m, double *H) {
+  const int Px = padded(nx), Py = padded(ny), Pz = padded(nz);
+  const size_t P = (size_t)Px * Py * Pz;
+  if (P > 8192) return 3;
+  double complex *Nr = malloc(6 * P * sizeof(double complex));
+  double complex *Nk = malloc(6 * P * sizeof(double complex));
+  double complex *mr = calloc(3 * P, sizeof(double complex));
+  double complex *mk = malloc(3 * P * sizeof(double complex));
+  double complex *hk = malloc(3 * P * sizeof(double complex));
+  if (!Nr || !Nk || !mr || !mk || !hk) return 2;
+  for (int comp = 0; comp < 6; ++comp) mirror_fill(N, nx, ny, nz, comp, Nr + comp * P);
+  for (int x = 0; x < nx; ++x)
+    for (int y = 0; y < ny; ++y)
+      for (int z = 0; z < nz; ++z)
+        for (int c = 0; c < 3; ++c)
+          mr[c * P + ((size_t)x * Py + y) * Pz + z] = m[(((size_t)x * ny + y) * nz + z) * 3 + c];
+  /* forward: X(k) = sum_r x(r) exp(-2 pi i (kx rx/Px + ky ry/Py + kz rz/Pz)) */
+#pragma omp parallel for schedule(static)
+  for (long kk = 0; kk < (long)P; ++kk) {
+    const int kx = (int)(kk / ((long)Py * Pz)), ky = (int)((kk / Pz) % Py), kz = (int)(kk % Pz);
+    double complex accN[6] = {0}, accm[3] = {0};
+    for (int a = 0; a < Px; ++a)
+      for (int b = 0; b < Py; ++b)
+        for (int c = 0; c < Pz; ++c) {
+          const double ph = -2.0 * M_PI *
+                            ((double)((long)kx * a % Px) / Px + (double)((long)ky * b % Py) / Py +
+                             (double)((long)kz * c % Pz) / Pz);
+          const double complex w = cos(ph) + I * sin(ph);
+          const size_t r = ((size_t)a * Py + b) * Pz + c;
+          for (int q = 0; q < 6; ++q) accN[q] += Nr[q * P + r] * w;
+          for (int q = 0; q < 3; ++q) accm[q] += mr[q * P + r] * w;
+        }
+    for (int q = 0; q < 6; ++q) Nk[q * P + kk] = accN[q];
+    for (int q = 0; q < 3; ++q) mk[q * P + kk] = accm[q];
+  }
+  for (size_t kk = 0; kk < P; ++kk)
+    for (int r = 0; r < 3; ++r) {
+      double complex s = 0;
+      for (int c = 0; c < 3; ++c) s += Nk[COMP_OF[r][c] * P + kk] * mk[c * P + kk];
+      hk[r * P + kk] = s;
+    }
+  /* inverse at the physical cells only, 1/P normalisation, times -Ms (O2) */
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int x = 0; x < nx; ++x)
+    for (int y = 0; y < ny; ++y)
+      for (int z = 0; z < nz; ++z) {
+        double complex acc[3] = {0};
+        for (int a = 0; a < Px; ++a)
+          for (int b = 0; b < Py; ++b)
+            for (int c = 0; c < Pz; ++c) {
+              const double ph = 2.0 * M_PI *
+                                ((double)((long)a * x % Px) / Px + (double)((long)b * y % Py) / Py +
+                                 (double)((long)c * z % Pz) / Pz);
+              const double complex w = cos(ph) + I * sin(ph);
+              const size_t k = ((size_t)a * Py + b) * Pz + c;
+              for (int r = 0; r < 3; ++r) acc[r] += hk[r * P + k] * w;
+            }
+        for (int r = 0; r < 3; ++r)
+          H[(((size_t)x * ny + y) * nz + z) * 3 + r] = -Ms * creal(acc[r]) / (double)P;
+      }
+  free(Nr); free(Nk); free(mr); free(mk); free(hk);
+  return 0;
+}
+
+/* ------------------------------------------------------------------ O5: own FFT path */
+
+static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
+
+/* Textbook iterative radix-2 decimation-in-time FFT on a contiguous buffer of length n
+ * (power of two).  sign = -1 forward, +1 inverse (unnormalised).  tw[q] = exp(sign 2 pi i q/n). */
+static void fft_radix2(double complex *a, int n, const double complex *tw) {
+  for (int i = 1, j = 0; i < n; ++i) { /* bit reversal */
+    int bit = n >> 1;
+    for (; j & bit; bit >>= 1) j ^= bit;
+    j ^= bit;
+    if (i < j) { double complex t = a[i]; a[i] = a[j]; a[j] = t; }
+  }
+  for (int len = 2; len <= n; len <<= 1) {
+    const int half = len >> 1, step = n / len;
+    for (int s = 0; s < n; s += len)
+      for (int q = 0; q < half; ++q) {
+        const double complex u = a[s + q], v = a[s + q + half] * tw[q * step];
+        a[s + q] = u + v;
+        a[s + q + half] = u - v;
+      }
+  }
+}
+
+static double complex *make_twiddles(int n, int sign) {
+  double complex *tw = malloc((size_t)(n > 0 ? n : 1) * sizeof(double complex));
+  for (int q = 0; q < n; ++q) {
+    const double ph = sign * 2.0 * M_PI * (double)q / (double)n;
+    tw[q] = cos(ph) + I * sin(ph);
+  }
+  return tw;
+}
+
+/* 1D FFTs along one axis of a [Px][Py][Pz] complex array, for index ranges
+ * x<limx, y<limy, z<limz of the *other* axes (pencils outside are known zero / unneeded). */
+static void fft_axis(double complex *A, int Px, int Py, int Pz, int axis, int sign, int lim0,
+                     int lim1) {
+  const int n = axis == 0 ? Px : (axis == 1 ? Py : Pz);
+  if (n == 1) return;
+  double complex *tw = make_twiddles(n, sign);
+#pragma omp parallel
+  {
+    double complex *buf = malloc((size_t)n * sizeof(double complex));
+#pragma omp for collapse(2) schedule(static)
+    for (int p = 0; p < lim0; ++p)
+      for (int q = 0; q < lim1; ++q) {
+        size_t base, stride;
+        if (axis == 2) { base = ((size_t)p * Py + q) * Pz; stride = 1; }            /* (x,y) */
+        else if (axis == 1) { base = (size_t)p * Py * Pz + q; stride = Pz; }       /* (x,z) */
+        else { base = (size_t)p * Pz + q; stride = (size_t)Py * Pz; }             /* (y,z) */
+        for (int t = 0; t < n; ++t) buf[t] = A[base + t * stride];
+        fft_radix2(buf, n, tw);
+        for (int t = 0; t < n; ++t) A[base + t * stride] = buf[t];
+      }
+    free(buf);
+  }
+  free(tw);
+}
+
+/* Fourier-space tensor: real part of the forward 3D FFT of the mirrored table,
+ * Nhat[6][Px][Py][Pz] (the imaginary part is analytically zero; its measured max is
+ * returned through max_imag if non-NULL). */
+int orc_demag_fft_nhat(int nx, int ny, int nz, const double *N, double *Nhat, double *max_imag) {
+  if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz)) return 1;
+  const int Px = padded(nx), Py = padded(ny), Pz = padded(nz);
+  const size_t P = (size_t)Px * Py * Pz;
+  double complex *A = malloc(P * sizeof(double complex));
+  if (!A) return 2;
+  double mi = 0.0;
+  for (int comp = 0; comp < 6; ++comp) {
+    mirror_fill(N, nx, ny, nz, comp, A);
+    fft_axis(A, Px, Py, Pz, 2, -1, Px, Py);
+    fft_axis(A, Px, Py, Pz, 1, -1, Px, Pz);
+    fft_axis(A, Px, Py, Pz, 0, -1, Py, Pz);
+    for (size_t k = 0; k < P; ++k) {
+      Nhat[comp * P + k] = creal(A[k]);
+      if (fabs(cimag(A[k])) > mi) mi = fabs(cimag(A[k]));
+    }
+  }
+  if (max_imag) *max_imag = mi;
+  free(A);
+  return 0;
+}
+
+/* H = -Ms * crop( IFFT( Nhat . FFT( pad(m) ) ) ), z then y then x forward,
+ * x then y then z inverse.  Pencils that are all zero (forward) or whose outputs are
+ * discarded (inverse) are skipped; that changes no value. */
+int orc_demag_fft(int nx, int ny, int nz, const double *Nhat, double Ms, const double *m,
+                  double *H) {
+  if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz)) return 1;
+  const int Px = padded(nx), Py = padded(ny), Pz = padded(nz);
+  const size_t P = (size_t)Px * Py * Pz;
+  double complex *A = calloc(3 * P, sizeof(double complex));
+  if (!A) return 2;
+  for (int c = 0; c < 3; ++c) {
+    double complex *Ac = A + c * P;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int x = 0; x < nx; ++x)
+      for (int y = 0; y < ny; ++y)
+        for (int z = 0; z < nz; ++z)
+          Ac[((size_t)x * Py + y) * Pz + z] = m[(((size_t)x * ny + y) * nz + z) * 3 + c];
+    fft_axis(Ac, Px, Py, Pz, 2, -1, nx, ny);
+    fft_axis(Ac, Px, Py, Pz, 1, -1, nx, Pz);
+    fft_axis(Ac, Px, Py, Pz, 0, -1, Py, Pz);
+  }
+#pragma omp parallel for schedule(static)
+  for (long k = 0; k < (long)P; ++k) {
+    double complex mk[3] = {A[k], A[P + k], A[2 * P + k]}, hk[3];
+    for (int r = 0; r < 3; ++r) {
+      hk[r] = 0;
+      for (int c = 0; c < 3; ++c) hk[r] += Nhat[COMP_OF[r][c] * P + k] * mk[c];
+    }
+    for (int r = 0; r < 3; ++r) A[r * P + k] = hk[r];
+  }
+  for (int c = 0; c < 3; ++c) {
+    double complex *Ac = A + c * P;
+    fft_axis(Ac, Px, Py, Pz, 0, +1, Py, Pz);
+    fft_axis(Ac, Px, Py, Pz, 1, +1, nx, Pz);
+    fft_axis(Ac, Px, Py, Pz, 2, +1, nx, ny);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int x = 0; x < nx; ++x)
+      for (int y = 0; y < ny; ++y)
+        for (int z = 0; z < nz; ++z)
+          H[(((size_t)x * ny + y) * nz + z) * 3 + c] =
+              -Ms * creal(Ac[((size_t)x * Py + y) * Pz + z]) / (double)P;
+  }
+  free(A);
+  return 0;
+}
+
+/* ------------------------------------------------------------------ O6, O7 local terms */
+
+/* H_ex = 2A/(mu0 Ms) sum_d [m(i+e_d) - 2 m(i) + m(i-e_d)] / D_d^2; a neighbour outside
+ * the mesh is replaced by m(i) (Neumann), so an axis with n_d = 1 contributes 0. */
+int orc_exchange(int nx, int ny, int nz, double dx, double dy, double dz, double Ms, double Aex,
+                 const double *m, double *H) {
+  const double pref = 2.0 * Aex / (ORC_MU0 * Ms);
+  const double inv[3] = {1.0 / (dx * dx), 1.0 / (dy * dy), 1.0 / (dz * dz)};
+  const int n[3] = {nx, ny, nz};
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int x = 0; x < nx; ++x)
+    for (int y = 0; y < ny; ++y)
+      for (int z = 0; z < nz; ++z) {
+        const int idx[3] = {x, y, z};
+        const size_t i0 = (((size_t)x * ny + y) * nz + z) * 3;
+        for (int c = 0; c < 3; ++c) {
+          double lap = 0.0;
+          for (int d = 0; d < 3; ++d) {
+            int ip[3] = {x, y, z}, im[3] = {x, y, z};
+            ip[d] = idx[d] + 1 < n[d] ? idx[d] + 1 : idx[d];
+            im[d] = idx[d] - 1 >= 0 ? idx[d] - 1 : idx[d];
+            const double mp = m[(((size_t)ip[0] * ny + ip[1]) * nz + ip[2]) * 3 + c];
+            const double mm = m[(((size_t)im[0] * ny + im[1]) * nz + im[2]) * 3 + c];
+            lap += (mp - 2.0 * m[i0 + c] + mm) * inv[d];
+          }
+          H[i0 + c] = pref * lap;
+        }
+      }
+  return 0;
+}
+
+/* H_an = 2Ku/(mu0 Ms) (m.u) u, u a unit vector. */
+int orc_anisotropy(size_t ncell, double Ms, double Ku, const double u[3], const double *m,
+                   double *H) {
+  const double pref = 2.0 * Ku / (ORC_MU0 * Ms);
+  for (size_t i = 0; i < ncell; ++i) {
+    const double d = m[3 * i] * u[0] + m[3 * i + 1] * u[1] + m[3 * i + 2] * u[2];
+    for (int c = 0; c < 3; ++c) H[3 * i + c] = pref * d * u[c];
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------ problem + O8, O9 */
+
+typedef struct {
+  int nx, ny, nz;
+  double dx, dy, dz;
+  double Ms, Aex, Ku, axis[3], alpha, gamma, Hext[3];
+  unsigned terms;
+  const double *Nhat; /* from orc_demag_fft_nhat; required if DEMAG is enabled */
+} orc_problem;
+
+/* H_eff = sum of enabled terms. */
+int orc_heff(const orc_problem *p, const double *m, double *H) {
+  const size_t n = (size_t)p->nx * p->ny * p->nz;
+  double *T = malloc(3 * n * sizeof(double));
+  if (!T) return 2;
+  memset(H, 0, 3 * n * sizeof(double));
+  if (p->terms & ORC_TERM_DEMAG) {
+    if (!p->Nhat) { free(T); return 3; }
+    int rc = orc_demag_fft(p->nx, p->ny, p->nz, p->Nhat, p->Ms, m, T);
+    if (rc) { free(T); return rc; }
+    for (size_t i = 0; i < 3 * n; ++i) H[i] += T[i];
+  }
+  if (p->terms & ORC_TERM_EXCHANGE) {
+    orc_exchange(p->nx, p->ny, p->nz, p->dx, p->dy, p->dz, p->Ms, p->Aex, m, T);
+    for (size_t i = 0; i < 3 * n; ++i) H[i] += T[i];
+  }
+  if (p->terms & ORC_TERM_ANISOTROPY) {
+    orc_anisotropy(n, p->Ms, p->Ku, p->axis, m, T);
+    for (size_t i = 0; i < 3 * n; ++i) H[i] += T[i];
+  }
+  if (p->terms & ORC_TERM_ZEEMAN)
+    for (size_t i = 0; i < n; ++i)
+      for (int c = 0; c < 3; ++c) H[3 * i + c] += p->Hext[c];
+  free(T);
+  return 0;
+}
+
+static void cross3(const double a[3], const double b[3], double o[3]) {
+  o[0] = a[1] * b[2] - a[2] * b[1];
+  o[1] = a[2] * b[0] - a[0] * b[2];
+  o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+/* dm/dt = -gamma/(1+alpha^2) [ m x H + alpha m x (m x H) ]   (eq. 1) */
+int orc_llg_torque(size_t ncell, double alpha, double gamma, const double *m, const double *H,
+                   double *dmdt) {
+  const double pref = -gamma / (1.0 + alpha * alpha);
+  for (size_t i = 0; i < ncell; ++i) {
+    double mxh[3], mxmxh[3];
+    cross3(m + 3 * i, H + 3 * i, mxh);
+    cross3(m + 3 * i, mxh, mxmxh);
+    for (int c = 0; c < 3; ++c) dmdt[3 * i + c] = pref * (mxh[c] + alpha * mxmxh[c]);
+  }
+  return 0;
+}
+
+int orc_llg_rhs(const orc_problem *p, const double *m, double *dmdt) {
+  const size_t n = (size_t)p->nx * p->ny * p->nz;
+  double *H = malloc(3 * n * sizeof(double));
+  if (!H) return 2;
+  int rc = orc_heff(p, m, H);
+  if (!rc) rc = orc_llg_torque(n, p->alpha, p->gamma, m, H, dmdt);
+  free(H);
+  return rc;
+}
+
+/* Classic RK4, then m <- m/|m| per cell; stage vectors are not renormalised. */
+int orc_rk4_step(const orc_problem *p, double *m, double dt) {
+  const size_t n3 = (size_t)p->nx * p->ny * p->nz * 3;
+  double *k1 = malloc(4 * n3 * sizeof(double)), *ms = malloc(n3 * sizeof(double));
+  if (!k1 || !ms) return 2;
+  double *k2 = k1 + n3, *k3 = k2 + n3, *k4 = k3 + n3;
+  int rc = orc_llg_rhs(p, m, k1);
+  for (size_t i = 0; i < n3; ++i) ms[i] = m[i] + 0.5 * dt * k1[i];
+  if (!rc) rc = orc_llg_rhs(p, ms, k2);
+  for (size_t i = 0; i < n3; ++i) ms[i] = m[i] + 0.5 * dt * k2[i];
+  if (!rc) rc = orc_llg_rhs(p, ms, k3);
+  for (size_t i = 0; i < n3; ++i) ms[i] = m[i] + dt * k3[i];
+  if (!rc) rc = orc_llg_rhs(p, ms, k4);
+  if (!rc) {
+    for (size_t i = 0; i < n3; ++i) m[i] += dt / 6.0 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+    for (size_t i = 0; i < n3; i += 3) {
+      const double nrm = sqrt(m[i] * m[i] + m[i + 1] * m[i + 1] + m[i + 2] * m[i + 2]);
+      m[i] /= nrm; m[i + 1] /= nrm; m[i + 2] /= nrm;
+    }
+  }
+  free(k1); free(ms);
+  return rc;
+}

@@ -1,0 +1,229 @@
+"""ctypes front end of the CPU oracle (oracle/mm_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this module.  It imports nothing from the
+CUDA package and the CUDA package imports nothing from here.
+
+All arrays are fp64 numpy arrays of shape [nx, ny, nz, 3] (PAPER.md:130-132 layout).
+Function-by-function citations are in the header of mm_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass, field
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mm_oracle.c")
+_LIB = os.path.join(_HERE, "libmm_oracle.so")
+
+MU0 = 4.0e-7 * np.pi  # reading Q8
+
+TERM_DEMAG, TERM_EXCHANGE, TERM_ANISOTROPY, TERM_ZEEMAN = 1, 2, 4, 8
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (quadmath + OpenMP).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC,
+               "-lquadmath", "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+class _Problem(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+                ("Ms", C.c_double), ("Aex", C.c_double), ("Ku", C.c_double),
+                ("axis", C.c_double * 3), ("alpha", C.c_double), ("gamma", C.c_double),
+                ("Hext", C.c_double * 3), ("terms", C.c_uint), ("Nhat", C.c_void_p)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with code {rc}")
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def newell_point(d, i, j, k):
+    """N(xx,yy,zz,xy,xz,yz) at cell offset (i,j,k) by the literal 27-point definition (O1)."""
+    out = np.zeros(6)
+    lib().orc_newell_point(C.c_double(d[0]), C.c_double(d[1]), C.c_double(d[2]),
+                           C.c_int(i), C.c_int(j), C.c_int(k), _p(out))
+    return out
+
+
+def newell_octant(n, d):
+    """Octant table N[6, nx, ny, nz] (O1)."""
+    N = np.zeros((6, n[0], n[1], n[2]))
+    _chk(lib().orc_newell_octant(C.c_int(n[0]), C.c_int(n[1]), C.c_int(n[2]), C.c_double(d[0]),
+                                 C.c_double(d[1]), C.c_double(d[2]), _p(N)), "newell_octant")
+    return N
+
+
+def demag_direct(N, Ms, m):
+    """O3: full O(n^2) real-space sum."""
+    m = _f64(m)
+    nx, ny, nz = m.shape[:3]
+    H = np.zeros_like(m)
+    _chk(lib().orc_demag_direct(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(N), C.c_double(Ms),
+                                _p(m), _p(H)), "demag_direct")
+    return H
+
+
+def demag_direct_sampled(N, Ms, m, cells):
+    """O3 at chosen flat cell indices; returns [nsamp, 3]."""
+    m = _f64(m)
+    nx, ny, nz = m.shape[:3]
+    cells = np.ascontiguousarray(cells, dtype=np.int64)
+    Hs = np.zeros((len(cells), 3))
+    _chk(lib().orc_demag_direct_sampled(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(N),
+                                        C.c_double(Ms), _p(m), C.c_int(len(cells)), _p(cells),
+                                        _p(Hs)), "demag_direct_sampled")
+    return Hs
+
+
+def demag_dft(N, Ms, m):
+    """O4: literal-DFT zero-padded convolution (tiny meshes only)."""
+    m = _f64(m)
+    nx, ny, nz = m.shape[:3]
+    H = np.zeros_like(m)
+    _chk(lib().orc_demag_dft(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(N), C.c_double(Ms), _p(m),
+                             _p(H)), "demag_dft")
+    return H
+
+
+def padded(n):
+    return 1 if n == 1 else 2 * n
+
+
+def demag_fft_nhat(N, return_max_imag=False):
+    """O5 set-up: real Fourier-space tensor Nhat[6, Px, Py, Pz]."""
+    _, nx, ny, nz = N.shape
+    Nhat = np.zeros((6, padded(nx), padded(ny), padded(nz)))
+    mi = C.c_double(0.0)
+    _chk(lib().orc_demag_fft_nhat(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(N), _p(Nhat),
+                                  C.byref(mi)), "demag_fft_nhat")
+    return (Nhat, mi.value) if return_max_imag else Nhat
+
+
+def demag_fft(Nhat, Ms, m):
+    """O5: demag field by the oracle's own FFT path."""
+    m = _f64(m)
+    nx, ny, nz = m.shape[:3]
+    H = np.zeros_like(m)
+    _chk(lib().orc_demag_fft(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(Nhat), C.c_double(Ms),
+                             _p(m), _p(H)), "demag_fft")
+    return H
+
+
+def exchange(d, Ms, Aex, m):
+    """O6."""
+    m = _f64(m)
+    nx, ny, nz = m.shape[:3]
+    H = np.zeros_like(m)
+    _chk(lib().orc_exchange(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(d[0]),
+                            C.c_double(d[1]), C.c_double(d[2]), C.c_double(Ms), C.c_double(Aex),
+                            _p(m), _p(H)), "exchange")
+    return H
+
+
+def anisotropy(Ms, Ku, axis, m):
+    """O7."""
+    m = _f64(m)
+    u = _f64(axis)
+    H = np.zeros_like(m)
+    _chk(lib().orc_anisotropy(C.c_size_t(m.size // 3), C.c_double(Ms), C.c_double(Ku), _p(u),
+                              _p(m), _p(H)), "anisotropy")
+    return H
+
+
+def llg_torque(alpha, gamma, m, H):
+    """O8 on a given field."""
+    m = _f64(m)
+    H = _f64(H)
+    out = np.zeros_like(m)
+    _chk(lib().orc_llg_torque(C.c_size_t(m.size // 3), C.c_double(alpha), C.c_double(gamma),
+                              _p(m), _p(H), _p(out)), "llg_torque")
+    return out
+
+
+@dataclass
+class Problem:
+    """Mesh + material + enabled terms; mirrors the paper's state.material / field-term list
+    (PAPER.md:84-161)."""
+    n: tuple
+    d: tuple
+    Ms: float
+    Aex: float = 0.0
+    Ku: float = 0.0
+    axis: tuple = (0.0, 0.0, 1.0)
+    alpha: float = 0.0
+    gamma: float = 2.211e5
+    Hext: tuple = (0.0, 0.0, 0.0)
+    terms: int = TERM_DEMAG | TERM_EXCHANGE
+    N: np.ndarray | None = field(default=None, repr=False)
+    Nhat: np.ndarray | None = field(default=None, repr=False)
+
+    def prepare(self):
+        """One-off: Newell table and its transform (excluded from any timing)."""
+        if self.terms & TERM_DEMAG and self.Nhat is None:
+            if self.N is None:
+                self.N = newell_octant(self.n, self.d)
+            self.Nhat = demag_fft_nhat(self.N)
+        return self
+
+    def _c(self):
+        s = _Problem()
+        s.nx, s.ny, s.nz = self.n
+        s.dx, s.dy, s.dz = self.d
+        s.Ms, s.Aex, s.Ku = self.Ms, self.Aex, self.Ku
+        s.axis[:] = list(self.axis)
+        s.alpha, s.gamma = self.alpha, self.gamma
+        s.Hext[:] = list(self.Hext)
+        s.terms = self.terms
+        s.Nhat = self.Nhat.ctypes.data if self.Nhat is not None else None
+        return s
+
+    def heff(self, m):
+        m = _f64(m)
+        H = np.zeros_like(m)
+        _chk(lib().orc_heff(C.byref(self._c()), _p(m), _p(H)), "heff")
+        return H
+
+    def llg_rhs(self, m):
+        m = _f64(m)
+        out = np.zeros_like(m)
+        _chk(lib().orc_llg_rhs(C.byref(self._c()), _p(m), _p(out)), "llg_rhs")
+        return out
+
+    def rk4_step(self, m, dt):
+        """O9; returns the new m (input untouched)."""
+        m = _f64(m).copy()
+        _chk(lib().orc_rk4_step(C.byref(self._c()), _p(m), C.c_double(dt)), "rk4_step")
+        return m

@@ -1,0 +1,124 @@
+"""Pins for the oracle's local terms, LLG right-hand side and RK4 (O6-O9): closed forms and
+invariants from SURVEY.md 8(c).  CPU only."""
+import numpy as np
+import pytest
+
+import workloads as w
+
+MU0 = 4e-7 * np.pi
+
+
+def test_exchange_zero_for_uniform(oracle):
+    m = np.zeros((6, 5, 4, 3))
+    m[...] = np.array([0.6, 0.0, 0.8])
+    H = oracle.exchange((1e-9, 2e-9, 3e-9), 8e5, 1.3e-11, m)
+    assert np.all(H == 0.0)
+
+
+@pytest.mark.parametrize("axis,q", [(0, 1), (0, 3), (1, 2), (2, 1)])
+def test_exchange_neumann_eigenvector(oracle, axis, q):
+    """m_x(j) = cos(pi q (j+1/2)/n)  =>  H_x = -(2A/mu0 Ms)(4/D^2) sin^2(pi q/2n) m_x exactly."""
+    n = (8, 6, 4)
+    d = (1e-9, 2e-9, 3e-9)
+    Ms, A = 8e5, 1.3e-11
+    j = np.arange(n[axis])
+    prof = np.cos(np.pi * q * (j + 0.5) / n[axis])
+    shape = [1, 1, 1]
+    shape[axis] = n[axis]
+    m = np.zeros(n + (3,))
+    m[..., 0] = prof.reshape(shape)
+    m[..., 1] = 0.25                                  # uniform component: no contribution
+    H = oracle.exchange(d, Ms, A, m)
+    lam = -(2 * A / (MU0 * Ms)) * (4 / d[axis] ** 2) * np.sin(np.pi * q / (2 * n[axis])) ** 2
+    assert np.allclose(H[..., 0], lam * m[..., 0], rtol=1e-12, atol=1e-9 * abs(lam))
+    assert np.allclose(H[..., 1], 0.0, atol=1e-9 * abs(lam))
+    assert np.all(H[..., 2] == 0.0)
+
+
+def test_exchange_single_axis_contributes_nothing(oracle):
+    m = w.random_unit_vectors(3, (1, 1, 1))
+    assert np.all(oracle.exchange((1e-9,) * 3, 8e5, 1e-11, m) == 0.0)
+    m = w.random_unit_vectors(3, (4, 1, 1))
+    H = oracle.exchange((1e-9, 5e-9, 7e-9), 8e5, 1e-11, m)
+    # hand stencil, first cell: neighbour on the left replaced by itself
+    pref = 2 * 1e-11 / (MU0 * 8e5) / 1e-18
+    assert np.allclose(H[0, 0, 0], pref * (m[1, 0, 0] - m[0, 0, 0]), rtol=1e-13)
+    assert np.allclose(H[2, 0, 0], pref * (m[3, 0, 0] - 2 * m[2, 0, 0] + m[1, 0, 0]), rtol=1e-12)
+
+
+def test_anisotropy_closed_forms(oracle):
+    Ms, Ku = 1e6, 5e5
+    u = np.array([0.0, 0.0, 1.0])
+    m = np.zeros((2, 1, 1, 3))
+    m[0, 0, 0] = u
+    m[1, 0, 0] = [1.0, 0.0, 0.0]
+    H = oracle.anisotropy(Ms, Ku, u, m)
+    assert np.allclose(H[0, 0, 0], 2 * Ku / (MU0 * Ms) * u, rtol=1e-15)
+    assert np.all(H[1, 0, 0] == 0.0)
+    u2 = np.array([1.0, 2.0, 2.0]) / 3.0
+    mm = w.random_unit_vectors(1, (3, 3, 3))
+    H = oracle.anisotropy(Ms, Ku, u2, mm)
+    assert np.allclose(H, 2 * Ku / (MU0 * Ms) * (mm @ u2)[..., None] * u2, rtol=1e-13)
+
+
+def test_llg_hand_example_and_invariants(oracle):
+    alpha, gamma, h = 0.3, 2.211e5, 1.0e5
+    m = np.array([[[[1.0, 0.0, 0.0]]]])
+    H = np.array([[[[0.0, h, 0.0]]]])
+    # m x H = h z ;  m x (m x H) = x x (h z) = -h y
+    want = -gamma / (1 + alpha**2) * np.array([0.0, -alpha * h, h])
+    assert np.allclose(oracle.llg_torque(alpha, gamma, m, H)[0, 0, 0], want, rtol=1e-15)
+    mm = w.random_unit_vectors(11, (4, 4, 4))
+    HH = 1e6 * w.normal_field(12, 4 * 4 * 4 * 3).reshape(4, 4, 4, 3)
+    t = oracle.llg_torque(alpha, gamma, mm, HH)
+    assert np.max(np.abs(np.sum(mm * t, axis=-1))) < 1e-15 * np.max(np.abs(t))   # m . dm/dt = 0
+    # H || m -> 0 (round-off of gamma*|H| only)
+    assert np.max(np.abs(oracle.llg_torque(alpha, gamma, mm, 3e5 * mm))) < 1e-15 * gamma * 3e5
+
+
+def _macrospin(oracle, dt, steps, alpha=0.1, Hz=1e6):
+    P = oracle.Problem(n=(2, 1, 1), d=(1e-9,) * 3, Ms=8e5, alpha=alpha, Hext=(0, 0, Hz),
+                       terms=oracle.TERM_ZEEMAN)
+    m0 = np.array([np.sin(1.0), 0.0, np.cos(1.0)])
+    m = np.tile(m0, (2, 1, 1, 1))
+    for _ in range(steps):
+        m = P.rk4_step(m, dt)
+    T = dt * steps
+    g = 2.211e5
+    mz = np.tanh(alpha * g * Hz * T / (1 + alpha**2) + np.arctanh(m0[2]))
+    phi = g * Hz * T / (1 + alpha**2)
+    s = np.sqrt(1 - mz * mz)
+    exact = np.array([s * np.cos(phi), s * np.sin(phi), mz])
+    return np.max(np.abs(m[0, 0, 0] - exact)), m
+
+
+def test_rk4_macrospin_closed_form_and_order(oracle):
+    """Uniform m in a constant field: m_z = tanh(a g H t/(1+a^2) + atanh m_z0), azimuth
+    g H t/(1+a^2); the global error of RK4 falls 16x when dt halves."""
+    e4, _ = _macrospin(oracle, 4e-13, 50)
+    e2, _ = _macrospin(oracle, 2e-13, 100)
+    e1, m = _macrospin(oracle, 1e-13, 200)
+    assert e1 < 1e-8 and e2 < 2e-7
+    assert 12 < e4 / e2 < 20 and 12 < e2 / e1 < 20
+    assert np.allclose(np.linalg.norm(m, axis=-1), 1.0, atol=1e-15)
+
+
+def test_heff_is_sum_of_terms(oracle):
+    c = w.get_config(1)
+    m = c.initial_m()
+    P = oracle.Problem(n=c.n, d=c.d, Ms=c.Ms, Aex=c.Aex, Ku=2e5, axis=(0, 0.6, 0.8), alpha=c.alpha,
+                       Hext=(1e4, -2e4, 3e4), terms=15).prepare()
+    H = P.heff(m)
+    parts = (oracle.demag_fft(P.Nhat, c.Ms, m) + oracle.exchange(c.d, c.Ms, c.Aex, m)
+             + oracle.anisotropy(c.Ms, 2e5, (0, 0.6, 0.8), m) + np.array([1e4, -2e4, 3e4]))
+    assert np.allclose(H, parts, rtol=1e-14, atol=1e-6)
+    assert np.allclose(P.llg_rhs(m), oracle.llg_torque(c.alpha, 2.211e5, m, H), rtol=1e-14)
+
+
+def test_rk4_conserves_norm_full_problem(oracle):
+    c = w.get_config(1)
+    P = oracle.Problem(n=c.n, d=c.d, Ms=c.Ms, Aex=c.Aex, alpha=c.alpha, terms=c.terms).prepare()
+    m = c.initial_m()
+    m1 = P.rk4_step(m, c.dt)
+    assert np.allclose(np.linalg.norm(m1, axis=-1), 1.0, atol=2e-16)
+    assert 0 < np.max(np.abs(m1 - m)) < 0.5
