@@ -1,0 +1,127 @@
+/*
+ * mm_b200.h -- C ABI of the B200-native micromagnetic hot path of arxiv/paper_2606_01114
+ * ("Magnum.np.distributed").  One GPU, one context per mesh, every step a hand-written
+ * sm_100a kernel; no cuFFT, no CPU fallback.
+ *
+ * Citations: PAPER.md = /root/reference/PAPER.md (line numbers), SURVEY = SURVEY.md.
+ *
+ * Conventions shared by every call
+ * --------------------------------
+ *  - Field arrays m, H, dmdt: contiguous [nx][ny][nz][3], component fastest, then z
+ *    (the paper's state tensor state.m[x,y,z,c]), element type float
+ *    (MM_F32) or double (MM_F64) as chosen at mm_ctx_create.  m is a dimensionless unit
+ *    vector per cell, H in A/m, dmdt in 1/s, lengths in metres.
+ *  - Pointers named m / H / dmdt / out are DEVICE pointers unless the function name ends
+ *    in _host; device pointers must be 16-byte aligned.  double[3] arguments and the
+ *    context handle are HOST pointers.
+ *  - Ownership: the caller owns every device buffer including the two workspaces; the
+ *    library never allocates or frees device memory (PyTorch does, in the binding).
+ *    The context owns only small host-side plan data.
+ *  - Execution: field/step calls enqueue kernels on the context's stream and return without
+ *    synchronising (CUDA-graph capturable, deterministic: no atomics).  mm_demag_init and
+ *    the *_host calls synchronise the stream before returning.
+ *  - Errors: every call returns mm_status; nothing is thrown across the ABI.  After a
+ *    non-OK status mm_last_error(ctx) holds a one-line explanation.
+ *  - Sizes: every n_d must be 1 or a power of two, nx, ny <= 1024, nz <= 512
+ *    (MM_ERR_UNSUPPORTED_SIZE otherwise).  An axis with n_d = 1 is neither padded nor
+ *    transformed (reading Q10 in DESIGN.md).
+ */
+#ifndef MM_B200_H
+#define MM_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mm_ctx mm_ctx; /* opaque, owned by the library */
+
+typedef enum { MM_F32 = 0, MM_F64 = 1 } mm_dtype;
+
+typedef enum {
+  MM_OK = 0,
+  MM_ERR_INVALID_ARG = 1,      /* NULL / misaligned pointer, non-positive size or cell, H == m */
+  MM_ERR_UNSUPPORTED_SIZE = 2, /* n_d not 1 or a power of two, or above the planned maximum */
+  MM_ERR_NOT_INITIALISED = 3,  /* workspace, material or mm_demag_init missing */
+  MM_ERR_WORKSPACE = 4,        /* workspace too small */
+  MM_ERR_CUDA = 5,             /* CUDA runtime / launch error, text in mm_last_error */
+  MM_ERR_NOT_IMPLEMENTED = 6
+} mm_status;
+
+/* Field terms of H_eff (H_eff is a sum of terms). */
+enum { MM_TERM_DEMAG = 1, MM_TERM_EXCHANGE = 2, MM_TERM_ANISOTROPY = 4, MM_TERM_ZEEMAN = 8 };
+
+/* Mesh of nx x ny x nz cells of size dx x dy x dz metres (Mesh(n, dx)). */
+mm_status mm_ctx_create(int nx, int ny, int nz, double dx, double dy, double dz, mm_dtype dtype,
+                        mm_ctx **out);
+mm_status mm_ctx_destroy(mm_ctx *ctx);
+
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default. */
+mm_status mm_ctx_set_stream(mm_ctx *ctx, void *cuda_stream);
+
+/* Bytes the caller must provide.  persistent: Fourier-space demag tensor, twiddle and index
+ * tables (written by mm_demag_init, read afterwards).  scratch: padded spectra, H_demag,
+ * RK4 stage buffers, host-call staging; contents are undefined between calls. */
+mm_status mm_ctx_workspace_bytes(const mm_ctx *ctx, size_t *persistent, size_t *scratch);
+mm_status mm_ctx_set_workspace(mm_ctx *ctx, void *persistent, size_t pbytes, void *scratch,
+                               size_t sbytes);
+
+/* Material (PAPER.md:92-100 state.material): Ms [A/m], Aex [J/m], Ku [J/m^3] with unit axis
+ * (normalised internally; ignored if Ku == 0), Gilbert alpha, gamma [m/(A s)] (2.211e5). */
+mm_status mm_set_material(mm_ctx *ctx, double Ms, double Aex, double Ku, const double axis[3],
+                          double alpha, double gamma);
+/* Uniform external field in A/m (PAPER.md:140-143 ExternalField(B/mu0)). */
+mm_status mm_set_zeeman(mm_ctx *ctx, const double Hext[3]);
+/* OR of MM_TERM_*; default DEMAG | EXCHANGE. */
+mm_status mm_set_terms(mm_ctx *ctx, unsigned term_mask);
+
+/* S0: Newell tensor (ref. 23 formula, evaluated in __float128 on the device
+ * for offsets i,j,k >= 0), its exact even/odd mirror expressed as separable cos/sin
+ * transforms in fp64, stored real in the layout the x pass consumes with 1/(Px Py Pz)
+ * folded in.  Needs both workspaces.  Idempotent.  Synchronises. */
+mm_status mm_demag_init(mm_ctx *ctx);
+
+/* Writes the Fourier-space tensor in natural order, [6][nx'][ny'][nz'] with n_d' = n_d+1
+ * (or 1 when n_d = 1), components xx yy zz xy xz yz, context dtype, unscaled: the real part
+ * of the forward DFT of the mirrored tensor at kx<=nx, ky<=ny, kz<=nz.  For tests. */
+mm_status mm_demag_nhat_export(mm_ctx *ctx, void *out);
+
+/* H := H_demag(m) = -Ms * crop(IFFT(Nhat . FFT(pad(m))))   (PAPER.md:45 eq. 4, :47, :53).
+ * Kernels S1..S5 of DESIGN.md.  H must not alias m. */
+mm_status mm_demag_field(mm_ctx *ctx, const void *m, void *H);
+/* H := 2A/(mu0 Ms) * 6-point Laplacian of m, Neumann boundary (eq. 2). */
+mm_status mm_exchange_field(mm_ctx *ctx, const void *m, void *H);
+/* H := sum of the enabled terms. */
+mm_status mm_heff(mm_ctx *ctx, const void *m, void *H);
+/* dmdt := -gamma/(1+alpha^2) [m x H_eff + alpha m x (m x H_eff)]  (eq. 1);
+ * H_eff is evaluated internally and not materialised. */
+mm_status mm_llg_rhs(mm_ctx *ctx, const void *m, void *dmdt);
+/* One classic RK4 step of size dt [s] followed by m <- m/|m|; m updated in place
+ * (fixed-step stand-in for the paper's RKF45; reading Q14). */
+mm_status mm_rk_step(mm_ctx *ctx, void *m_inout, double dt);
+
+/* Same operations on HOST buffers (pageable or pinned): copies m host->device into scratch
+ * staging, runs the device path, copies the result device->host, synchronises.  These are
+ * what bench.py's end-to-end leg times. */
+mm_status mm_demag_field_host(mm_ctx *ctx, const void *m_host, void *H_host);
+mm_status mm_heff_host(mm_ctx *ctx, const void *m_host, void *H_host);
+mm_status mm_llg_rhs_host(mm_ctx *ctx, const void *m_host, void *dmdt_host);
+mm_status mm_rk_step_host(mm_ctx *ctx, void *m_inout_host, double dt);
+
+/* Number of kernel launches the library has enqueued on this context since creation
+ * (bench.py reports the difference over its timed region as gpu_launches). */
+mm_status mm_ctx_launch_count(const mm_ctx *ctx, unsigned long long *count);
+
+/* Tuning knobs for experiments (tile widths of the FFT passes); 0 keeps the default.
+ * Must be called before mm_demag_init. */
+mm_status mm_ctx_set_tiles(mm_ctx *ctx, int bz, int by, int bk);
+
+/* Last error text of this context (or of the last failed mm_ctx_create if ctx is NULL).
+ * Not thread-safe. */
+const char *mm_last_error(const mm_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MM_B200_H */

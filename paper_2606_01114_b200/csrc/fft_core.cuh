@@ -1,0 +1,203 @@
+// In-register radix-R DFT butterflies and in-place shared-memory FFT stages.
+//
+// Scheme: a tile holds N rows x B columns of complex
+// values, column = one independent pencil ("lanes along batch": consecutive threads own
+// consecutive columns, so every shared-memory access of a warp is a contiguous run and
+// twiddles are warp-uniform).  Forward = decimation in frequency, in place, natural order
+// in -> digit-reversed order out; inverse = the exact mirror image (decimation in time,
+// digit-reversed in -> natural out).  The pointwise multiply with the demag tensor happens
+// in digit-reversed order, so no reordering pass is ever executed (FFT,
+// pointwise multiplication, inverse FFT).
+#pragma once
+#include <utility>
+
+#include "mm_common.cuh"
+
+namespace mm {
+
+// cos(2 pi k / 32), k = 0..8
+constexpr double kCos32[9] = {1.0,
+                                         0.98078528040323044913,
+                                         0.92387953251128675613,
+                                         0.83146961230254523708,
+                                         0.70710678118654752440,
+                                         0.55557023301960222474,
+                                         0.38268343236508977173,
+                                         0.19509032201612826785,
+                                         0.0};
+
+template <int R, int S> constexpr double root_cos() {
+  constexpr int a = (S % R) * (32 / R);  // angle in 1/32 turns, 0..31
+  if (a <= 8) return kCos32[a];
+  if (a <= 16) return -kCos32[16 - a];
+  if (a <= 24) return -kCos32[a - 16];
+  return kCos32[32 - a];
+}
+template <int R, int S> constexpr double root_sin() {
+  constexpr int a = (S % R) * (32 / R);
+  if (a <= 8) return kCos32[8 - a];
+  if (a <= 16) return kCos32[a - 8];
+  if (a <= 24) return -kCos32[24 - a];
+  return -kCos32[a - 24];
+}
+
+// v * w_R^S with w_R = exp(-2 pi i / R) (forward) or its conjugate (INV).
+template <typename T, int R, int S, bool INV> __device__ __forceinline__ Cx<T> mul_root(Cx<T> v) {
+  constexpr int s = S % R;
+  if constexpr (s == 0) {
+    return v;
+  } else if constexpr (4 * s == R) {  // -i (forward)
+    return INV ? mk<T>(-v.y, v.x) : mk<T>(v.y, -v.x);
+  } else if constexpr (2 * s == R) {
+    return mk<T>(-v.x, -v.y);
+  } else if constexpr (4 * s == 3 * R) {  // +i (forward)
+    return INV ? mk<T>(v.y, -v.x) : mk<T>(-v.y, v.x);
+  } else if constexpr (8 * s == R) {  // (1 - i)/sqrt2 (forward)
+    constexpr T h = (T)0.70710678118654752440;
+    return INV ? mk<T>((v.x - v.y) * h, (v.x + v.y) * h) : mk<T>((v.x + v.y) * h, (v.y - v.x) * h);
+  } else if constexpr (8 * s == 3 * R) {  // (-1 - i)/sqrt2 (forward)
+    constexpr T h = (T)0.70710678118654752440;
+    return INV ? mk<T>((-v.x - v.y) * h, (v.x - v.y) * h) : mk<T>((v.y - v.x) * h, (-v.x - v.y) * h);
+  } else {
+    constexpr T c = (T)root_cos<R, s>();
+    constexpr T sn = (T)root_sin<R, s>();
+    // forward: (c - i sn); inverse: (c + i sn)
+    return INV ? mk<T>(v.x * c - v.y * sn, v.y * c + v.x * sn)
+               : mk<T>(v.x * c + v.y * sn, v.y * c - v.x * sn);
+  }
+}
+
+// Radix-R DFT of v[0..R) in registers, natural order in and out, unnormalised.
+// Decimation in frequency: sums -> even outputs, twiddled differences -> odd outputs.
+template <typename T, int R, bool INV> struct Dft {
+  template <int... I>
+  static __device__ __forceinline__ void split(const Cx<T>* v, Cx<T>* a, Cx<T>* b,
+                                               std::integer_sequence<int, I...>) {
+    ((a[I] = cadd(v[I], v[I + R / 2])), ...);
+    ((b[I] = mul_root<T, R, I, INV>(csub(v[I], v[I + R / 2]))), ...);
+  }
+  static __device__ __forceinline__ void run(Cx<T>* v) {
+    Cx<T> a[R / 2], b[R / 2];
+    split(v, a, b, std::make_integer_sequence<int, R / 2>{});
+    Dft<T, R / 2, INV>::run(a);
+    Dft<T, R / 2, INV>::run(b);
+#pragma unroll
+    for (int k = 0; k < R / 2; ++k) {
+      v[2 * k] = a[k];
+      v[2 * k + 1] = b[k];
+    }
+  }
+};
+template <typename T, bool INV> struct Dft<T, 1, INV> {
+  static __device__ __forceinline__ void run(Cx<T>*) {}
+};
+
+// One forward stage of span S (radix R) over a tile of N rows x B columns in shared memory,
+// row r of column c at sm[r * B + c].  Thread (col, tt) with NT threads per column.
+// W[q] = exp(-2 pi i q / P); wstep = P / S so that w_S^(t u) = W[t u wstep].
+template <typename T, int R>
+__device__ __forceinline__ void stage_fwd(Cx<T>* sm, int B, int col, int tt, int NT, int N, int S,
+                                          const Cx<T>* __restrict__ W, int wstep) {
+  const int q = S / R;
+  for (int b = tt; b < N / R; b += NT) {
+    const int blk = b / q, t = b - blk * q;
+    Cx<T>* p = sm + (size_t)(blk * S + t) * B + col;
+    Cx<T> v[R];
+#pragma unroll
+    for (int s = 0; s < R; ++s) v[s] = p[(size_t)s * q * B];
+    Dft<T, R, false>::run(v);
+    if (q > 1) {
+#pragma unroll
+      for (int u = 1; u < R; ++u) v[u] = cmul(v[u], __ldg(W + t * u * wstep));
+    }
+#pragma unroll
+    for (int u = 0; u < R; ++u) p[(size_t)u * q * B] = v[u];
+  }
+}
+
+// Exact mirror of stage_fwd: conj twiddle, inverse butterfly (unnormalised).
+template <typename T, int R>
+__device__ __forceinline__ void stage_inv(Cx<T>* sm, int B, int col, int tt, int NT, int N, int S,
+                                          const Cx<T>* __restrict__ W, int wstep) {
+  const int q = S / R;
+  for (int b = tt; b < N / R; b += NT) {
+    const int blk = b / q, t = b - blk * q;
+    Cx<T>* p = sm + (size_t)(blk * S + t) * B + col;
+    Cx<T> v[R];
+#pragma unroll
+    for (int u = 0; u < R; ++u) v[u] = p[(size_t)u * q * B];
+    if (q > 1) {
+#pragma unroll
+      for (int u = 1; u < R; ++u) v[u] = cmulc(v[u], __ldg(W + t * u * wstep));
+    }
+    Dft<T, R, true>::run(v);
+#pragma unroll
+    for (int s = 0; s < R; ++s) p[(size_t)s * q * B] = v[s];
+  }
+}
+
+// All forward stages of the length-L sub-transforms tiling the N rows (N multiple of L).
+template <typename T>
+__device__ __forceinline__ void run_stages_fwd(Cx<T>* sm, int B, int col, int tt, int NT, int N,
+                                               const FftPlan& pl, const Cx<T>* __restrict__ W) {
+  int S = pl.L;
+  for (int i = 0; i < pl.nstages; ++i) {
+    const int R = pl.radix[i];
+    const int wstep = pl.P / S;
+    switch (R) {
+      case 16: stage_fwd<T, 16>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 8: stage_fwd<T, 8>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 4: stage_fwd<T, 4>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      default: stage_fwd<T, 2>(sm, B, col, tt, NT, N, S, W, wstep); break;
+    }
+    S /= R;
+    __syncthreads();
+  }
+}
+
+template <typename T>
+__device__ __forceinline__ void run_stages_inv(Cx<T>* sm, int B, int col, int tt, int NT, int N,
+                                               const FftPlan& pl, const Cx<T>* __restrict__ W) {
+  int S = 1;
+  for (int i = pl.nstages - 1; i >= 0; --i) {
+    const int R = pl.radix[i];
+    S *= R;
+    const int wstep = pl.P / S;
+    switch (R) {
+      case 16: stage_inv<T, 16>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 8: stage_inv<T, 8>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 4: stage_inv<T, 4>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      default: stage_inv<T, 2>(sm, B, col, tt, NT, N, S, W, wstep); break;
+    }
+    __syncthreads();
+  }
+}
+
+// Host side: position of frequency k in the digit-reversed output of the pruned length-P
+// transform (first a radix-2 split into even/odd outputs, then the plan's stages on L).
+//   k = u0 + 2 (u1 + R1 (u2 + R2 (...)))  ->  pos = u0 L + u1 L/R1 + u2 L/(R1 R2) + ...
+inline int pos_of_freq(const FftPlan& pl, int k) {
+  if (pl.P == 1) return 0;
+  int pos = (k & 1) * pl.L;
+  int kk = k >> 1, span = pl.L;
+  for (int i = 0; i < pl.nstages; ++i) {
+    const int R = pl.radix[i];
+    span /= R;
+    pos += (kk % R) * span;
+    kk /= R;
+  }
+  return pos;
+}
+
+inline FftPlan make_plan(int n) {
+  FftPlan pl{};
+  pl.L = n;
+  pl.P = n == 1 ? 1 : 2 * n;
+  pl.nstages = 0;
+  int rem = n;
+  while (rem >= 8) { pl.radix[pl.nstages++] = 8; rem /= 8; }
+  if (rem > 1) pl.radix[pl.nstages++] = rem;
+  return pl;
+}
+
+}  // namespace mm

@@ -1,0 +1,483 @@
+// C ABI of include/mm_b200.h: context, workspace carve-up, call sequencing.  Every numeric
+// step runs in the kernels of demag_passes.cu / demag_init.cu / pointwise.cu; this file only
+// validates arguments and enqueues launches on the context's stream.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/mm_b200.h"
+#include "demag_init.cuh"
+#include "demag_passes.cuh"
+#include "fft_core.cuh"
+#include "pointwise.cuh"
+
+using namespace mm;
+
+static const double kMu0 = 4.0e-7 * 3.14159265358979323846;  // reading Q8
+static char g_create_error[256] = "";
+
+struct mm_ctx {
+  int nx, ny, nz;
+  double dx, dy, dz;
+  mm_dtype dtype;
+  size_t es;  // bytes per real
+  cudaStream_t stream = nullptr;
+  // material / terms
+  bool have_material = false;
+  double Ms = 0, Aex = 0, Ku = 0, axis[3] = {0, 0, 1}, alpha = 0, gamma = 2.211e5;
+  double Hext[3] = {0, 0, 0};
+  unsigned terms = MM_TERM_DEMAG | MM_TERM_EXCHANGE;
+  // plan
+  DemagGeom geom{};
+  InitGeom igeom{};
+  bool tiles_locked = false;
+  int want_bz = 0, want_by = 0, want_bk = 0;
+  // workspaces
+  unsigned char* pers = nullptr;
+  unsigned char* scr = nullptr;
+  size_t pers_bytes = 0, scr_bytes = 0;
+  bool demag_ready = false;
+  // persistent offsets
+  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, pers_need;
+  // scratch offsets
+  size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, scr_need;
+  unsigned long long launches = 0;
+  char err[256] = "";
+};
+
+static mm_status fail(mm_ctx* c, mm_status s, const char* fmt, ...) {
+  char* dst = c ? c->err : g_create_error;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 256, fmt, ap);
+  va_end(ap);
+  return s;
+}
+
+static bool pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
+static size_t align256(size_t v) { return (v + 255) / 256 * 256; }
+static int padded(int n) { return n == 1 ? 1 : 2 * n; }
+
+static int pick_tile(int limit, size_t bytes_per_col, size_t budget, int cap) {
+  int b = 1;
+  while (b * 2 <= limit && b * 2 <= cap && (size_t)(b * 2) * bytes_per_col <= budget) b *= 2;
+  return b;
+}
+
+// Tile widths and workspace layout; called at create and again if tiles change.
+static void plan_layout(mm_ctx* c) {
+  DemagGeom& g = c->geom;
+  g.nx = c->nx; g.ny = c->ny; g.nz = c->nz;
+  g.Px = padded(c->nx); g.Py = padded(c->ny); g.Pz = padded(c->nz);
+  g.Kz = g.Pz == 1 ? 1 : g.Pz / 2 + 1;
+  g.px = make_plan(c->nx); g.py = make_plan(c->ny); g.pz = make_plan(c->nz);
+  const size_t cs = 2 * c->es;
+  const size_t kMax = 200 * 1024;  // usable dynamic shared memory we plan for (227 KB limit)
+  g.Bz = c->want_bz ? c->want_bz : pick_tile(c->nx, 3 * g.Pz * cs, 100 * 1024, 32);
+  g.By = c->want_by ? c->want_by : pick_tile(c->nx, g.Py * cs, 100 * 1024, 32);
+  g.Bk = c->want_bk ? c->want_bk : pick_tile(g.Py, 3 * g.Px * cs, kMax, 32);
+  if (g.Bz > c->nx) g.Bz = c->nx;
+  if (g.By > c->nx) g.By = c->nx;
+  if (g.Bk > g.Py) g.Bk = g.Py;
+  InitGeom& ig = c->igeom;
+  ig.nx = c->nx; ig.ny = c->ny; ig.nz = c->nz;
+  ig.Px = g.Px; ig.Py = g.Py; ig.Pz = g.Pz; ig.Kz = g.Kz;
+  ig.ox = c->nx == 1 ? 1 : c->nx + 1;
+  ig.oy = c->ny == 1 ? 1 : c->ny + 1;
+  ig.oz = c->nz == 1 ? 1 : c->nz + 1;
+  ig.Bk = g.Bk;
+  // persistent
+  size_t o = 0;
+  c->off_table = o; o += align256((size_t)g.Kz * g.Py * g.Px * 6 * c->es);
+  c->off_wx = o; o += align256((size_t)g.Px * cs);
+  c->off_wy = o; o += align256((size_t)g.Py * cs);
+  c->off_wz = o; o += align256((size_t)g.Pz * cs);
+  c->off_posz = o; o += align256((size_t)g.Pz * 2);
+  c->off_fx = o; o += align256((size_t)g.Px * 2);
+  c->off_fy = o; o += align256((size_t)g.Py * 2);
+  c->off_posx = o; o += align256((size_t)g.Px * 2);
+  c->off_posy = o; o += align256((size_t)g.Py * 2);
+  c->pers_need = o;
+  // scratch
+  const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
+  o = 0;
+  c->off_a1 = o; o += align256((size_t)3 * g.Kz * g.ny * g.nx * cs);
+  c->off_a2 = o; o += align256((size_t)3 * g.Kz * g.Py * g.nx * cs);
+  const size_t spectra = o;
+  c->off_hd = o; o += align256(n3);
+  c->off_msa = o; o += align256(n3);
+  c->off_msb = o; o += align256(n3);
+  c->off_acc = o; o += align256(n3);
+  c->off_sin = o; o += align256(n3);
+  c->off_sout = o; o += align256(n3);
+  (void)spectra;
+  const size_t init_need = demag_init_scratch_bytes(ig);  // aliases the start of scratch
+  c->scr_need = o > init_need ? o : init_need;
+}
+
+extern "C" {
+
+mm_status mm_ctx_create(int nx, int ny, int nz, double dx, double dy, double dz, mm_dtype dtype,
+                        mm_ctx** out) {
+  if (!out) return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: out is NULL");
+  *out = nullptr;
+  if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0))
+    return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: sizes and cell lengths must be positive");
+  if (dtype != MM_F32 && dtype != MM_F64)
+    return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: unknown dtype %d", (int)dtype);
+  if (!pow2(nx) || !pow2(ny) || !pow2(nz) || nx > 1024 || ny > 1024 || nz > 512)
+    return fail(nullptr, MM_ERR_UNSUPPORTED_SIZE,
+                "mm_ctx_create: %dx%dx%d unsupported (each n must be 1 or a power of two, "
+                "nx,ny <= 1024, nz <= 512)", nx, ny, nz);
+  mm_ctx* c = new (std::nothrow) mm_ctx();
+  if (!c) return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: out of host memory");
+  c->nx = nx; c->ny = ny; c->nz = nz;
+  c->dx = dx; c->dy = dy; c->dz = dz;
+  c->dtype = dtype;
+  c->es = dtype == MM_F32 ? 4 : 8;
+  plan_layout(c);
+  *out = c;
+  return MM_OK;
+}
+
+mm_status mm_ctx_destroy(mm_ctx* ctx) {
+  delete ctx;
+  return MM_OK;
+}
+
+mm_status mm_ctx_set_stream(mm_ctx* ctx, void* cuda_stream) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+  return MM_OK;
+}
+
+mm_status mm_ctx_set_tiles(mm_ctx* ctx, int bz, int by, int bk) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (ctx->demag_ready) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: call before mm_demag_init");
+  const int v[3] = {bz, by, bk};
+  for (int i = 0; i < 3; ++i)
+    if (v[i] < 0 || (v[i] > 0 && !pow2(v[i])) || v[i] > 64)
+      return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: tile widths must be 0 or a power of two <= 64");
+  ctx->want_bz = bz; ctx->want_by = by; ctx->want_bk = bk;
+  plan_layout(ctx);
+  const size_t cs = 2 * ctx->es;
+  const DemagGeom& g = ctx->geom;
+  const size_t lim = 227 * 1024;
+  if ((size_t)3 * g.Pz * g.Bz * cs > lim || (size_t)g.Py * g.By * cs > lim ||
+      (size_t)3 * g.Px * g.Bk * cs > lim) {
+    ctx->want_bz = ctx->want_by = ctx->want_bk = 0;
+    plan_layout(ctx);
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: tile exceeds 227 KB of shared memory");
+  }
+  return MM_OK;
+}
+
+mm_status mm_ctx_workspace_bytes(const mm_ctx* ctx, size_t* persistent, size_t* scratch) {
+  if (!ctx || !persistent || !scratch) return MM_ERR_INVALID_ARG;
+  *persistent = ctx->pers_need;
+  *scratch = ctx->scr_need;
+  return MM_OK;
+}
+
+mm_status mm_ctx_set_workspace(mm_ctx* ctx, void* persistent, size_t pbytes, void* scratch,
+                               size_t sbytes) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!persistent || !scratch || ((uintptr_t)persistent & 255) || ((uintptr_t)scratch & 255))
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_workspace: NULL or not 256-byte aligned");
+  if (pbytes < ctx->pers_need || sbytes < ctx->scr_need)
+    return fail(ctx, MM_ERR_WORKSPACE, "mm_ctx_set_workspace: need %zu + %zu bytes, got %zu + %zu",
+                ctx->pers_need, ctx->scr_need, pbytes, sbytes);
+  ctx->pers = static_cast<unsigned char*>(persistent);
+  ctx->scr = static_cast<unsigned char*>(scratch);
+  ctx->pers_bytes = pbytes;
+  ctx->scr_bytes = sbytes;
+  ctx->demag_ready = false;
+  return MM_OK;
+}
+
+mm_status mm_set_material(mm_ctx* ctx, double Ms, double Aex, double Ku, const double axis[3],
+                          double alpha, double gamma) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!(Ms > 0) || Aex < 0 || alpha < 0 || !(gamma > 0))
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_material: need Ms > 0, Aex >= 0, alpha >= 0, gamma > 0");
+  double u[3] = {0, 0, 1};
+  if (Ku != 0.0) {
+    if (!axis) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_material: Ku != 0 needs an axis");
+    const double n = std::sqrt(axis[0] * axis[0] + axis[1] * axis[1] + axis[2] * axis[2]);
+    if (!(n > 0)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_material: zero anisotropy axis");
+    for (int i = 0; i < 3; ++i) u[i] = axis[i] / n;
+  }
+  ctx->Ms = Ms; ctx->Aex = Aex; ctx->Ku = Ku;
+  for (int i = 0; i < 3; ++i) ctx->axis[i] = u[i];
+  ctx->alpha = alpha; ctx->gamma = gamma;
+  ctx->have_material = true;
+  return MM_OK;
+}
+
+mm_status mm_set_zeeman(mm_ctx* ctx, const double Hext[3]) {
+  if (!ctx || !Hext) return MM_ERR_INVALID_ARG;
+  for (int i = 0; i < 3; ++i) ctx->Hext[i] = Hext[i];
+  return MM_OK;
+}
+
+mm_status mm_set_terms(mm_ctx* ctx, unsigned term_mask) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (term_mask & ~15u) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_terms: unknown term bits 0x%x", term_mask);
+  ctx->terms = term_mask;
+  return MM_OK;
+}
+
+mm_status mm_ctx_launch_count(const mm_ctx* ctx, unsigned long long* count) {
+  if (!ctx || !count) return MM_ERR_INVALID_ARG;
+  *count = ctx->launches;
+  return MM_OK;
+}
+
+const char* mm_last_error(const mm_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ internals
+
+static mm_status cuda_fail(mm_ctx* c, const char* what, cudaError_t e) {
+  return fail(c, MM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+template <typename T> static void fill_twiddles(std::vector<unsigned char>& buf, size_t off, int P) {
+  Cx<T>* w = reinterpret_cast<Cx<T>*>(buf.data() + off);
+  for (int q = 0; q < P; ++q) {
+    // exact octant reduction through the integer phase keeps the table symmetric
+    const long double ph = -2.0L * 3.14159265358979323846264338327950288L * (long double)q / (long double)P;
+    w[q] = mk<T>((T)cosl(ph), (T)sinl(ph));
+  }
+}
+
+template <typename T> static mm_status demag_init_t(mm_ctx* c) {
+  const DemagGeom& g = c->geom;
+  // small tables: twiddles and digit-reversal maps, built on the host, uploaded once
+  const size_t small_off = c->off_wx, small_bytes = c->pers_need - c->off_wx;
+  std::vector<unsigned char> host(small_bytes, 0);
+  fill_twiddles<T>(host, c->off_wx - small_off, g.Px);
+  fill_twiddles<T>(host, c->off_wy - small_off, g.Py);
+  fill_twiddles<T>(host, c->off_wz - small_off, g.Pz);
+  auto u16 = [&](size_t off) { return reinterpret_cast<uint16_t*>(host.data() + (off - small_off)); };
+  for (int k = 0; k < g.Pz; ++k) u16(c->off_posz)[k] = (uint16_t)pos_of_freq(g.pz, k);
+  for (int k = 0; k < g.Px; ++k) {
+    const int p = pos_of_freq(g.px, k);
+    u16(c->off_posx)[k] = (uint16_t)p;
+    u16(c->off_fx)[p] = (uint16_t)k;
+  }
+  for (int k = 0; k < g.Py; ++k) {
+    const int p = pos_of_freq(g.py, k);
+    u16(c->off_posy)[k] = (uint16_t)p;
+    u16(c->off_fy)[p] = (uint16_t)k;
+  }
+  cudaError_t e = cudaMemcpyAsync(c->pers + small_off, host.data(), small_bytes,
+                                  cudaMemcpyHostToDevice, c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: table upload", e);
+  e = demag_init_launch<T>(c->igeom, c->dx, c->dy, c->dz, c->scr,
+                           reinterpret_cast<const uint16_t*>(c->pers + c->off_fx),
+                           reinterpret_cast<const uint16_t*>(c->pers + c->off_fy),
+                           reinterpret_cast<T*>(c->pers + c->off_table), c->stream, &c->launches);
+  if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: launch", e);
+  e = cudaStreamSynchronize(c->stream);  // also keeps `host` alive until the copy is done
+  if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: execution", e);
+  c->demag_ready = true;
+  return MM_OK;
+}
+
+template <typename T> static DemagBufs<T> bufs_of(mm_ctx* c) {
+  DemagBufs<T> b;
+  b.Wx = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wx);
+  b.Wy = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wy);
+  b.Wz = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wz);
+  b.posz = reinterpret_cast<const uint16_t*>(c->pers + c->off_posz);
+  b.table = reinterpret_cast<const T*>(c->pers + c->off_table);
+  b.A1 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a1);
+  b.A2 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a2);
+  return b;
+}
+
+template <typename T> static PwParams<T> pw_of(const mm_ctx* c, unsigned terms) {
+  PwParams<T> p{};
+  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+  p.terms = terms;
+  const double pe = 2.0 * c->Aex / (kMu0 * c->Ms);
+  p.ex[0] = (T)(pe / (c->dx * c->dx));
+  p.ex[1] = (T)(pe / (c->dy * c->dy));
+  p.ex[2] = (T)(pe / (c->dz * c->dz));
+  p.kan = (T)(2.0 * c->Ku / (kMu0 * c->Ms));
+  for (int i = 0; i < 3; ++i) { p.u[i] = (T)c->axis[i]; p.hext[i] = (T)c->Hext[i]; }
+  p.pref = (T)(-c->gamma / (1.0 + c->alpha * c->alpha));
+  p.alpha = (T)c->alpha;
+  p.first = 0; p.wk = (T)1; p.a = (T)0;
+  return p;
+}
+
+static mm_status check_ptr(mm_ctx* c, const char* fn, const void* a, const void* b) {
+  if (!a || !b || ((uintptr_t)a & 15) || ((uintptr_t)b & 15))
+    return fail(c, MM_ERR_INVALID_ARG, "%s: NULL or not 16-byte aligned device pointer", fn);
+  return MM_OK;
+}
+
+static mm_status need_ready(mm_ctx* c, const char* fn, bool demag) {
+  if (!c->have_material) return fail(c, MM_ERR_NOT_INITIALISED, "%s: mm_set_material not called", fn);
+  if (!c->scr || !c->pers) return fail(c, MM_ERR_NOT_INITIALISED, "%s: mm_ctx_set_workspace not called", fn);
+  if (demag && !c->demag_ready) return fail(c, MM_ERR_NOT_INITIALISED, "%s: mm_demag_init not called", fn);
+  return MM_OK;
+}
+
+template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H) {
+  cudaError_t e = demag_field_launch<T>(c->geom, bufs_of<T>(c), static_cast<const T*>(m),
+                                        static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches);
+  return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag launch", e);
+}
+
+// H_eff-type evaluations: optional demag into scratch, then the fused pointwise pass.
+template <typename T>
+static mm_status eval_t(mm_ctx* c, int mode, const void* m, void* out, void* m0, const PwParams<T>& p) {
+  T* Hd = reinterpret_cast<T*>(c->scr + c->off_hd);
+  if (mode != PW_EXCHANGE && (p.terms & MM_TERM_DEMAG)) {
+    mm_status s = demag_t<T>(c, m, Hd);
+    if (s != MM_OK) return s;
+  }
+  cudaError_t e = pointwise_launch<T>(mode, p, static_cast<const T*>(m), Hd, static_cast<T*>(out),
+                                      static_cast<T*>(m0), reinterpret_cast<T*>(c->scr + c->off_acc),
+                                      c->stream, &c->launches);
+  return e == cudaSuccess ? MM_OK : cuda_fail(c, "pointwise launch", e);
+}
+
+template <typename T> static mm_status rk_t(mm_ctx* c, void* m, double dt) {
+  T* msa = reinterpret_cast<T*>(c->scr + c->off_msa);
+  T* msb = reinterpret_cast<T*>(c->scr + c->off_msb);
+  PwParams<T> p = pw_of<T>(c, c->terms);
+  mm_status s;
+  p.first = 1; p.wk = (T)1; p.a = (T)(0.5 * dt);
+  if ((s = eval_t<T>(c, PW_RK_STAGE, m, msa, m, p)) != MM_OK) return s;
+  p.first = 0; p.wk = (T)2; p.a = (T)(0.5 * dt);
+  if ((s = eval_t<T>(c, PW_RK_STAGE, msa, msb, m, p)) != MM_OK) return s;
+  p.wk = (T)2; p.a = (T)dt;
+  if ((s = eval_t<T>(c, PW_RK_STAGE, msb, msa, m, p)) != MM_OK) return s;
+  p.a = (T)(dt / 6.0);
+  return eval_t<T>(c, PW_RK_FINAL, msa, nullptr, m, p);
+}
+
+static mm_status dispatch_eval(mm_ctx* c, int mode, unsigned terms, const void* m, void* out) {
+  if (c->dtype == MM_F32) return eval_t<float>(c, mode, m, out, nullptr, pw_of<float>(c, terms));
+  return eval_t<double>(c, mode, m, out, nullptr, pw_of<double>(c, terms));
+}
+
+extern "C" {
+
+mm_status mm_demag_init(mm_ctx* ctx) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!ctx->scr || !ctx->pers)
+    return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_demag_init: mm_ctx_set_workspace not called");
+  if (ctx->demag_ready) return MM_OK;
+  return ctx->dtype == MM_F32 ? demag_init_t<float>(ctx) : demag_init_t<double>(ctx);
+}
+
+mm_status mm_demag_nhat_export(mm_ctx* ctx, void* out) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!ctx->demag_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_demag_nhat_export: mm_demag_init not called");
+  if (!out || ((uintptr_t)out & 15)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_demag_nhat_export: bad pointer");
+  const uint16_t* posx = reinterpret_cast<const uint16_t*>(ctx->pers + ctx->off_posx);
+  const uint16_t* posy = reinterpret_cast<const uint16_t*>(ctx->pers + ctx->off_posy);
+  cudaError_t e;
+  if (ctx->dtype == MM_F32)
+    e = demag_export_launch<float>(ctx->igeom, reinterpret_cast<const float*>(ctx->pers + ctx->off_table),
+                                   posx, posy, static_cast<float*>(out), ctx->stream, &ctx->launches);
+  else
+    e = demag_export_launch<double>(ctx->igeom, reinterpret_cast<const double*>(ctx->pers + ctx->off_table),
+                                    posx, posy, static_cast<double*>(out), ctx->stream, &ctx->launches);
+  return e == cudaSuccess ? MM_OK : cuda_fail(ctx, "mm_demag_nhat_export", e);
+}
+
+mm_status mm_demag_field(mm_ctx* ctx, const void* m, void* H) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_demag_field", m, H)) != MM_OK) return s;
+  if (m == H) return fail(ctx, MM_ERR_INVALID_ARG, "mm_demag_field: H must not alias m");
+  if ((s = need_ready(ctx, "mm_demag_field", true)) != MM_OK) return s;
+  return ctx->dtype == MM_F32 ? demag_t<float>(ctx, m, H) : demag_t<double>(ctx, m, H);
+}
+
+mm_status mm_exchange_field(mm_ctx* ctx, const void* m, void* H) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_exchange_field", m, H)) != MM_OK) return s;
+  if (m == H) return fail(ctx, MM_ERR_INVALID_ARG, "mm_exchange_field: H must not alias m");
+  if (!ctx->have_material) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_exchange_field: mm_set_material not called");
+  return dispatch_eval(ctx, PW_EXCHANGE, MM_TERM_EXCHANGE, m, H);
+}
+
+mm_status mm_heff(mm_ctx* ctx, const void* m, void* H) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_heff", m, H)) != MM_OK) return s;
+  if (m == H) return fail(ctx, MM_ERR_INVALID_ARG, "mm_heff: H must not alias m");
+  if ((s = need_ready(ctx, "mm_heff", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
+  return dispatch_eval(ctx, PW_HEFF, ctx->terms, m, H);
+}
+
+mm_status mm_llg_rhs(mm_ctx* ctx, const void* m, void* dmdt) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_llg_rhs", m, dmdt)) != MM_OK) return s;
+  if (m == dmdt) return fail(ctx, MM_ERR_INVALID_ARG, "mm_llg_rhs: dmdt must not alias m");
+  if ((s = need_ready(ctx, "mm_llg_rhs", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
+  return dispatch_eval(ctx, PW_RHS, ctx->terms, m, dmdt);
+}
+
+mm_status mm_rk_step(mm_ctx* ctx, void* m_inout, double dt) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_rk_step", m_inout, m_inout)) != MM_OK) return s;
+  if (!(dt > 0)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_rk_step: dt must be positive");
+  if ((s = need_ready(ctx, "mm_rk_step", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
+  return ctx->dtype == MM_F32 ? rk_t<float>(ctx, m_inout, dt) : rk_t<double>(ctx, m_inout, dt);
+}
+
+// ---- host-buffer variants: H2D, device path, D2H, synchronise
+
+static mm_status host_call(mm_ctx* ctx, const char* fn, int which, const void* in_host, void* out_host,
+                           double dt) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!in_host || !out_host) return fail(ctx, MM_ERR_INVALID_ARG, "%s: NULL host pointer", fn);
+  if (!ctx->scr) return fail(ctx, MM_ERR_NOT_INITIALISED, "%s: mm_ctx_set_workspace not called", fn);
+  const size_t n3 = (size_t)ctx->nx * ctx->ny * ctx->nz * 3 * ctx->es;
+  void* din = ctx->scr + ctx->off_sin;
+  void* dout = ctx->scr + ctx->off_sout;
+  cudaError_t e = cudaMemcpyAsync(din, in_host, n3, cudaMemcpyHostToDevice, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, fn, e);
+  mm_status s;
+  switch (which) {
+    case 0: s = mm_demag_field(ctx, din, dout); break;
+    case 1: s = mm_heff(ctx, din, dout); break;
+    case 2: s = mm_llg_rhs(ctx, din, dout); break;
+    default: s = mm_rk_step(ctx, din, dt); dout = din; break;
+  }
+  if (s != MM_OK) return s;
+  e = cudaMemcpyAsync(out_host, dout, n3, cudaMemcpyDeviceToHost, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, fn, e);
+  e = cudaStreamSynchronize(ctx->stream);
+  return e == cudaSuccess ? MM_OK : cuda_fail(ctx, fn, e);
+}
+
+mm_status mm_demag_field_host(mm_ctx* ctx, const void* m_host, void* H_host) {
+  return host_call(ctx, "mm_demag_field_host", 0, m_host, H_host, 0);
+}
+mm_status mm_heff_host(mm_ctx* ctx, const void* m_host, void* H_host) {
+  return host_call(ctx, "mm_heff_host", 1, m_host, H_host, 0);
+}
+mm_status mm_llg_rhs_host(mm_ctx* ctx, const void* m_host, void* dmdt_host) {
+  return host_call(ctx, "mm_llg_rhs_host", 2, m_host, dmdt_host, 0);
+}
+mm_status mm_rk_step_host(mm_ctx* ctx, void* m_inout_host, double dt) {
+  return host_call(ctx, "mm_rk_step_host", 3, m_inout_host, m_inout_host, dt);
+}
+
+}  // extern "C"

@@ -1,0 +1,39 @@
+// Shared device helpers of the CUDA path: complex arithmetic on float2/double2, plan
+// descriptors.  (No code is shared with oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mm {
+
+template <typename T> struct cx_of;
+template <> struct cx_of<float> { using type = float2; };
+template <> struct cx_of<double> { using type = double2; };
+template <typename T> using Cx = typename cx_of<T>::type;
+
+template <typename T> __host__ __device__ __forceinline__ Cx<T> mk(T a, T b) {
+  Cx<T> r; r.x = a; r.y = b; return r;
+}
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { a.x += b.x; a.y += b.y; return a; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
+// a * b
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
+  C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+// a * conj(b)
+template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {
+  C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r;
+}
+template <typename C> __device__ __forceinline__ C cconj(C a) { a.y = -a.y; return a; }
+
+constexpr int MM_MAX_STAGES = 6;
+
+// Radix plan of one in-place power-of-two transform of length L: L = prod radix[i].
+struct FftPlan {
+  int L;        // sub-transform length (n_d); the padded length is P = 2L (or 1)
+  int P;
+  int nstages;
+  int radix[MM_MAX_STAGES];
+};
+
+}  // namespace mm

@@ -1,0 +1,260 @@
+// S6/S7: one pass over the mesh computes the 6-point exchange stencil
+// (eq. 2, Neumann boundary), uniaxial anisotropy, Zeeman
+// (PAPER.md:140-143), adds H_demag, forms the LLG right-hand side (eq. 1) and
+// applies the RK4 stage arithmetic, so H_eff and k_i are never written to HBM.
+// HBM-bound: 128-bit loads/stores, 4 consecutive z cells (12 reals) per thread; the six
+// neighbours come from L1/L2.
+#include "pointwise.cuh"
+
+#include "../../include/mm_b200.h"
+
+namespace mm {
+
+template <typename T> struct V12;  // 12 consecutive reals, 16-byte aligned
+template <> struct V12<float> {
+  static __device__ __forceinline__ void ld(const float* p, float (&v)[12]) {
+    const float4* q = reinterpret_cast<const float4*>(p);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const float4 t = q[i];
+      v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
+    }
+  }
+  static __device__ __forceinline__ void st(float* p, const float (&v)[12]) {
+    float4* q = reinterpret_cast<float4*>(p);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) q[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+  }
+};
+template <> struct V12<double> {
+  static __device__ __forceinline__ void ld(const double* p, double (&v)[12]) {
+    const double2* q = reinterpret_cast<const double2*>(p);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      const double2 t = q[i];
+      v[2 * i] = t.x; v[2 * i + 1] = t.y;
+    }
+  }
+  static __device__ __forceinline__ void st(double* p, const double (&v)[12]) {
+    double2* q = reinterpret_cast<double2*>(p);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) q[i] = make_double2(v[2 * i], v[2 * i + 1]);
+  }
+};
+
+// Everything that happens in one cell once its neighbours are known.
+// mc: m at the cell; lap: exchange field already summed; hd: demag field (or 0);
+// m0v / accv: RK4 step-start state and running sum (only read in RK modes).
+// Returns through o[3] the value to store in `out` (or m0 for PW_RK_FINAL); accv is updated.
+template <typename T, int MODE>
+__device__ __forceinline__ void cell_update(const PwParams<T>& p, const T* mc, const T* lap,
+                                            const T* hd, const T* m0v, T* accv, T* o) {
+  T h[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) h[c] = (p.terms & MM_TERM_EXCHANGE) ? lap[c] : (T)0;
+  if (MODE == PW_EXCHANGE) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) o[c] = lap[c];
+    return;
+  }
+  if (p.terms & MM_TERM_DEMAG) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) h[c] += hd[c];
+  }
+  if (p.terms & MM_TERM_ANISOTROPY) {
+    const T d = p.kan * (mc[0] * p.u[0] + mc[1] * p.u[1] + mc[2] * p.u[2]);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) h[c] += d * p.u[c];
+  }
+  if (p.terms & MM_TERM_ZEEMAN) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) h[c] += p.hext[c];
+  }
+  if (MODE == PW_HEFF) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) o[c] = h[c];
+    return;
+  }
+  // m x H, then m x (m x H) as a genuine double cross product (keeps m . dm/dt = 0)
+  const T t0 = mc[1] * h[2] - mc[2] * h[1];
+  const T t1 = mc[2] * h[0] - mc[0] * h[2];
+  const T t2 = mc[0] * h[1] - mc[1] * h[0];
+  const T d0 = mc[1] * t2 - mc[2] * t1;
+  const T d1 = mc[2] * t0 - mc[0] * t2;
+  const T d2 = mc[0] * t1 - mc[1] * t0;
+  T k[3] = {p.pref * (t0 + p.alpha * d0), p.pref * (t1 + p.alpha * d1),
+            p.pref * (t2 + p.alpha * d2)};
+  if (MODE == PW_RHS) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) o[c] = k[c];
+  } else if (MODE == PW_RK_STAGE) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      accv[c] = p.first ? k[c] : accv[c] + p.wk * k[c];
+      o[c] = m0v[c] + p.a * k[c];
+    }
+  } else {  // PW_RK_FINAL
+    T v[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) v[c] = m0v[c] + p.a * (accv[c] + k[c]);
+    const T inv = (T)1 / sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) o[c] = v[c] * inv;
+  }
+}
+
+// Vector path: nz % 4 == 0.  Thread = 4 consecutive z cells of one (x, y) line.
+template <typename T, int MODE>
+__global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __restrict__ m,
+                                                     const T* __restrict__ Hd, T* __restrict__ out,
+                                                     T* __restrict__ m0, T* __restrict__ acc) {
+  const int nzq = p.nz >> 2;
+  const size_t total = (size_t)p.nx * p.ny * nzq;
+  const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= total) return;
+  const int zq = (int)(g % nzq);
+  const int y = (int)((g / nzq) % p.ny);
+  const int x = (int)(g / ((size_t)nzq * p.ny));
+  const size_t sy = (size_t)p.nz * 3, sx = sy * p.ny;
+  const size_t base = (size_t)x * sx + (size_t)y * sy + (size_t)zq * 12;
+  const bool need_lap = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE;
+
+  T mc[12], lap[12];
+  V12<T>::ld(m + base, mc);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) lap[i] = 0;
+  if (need_lap) {
+    T nb[12];
+    if (p.nx > 1) {
+      V12<T>::ld(m + (x > 0 ? base - sx : base), nb);
+#pragma unroll
+      for (int i = 0; i < 12; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
+      V12<T>::ld(m + (x + 1 < p.nx ? base + sx : base), nb);
+#pragma unroll
+      for (int i = 0; i < 12; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
+    }
+    if (p.ny > 1) {
+      V12<T>::ld(m + (y > 0 ? base - sy : base), nb);
+#pragma unroll
+      for (int i = 0; i < 12; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
+      V12<T>::ld(m + (y + 1 < p.ny ? base + sy : base), nb);
+#pragma unroll
+      for (int i = 0; i < 12; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
+    }
+    {
+      T lo[3], hi[3];
+      const bool has_lo = zq > 0, has_hi = zq + 1 < nzq;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        lo[c] = has_lo ? m[base - 3 + c] : mc[c];
+        hi[c] = has_hi ? m[base + 12 + c] : mc[9 + c];
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const T below = j == 0 ? lo[c] : mc[3 * (j - 1) + c];
+          const T above = j == 3 ? hi[c] : mc[3 * (j + 1) + c];
+          lap[3 * j + c] += p.ex[2] * ((below - mc[3 * j + c]) + (above - mc[3 * j + c]));
+        }
+    }
+  }
+  T hd[12], m0v[12], accv[12], o[12];
+#pragma unroll
+  for (int i = 0; i < 12; ++i) hd[i] = m0v[i] = accv[i] = 0;
+  if (MODE != PW_EXCHANGE && (p.terms & MM_TERM_DEMAG)) V12<T>::ld(Hd + base, hd);
+  if (MODE == PW_RK_STAGE || MODE == PW_RK_FINAL) {
+    V12<T>::ld(m0 + base, m0v);
+    if (!(MODE == PW_RK_STAGE && p.first)) V12<T>::ld(acc + base, accv);
+  }
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+    cell_update<T, MODE>(p, mc + 3 * j, lap + 3 * j, hd + 3 * j, m0v + 3 * j, accv + 3 * j,
+                         o + 3 * j);
+  if (MODE == PW_RK_STAGE) V12<T>::st(acc + base, accv);
+  V12<T>::st((MODE == PW_RK_FINAL ? m0 : out) + base, o);
+}
+
+// Scalar path for nz in {1, 2} (thin films): thread = one cell.
+template <typename T, int MODE>
+__global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __restrict__ m,
+                                                      const T* __restrict__ Hd, T* __restrict__ out,
+                                                      T* __restrict__ m0, T* __restrict__ acc) {
+  const size_t total = (size_t)p.nx * p.ny * p.nz;
+  const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= total) return;
+  const int z = (int)(g % p.nz);
+  const int y = (int)((g / p.nz) % p.ny);
+  const int x = (int)(g / ((size_t)p.nz * p.ny));
+  const size_t sy = (size_t)p.nz * 3, sx = sy * p.ny;
+  const size_t base = g * 3;
+  const bool need_lap = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE;
+  T mc[3], lap[3] = {0, 0, 0};
+#pragma unroll
+  for (int c = 0; c < 3; ++c) mc[c] = m[base + c];
+  if (need_lap) {
+    const size_t off[3] = {sx, sy, 3};
+    const int idx[3] = {x, y, z}, n[3] = {p.nx, p.ny, p.nz};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const size_t lo = idx[d] > 0 ? base - off[d] : base;
+      const size_t hi = idx[d] + 1 < n[d] ? base + off[d] : base;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) lap[c] += p.ex[d] * ((m[lo + c] - mc[c]) + (m[hi + c] - mc[c]));
+    }
+  }
+  T hd[3] = {0, 0, 0}, m0v[3] = {0, 0, 0}, accv[3] = {0, 0, 0}, o[3];
+  if (MODE != PW_EXCHANGE && (p.terms & MM_TERM_DEMAG)) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) hd[c] = Hd[base + c];
+  }
+  if (MODE == PW_RK_STAGE || MODE == PW_RK_FINAL) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      m0v[c] = m0[base + c];
+      if (!(MODE == PW_RK_STAGE && p.first)) accv[c] = acc[base + c];
+    }
+  }
+  cell_update<T, MODE>(p, mc, lap, hd, m0v, accv, o);
+  T* dst = MODE == PW_RK_FINAL ? m0 : out;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    if (MODE == PW_RK_STAGE) acc[base + c] = accv[c];
+    dst[base + c] = o[c];
+  }
+}
+
+template <typename T, int MODE>
+static void launch_mode(const PwParams<T>& p, const T* m, const T* Hd, T* out, T* m0, T* acc,
+                        cudaStream_t st) {
+  if (p.nz % 4 == 0) {
+    const size_t total = (size_t)p.nx * p.ny * (p.nz / 4);
+    pw_vec_kernel<T, MODE><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
+  } else {
+    const size_t total = (size_t)p.nx * p.ny * p.nz;
+    pw_cell_kernel<T, MODE><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
+  }
+}
+
+template <typename T>
+cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T* Hd, T* out,
+                             T* m0, T* acc, cudaStream_t st, unsigned long long* launches) {
+  switch (mode) {
+    case PW_EXCHANGE: launch_mode<T, PW_EXCHANGE>(p, m, Hd, out, m0, acc, st); break;
+    case PW_HEFF: launch_mode<T, PW_HEFF>(p, m, Hd, out, m0, acc, st); break;
+    case PW_RHS: launch_mode<T, PW_RHS>(p, m, Hd, out, m0, acc, st); break;
+    case PW_RK_STAGE: launch_mode<T, PW_RK_STAGE>(p, m, Hd, out, m0, acc, st); break;
+    default: launch_mode<T, PW_RK_FINAL>(p, m, Hd, out, m0, acc, st); break;
+  }
+  ++*launches;
+  return cudaGetLastError();
+}
+
+template cudaError_t pointwise_launch<float>(int, const PwParams<float>&, const float*,
+                                             const float*, float*, float*, float*, cudaStream_t,
+                                             unsigned long long*);
+template cudaError_t pointwise_launch<double>(int, const PwParams<double>&, const double*,
+                                              const double*, double*, double*, double*,
+                                              cudaStream_t, unsigned long long*);
+
+}  // namespace mm

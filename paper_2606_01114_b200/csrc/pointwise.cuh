@@ -1,0 +1,32 @@
+// S6/S7: fused local field terms + LLG right-hand side + RK4 stage arithmetic.
+#pragma once
+#include "mm_common.cuh"
+
+namespace mm {
+
+enum PwMode {
+  PW_EXCHANGE = 0,  // out := H_exchange(m)
+  PW_HEFF = 1,      // out := sum of enabled terms (Hd added when the demag term is on)
+  PW_RHS = 2,       // out := LLG right-hand side at H_eff
+  PW_RK_STAGE = 3,  // k := RHS; acc := (first ? k : acc + wk k); out := m0 + a k
+  PW_RK_FINAL = 4   // k := RHS; m0 := normalise(m0 + b (acc + k))
+};
+
+template <typename T> struct PwParams {
+  int nx, ny, nz;
+  unsigned terms;     // MM_TERM_* mask actually applied
+  T ex[3];            // 2A/(mu0 Ms) / d_d^2
+  T kan, u[3];        // 2Ku/(mu0 Ms), unit axis
+  T hext[3];          // A/m
+  T pref, alpha;      // -gamma/(1+alpha^2), alpha
+  // RK4 bookkeeping
+  int first;          // stage 1: acc is written, not accumulated
+  T wk;               // weight of k in acc (1 or 2)
+  T a;                // stage step a_i * dt  (PW_RK_STAGE)  /  dt/6 (PW_RK_FINAL)
+};
+
+template <typename T>
+cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T* Hd, T* out,
+                             T* m0, T* acc, cudaStream_t st, unsigned long long* launches);
+
+}  // namespace mm

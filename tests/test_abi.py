@@ -1,0 +1,62 @@
+"""The C-ABI library loads and exports every symbol include/mm_b200.h declares; host-only
+argument validation (no kernel is launched, no GPU needed)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_01114_b200 import build, load_library
+    build.build()
+    return load_library()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "mm_b200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mm_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    syms = declared_symbols()
+    assert len(syms) >= 20 and "mm_rk_step" in syms and "mm_demag_field" in syms
+    for s in syms:
+        assert hasattr(lib, s), s
+
+
+def test_create_validates_arguments(lib):
+    h = C.c_void_p()
+    assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 0
+    p, s = C.c_size_t(), C.c_size_t()
+    assert lib.mm_ctx_workspace_bytes(h, C.byref(p), C.byref(s)) == 0
+    assert p.value > 0 and s.value > 0
+    # not initialised: no workspace yet
+    assert lib.mm_demag_init(h) == 3
+    assert b"workspace" in lib.mm_last_error(h)
+    assert lib.mm_set_terms(h, 64) == 1
+    assert lib.mm_ctx_destroy(h) == 0
+    assert lib.mm_ctx_create(12, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 2     # not a power of two
+    assert b"power of two" in lib.mm_last_error(None)
+    assert lib.mm_ctx_create(2048, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 2   # above the plan
+    assert lib.mm_ctx_create(16, 16, 2, 0.0, 5e-9, 3e-9, 1, C.byref(h)) == 1
+    assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 7, C.byref(h)) == 1
+    assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 0, None) == 1
+
+
+def test_workspace_sizes_match_design(lib):
+    """Config 4 fp32: table 6*129*1024*1024*4 B, spectra 3*129*(512+1024)*512*8 B."""
+    h = C.c_void_p()
+    assert lib.mm_ctx_create(512, 512, 128, 4e-9, 4e-9, 4e-9, 0, C.byref(h)) == 0
+    p, s = C.c_size_t(), C.c_size_t()
+    lib.mm_ctx_workspace_bytes(h, C.byref(p), C.byref(s))
+    table = 6 * 129 * 1024 * 1024 * 4
+    spectra = 3 * 129 * (512 + 1024) * 512 * 8
+    fields = 6 * 512 * 512 * 128 * 3 * 4
+    assert table <= p.value < table + (1 << 20)
+    assert spectra + fields <= s.value < spectra + fields + (1 << 20)
+    lib.mm_ctx_destroy(h)

@@ -1,0 +1,176 @@
+"""CUDA path vs CPU oracle, element by element, on the same seeded inputs, through the C ABI.
+Tolerances are BASELINE.json north_star's: rel-L2 per component (relative to max|H|) <= 1e-12
+(fp64) / 2e-5 (fp32); RK4 trajectories within 1e-10 / 1e-4 in m."""
+import numpy as np
+import pytest
+import torch
+
+import workloads as w
+from gpu_util import TOL, TRAJ_TOL, make_ctx, make_problem, round_input, to_dev
+
+pytestmark = pytest.mark.gpu
+
+SMALL = [((16, 16, 2), (5e-9, 5e-9, 3e-9)), ((8, 4, 1), (3e-9, 4e-9, 5e-9)),
+         ((4, 1, 8), (2e-9, 2e-9, 1e-9)), ((1, 1, 4), (1e-9, 2e-9, 3e-9)),
+         ((1, 1, 1), (1e-9, 2e-9, 3e-9)), ((2, 2, 2), (1e-9, 1e-9, 1e-9)),
+         ((1, 8, 1), (1e-9, 2e-9, 3e-9)), ((32, 16, 8), (4e-9, 3e-9, 2e-9)),
+         ((128, 32, 1), (3.90625e-9, 3.90625e-9, 3e-9))]
+
+
+def cfg_for(n, d, **kw):
+    base = w.get_config(1)
+    return w.Config(**{**base.__dict__, "n": n, "d": d, "name": "t", **kw})
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n,d", SMALL)
+def test_nhat_matches_oracle(oracle, n, d, dt):
+    """S0: the exported Fourier-space tensor equals the real part of the oracle's FFT of the
+    mirrored table on the octant kx<=nx, ky<=ny, kz<=nz."""
+    cfg = cfg_for(n, d)
+    ctx = make_ctx(cfg, dt)
+    got = ctx.nhat_export().cpu().numpy().astype(np.float64)
+    Nhat = oracle.demag_fft_nhat(oracle.newell_octant(n, d))
+    o = tuple(1 if v == 1 else v + 1 for v in n)
+    ref = Nhat[:, :o[0], :o[1], :o[2]]
+    tol = 5e-14 if dt == "f64" else 2e-7
+    assert np.max(np.abs(got - ref)) < tol
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n,d", SMALL)
+def test_demag_vs_direct_sum(oracle, n, d, dt):
+    """S1-S5 against the O(n^2) real-space sum (ground truth O3)."""
+    cfg = cfg_for(n, d)
+    m, m64 = round_input(w.random_unit_vectors(101, n), dt)
+    ref = oracle.demag_direct(oracle.newell_octant(n, d), cfg.Ms, m64)
+    ctx = make_ctx(cfg, dt)
+    got = ctx.demag_field(to_dev(m)).cpu().numpy()
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL[dt], (l2, mx)
+    assert mx <= 10 * TOL[dt]
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n", [(64, 64, 16), (128, 64, 32), (16, 256, 4), (256, 8, 64)])
+def test_demag_vs_oracle_fft_medium(oracle, n, dt):
+    """Several tiles per pass and ragged tile counts; reference = oracle FFT path O5."""
+    cfg = cfg_for(n, (4e-9, 3e-9, 2e-9))
+    m, m64 = round_input(w.random_unit_vectors(202, n), dt)
+    P = make_problem(oracle, cfg, terms=1)
+    ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
+    ctx = make_ctx(cfg, dt)
+    got = ctx.demag_field(to_dev(m)).cpu().numpy()
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL[dt], (l2, mx)
+    # deterministic: bit-identical on repetition
+    again = ctx.demag_field(to_dev(m)).cpu().numpy()
+    assert np.array_equal(got, again)
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n,d", [((16, 16, 2), (5e-9, 5e-9, 3e-9)), ((8, 4, 1), (3e-9, 4e-9, 5e-9)),
+                                 ((32, 16, 8), (4e-9, 3e-9, 2e-9)), ((1, 1, 4), (1e-9, 2e-9, 3e-9)),
+                                 ((64, 32, 16), (2e-9, 2e-9, 2e-9))])
+def test_exchange_field(oracle, n, d, dt):
+    cfg = cfg_for(n, d)
+    m, m64 = round_input(w.random_unit_vectors(303, n), dt)
+    ref = oracle.exchange(d, cfg.Ms, cfg.Aex, m64)
+    ctx = make_ctx(cfg, dt, terms=2)
+    got = ctx.exchange_field(to_dev(m)).cpu().numpy()
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n", [(16, 16, 2), (32, 16, 8), (128, 32, 1)])
+def test_heff_and_llg_rhs_all_terms(oracle, n, dt):
+    cfg = cfg_for(n, (5e-9, 5e-9, 3e-9), Ku=5e5, axis=(0.0, 0.6, 0.8), alpha=0.1,
+                  Hext=(1e4, -2e4, 3e4), terms=15)
+    m, m64 = round_input(cfg.initial_m(), dt)
+    P = make_problem(oracle, cfg)
+    ctx = make_ctx(cfg, dt)
+    md = to_dev(m)
+    H = ctx.heff(md).cpu().numpy()
+    l2, mx = w.field_errors(H, P.heff(m64))
+    assert l2 <= TOL[dt], (l2, mx)
+    k = ctx.llg_rhs(md).cpu().numpy()
+    l2, mx = w.field_errors(k, P.llg_rhs(m64))
+    assert l2 <= TOL[dt], (l2, mx)
+    # each term alone
+    for t in (1, 2, 4, 8):
+        ctx.set_terms(t)
+        Pt = make_problem(oracle, cfg, terms=t, N=P.N)
+        l2, mx = w.field_errors(ctx.heff(md).cpu().numpy(), Pt.heff(m64))
+        assert l2 <= TOL[dt], (t, l2, mx)
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+def test_config1_rk4_trajectory(oracle, dt):
+    """Config 1: 10 RK4 steps at dt = 1e-13 s, demag + exchange, alpha = 0.5."""
+    cfg = w.get_config(1)
+    m, m64 = round_input(cfg.initial_m(), dt)
+    P = make_problem(oracle, cfg)
+    ctx = make_ctx(cfg, dt)
+    md = to_dev(m)
+    ref = m64
+    for step in range(10):
+        ctx.rk_step(md, cfg.dt)
+        ref = P.rk4_step(ref, cfg.dt)
+        assert w.traj_error(md.cpu().numpy(), ref) <= TRAJ_TOL[dt], step
+    assert abs(np.linalg.norm(md.cpu().numpy(), axis=-1) - 1).max() < (1e-14 if dt == "f64" else 1e-6)
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+def test_config2_first_100_steps(oracle, dt):
+    """Config 2 (SP4-shaped strip, driven phase): first 100 RK4 steps pointwise."""
+    cfg = w.get_config(2)
+    m, m64 = round_input(cfg.initial_m(), dt)
+    P = make_problem(oracle, cfg)
+    ctx = make_ctx(cfg, dt)
+    md = to_dev(m)
+    ref = m64
+    worst = 0.0
+    for step in range(100):
+        ctx.rk_step(md, cfg.dt)
+        ref = P.rk4_step(ref, cfg.dt)
+        if step % 10 == 9:
+            worst = max(worst, w.traj_error(md.cpu().numpy(), ref))
+    assert worst <= TRAJ_TOL[dt], worst
+
+
+def test_host_calls_match_device_calls(oracle):
+    cfg = cfg_for((32, 16, 8), (4e-9, 3e-9, 2e-9))
+    ctx = make_ctx(cfg, "f32")
+    m = w.random_unit_vectors(7, cfg.n).astype(np.float32)
+    md = to_dev(m)
+    assert np.array_equal(ctx.demag_field_host(m), ctx.demag_field(md).cpu().numpy())
+    assert np.array_equal(ctx.heff_host(m), ctx.heff(md).cpu().numpy())
+    assert np.array_equal(ctx.llg_rhs_host(m), ctx.llg_rhs(md).cpu().numpy())
+    m2 = m.copy()
+    ctx.rk_step_host(m2, 1e-13)
+    ctx.rk_step(md, 1e-13)
+    assert np.array_equal(m2, md.cpu().numpy())
+
+
+def test_error_paths_on_device():
+    from paper_2606_01114_b200 import Context, MMError
+    ctx = Context((8, 8, 2), (1e-9,) * 3, dtype=torch.float32)
+    m = torch.zeros(8, 8, 2, 3, device="cuda")
+    with pytest.raises(MMError) as e:
+        ctx.heff(m)
+    assert e.value.status == 3                      # material missing
+    ctx.set_material(8e5, 1.3e-11)
+    with pytest.raises(MMError) as e:
+        ctx.demag_field(m)
+    assert e.value.status == 3                      # demag_init missing
+    ctx.demag_init()
+    with pytest.raises(MMError) as e:
+        ctx._call("mm_demag_field", m.data_ptr(), m.data_ptr())
+    assert e.value.status == 1                      # aliasing
+    with pytest.raises(MMError) as e:
+        ctx._call("mm_demag_field", m.data_ptr() + 4, m.data_ptr())
+    assert e.value.status == 1                      # misaligned
+    n0 = ctx.launch_count
+    ctx.demag_field(m)
+    assert ctx.launch_count - n0 == 5
