@@ -113,6 +113,17 @@ mm_status mm_rk_step_host(mm_ctx *ctx, void *m_inout_host, double dt);
  * (bench.py reports the difference over its timed region as gpu_launches). */
 mm_status mm_ctx_launch_count(const mm_ctx *ctx, unsigned long long *count);
 
+/* Per-kernel timing for the roofline report.  While enabled, every field/step call records
+ * CUDA events on the context's stream around each kernel it enqueues (a few microseconds of
+ * host time per launch; at most 8192 marks are kept between two reads).
+ * mm_ctx_kernel_times synchronises the stream and returns, per kernel kind, the summed
+ * duration in milliseconds and the number of launches since the last reset:
+ *   0 S1 forward z   1 S2 forward y   2 S3 fused x pass   3 S4 inverse y   4 S5 inverse z
+ *   5 S6/S7 fused pointwise pass      6, 7 unused */
+mm_status mm_ctx_set_profiling(mm_ctx *ctx, int enable);
+mm_status mm_ctx_kernel_times(mm_ctx *ctx, int reset, double ms_sum[8],
+                              unsigned long long count[8]);
+
 /* Tuning knobs for experiments (tile widths of the FFT passes); 0 keeps the default.
  * Must be called before mm_demag_init. */
 mm_status mm_ctx_set_tiles(mm_ctx *ctx, int bz, int by, int bk);

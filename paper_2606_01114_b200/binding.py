@@ -63,6 +63,8 @@ def load_library():
         "mm_rk_step_host": [vp, vp, dbl],
         "mm_ctx_launch_count": [vp, C.POINTER(C.c_ulonglong)],
         "mm_ctx_set_tiles": [vp, i32, i32, i32],
+        "mm_ctx_set_profiling": [vp, i32],
+        "mm_ctx_kernel_times": [vp, i32, C.POINTER(dbl), C.POINTER(C.c_ulonglong)],
     }
     for name, args in sigs.items():
         fn = getattr(lib, name)
@@ -158,6 +160,18 @@ class Context:
         v = C.c_ulonglong()
         self._call("mm_ctx_launch_count", C.byref(v))
         return v.value
+
+    def set_profiling(self, on=True):
+        self._call("mm_ctx_set_profiling", 1 if on else 0)
+
+    KERNEL_NAMES = ("S1_zf", "S2_yf", "S3_xp", "S4_yi", "S5_zi", "S6_pointwise")
+
+    def kernel_times(self, reset=True):
+        """{kernel: (total ms, launches)} since the last reset; synchronises."""
+        ms = (C.c_double * 8)()
+        cnt = (C.c_ulonglong * 8)()
+        self._call("mm_ctx_kernel_times", 1 if reset else 0, ms, cnt)
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_NAMES)}
 
     # -- device calls
     def _check(self, t):

@@ -221,7 +221,7 @@ static int pick_threads(int B, int rows) {
 
 template <typename T>
 cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const T* m, T* H,
-                               T scale, cudaStream_t st, unsigned long long* launches) {
+                               T scale, cudaStream_t st, unsigned long long* launches, Prof* prof) {
   cudaError_t err;
   const size_t cs = sizeof(Cx<T>);
   Cx<T>* A2 = g.Py > 1 ? b.A2 : b.A1;  // ny == 1: the y pass is the identity
@@ -229,6 +229,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     const size_t sb = (size_t)3 * g.Pz * g.Bz * cs;
     if ((err = set_smem(zf_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.Bz, (g.ny + 1) / 2);
+    prof->mark(0, st);
     zf_kernel<T><<<grid, pick_threads(g.Bz, 3 * g.Pz), sb, st>>>(g, m, b.A1, b.Wz, b.posz);
     ++*launches;
   }
@@ -236,6 +237,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     const size_t sb = (size_t)g.Py * g.By * cs;
     if ((err = set_smem(yf_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.By, g.Kz, 3);
+    prof->mark(1, st);
     yf_kernel<T><<<grid, pick_threads(g.By, g.Py), sb, st>>>(g, b.A1, b.A2, b.Wy);
     ++*launches;
   }
@@ -243,6 +245,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     const size_t sb = (size_t)3 * g.Px * g.Bk * cs;
     if ((err = set_smem(xp_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.Py / g.Bk, g.Kz);
+    prof->mark(2, st);
     xp_kernel<T><<<grid, pick_threads(g.Bk, 3 * g.Px), sb, st>>>(g, A2, b.table, b.Wx);
     ++*launches;
   }
@@ -250,6 +253,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     const size_t sb = (size_t)g.Py * g.By * cs;
     if ((err = set_smem(yi_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.By, g.Kz, 3);
+    prof->mark(3, st);
     yi_kernel<T><<<grid, pick_threads(g.By, g.Py), sb, st>>>(g, b.A2, b.A1, b.Wy);
     ++*launches;
   }
@@ -257,17 +261,19 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     const size_t sb = (size_t)3 * g.Pz * g.Bz * cs;
     if ((err = set_smem(zi_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.Bz, (g.ny + 1) / 2);
+    prof->mark(4, st);
     zi_kernel<T><<<grid, pick_threads(g.Bz, 3 * g.Pz), sb, st>>>(g, b.A1, H, b.Wz, b.posz, scale);
     ++*launches;
   }
+  prof->mark(-1, st);
   return cudaGetLastError();
 }
 
 template cudaError_t demag_field_launch<float>(const DemagGeom&, const DemagBufs<float>&,
                                                const float*, float*, float, cudaStream_t,
-                                               unsigned long long*);
+                                               unsigned long long*, Prof*);
 template cudaError_t demag_field_launch<double>(const DemagGeom&, const DemagBufs<double>&,
                                                 const double*, double*, double, cudaStream_t,
-                                                unsigned long long*);
+                                                unsigned long long*, Prof*);
 
 }  // namespace mm

@@ -26,6 +26,6 @@ template <typename T> struct DemagBufs {
 // Enqueues S1..S5: H := scale * crop(IFFT(table . FFT(pad(m)))).
 template <typename T>
 cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const T* m, T* H,
-                               T scale, cudaStream_t st, unsigned long long* launches);
+                               T scale, cudaStream_t st, unsigned long long* launches, Prof* prof);
 
 }  // namespace mm

@@ -45,6 +45,9 @@ struct mm_ctx {
   // scratch offsets
   size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, scr_need;
   unsigned long long launches = 0;
+  Prof prof;
+  double prof_ms[Prof::kKinds] = {0};
+  unsigned long long prof_cnt[Prof::kKinds] = {0};
   char err[256] = "";
 };
 
@@ -238,6 +241,34 @@ mm_status mm_ctx_launch_count(const mm_ctx* ctx, unsigned long long* count) {
 
 const char* mm_last_error(const mm_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
 
+mm_status mm_ctx_set_profiling(mm_ctx* ctx, int enable) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  ctx->prof.on = enable != 0;
+  return MM_OK;
+}
+
+mm_status mm_ctx_kernel_times(mm_ctx* ctx, int reset, double ms_sum[8], unsigned long long count[8]) {
+  if (!ctx || !ms_sum || !count) return MM_ERR_INVALID_ARG;
+  cudaError_t e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) { snprintf(ctx->err, 256, "mm_ctx_kernel_times: %s", cudaGetErrorString(e)); return MM_ERR_CUDA; }
+  Prof& p = ctx->prof;
+  for (int i = 0; i + 1 < p.n; ++i) {
+    if (p.kind[i] < 0) continue;
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, p.ev[i], p.ev[i + 1]) == cudaSuccess) {
+      ctx->prof_ms[p.kind[i]] += ms;
+      ctx->prof_cnt[p.kind[i]] += 1;
+    }
+  }
+  p.n = 0;
+  for (int k = 0; k < Prof::kKinds; ++k) {
+    ms_sum[k] = ctx->prof_ms[k];
+    count[k] = ctx->prof_cnt[k];
+    if (reset) { ctx->prof_ms[k] = 0; ctx->prof_cnt[k] = 0; }
+  }
+  return MM_OK;
+}
+
 }  // extern "C"
 
 // ------------------------------------------------------------------ internals
@@ -332,7 +363,8 @@ static mm_status need_ready(mm_ctx* c, const char* fn, bool demag) {
 
 template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H) {
   cudaError_t e = demag_field_launch<T>(c->geom, bufs_of<T>(c), static_cast<const T*>(m),
-                                        static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches);
+                                        static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches,
+                                        &c->prof);
   return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag launch", e);
 }
 
@@ -346,7 +378,7 @@ static mm_status eval_t(mm_ctx* c, int mode, const void* m, void* out, void* m0,
   }
   cudaError_t e = pointwise_launch<T>(mode, p, static_cast<const T*>(m), Hd, static_cast<T*>(out),
                                       static_cast<T*>(m0), reinterpret_cast<T*>(c->scr + c->off_acc),
-                                      c->stream, &c->launches);
+                                      c->stream, &c->launches, &c->prof);
   return e == cudaSuccess ? MM_OK : cuda_fail(c, "pointwise launch", e);
 }
 

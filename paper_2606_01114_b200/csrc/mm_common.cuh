@@ -36,4 +36,36 @@ struct FftPlan {
   int radix[MM_MAX_STAGES];
 };
 
+
+// Optional per-kernel timing with CUDA events on the launching stream (bench.py's roofline
+// leg).  mark(id) is called immediately before kernel `id` is enqueued, mark(-1) after the
+// last kernel of a call; the time between two consecutive marks belongs to the first.
+struct Prof {
+  static constexpr int kKinds = 8;
+  static constexpr int kMaxMarks = 8192;
+  bool on = false;
+  cudaEvent_t* ev = nullptr;
+  int* kind = nullptr;
+  int n = 0, cap = 0;
+  void mark(int id, cudaStream_t st) {
+    if (!on || n >= kMaxMarks) return;
+    if (n == cap) {
+      const int ncap = cap ? cap * 2 : 64;
+      cudaEvent_t* e2 = new cudaEvent_t[ncap];
+      int* k2 = new int[ncap];
+      for (int i = 0; i < cap; ++i) { e2[i] = ev[i]; k2[i] = kind[i]; }
+      for (int i = cap; i < ncap; ++i) cudaEventCreate(&e2[i]);
+      delete[] ev; delete[] kind;
+      ev = e2; kind = k2; cap = ncap;
+    }
+    kind[n] = id;
+    cudaEventRecord(ev[n], st);
+    ++n;
+  }
+  ~Prof() {
+    for (int i = 0; i < cap; ++i) cudaEventDestroy(ev[i]);
+    delete[] ev; delete[] kind;
+  }
+};
+
 }  // namespace mm

@@ -238,7 +238,9 @@ static void launch_mode(const PwParams<T>& p, const T* m, const T* Hd, T* out, T
 
 template <typename T>
 cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T* Hd, T* out,
-                             T* m0, T* acc, cudaStream_t st, unsigned long long* launches) {
+                             T* m0, T* acc, cudaStream_t st, unsigned long long* launches,
+                             Prof* prof) {
+  prof->mark(5, st);
   switch (mode) {
     case PW_EXCHANGE: launch_mode<T, PW_EXCHANGE>(p, m, Hd, out, m0, acc, st); break;
     case PW_HEFF: launch_mode<T, PW_HEFF>(p, m, Hd, out, m0, acc, st); break;
@@ -247,14 +249,15 @@ cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T
     default: launch_mode<T, PW_RK_FINAL>(p, m, Hd, out, m0, acc, st); break;
   }
   ++*launches;
+  prof->mark(-1, st);
   return cudaGetLastError();
 }
 
 template cudaError_t pointwise_launch<float>(int, const PwParams<float>&, const float*,
                                              const float*, float*, float*, float*, cudaStream_t,
-                                             unsigned long long*);
+                                             unsigned long long*, Prof*);
 template cudaError_t pointwise_launch<double>(int, const PwParams<double>&, const double*,
                                               const double*, double*, double*, double*,
-                                              cudaStream_t, unsigned long long*);
+                                              cudaStream_t, unsigned long long*, Prof*);
 
 }  // namespace mm

@@ -27,6 +27,7 @@ template <typename T> struct PwParams {
 
 template <typename T>
 cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T* Hd, T* out,
-                             T* m0, T* acc, cudaStream_t st, unsigned long long* launches);
+                             T* m0, T* acc, cudaStream_t st, unsigned long long* launches,
+                             Prof* prof);
 
 }  // namespace mm
