@@ -125,8 +125,18 @@ mm_status mm_ctx_kernel_times(mm_ctx *ctx, int reset, double ms_sum[8],
                               unsigned long long count[8]);
 
 /* Tuning knobs for experiments (tile widths of the FFT passes); 0 keeps the default.
- * Must be called before mm_demag_init. */
+ * Applies to the generic passes.  Must be called before mm_ctx_set_workspace. */
 mm_status mm_ctx_set_tiles(mm_ctx *ctx, int bz, int by, int bk);
+
+/* Demag path selection (experiments and tests).  path: 0 = automatic (the x-first fast kernels
+ * of demag_fast.cu where they cover the mesh: nx, ny in {64..1024}, nz in {64, 128}; otherwise
+ * the generic z-first passes), 1 = generic passes always, 2 = fast kernels required
+ * (MM_ERR_UNSUPPORTED_SIZE if they do not cover the mesh).  kchunk: number of kx planes the
+ * y/z/y passes of the fast path process per launch group through one reused (L2-sized)
+ * buffer; 0 = all planes at once.  Changes the workspace sizes: call before
+ * mm_ctx_workspace_bytes / mm_ctx_set_workspace.  mm_ctx_path reports what is selected. */
+mm_status mm_ctx_set_path(mm_ctx *ctx, int path, int kchunk);
+mm_status mm_ctx_path(const mm_ctx *ctx, int *fast, int *kchunk);
 
 /* Last error text of this context (or of the last failed mm_ctx_create if ctx is NULL).
  * Not thread-safe. */

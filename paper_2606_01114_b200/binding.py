@@ -63,6 +63,8 @@ def load_library():
         "mm_rk_step_host": [vp, vp, dbl],
         "mm_ctx_launch_count": [vp, C.POINTER(C.c_ulonglong)],
         "mm_ctx_set_tiles": [vp, i32, i32, i32],
+        "mm_ctx_set_path": [vp, i32, i32],
+        "mm_ctx_path": [vp, C.POINTER(i32), C.POINTER(i32)],
         "mm_ctx_set_profiling": [vp, i32],
         "mm_ctx_kernel_times": [vp, i32, C.POINTER(dbl), C.POINTER(C.c_ulonglong)],
     }
@@ -88,7 +90,8 @@ class Context:
     """One mesh on one GPU (mm_ctx).  Mirrors Mesh(n, dx) + State.material + the field-term
     list of the paper's scripts."""
 
-    def __init__(self, n, d, dtype=torch.float32, device="cuda:0", tiles=None, allocate=True):
+    def __init__(self, n, d, dtype=torch.float32, device="cuda:0", tiles=None, allocate=True,
+                 path=0, kchunk=0):
         self.lib = load_library()
         self.n = tuple(int(v) for v in n)
         self.d = tuple(float(v) for v in d)
@@ -100,6 +103,8 @@ class Context:
             raise MMError(st, self.lib.mm_last_error(None).decode())
         if tiles is not None:
             self._call("mm_ctx_set_tiles", *[int(t) for t in tiles])
+        if path or kchunk:
+            self._call("mm_ctx_set_path", int(path), int(kchunk))
         self._ws = None
         if allocate:
             self.allocate()
@@ -154,6 +159,13 @@ class Context:
 
     def demag_init(self):
         self._call("mm_demag_init")
+
+    @property
+    def path(self):
+        """(fast, kchunk): whether the x-first fast kernels are selected, planes per chunk."""
+        f, k = C.c_int(), C.c_int()
+        self._call("mm_ctx_path", C.byref(f), C.byref(k))
+        return bool(f.value), k.value
 
     @property
     def launch_count(self):

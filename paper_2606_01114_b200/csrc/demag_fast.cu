@@ -1,0 +1,727 @@
+// K1..K5 of the fast demag path.
+//
+//   K1 xf : m [x][y][z][c] real      -> A1[kx<=nx][y][q]      x forward, r2c, pruned   (S1)
+//   K2 yf : A1                       -> A2[kx][ky'][q]        y forward, pruned        (S2)
+//   K3 zp : A2 in place, x Nhat                               z forward, tensor
+//                                                             multiply, z inverse      (S3)
+//   K4 yi : A2                       -> A1[kx][y][q]          y inverse, truncated     (S4)
+//   K5 xi : A1                       -> H [x][y][z][c] real   x inverse, c2r, truncated(S5)
+// q = 3 z + c is the flattened (z, component) index, the fastest axis everywhere.
+//
+// K1, K2, K4, K5 ("strided passes"): the transform axis is strided, 64 bytes of q are the
+// batch.  A CTA owns a tile of 2L rows x 64 B in shared memory (L = n_d; rows [0, L) hold the
+// even-output half, rows [L, 2L) the odd-output half of the pruned length-2L transform); lanes
+// run along the batch so every global access is a run of 64-byte row segments and every shared
+// access of a quarter/half warp is conflict-free (rows of a warp's neighbouring tasks differ
+// in bit 0; the last stage's rows are made to differ by the XOR swizzle below).  Three radix
+// stages: the first straight from global memory in registers, the middle one in shared
+// memory, the last one straight to global memory.
+//
+// K3 ("contiguous pass"): the z pencil of one (kx, ky') is 3 nz contiguous complex values.  A
+// group of G = Pz/16 lanes owns a pencil, each lane 16 values of each component in registers:
+// pruned radix-16 stage, one exchange through shared memory, radix-G stage, 3x3 real-symmetric
+// multiply in registers, and the mirror image back.  Pencils move by bulk async copies.
+#include "demag_fast.cuh"
+
+#include <cuda/std/cstdint>
+
+#include "fft_core.cuh"
+
+namespace mm {
+
+constexpr int kStrideThreads = 256;
+
+constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v / 2); }
+
+// Radix plan of the length-L sub-transforms of the strided passes: L = R1 R2 R3.
+template <int L> struct FastPlan;
+template <> struct FastPlan<64> { static constexpr int R1 = 4, R2 = 4, R3 = 4; };
+template <> struct FastPlan<128> { static constexpr int R1 = 8, R2 = 4, R3 = 4; };
+template <> struct FastPlan<256> { static constexpr int R1 = 8, R2 = 8, R3 = 4; };
+template <> struct FastPlan<512> { static constexpr int R1 = 8, R2 = 8, R3 = 8; };
+template <> struct FastPlan<1024> { static constexpr int R1 = 16, R2 = 8, R3 = 8; };
+
+static void plan_of(int L, int& R1, int& R2, int& R3) {
+  switch (L) {
+    case 64: R1 = 4; R2 = 4; R3 = 4; break;
+    case 128: R1 = 8; R2 = 4; R3 = 4; break;
+    case 256: R1 = 8; R2 = 8; R3 = 4; break;
+    case 512: R1 = 8; R2 = 8; R3 = 8; break;
+    default: R1 = 16; R2 = 8; R3 = 8; break;
+  }
+}
+
+// k = h + 2 (u1 + R1 (u2 + R2 u3))  ->  row h L + u1 R2 R3 + u2 R3 + u3
+int fast_pos_logical(int L, int k) {
+  int R1, R2, R3;
+  plan_of(L, R1, R2, R3);
+  const int h = k & 1;
+  int kk = k >> 1;
+  const int u1 = kk % R1; kk /= R1;
+  const int u2 = kk % R2; kk /= R2;
+  return h * L + u1 * R2 * R3 + u2 * R3 + kk;
+}
+int fast_swizzle(int L, int row) {
+  int R1, R2, R3;
+  plan_of(L, R1, R2, R3);
+  return row ^ ((row >> ilog2c(R3)) & 1);
+}
+
+template <typename T, int L> struct Tile {
+  using P = FastPlan<L>;
+  static constexpr int R1 = P::R1, R2 = P::R2, R3 = P::R3;
+  static constexpr int q1 = R2 * R3, q2 = R3;
+  static constexpr int B = 64 / (int)sizeof(Cx<T>);   // lanes along the batch (64-byte rows)
+  static constexpr int NS = kStrideThreads / B;       // task slots
+  static constexpr int LOG3 = ilog2c(R3);
+  static constexpr int smem_bytes = 2 * L * 64;
+  // resident CTAs per SM the kernels are compiled for (shared memory and registers)
+  static constexpr int min_blocks =
+      smem_bytes <= 72 * 1024 ? (sizeof(T) == 4 ? 3 : 2) : (smem_bytes <= 110 * 1024 ? 2 : 1);
+};
+
+// ------------------------------------------------------------------ strided-pass stages
+// Shared-memory element (logical row r, lane): sm[(r ^ ((r >> LOG3) & 1)) * B + lane].
+
+// Forward first stage for butterfly bf: v[s] holds input row bf + q1 s.  Writes the even half
+// (rows u1 q1 + bf) and the odd half (+L) after the inter-stage twiddle w_L^(bf u1).
+template <typename T, int L>
+__device__ __forceinline__ void fwd_first(Cx<T>* sm, const Cx<T>* __restrict__ W, int lane,
+                                          int bf, Cx<T>* v) {
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, q1 = TL::q1, B = TL::B;
+  const int rb = bf ^ ((bf >> TL::LOG3) & 1);
+  Cx<T> tw[R1];
+#pragma unroll
+  for (int u = 1; u < R1; ++u) tw[u] = __ldg(W + 2 * bf * u);
+  Cx<T> e[R1];
+#pragma unroll
+  for (int s = 0; s < R1; ++s) e[s] = v[s];
+  Dft<T, R1, false>::run(e);
+#pragma unroll
+  for (int u = 0; u < R1; ++u)
+    sm[(u * q1 + rb) * B + lane] = u ? cmul(e[u], tw[u]) : e[0];
+#pragma unroll
+  for (int s = 0; s < R1; ++s) v[s] = cmul(v[s], __ldg(W + bf + q1 * s));
+  Dft<T, R1, false>::run(v);
+#pragma unroll
+  for (int u = 0; u < R1; ++u)
+    sm[(L + u * q1 + rb) * B + lane] = u ? cmul(v[u], tw[u]) : v[0];
+}
+
+// Forward middle stage over both halves, in place.
+template <typename T, int L>
+__device__ __forceinline__ void fwd_middle(Cx<T>* sm, const Cx<T>* __restrict__ W, int lane,
+                                           int slot) {
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, R2 = TL::R2, q1 = TL::q1, q2 = TL::q2, B = TL::B, NS = TL::NS;
+  constexpr int NTASK = 2 * R1 * q2;
+#pragma unroll
+  for (int i0 = 0; i0 < NTASK; i0 += NS) {
+    const int i = i0 + slot;
+    if (NTASK % NS != 0 && i >= NTASK) break;
+    const int t2 = i % q2, hu = i / q2;
+    const int b0 = hu * q1 + t2, b1 = b0 ^ 1;
+    Cx<T> v[R2];
+#pragma unroll
+    for (int s = 0; s < R2; ++s) v[s] = sm[(((s & 1) ? b1 : b0) + q2 * s) * B + lane];
+    Dft<T, R2, false>::run(v);
+#pragma unroll
+    for (int u = 1; u < R2; ++u) v[u] = cmul(v[u], __ldg(W + 2 * R1 * t2 * u));
+#pragma unroll
+    for (int u = 0; u < R2; ++u) sm[(((u & 1) ? b1 : b0) + q2 * u) * B + lane] = v[u];
+  }
+}
+
+// Forward last stage of task i (rows i R3 .. i R3 + R3 - 1): loads and transforms; v[u3] is
+// the value of logical row i R3 + u3.
+template <typename T, int L>
+__device__ __forceinline__ void fwd_last(const Cx<T>* sm, int lane, int i, Cx<T>* v) {
+  using TL = Tile<T, L>;
+  constexpr int R3 = TL::R3, B = TL::B;
+  const int g = i & 1, base = i * R3;
+  const int pe = base + g, po = base - g;
+#pragma unroll
+  for (int s = 0; s < R3; ++s) v[s] = sm[(((s & 1) ? po : pe) + s) * B + lane];
+  Dft<T, R3, false>::run(v);
+}
+
+// Inverse first stage (mirror of fwd_last): v[u3] = value of logical row i R3 + u3 on entry;
+// the inverse butterfly's outputs are stored at rows i R3 + s.
+template <typename T, int L>
+__device__ __forceinline__ void inv_first(Cx<T>* sm, int lane, int i, Cx<T>* v) {
+  using TL = Tile<T, L>;
+  constexpr int R3 = TL::R3, B = TL::B;
+  const int g = i & 1, base = i * R3;
+  const int pe = base + g, po = base - g;
+  Dft<T, R3, true>::run(v);
+#pragma unroll
+  for (int s = 0; s < R3; ++s) sm[(((s & 1) ? po : pe) + s) * B + lane] = v[s];
+}
+
+// Inverse middle stage (mirror of fwd_middle).
+template <typename T, int L>
+__device__ __forceinline__ void inv_middle(Cx<T>* sm, const Cx<T>* __restrict__ W, int lane,
+                                           int slot) {
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, R2 = TL::R2, q1 = TL::q1, q2 = TL::q2, B = TL::B, NS = TL::NS;
+  constexpr int NTASK = 2 * R1 * q2;
+#pragma unroll
+  for (int i0 = 0; i0 < NTASK; i0 += NS) {
+    const int i = i0 + slot;
+    if (NTASK % NS != 0 && i >= NTASK) break;
+    const int t2 = i % q2, hu = i / q2;
+    const int b0 = hu * q1 + t2, b1 = b0 ^ 1;
+    Cx<T> v[R2];
+#pragma unroll
+    for (int u = 0; u < R2; ++u) v[u] = sm[(((u & 1) ? b1 : b0) + q2 * u) * B + lane];
+#pragma unroll
+    for (int u = 1; u < R2; ++u) v[u] = cmulc(v[u], __ldg(W + 2 * R1 * t2 * u));
+    Dft<T, R2, true>::run(v);
+#pragma unroll
+    for (int s = 0; s < R2; ++s) sm[(((s & 1) ? b1 : b0) + q2 * s) * B + lane] = v[s];
+  }
+}
+
+// Inverse last stage for butterfly bf (mirror of fwd_first) with the truncation combine:
+// v[s] = e_s + conj(w_2L^(bf + q1 s)) o_s = output sample bf + q1 s.
+template <typename T, int L>
+__device__ __forceinline__ void inv_last(const Cx<T>* sm, const Cx<T>* __restrict__ W, int lane,
+                                         int bf, Cx<T>* v) {
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, q1 = TL::q1, B = TL::B;
+  const int rb = bf ^ ((bf >> TL::LOG3) & 1);
+  Cx<T> tw[R1];
+#pragma unroll
+  for (int u = 1; u < R1; ++u) tw[u] = __ldg(W + 2 * bf * u);
+  Cx<T> o[R1];
+#pragma unroll
+  for (int u = 0; u < R1; ++u) {
+    const Cx<T> a = sm[(u * q1 + rb) * B + lane], b = sm[(L + u * q1 + rb) * B + lane];
+    v[u] = u ? cmulc(a, tw[u]) : a;
+    o[u] = u ? cmulc(b, tw[u]) : b;
+  }
+  Dft<T, R1, true>::run(v);
+  Dft<T, R1, true>::run(o);
+#pragma unroll
+  for (int s = 0; s < R1; ++s) v[s] = cadd(v[s], cmulc(o[s], __ldg(W + bf + q1 * s)));
+}
+
+// two adjacent complex values as one vector access where the type allows it
+template <typename T> struct Pair2;
+template <> struct Pair2<float> {
+  static __device__ __forceinline__ void st(float2* p, float2 a, float2 b) {
+    *reinterpret_cast<float4*>(p) = make_float4(a.x, a.y, b.x, b.y);
+  }
+  static __device__ __forceinline__ void ld(const float2* p, float2& a, float2& b) {
+    const float4 t = *reinterpret_cast<const float4*>(p);
+    a = make_float2(t.x, t.y);
+    b = make_float2(t.z, t.w);
+  }
+};
+template <> struct Pair2<double> {
+  static __device__ __forceinline__ void st(double2* p, double2 a, double2 b) { p[0] = a; p[1] = b; }
+  static __device__ __forceinline__ void ld(const double2* p, double2& a, double2& b) { a = p[0]; b = p[1]; }
+};
+
+#define MM_TILE_PROLOGUE                                                   \
+  extern __shared__ __align__(16) unsigned char smem_raw[];                \
+  Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);                          \
+  using TL = Tile<T, L>;                                                   \
+  constexpr int R1 = TL::R1, R2 = TL::R2, R3 = TL::R3, q1 = TL::q1, B = TL::B, NS = TL::NS; \
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B;                \
+  (void)R2; (void)R3;
+
+// ---------------------------------------------------------------- K2: forward y (S2)
+// grid (Q / B, planes).  A1, A2 point at the first plane of the launch.
+template <typename T, int L>
+__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+yf_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>* __restrict__ W, int Q) {
+  MM_TILE_PROLOGUE
+  const size_t col = (size_t)blockIdx.x * B + lane;
+  const Cx<T>* in = A1 + (size_t)blockIdx.y * L * Q + col;
+  Cx<T>* out = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
+#pragma unroll 1
+  for (int bf = slot; bf < q1; bf += NS) {
+    Cx<T> v[R1];
+#pragma unroll
+    for (int s = 0; s < R1; ++s) v[s] = in[(size_t)(bf + q1 * s) * Q];
+    fwd_first<T, L>(sm, W, lane, bf, v);
+  }
+  __syncthreads();
+  fwd_middle<T, L>(sm, W, lane, slot);
+  __syncthreads();
+#pragma unroll 1
+  for (int i = slot; i < 2 * R1 * R2; i += NS) {
+    Cx<T> v[R3];
+    fwd_last<T, L>(sm, lane, i, v);
+#pragma unroll
+    for (int u = 0; u < R3; ++u) out[(size_t)(i * R3 + u) * Q] = v[u];
+  }
+}
+
+// ---------------------------------------------------------------- K4: inverse y (S4)
+template <typename T, int L>
+__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+yi_fast_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W, int Q) {
+  MM_TILE_PROLOGUE
+  const size_t col = (size_t)blockIdx.x * B + lane;
+  const Cx<T>* in = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
+  Cx<T>* out = A1 + (size_t)blockIdx.y * L * Q + col;
+#pragma unroll 1
+  for (int i = slot; i < 2 * R1 * R2; i += NS) {
+    Cx<T> v[R3];
+#pragma unroll
+    for (int u = 0; u < R3; ++u) v[u] = in[(size_t)(i * R3 + u) * Q];
+    inv_first<T, L>(sm, lane, i, v);
+  }
+  __syncthreads();
+  inv_middle<T, L>(sm, W, lane, slot);
+  __syncthreads();
+#pragma unroll 1
+  for (int bf = slot; bf < q1; bf += NS) {
+    Cx<T> v[R1];
+    inv_last<T, L>(sm, W, lane, bf, v);
+#pragma unroll
+    for (int s = 0; s < R1; ++s) out[(size_t)(bf + q1 * s) * Q] = v[s];
+  }
+}
+
+// ---------------------------------------------------------------- K1: forward x, r2c (S1)
+// The real array m[x][y][q] is read as complex pairs (q, q+1): Z = FFT(a + i b) of two real
+// signals, separated afterwards with A[k] = (Z[k] + conj Z[-k])/2, B[k] = (Z[k] - conj Z[-k])/(2i)
+// for k <= nx.  grid (ny Q / 2 / B).  npairs = ny Q / 2 (pairs per x row); rowc = ny Q.
+template <typename T, int L>
+__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+xf_fast_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W,
+               const uint16_t* __restrict__ pos, size_t npairs) {
+  MM_TILE_PROLOGUE
+  const size_t pair = (size_t)blockIdx.x * B + lane;
+  const Cx<T>* in = mp + pair;
+#pragma unroll 1
+  for (int bf = slot; bf < q1; bf += NS) {
+    Cx<T> v[R1];
+#pragma unroll
+    for (int s = 0; s < R1; ++s) v[s] = in[(size_t)(bf + q1 * s) * npairs];
+    fwd_first<T, L>(sm, W, lane, bf, v);
+  }
+  __syncthreads();
+  fwd_middle<T, L>(sm, W, lane, slot);
+  __syncthreads();
+#pragma unroll 1
+  for (int i = slot; i < 2 * R1 * R2; i += NS) {
+    Cx<T> v[R3];
+    fwd_last<T, L>(sm, lane, i, v);
+    const int g = i & 1, base = i * R3, pe = base + g, po = base - g;
+#pragma unroll
+    for (int u = 0; u < R3; ++u) sm[(((u & 1) ? po : pe) + u) * B + lane] = v[u];
+  }
+  __syncthreads();
+  Cx<T>* out = A1 + 2 * pair;
+  const size_t rowc = 2 * npairs;
+#pragma unroll 1
+  for (int k = slot; k <= L; k += NS) {
+    const int p1 = pos[k], p2 = pos[(2 * L - k) & (2 * L - 1)];
+    const Cx<T> z1 = sm[p1 * B + lane], z2 = cconj(sm[p2 * B + lane]);
+    const Cx<T> s = cadd(z1, z2), d = csub(z1, z2);
+    Pair2<T>::st(out + (size_t)k * rowc, mk<T>((T)0.5 * s.x, (T)0.5 * s.y),
+                 mk<T>((T)0.5 * d.y, (T)-0.5 * d.x));
+  }
+}
+
+// ---------------------------------------------------------------- K5: inverse x, c2r (S5)
+// Z[k] = A[k] + i B[k], Z[Px - k] = conj A[k] + i conj B[k]; the truncated inverse gives
+// h_q(x) + i h_{q+1}(x), written as the real pair (q, q+1) of H, times scale (-Ms).
+template <typename T, int L>
+__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+xi_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>* __restrict__ W,
+               const uint16_t* __restrict__ pos, size_t npairs, T scale) {
+  MM_TILE_PROLOGUE
+  const size_t pair = (size_t)blockIdx.x * B + lane;
+  const Cx<T>* in = A1 + 2 * pair;
+  const size_t rowc = 2 * npairs;
+#pragma unroll 1
+  for (int k = slot; k <= L; k += NS) {
+    Cx<T> a, b;
+    Pair2<T>::ld(in + (size_t)k * rowc, a, b);
+    sm[pos[k] * B + lane] = mk<T>(a.x - b.y, a.y + b.x);
+    if (k != 0 && k != L) sm[pos[2 * L - k] * B + lane] = mk<T>(a.x + b.y, b.x - a.y);
+  }
+  __syncthreads();
+#pragma unroll 1
+  for (int i = slot; i < 2 * R1 * R2; i += NS) {
+    Cx<T> v[R3];
+    const int g = i & 1, base = i * R3, pe = base + g, po = base - g;
+#pragma unroll
+    for (int u = 0; u < R3; ++u) v[u] = sm[(((u & 1) ? po : pe) + u) * B + lane];
+    inv_first<T, L>(sm, lane, i, v);
+  }
+  __syncthreads();
+  inv_middle<T, L>(sm, W, lane, slot);
+  __syncthreads();
+  Cx<T>* out = Hp + pair;
+#pragma unroll 1
+  for (int bf = slot; bf < q1; bf += NS) {
+    Cx<T> v[R1];
+    inv_last<T, L>(sm, W, lane, bf, v);
+#pragma unroll
+    for (int s = 0; s < R1; ++s)
+      out[(size_t)(bf + q1 * s) * npairs] = mk<T>(scale * v[s].x, scale * v[s].y);
+  }
+}
+
+// ---------------------------------------------------------------- K3: fused z pass (S3)
+// Bulk asynchronous copies (global <-> shared, completion on an mbarrier / bulk group).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* dst_smem, const void* src_gmem, uint32_t bytes,
+                                          uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* dst_gmem, const void* src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem),
+               "r"(smem_u32(src_smem)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() {
+  asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+template <typename T, int G> struct ZpCfg {
+  static constexpr int nz = 8 * G, Pz = 16 * G, Q = 3 * nz;
+  static constexpr int NPW = 32 / G;        // pencils per warp
+  static constexpr int NSUB = 16 / G;       // second-stage sub-transforms per lane
+  static constexpr int PITCH = G + 1;       // exchange row pitch (conflict-free transposition)
+  static constexpr int XB = 16 * PITCH;     // exchange elements per pencil
+  static constexpr int WARPS = sizeof(T) == 4 ? 4 : 2;
+  static constexpr int MINB = 3;
+  static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
+  static constexpr int warp_elems = 2 * NPW * Q + NPW * XB;  // two stages of pencils + exchange
+  static constexpr int smem_bytes = 128 + WARPS * warp_elems * (int)sizeof(Cx<T>);
+};
+
+// Forward z transform of one component of one pencil: in = pencil (component-interleaved),
+// X[i G + v] = spectrum at kz = NSUB t + i + 16 v.
+template <typename T, int G>
+__device__ __forceinline__ void zp_forward(const Cx<T>* in, Cx<T>* xb, const Cx<T>* tw, int t, int c,
+                                           Cx<T>* X) {
+  using C = ZpCfg<T, G>;
+  Cx<T> e[8], o[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) e[j] = in[(t + G * j) * 3 + c];
+  // pruned radix 16 (inputs 8..15 are the zero padding): even outputs = DFT8(a), odd = DFT8(a w16^j)
+  o[0] = e[0];
+  o[1] = mul_root<T, 16, 1, false>(e[1]);
+  o[2] = mul_root<T, 16, 2, false>(e[2]);
+  o[3] = mul_root<T, 16, 3, false>(e[3]);
+  o[4] = mul_root<T, 16, 4, false>(e[4]);
+  o[5] = mul_root<T, 16, 5, false>(e[5]);
+  o[6] = mul_root<T, 16, 6, false>(e[6]);
+  o[7] = mul_root<T, 16, 7, false>(e[7]);
+  Dft<T, 8, false>::run(e);
+  Dft<T, 8, false>::run(o);
+  xb[t] = e[0];
+#pragma unroll
+  for (int v = 0; v < 8; ++v) {
+    if (v) xb[(2 * v) * C::PITCH + t] = cmul(e[v], tw[2 * v]);
+    xb[(2 * v + 1) * C::PITCH + t] = cmul(o[v], tw[2 * v + 1]);
+  }
+  __syncwarp();
+#pragma unroll
+  for (int i = 0; i < C::NSUB; ++i) {
+    Cx<T> b[G];
+#pragma unroll
+    for (int tp = 0; tp < G; ++tp) b[tp] = xb[(C::NSUB * t + i) * C::PITCH + tp];
+    Dft<T, G, false>::run(b);
+#pragma unroll
+    for (int v = 0; v < G; ++v) X[i * G + v] = b[v];
+  }
+  __syncwarp();
+}
+
+// Mirror image: X -> truncated samples written to out (component-interleaved pencil).
+template <typename T, int G>
+__device__ __forceinline__ void zp_inverse(Cx<T>* out, Cx<T>* xb, const Cx<T>* tw, int t, int c,
+                                           const Cx<T>* X) {
+  using C = ZpCfg<T, G>;
+#pragma unroll
+  for (int i = 0; i < C::NSUB; ++i) {
+    Cx<T> b[G];
+#pragma unroll
+    for (int v = 0; v < G; ++v) b[v] = X[i * G + v];
+    Dft<T, G, true>::run(b);
+#pragma unroll
+    for (int tp = 0; tp < G; ++tp) xb[(C::NSUB * t + i) * C::PITCH + tp] = b[tp];
+  }
+  __syncwarp();
+  Cx<T> e[8], o[8];
+  e[0] = xb[t];
+#pragma unroll
+  for (int v = 0; v < 8; ++v) {
+    if (v) e[v] = cmulc(xb[(2 * v) * C::PITCH + t], tw[2 * v]);
+    o[v] = cmulc(xb[(2 * v + 1) * C::PITCH + t], tw[2 * v + 1]);
+  }
+  __syncwarp();
+  Dft<T, 8, true>::run(e);
+  Dft<T, 8, true>::run(o);
+  out[t * 3 + c] = cadd(e[0], o[0]);
+  out[(t + G * 1) * 3 + c] = cadd(e[1], mul_root<T, 16, 1, true>(o[1]));
+  out[(t + G * 2) * 3 + c] = cadd(e[2], mul_root<T, 16, 2, true>(o[2]));
+  out[(t + G * 3) * 3 + c] = cadd(e[3], mul_root<T, 16, 3, true>(o[3]));
+  out[(t + G * 4) * 3 + c] = cadd(e[4], mul_root<T, 16, 4, true>(o[4]));
+  out[(t + G * 5) * 3 + c] = cadd(e[5], mul_root<T, 16, 5, true>(o[5]));
+  out[(t + G * 6) * 3 + c] = cadd(e[6], mul_root<T, 16, 6, true>(o[6]));
+  out[(t + G * 7) * 3 + c] = cadd(e[7], mul_root<T, 16, 7, true>(o[7]));
+}
+
+// A2 points at the first plane of the launch, whose kx is kx0.  One warp task = NPW pencils =
+// NPW/2 mirror pairs (ky, Py - ky) of one plane, which share their Nhat rows.
+template <typename T, int G>
+__global__ void __launch_bounds__(ZpCfg<T, G>::WARPS * 32, ZpCfg<T, G>::MINB)
+zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
+               const uint16_t* __restrict__ posy, int ny, int kx0, int ntask) {
+  using C = ZpCfg<T, G>;
+  constexpr int nz = C::nz, Pz = C::Pz, Q = C::Q, NPW = C::NPW;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 2 * warp;
+  Cx<T>* wbase = reinterpret_cast<Cx<T>*>(smem_raw + 128) + (size_t)warp * C::warp_elems;
+  const int t = lane % G, pw = lane / G;
+  Cx<T>* xb = wbase + 2 * NPW * Q + pw * C::XB;
+  const int Py = 2 * ny;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 2 * C::WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  Cx<T> tw[16];
+#pragma unroll
+  for (int u = 1; u < 16; ++u) tw[u] = __ldg(Wz + t * u);
+  tw[0] = mk<T>(1, 0);
+
+  const int gw = blockIdx.x * C::WARPS + warp, stride = gridDim.x * C::WARPS;
+  auto pencil_ptr = [&](int task, int p) -> Cx<T>* {
+    const int pair = task * (NPW / 2) + (p >> 1);
+    const int plane = pair / ny, i = pair - plane * ny;
+    const int ky = (p & 1) ? (i == 0 ? ny : Py - i) : i;
+    return A2 + ((size_t)plane * Py + posy[ky]) * Q;
+  };
+  auto issue = [&](int task, int stage) {
+    mbar_expect_tx(bars + stage, NPW * C::pencil_bytes);
+    for (int p = 0; p < NPW; ++p)
+      bulk_load(wbase + (stage * NPW + p) * Q, pencil_ptr(task, p), C::pencil_bytes, bars + stage);
+  };
+  if (lane == 0 && gw < ntask) issue(gw, 0);
+  int it = 0;
+  for (int task = gw; task < ntask; task += stride, ++it) {
+    const int stage = it & 1;
+    if (lane == 0) {
+      bulk_wait_read0();  // the previous task's store has finished reading the other stage
+      if (task + stride < ntask) issue(task + stride, stage ^ 1);
+    }
+    __syncwarp();
+    mbar_wait(bars + stage, (it >> 1) & 1);
+    Cx<T>* pen = wbase + (stage * NPW + pw) * Q;
+    // ---- forward
+    Cx<T> X[3][16];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) zp_forward<T, G>(pen, xb, tw, t, c, X[c]);
+    // ---- tensor multiply
+    {
+      const int pair = task * (NPW / 2) + (pw >> 1);
+      const int plane = pair / ny, i = pair - plane * ny;
+      const int kyo = (pw & 1) ? (i == 0 ? ny : i) : i;
+      const T sy = ((pw & 1) && i != 0) ? (T)-1 : (T)1;
+      const T* nrow = tab + ((size_t)(kx0 + plane) * (ny + 1) + kyo) * 6 * (nz + 1);
+#pragma unroll
+      for (int f = 0; f < 16; ++f) {
+        const int kz = C::NSUB * t + (f / G) + 16 * (f % G);
+        const bool mir = kz > nz;
+        const int idx = mir ? Pz - kz : kz;
+        const T sz = mir ? (T)-1 : (T)1;
+        const T nxx = __ldg(nrow + idx), nyy = __ldg(nrow + (nz + 1) + idx),
+                nzz = __ldg(nrow + 2 * (nz + 1) + idx), nxy = sy * __ldg(nrow + 3 * (nz + 1) + idx),
+                nxz = sz * __ldg(nrow + 4 * (nz + 1) + idx),
+                nyz = sy * sz * __ldg(nrow + 5 * (nz + 1) + idx);
+        const Cx<T> a = X[0][f], b = X[1][f], c = X[2][f];
+        X[0][f] = mk<T>(nxx * a.x + nxy * b.x + nxz * c.x, nxx * a.y + nxy * b.y + nxz * c.y);
+        X[1][f] = mk<T>(nxy * a.x + nyy * b.x + nyz * c.x, nxy * a.y + nyy * b.y + nyz * c.y);
+        X[2][f] = mk<T>(nxz * a.x + nyz * b.x + nzz * c.x, nxz * a.y + nyz * b.y + nzz * c.y);
+      }
+    }
+    // ---- inverse, in place in the staged pencil
+#pragma unroll
+    for (int c = 0; c < 3; ++c) zp_inverse<T, G>(pen, xb, tw, t, c, X[c]);
+    fence_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+      for (int p = 0; p < NPW; ++p)
+        bulk_store(pencil_ptr(task, p), wbase + (stage * NPW + p) * Q, C::pencil_bytes);
+      bulk_commit();
+    }
+  }
+  if (lane == 0) bulk_wait0();
+}
+
+// ---------------------------------------------------------------- host side
+
+bool fast_supported(int nx, int ny, int nz, size_t /*real_bytes*/) {
+  auto okxy = [](int n) { return n == 64 || n == 128 || n == 256 || n == 512 || n == 1024; };
+  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128);
+}
+
+template <typename K> static cudaError_t opt_in_smem(K kernel, int bytes) {
+  if (bytes <= 48 * 1024) return cudaSuccess;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+static int g_sm_count = 0;
+static int sm_count() {
+  if (!g_sm_count) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        g_sm_count <= 0)
+      g_sm_count = 148;
+  }
+  return g_sm_count;
+}
+
+template <typename T, int L>
+static cudaError_t launch_xf(const FastGeom& g, const FastBufs<T>& b, const T* m, cudaStream_t st) {
+  using TL = Tile<T, L>;
+  cudaError_t e = opt_in_smem(xf_fast_kernel<T, L>, TL::smem_bytes);
+  if (e != cudaSuccess) return e;
+  const size_t npairs = (size_t)g.ny * g.Q / 2;
+  xf_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), kStrideThreads, TL::smem_bytes, st>>>(
+      reinterpret_cast<const Cx<T>*>(m), b.A1, b.Wx, b.posx, npairs);
+  return cudaSuccess;
+}
+template <typename T, int L>
+static cudaError_t launch_xi(const FastGeom& g, const FastBufs<T>& b, T* H, T scale, cudaStream_t st) {
+  using TL = Tile<T, L>;
+  cudaError_t e = opt_in_smem(xi_fast_kernel<T, L>, TL::smem_bytes);
+  if (e != cudaSuccess) return e;
+  const size_t npairs = (size_t)g.ny * g.Q / 2;
+  xi_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), kStrideThreads, TL::smem_bytes, st>>>(
+      b.A1, reinterpret_cast<Cx<T>*>(H), b.Wx, b.posx, npairs, scale);
+  return cudaSuccess;
+}
+template <typename T, int L>
+static cudaError_t launch_yf(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
+  using TL = Tile<T, L>;
+  cudaError_t e = opt_in_smem(yf_fast_kernel<T, L>, TL::smem_bytes);
+  if (e != cudaSuccess) return e;
+  dim3 grid(g.Q / TL::B, nk);
+  yf_fast_kernel<T, L><<<grid, kStrideThreads, TL::smem_bytes, st>>>(
+      b.A1 + (size_t)k0 * g.ny * g.Q, b.A2, b.Wy, g.Q);
+  return cudaSuccess;
+}
+template <typename T, int L>
+static cudaError_t launch_yi(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
+  using TL = Tile<T, L>;
+  cudaError_t e = opt_in_smem(yi_fast_kernel<T, L>, TL::smem_bytes);
+  if (e != cudaSuccess) return e;
+  dim3 grid(g.Q / TL::B, nk);
+  yi_fast_kernel<T, L><<<grid, kStrideThreads, TL::smem_bytes, st>>>(
+      b.A2, b.A1 + (size_t)k0 * g.ny * g.Q, b.Wy, g.Q);
+  return cudaSuccess;
+}
+template <typename T, int G>
+static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
+  using C = ZpCfg<T, G>;
+  cudaError_t e = opt_in_smem(zp_fast_kernel<T, G>, C::smem_bytes);
+  if (e != cudaSuccess) return e;
+  const int ntask = (int)((size_t)nk * g.ny * 2 / C::NPW);
+  int grid = sm_count() * C::MINB;
+  if (grid * C::WARPS > ntask) grid = (ntask + C::WARPS - 1) / C::WARPS;
+  zp_fast_kernel<T, G><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(
+      b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask);
+  return cudaSuccess;
+}
+
+#define MM_DISPATCH_L(L, CALL)                       \
+  switch (L) {                                       \
+    case 64: e = CALL(64); break;                    \
+    case 128: e = CALL(128); break;                  \
+    case 256: e = CALL(256); break;                  \
+    case 512: e = CALL(512); break;                  \
+    case 1024: e = CALL(1024); break;                \
+    default: e = cudaErrorInvalidValue; break;       \
+  }
+
+template <typename T>
+cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
+                              cudaStream_t st, unsigned long long* launches, Prof* prof) {
+  cudaError_t e = cudaSuccess;
+  prof->mark(0, st);
+#define CALL_XF(L) launch_xf<T, L>(g, b, m, st)
+  MM_DISPATCH_L(g.nx, CALL_XF)
+#undef CALL_XF
+  if (e != cudaSuccess) return e;
+  ++*launches;
+  const int nplanes = g.nx + 1;
+  const int kc = g.kchunk > 0 ? g.kchunk : nplanes;
+  for (int k0 = 0; k0 < nplanes; k0 += kc) {
+    const int nk = nplanes - k0 < kc ? nplanes - k0 : kc;
+    prof->mark(1, st);
+#define CALL_YF(L) launch_yf<T, L>(g, b, k0, nk, st)
+    MM_DISPATCH_L(g.ny, CALL_YF)
+#undef CALL_YF
+    if (e != cudaSuccess) return e;
+    prof->mark(2, st);
+    e = g.nz == 128 ? launch_zp<T, 16>(g, b, k0, nk, st) : launch_zp<T, 8>(g, b, k0, nk, st);
+    if (e != cudaSuccess) return e;
+    prof->mark(3, st);
+#define CALL_YI(L) launch_yi<T, L>(g, b, k0, nk, st)
+    MM_DISPATCH_L(g.ny, CALL_YI)
+#undef CALL_YI
+    if (e != cudaSuccess) return e;
+    *launches += 3;
+  }
+  prof->mark(4, st);
+#define CALL_XI(L) launch_xi<T, L>(g, b, H, scale, st)
+  MM_DISPATCH_L(g.nx, CALL_XI)
+#undef CALL_XI
+  if (e != cudaSuccess) return e;
+  ++*launches;
+  prof->mark(-1, st);
+  return cudaGetLastError();
+}
+
+template cudaError_t demag_fast_launch<float>(const FastGeom&, const FastBufs<float>&, const float*,
+                                              float*, float, cudaStream_t, unsigned long long*, Prof*);
+template cudaError_t demag_fast_launch<double>(const FastGeom&, const FastBufs<double>&,
+                                               const double*, double*, double, cudaStream_t,
+                                               unsigned long long*, Prof*);
+
+}  // namespace mm

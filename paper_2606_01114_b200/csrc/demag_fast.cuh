@@ -1,0 +1,43 @@
+// Fast demag path ("x-first"): geometry, buffers and the host launcher.
+//
+// Same operation as demag_passes.cu (PAPER.md:45 eq. 4, :47, :53: zero-padded FFT of m, pointwise
+// multiply with the Fourier-space demag tensor, inverse FFT, crop) but with the axes visited in
+// the order x (r2c) -> y -> z.Nhat.z^-1 -> y^-1 -> x^-1 (c2r), which on the [x][y][z][3] state
+// layout makes every pass coalesced without any transposition and puts the
+// shortest transforms on the largest (fully padded) data.  See DESIGN.md section 5.
+#pragma once
+#include "mm_common.cuh"
+
+namespace mm {
+
+struct FastGeom {
+  int nx, ny, nz;
+  int Px, Py, Pz;  // 2 n_d
+  int Q;           // complex columns per (kx, y) row: 3 nz
+  int kchunk;      // kx planes per launch of K2..K4 (0 = all nx + 1 planes at once)
+};
+
+// true if the fast kernels cover this mesh (otherwise the generic path of demag_passes.cu runs)
+bool fast_supported(int nx, int ny, int nz, size_t real_bytes);
+
+template <typename T> struct FastBufs {
+  const Cx<T>* Wx;        // Wx[q] = exp(-2 pi i q / Px), q < Px
+  const Cx<T>* Wy;        // ... / Py
+  const Cx<T>* Wz;        // ... / Pz
+  const uint16_t* posx;   // shared-memory row (swizzled) of x frequency k in the K1/K5 tile, k < Px
+  const uint16_t* posy;   // row of y frequency k in A2, k < Py
+  const T* table;         // Nhat[kx <= nx][ky <= ny][6][kz <= nz], scaled by -1/(Px Py Pz) parity sign
+  Cx<T>* A1;              // [nx + 1][ny][Q]
+  Cx<T>* A2;              // [kchunk planes][Py][Q] (rows in digit-reversed ky order), reused by every chunk
+};
+
+// Enqueues K1..K5: H := scale * crop(IFFT(table . FFT(pad(m)))).
+template <typename T>
+cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
+                              cudaStream_t st, unsigned long long* launches, Prof* prof);
+
+// Host helpers for the tables above (plan order of the fast kernels).
+int fast_pos_logical(int L, int k);   // row of frequency k < 2L in the [even half | odd half] layout
+int fast_swizzle(int L, int row);     // shared-memory row of logical row
+
+}  // namespace mm

@@ -174,12 +174,37 @@ __global__ void unpack_table_kernel(int comp, InitGeom g, const T* __restrict__ 
   out[e] = (T)((double)v * unscale);
 }
 
+// Fast path (demag_fast.cu): the natural-order octant itself, T[kx][ky][6][kz], with the
+// (-i)^2 of the two odd axes and the normalisation folded in; the mirror signs are applied
+// by the z pass.
+template <typename T>
+__global__ void pack_fast_kernel(int comp, InitGeom g, const double* __restrict__ oct,
+                                 T* __restrict__ table, double scale) {
+  const size_t total = (size_t)g.ox * g.oy * g.oz;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= total) return;
+  const int kz = (int)(e % g.oz);
+  const size_t xy = e / g.oz;
+  const double v = comp >= 3 ? -oct[e] : oct[e];
+  table[(xy * 6 + comp) * g.oz + kz] = (T)(v * scale);
+}
+template <typename T>
+__global__ void unpack_fast_kernel(int comp, InitGeom g, const T* __restrict__ table,
+                                   T* __restrict__ out, double unscale) {
+  const size_t total = (size_t)g.ox * g.oy * g.oz;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= total) return;
+  const int kz = (int)(e % g.oz);
+  const size_t xy = e / g.oz;
+  out[e] = (T)((double)table[(xy * 6 + comp) * g.oz + kz] * unscale);
+}
+
 static unsigned blocks_for(size_t n, int t) { return (unsigned)((n + t - 1) / t); }
 
 template <typename T>
 cudaError_t demag_init_launch(const InitGeom& g, double dx, double dy, double dz, void* scratch,
-                              const uint16_t* fx, const uint16_t* fy, T* table, cudaStream_t st,
-                              unsigned long long* launches) {
+                              const uint16_t* fx, const uint16_t* fy, T* table, int fast,
+                              cudaStream_t st, unsigned long long* launches) {
   // scratch carve-up: F lattice (fp128) | octant ping | octant pong | trig tables
   unsigned char* p = static_cast<unsigned char*>(scratch);
   const size_t nF = (size_t)(g.nx + 2) * (g.ny + 2) * (g.nz + 2);
@@ -213,8 +238,11 @@ cudaError_t demag_init_launch(const InitGeom& g, double dx, double dy, double dz
     trig_table_kernel<<<blocks_for(g.Pz, 128), 128, 0, st>>>(g.Pz, c, s);
     parity_transform_kernel<<<blocks_for(nO, 256), 256, 0, st>>>(
         ping, pong, (size_t)g.ox * g.oy, g.nz, g.oz, 1, g.Pz, odd[comp][2], c, s);
-    pack_table_kernel<T><<<blocks_for((size_t)g.Kz * g.Py * g.Px, 256), 256, 0, st>>>(
-        comp, g, pong, fx, fy, table, scale);
+    if (fast)
+      pack_fast_kernel<T><<<blocks_for(nO, 256), 256, 0, st>>>(comp, g, pong, table, scale);
+    else
+      pack_table_kernel<T><<<blocks_for((size_t)g.Kz * g.Py * g.Px, 256), 256, 0, st>>>(
+          comp, g, pong, fx, fy, table, scale);
     *launches += 7;
   }
   return cudaGetLastError();
@@ -228,29 +256,33 @@ size_t demag_init_scratch_bytes(const InitGeom& g) {
 
 template <typename T>
 cudaError_t demag_export_launch(const InitGeom& g, const T* table, const uint16_t* posx,
-                                const uint16_t* posy, T* out, cudaStream_t st,
+                                const uint16_t* posy, T* out, int fast, cudaStream_t st,
                                 unsigned long long* launches) {
   const size_t nO = (size_t)g.ox * g.oy * g.oz;
   const double unscale = (double)g.Px * (double)g.Py * (double)g.Pz;
   for (int comp = 0; comp < 6; ++comp) {
-    unpack_table_kernel<T><<<blocks_for(nO, 256), 256, 0, st>>>(comp, g, table, posx, posy,
-                                                                 out + comp * nO, unscale);
+    if (fast)
+      unpack_fast_kernel<T><<<blocks_for(nO, 256), 256, 0, st>>>(comp, g, table, out + comp * nO,
+                                                                 unscale);
+    else
+      unpack_table_kernel<T><<<blocks_for(nO, 256), 256, 0, st>>>(comp, g, table, posx, posy,
+                                                                   out + comp * nO, unscale);
     ++*launches;
   }
   return cudaGetLastError();
 }
 
 template cudaError_t demag_init_launch<float>(const InitGeom&, double, double, double, void*,
-                                              const uint16_t*, const uint16_t*, float*,
+                                              const uint16_t*, const uint16_t*, float*, int,
                                               cudaStream_t, unsigned long long*);
 template cudaError_t demag_init_launch<double>(const InitGeom&, double, double, double, void*,
-                                               const uint16_t*, const uint16_t*, double*,
+                                               const uint16_t*, const uint16_t*, double*, int,
                                                cudaStream_t, unsigned long long*);
 template cudaError_t demag_export_launch<float>(const InitGeom&, const float*, const uint16_t*,
-                                                const uint16_t*, float*, cudaStream_t,
+                                                const uint16_t*, float*, int, cudaStream_t,
                                                 unsigned long long*);
 template cudaError_t demag_export_launch<double>(const InitGeom&, const double*, const uint16_t*,
-                                                 const uint16_t*, double*, cudaStream_t,
+                                                 const uint16_t*, double*, int, cudaStream_t,
                                                  unsigned long long*);
 
 }  // namespace mm

@@ -15,15 +15,16 @@ struct InitGeom {
 size_t demag_init_scratch_bytes(const InitGeom& g);
 
 // fx[pos] / fy[pos]: frequency held at position pos of the digit-reversed x / y transform.
+// fast != 0: pack the natural-order octant T[kx][ky][6][kz] for demag_fast.cu instead.
 template <typename T>
 cudaError_t demag_init_launch(const InitGeom& g, double dx, double dy, double dz, void* scratch,
-                              const uint16_t* fx, const uint16_t* fy, T* table, cudaStream_t st,
-                              unsigned long long* launches);
+                              const uint16_t* fx, const uint16_t* fy, T* table, int fast,
+                              cudaStream_t st, unsigned long long* launches);
 
 // posx[k] / posy[k]: position of frequency k.  out: [6][ox][oy][oz], unscaled.
 template <typename T>
 cudaError_t demag_export_launch(const InitGeom& g, const T* table, const uint16_t* posx,
-                                const uint16_t* posy, T* out, cudaStream_t st,
+                                const uint16_t* posy, T* out, int fast, cudaStream_t st,
                                 unsigned long long* launches);
 
 }  // namespace mm

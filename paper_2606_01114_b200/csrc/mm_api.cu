@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "../../include/mm_b200.h"
+#include "demag_fast.cuh"
 #include "demag_init.cuh"
 #include "demag_passes.cuh"
 #include "fft_core.cuh"
@@ -33,7 +34,10 @@ struct mm_ctx {
   // plan
   DemagGeom geom{};
   InitGeom igeom{};
-  bool tiles_locked = false;
+  FastGeom fgeom{};
+  bool fast = false;     // the x-first kernels of demag_fast.cu cover this mesh and are selected
+  int path_pref = 0;     // 0 auto, 1 generic (demag_passes.cu), 2 fast required
+  int kchunk = 0;        // kx planes per K2..K4 launch group (0 = all)
   int want_bz = 0, want_by = 0, want_bk = 0;
   // workspaces
   unsigned char* pers = nullptr;
@@ -92,9 +96,17 @@ static void plan_layout(mm_ctx* c) {
   ig.oy = c->ny == 1 ? 1 : c->ny + 1;
   ig.oz = c->nz == 1 ? 1 : c->nz + 1;
   ig.Bk = g.Bk;
+  c->fast = c->path_pref != 1 && fast_supported(c->nx, c->ny, c->nz, c->es);
+  FastGeom& fg = c->fgeom;
+  fg.nx = c->nx; fg.ny = c->ny; fg.nz = c->nz;
+  fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;
+  fg.Q = 3 * c->nz;
+  fg.kchunk = (c->kchunk > 0 && c->kchunk < c->nx + 1) ? c->kchunk : 0;
   // persistent
   size_t o = 0;
-  c->off_table = o; o += align256((size_t)g.Kz * g.Py * g.Px * 6 * c->es);
+  c->off_table = o;
+  o += c->fast ? align256((size_t)ig.ox * ig.oy * ig.oz * 6 * c->es)
+               : align256((size_t)g.Kz * g.Py * g.Px * 6 * c->es);
   c->off_wx = o; o += align256((size_t)g.Px * cs);
   c->off_wy = o; o += align256((size_t)g.Py * cs);
   c->off_wz = o; o += align256((size_t)g.Pz * cs);
@@ -107,8 +119,14 @@ static void plan_layout(mm_ctx* c) {
   // scratch
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
   o = 0;
-  c->off_a1 = o; o += align256((size_t)3 * g.Kz * g.ny * g.nx * cs);
-  c->off_a2 = o; o += align256((size_t)3 * g.Kz * g.Py * g.nx * cs);
+  if (c->fast) {
+    const size_t planes2 = fg.kchunk ? fg.kchunk : c->nx + 1;
+    c->off_a1 = o; o += align256((size_t)(c->nx + 1) * g.ny * fg.Q * cs);
+    c->off_a2 = o; o += align256(planes2 * g.Py * fg.Q * cs);
+  } else {
+    c->off_a1 = o; o += align256((size_t)3 * g.Kz * g.ny * g.nx * cs);
+    c->off_a2 = o; o += align256((size_t)3 * g.Kz * g.Py * g.nx * cs);
+  }
   const size_t spectra = o;
   c->off_hd = o; o += align256(n3);
   c->off_msa = o; o += align256(n3);
@@ -159,7 +177,7 @@ mm_status mm_ctx_set_stream(mm_ctx* ctx, void* cuda_stream) {
 
 mm_status mm_ctx_set_tiles(mm_ctx* ctx, int bz, int by, int bk) {
   if (!ctx) return MM_ERR_INVALID_ARG;
-  if (ctx->demag_ready) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: call before mm_demag_init");
+  if (ctx->pers) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: call before mm_ctx_set_workspace");
   const int v[3] = {bz, by, bk};
   for (int i = 0; i < 3; ++i)
     if (v[i] < 0 || (v[i] > 0 && !pow2(v[i])) || v[i] > 64)
@@ -175,6 +193,27 @@ mm_status mm_ctx_set_tiles(mm_ctx* ctx, int bz, int by, int bk) {
     plan_layout(ctx);
     return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: tile exceeds 227 KB of shared memory");
   }
+  return MM_OK;
+}
+
+mm_status mm_ctx_set_path(mm_ctx* ctx, int path, int kchunk) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (ctx->pers) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: call before mm_ctx_set_workspace");
+  if (path < 0 || path > 2 || kchunk < 0)
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: path must be 0, 1 or 2 and kchunk >= 0");
+  if (path == 2 && !fast_supported(ctx->nx, ctx->ny, ctx->nz, ctx->es))
+    return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_path: the fast kernels do not cover %dx%dx%d",
+                ctx->nx, ctx->ny, ctx->nz);
+  ctx->path_pref = path;
+  ctx->kchunk = kchunk;
+  plan_layout(ctx);
+  return MM_OK;
+}
+
+mm_status mm_ctx_path(const mm_ctx* ctx, int* fast, int* kchunk) {
+  if (!ctx || !fast || !kchunk) return MM_ERR_INVALID_ARG;
+  *fast = ctx->fast ? 1 : 0;
+  *kchunk = ctx->fgeom.kchunk;
   return MM_OK;
 }
 
@@ -298,12 +337,12 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   for (int k = 0; k < g.Pz; ++k) u16(c->off_posz)[k] = (uint16_t)pos_of_freq(g.pz, k);
   for (int k = 0; k < g.Px; ++k) {
     const int p = pos_of_freq(g.px, k);
-    u16(c->off_posx)[k] = (uint16_t)p;
+    u16(c->off_posx)[k] = (uint16_t)(c->fast ? fast_swizzle(c->nx, fast_pos_logical(c->nx, k)) : p);
     u16(c->off_fx)[p] = (uint16_t)k;
   }
   for (int k = 0; k < g.Py; ++k) {
     const int p = pos_of_freq(g.py, k);
-    u16(c->off_posy)[k] = (uint16_t)p;
+    u16(c->off_posy)[k] = (uint16_t)(c->fast ? fast_pos_logical(c->ny, k) : p);
     u16(c->off_fy)[p] = (uint16_t)k;
   }
   cudaError_t e = cudaMemcpyAsync(c->pers + small_off, host.data(), small_bytes,
@@ -312,7 +351,8 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   e = demag_init_launch<T>(c->igeom, c->dx, c->dy, c->dz, c->scr,
                            reinterpret_cast<const uint16_t*>(c->pers + c->off_fx),
                            reinterpret_cast<const uint16_t*>(c->pers + c->off_fy),
-                           reinterpret_cast<T*>(c->pers + c->off_table), c->stream, &c->launches);
+                           reinterpret_cast<T*>(c->pers + c->off_table), c->fast ? 1 : 0, c->stream,
+                           &c->launches);
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: launch", e);
   e = cudaStreamSynchronize(c->stream);  // also keeps `host` alive until the copy is done
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: execution", e);
@@ -361,7 +401,26 @@ static mm_status need_ready(mm_ctx* c, const char* fn, bool demag) {
   return MM_OK;
 }
 
+template <typename T> static FastBufs<T> fast_bufs_of(mm_ctx* c) {
+  FastBufs<T> b;
+  b.Wx = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wx);
+  b.Wy = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wy);
+  b.Wz = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wz);
+  b.posx = reinterpret_cast<const uint16_t*>(c->pers + c->off_posx);
+  b.posy = reinterpret_cast<const uint16_t*>(c->pers + c->off_posy);
+  b.table = reinterpret_cast<const T*>(c->pers + c->off_table);
+  b.A1 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a1);
+  b.A2 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a2);
+  return b;
+}
+
 template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H) {
+  if (c->fast) {
+    cudaError_t e = demag_fast_launch<T>(c->fgeom, fast_bufs_of<T>(c), static_cast<const T*>(m),
+                                         static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches,
+                                         &c->prof);
+    return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag (fast path) launch", e);
+  }
   cudaError_t e = demag_field_launch<T>(c->geom, bufs_of<T>(c), static_cast<const T*>(m),
                                         static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches,
                                         &c->prof);
@@ -421,10 +480,12 @@ mm_status mm_demag_nhat_export(mm_ctx* ctx, void* out) {
   cudaError_t e;
   if (ctx->dtype == MM_F32)
     e = demag_export_launch<float>(ctx->igeom, reinterpret_cast<const float*>(ctx->pers + ctx->off_table),
-                                   posx, posy, static_cast<float*>(out), ctx->stream, &ctx->launches);
+                                   posx, posy, static_cast<float*>(out), ctx->fast ? 1 : 0, ctx->stream,
+                                   &ctx->launches);
   else
     e = demag_export_launch<double>(ctx->igeom, reinterpret_cast<const double*>(ctx->pers + ctx->off_table),
-                                    posx, posy, static_cast<double*>(out), ctx->stream, &ctx->launches);
+                                    posx, posy, static_cast<double*>(out), ctx->fast ? 1 : 0, ctx->stream,
+                                    &ctx->launches);
   return e == cudaSuccess ? MM_OK : cuda_fail(ctx, "mm_demag_nhat_export", e);
 }
 

@@ -49,14 +49,27 @@ def test_create_validates_arguments(lib):
 
 
 def test_workspace_sizes_match_design(lib):
-    """Config 4 fp32: table 6*129*1024*1024*4 B, spectra 3*129*(512+1024)*512*8 B."""
-    h = C.c_void_p()
-    assert lib.mm_ctx_create(512, 512, 128, 4e-9, 4e-9, 4e-9, 0, C.byref(h)) == 0
-    p, s = C.c_size_t(), C.c_size_t()
-    lib.mm_ctx_workspace_bytes(h, C.byref(p), C.byref(s))
-    table = 6 * 129 * 1024 * 1024 * 4
-    spectra = 3 * 129 * (512 + 1024) * 512 * 8
+    """Config 4 fp32.  Generic passes: table 6*129*1024*1024*4 B, spectra 3*129*(512+1024)*512*8 B.
+    Fast path (selected automatically): octant table 6*513*513*129*4 B, A1 513*512*384*8 B,
+    A2 = kchunk (or 513) planes of 1024*384*8 B."""
     fields = 6 * 512 * 512 * 128 * 3 * 4
-    assert table <= p.value < table + (1 << 20)
-    assert spectra + fields <= s.value < spectra + fields + (1 << 20)
+    p, s = C.c_size_t(), C.c_size_t()
+    fast, kc = C.c_int(), C.c_int()
+    for path, kchunk, table, spectra in (
+            (1, 0, 6 * 129 * 1024 * 1024 * 4, 3 * 129 * (512 + 1024) * 512 * 8),
+            (0, 0, 6 * 513 * 513 * 129 * 4, 513 * 512 * 384 * 8 + 513 * 1024 * 384 * 8),
+            (2, 16, 6 * 513 * 513 * 129 * 4, 513 * 512 * 384 * 8 + 16 * 1024 * 384 * 8)):
+        h = C.c_void_p()
+        assert lib.mm_ctx_create(512, 512, 128, 4e-9, 4e-9, 4e-9, 0, C.byref(h)) == 0
+        assert lib.mm_ctx_set_path(h, path, kchunk) == 0
+        lib.mm_ctx_workspace_bytes(h, C.byref(p), C.byref(s))
+        assert table <= p.value < table + (1 << 20)
+        assert spectra + fields <= s.value < spectra + fields + (1 << 20)
+        assert lib.mm_ctx_path(h, C.byref(fast), C.byref(kc)) == 0
+        assert fast.value == (0 if path == 1 else 1) and kc.value == kchunk
+        lib.mm_ctx_destroy(h)
+    h = C.c_void_p()
+    assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 0, C.byref(h)) == 0
+    assert lib.mm_ctx_set_path(h, 2, 0) == 2          # fast kernels do not cover thin films
+    assert lib.mm_ctx_set_path(h, 3, 0) == 1
     lib.mm_ctx_destroy(h)

@@ -1,0 +1,68 @@
+"""The x-first fast demag kernels (demag_fast.cu, K1..K5) against the oracle and against the
+generic z-first passes, through the C ABI: several tiles per pass, every supported radix plan,
+chunked and unchunked plane groups (with a ragged last chunk)."""
+import numpy as np
+import pytest
+
+import workloads as w
+from gpu_util import TOL, make_ctx, make_problem, round_input, to_dev
+
+pytestmark = pytest.mark.gpu
+
+MESHES = [(64, 64, 64), (128, 64, 64), (64, 256, 128), (256, 128, 64), (64, 64, 128)]
+
+
+def cfg_for(n, d=(4e-9, 3e-9, 2e-9)):
+    base = w.get_config(1)
+    return w.Config(**{**base.__dict__, "n": n, "d": d, "name": "t"})
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n", MESHES)
+def test_fast_demag_vs_oracle_fft(oracle, n, dt):
+    cfg = cfg_for(n)
+    m, m64 = round_input(w.random_unit_vectors(404, n), dt)
+    P = make_problem(oracle, cfg, terms=1)
+    ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
+    md = to_dev(m)
+    results = []
+    for kchunk in (0, 7):
+        ctx = make_ctx(cfg, dt, terms=1, path=2, kchunk=kchunk)
+        assert ctx.path == (True, kchunk)
+        got = ctx.demag_field(md).cpu().numpy()
+        l2, mx = w.field_errors(got, ref)
+        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (kchunk, l2, mx)
+        assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())      # deterministic
+        results.append(got)
+        ctx.close()
+    assert np.array_equal(results[0], results[1])                           # chunking changes nothing
+    # the generic passes agree with the fast kernels to rounding
+    ctx = make_ctx(cfg, dt, terms=1, path=1)
+    assert ctx.path[0] is False
+    l2, mx = w.field_errors(ctx.demag_field(md).cpu().numpy(), results[0])
+    assert l2 <= TOL[dt], (l2, mx)
+    ctx.close()
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+def test_fast_nhat_export(oracle, dt):
+    n, d = (64, 64, 64), (4e-9, 3e-9, 2e-9)
+    ctx = make_ctx(cfg_for(n, d), dt, terms=1, path=2)
+    got = ctx.nhat_export().cpu().numpy().astype(np.float64)
+    Nhat = oracle.demag_fft_nhat(oracle.newell_octant(n, d))
+    ref = Nhat[:, :n[0] + 1, :n[1] + 1, :n[2] + 1]
+    assert np.max(np.abs(got - ref)) < (5e-14 if dt == "f64" else 2e-7)
+
+
+def test_fast_vs_direct_sum_sampled(oracle):
+    """No FFT on the reference side: sampled O(n) direct sums on a 64x64x64 mesh, fp64."""
+    n, d = (64, 64, 64), (5e-9, 5e-9, 3e-9)
+    cfg = cfg_for(n, d)
+    m, m64 = round_input(w.random_unit_vectors(505, n), "f64")
+    N = oracle.newell_octant(n, d)
+    cells = w.sample_cells(9, n, 60)
+    ref = oracle.demag_direct_sampled(N, cfg.Ms, m64, cells)
+    ctx = make_ctx(cfg, "f64", terms=1, path=2)
+    got = ctx.demag_field(to_dev(m)).cpu().numpy().reshape(-1, 3)[cells]
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL["f64"], (l2, mx)
