@@ -98,14 +98,20 @@ class ClockSampler:
 
 # ------------------------------------------------------------------ byte model
 
-def byte_model(n, s):
-    """Algorithmic bytes per evaluation and per kernel (exact form)."""
+def byte_model(n, s, fast=False):
+    """Algorithmic bytes per evaluation and per kernel (exact form).
+    The half-spectrum axis is z (nz + 1 planes) in the generic passes, x (nx + 1 planes) in the
+    x-first fast kernels; the model is the same 84 s B/cell otherwise."""
     nx, ny, nz = n
     ncell = nx * ny * nz
     Kz = 1 if nz == 1 else nz + 1
     Py = 1 if ny == 1 else 2 * ny
-    a1 = 3 * nx * ny * Kz * 2 * s
-    a2 = 3 * nx * Py * Kz * 2 * s
+    if fast:
+        a1 = 3 * (nx + 1) * ny * nz * 2 * s
+        a2 = 3 * (nx + 1) * Py * nz * 2 * s
+    else:
+        a1 = 3 * nx * ny * Kz * 2 * s
+        a2 = 3 * nx * Py * Kz * 2 * s
     octant = 6 * (nx + 1) * (ny + 1) * Kz * s
     k = {"S1_zf": 3 * ncell * s + a1, "S2_yf": a1 + a2, "S3_xp": 2 * a2 + octant,
          "S4_yi": a2 + a1, "S5_zi": a1 + 3 * ncell * s, "S6_pointwise": 9 * ncell * s}
@@ -200,7 +206,7 @@ def run_ours(args, cfg):
 
     tdt = torch.float32 if args.dtype == "f32" else torch.float64
     s = 4 if args.dtype == "f32" else 8
-    ctx = Context(cfg.n, cfg.d, dtype=tdt, device=f"cuda:{local}")
+    ctx = Context(cfg.n, cfg.d, dtype=tdt, device=f"cuda:{local}", path=args.path, kchunk=args.kchunk)
     ctx.set_material(cfg.Ms, cfg.Aex, cfg.Ku, cfg.axis, cfg.alpha, cfg.gamma)
     ctx.set_zeeman(cfg.Hext)
     ctx.set_terms(cfg.terms)
@@ -267,7 +273,7 @@ def run_ours(args, cfg):
         return 0
 
     ncell = cfg.ncell
-    kbytes, total_bytes = byte_model(cfg.n, s)
+    kbytes, total_bytes = byte_model(cfg.n, s, fast=ctx.path[0])
     peak, peak_src = measured_peak()
     per_kernel = {}
     for k, (tot, cnt) in ktimes.items():
@@ -329,6 +335,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic passes, 2 fast kernels (experiments)")
+    ap.add_argument("--kchunk", type=int, default=0, help="kx planes per y/z/y launch group (experiments)")
     ap.add_argument("--mesh", default=None, help="override mesh, e.g. 256x256x64 (experiments)")
     args = ap.parse_args()
     cfg = w.get_config(4)
