@@ -418,27 +418,33 @@ __device__ __forceinline__ void fence_async_smem() {
 
 template <typename T, int G> struct ZpCfg {
   static constexpr int nz = 8 * G, Pz = 16 * G, Q = 3 * nz;
-  static constexpr int NPW = 32 / G;        // pencils per warp
+  static constexpr int OZP = nz + 2;        // kz pitch of a table row (InitGeom::ozp)
+  static constexpr int NPW = 32 / G;        // pencils per warp task
   static constexpr int NSUB = 16 / G;       // second-stage sub-transforms per lane
   static constexpr int PITCH = G + 1;       // exchange row pitch (conflict-free transposition)
-  static constexpr int XB = 16 * PITCH;     // exchange elements per pencil
+  static constexpr int XB = 16 * PITCH;     // exchange elements per pencil (aliases the pencil)
   static constexpr int WARPS = sizeof(T) == 4 ? 4 : 2;
   static constexpr int MINB = 3;
   static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
-  static constexpr int warp_elems = 2 * NPW * Q + NPW * XB;  // two stages of pencils + exchange
-  static constexpr int smem_bytes = 128 + WARPS * warp_elems * (int)sizeof(Cx<T>);
+  static constexpr int table_bytes = 6 * OZP * (int)sizeof(T);  // one (kx, ky) row, 16 B multiple
+  // per warp: two stages of NPW pencils + the table rows of the NPW / 2 mirror pairs + one slot
+  // for the row ky = ny (the partner of ky = 0, the only pair that does not share its row)
+  static constexpr int warp_bytes = 2 * NPW * pencil_bytes + (NPW / 2 + 1) * table_bytes;
+  static constexpr int smem_bytes = 128 + WARPS * warp_bytes;
+  static_assert(XB <= Q, "exchange buffer must fit in the pencil it aliases");
+  static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0, "bulk copies need 16 B multiples");
 };
 
-// Forward z transform of one component of one pencil: in = pencil (component-interleaved),
-// X[i G + v] = spectrum at kz = NSUB t + i + 16 v.
+// Forward z transform of one component of one pencil.  a[j] = sample z = t + G j (j < 8; the
+// samples j >= 8 are the zero padding).  X[i G + v] = spectrum at kz = NSUB t + i + 16 v.
 template <typename T, int G>
-__device__ __forceinline__ void zp_forward(const Cx<T>* in, Cx<T>* xb, const Cx<T>* tw, int t, int c,
+__device__ __forceinline__ void zp_forward(const Cx<T>* a, Cx<T>* xb, const Cx<T>* tw, int t,
                                            Cx<T>* X) {
   using C = ZpCfg<T, G>;
   Cx<T> e[8], o[8];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) e[j] = in[(t + G * j) * 3 + c];
-  // pruned radix 16 (inputs 8..15 are the zero padding): even outputs = DFT8(a), odd = DFT8(a w16^j)
+  for (int j = 0; j < 8; ++j) e[j] = a[j];
+  // pruned radix 16: even outputs = DFT8(a), odd outputs = DFT8(a w16^j)
   o[0] = e[0];
   o[1] = mul_root<T, 16, 1, false>(e[1]);
   o[2] = mul_root<T, 16, 2, false>(e[2]);
@@ -468,9 +474,9 @@ __device__ __forceinline__ void zp_forward(const Cx<T>* in, Cx<T>* xb, const Cx<
   __syncwarp();
 }
 
-// Mirror image: X -> truncated samples written to out (component-interleaved pencil).
+// Mirror image: X -> the 8 truncated samples z = t + G j of this lane, in r[j].
 template <typename T, int G>
-__device__ __forceinline__ void zp_inverse(Cx<T>* out, Cx<T>* xb, const Cx<T>* tw, int t, int c,
+__device__ __forceinline__ void zp_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw, int t,
                                            const Cx<T>* X) {
   using C = ZpCfg<T, G>;
 #pragma unroll
@@ -493,33 +499,59 @@ __device__ __forceinline__ void zp_inverse(Cx<T>* out, Cx<T>* xb, const Cx<T>* t
   __syncwarp();
   Dft<T, 8, true>::run(e);
   Dft<T, 8, true>::run(o);
-  out[t * 3 + c] = cadd(e[0], o[0]);
-  out[(t + G * 1) * 3 + c] = cadd(e[1], mul_root<T, 16, 1, true>(o[1]));
-  out[(t + G * 2) * 3 + c] = cadd(e[2], mul_root<T, 16, 2, true>(o[2]));
-  out[(t + G * 3) * 3 + c] = cadd(e[3], mul_root<T, 16, 3, true>(o[3]));
-  out[(t + G * 4) * 3 + c] = cadd(e[4], mul_root<T, 16, 4, true>(o[4]));
-  out[(t + G * 5) * 3 + c] = cadd(e[5], mul_root<T, 16, 5, true>(o[5]));
-  out[(t + G * 6) * 3 + c] = cadd(e[6], mul_root<T, 16, 6, true>(o[6]));
-  out[(t + G * 7) * 3 + c] = cadd(e[7], mul_root<T, 16, 7, true>(o[7]));
+  r[0] = cadd(e[0], o[0]);
+  r[1] = cadd(e[1], mul_root<T, 16, 1, true>(o[1]));
+  r[2] = cadd(e[2], mul_root<T, 16, 2, true>(o[2]));
+  r[3] = cadd(e[3], mul_root<T, 16, 3, true>(o[3]));
+  r[4] = cadd(e[4], mul_root<T, 16, 4, true>(o[4]));
+  r[5] = cadd(e[5], mul_root<T, 16, 5, true>(o[5]));
+  r[6] = cadd(e[6], mul_root<T, 16, 6, true>(o[6]));
+  r[7] = cadd(e[7], mul_root<T, 16, 7, true>(o[7]));
+}
+
+// Hhat = Nhat mhat at the 16 frequencies of this lane.  trow: the (kx, ky) table row in shared
+// memory, [6][OZP]; sy = -1 on the mirrored ky half (N_xy, N_yz are odd in ky), the kz mirror
+// (N_xz, N_yz odd in kz) is resolved per frequency.
+template <typename T, int G>
+__device__ __forceinline__ void zp_multiply(const T* trow, int t, T sy, Cx<T>* X0, Cx<T>* X1,
+                                            Cx<T>* X2) {
+  using C = ZpCfg<T, G>;
+#pragma unroll
+  for (int f = 0; f < 16; ++f) {
+    const int kz = C::NSUB * t + (f / G) + 16 * (f % G);
+    const bool mir = kz > C::nz;
+    const int idx = mir ? C::Pz - kz : kz;
+    const T sz = mir ? (T)-1 : (T)1;
+    const T nxx = trow[idx], nyy = trow[C::OZP + idx], nzz = trow[2 * C::OZP + idx],
+            nxy = sy * trow[3 * C::OZP + idx], nxz = sz * trow[4 * C::OZP + idx],
+            nyz = sy * sz * trow[5 * C::OZP + idx];
+    const Cx<T> a = X0[f], b = X1[f], c = X2[f];
+    X0[f] = mk<T>(nxx * a.x + nxy * b.x + nxz * c.x, nxx * a.y + nxy * b.y + nxz * c.y);
+    X1[f] = mk<T>(nxy * a.x + nyy * b.x + nyz * c.x, nxy * a.y + nyy * b.y + nyz * c.y);
+    X2[f] = mk<T>(nxz * a.x + nyz * b.x + nzz * c.x, nxz * a.y + nyz * b.y + nzz * c.y);
+  }
 }
 
 // A2 points at the first plane of the launch, whose kx is kx0.  One warp task = NPW pencils =
-// NPW/2 mirror pairs (ky, Py - ky) of one plane, which share their Nhat rows.
+// NPW/2 mirror pairs (ky, Py - ky) of one plane, which share their Nhat rows.  Pencils and
+// table rows arrive by bulk asynchronous copies one task ahead; the pencil's own buffer is
+// the exchange buffer of its transforms once its samples sit in registers.
 template <typename T, int G>
 __global__ void __launch_bounds__(ZpCfg<T, G>::WARPS * 32, ZpCfg<T, G>::MINB)
 zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
                const uint16_t* __restrict__ posy, int ny, int kx0, int ntask) {
   using C = ZpCfg<T, G>;
-  constexpr int nz = C::nz, Pz = C::Pz, Q = C::Q, NPW = C::NPW;
+  constexpr int Q = C::Q, NPW = C::NPW;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 2 * warp;
-  Cx<T>* wbase = reinterpret_cast<Cx<T>*>(smem_raw + 128) + (size_t)warp * C::warp_elems;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 3 * warp;  // stage 0, stage 1, table
+  unsigned char* wraw = smem_raw + 128 + (size_t)warp * C::warp_bytes;
+  Cx<T>* pbase = reinterpret_cast<Cx<T>*>(wraw);
+  T* tbase = reinterpret_cast<T*>(wraw + 2 * NPW * C::pencil_bytes);
   const int t = lane % G, pw = lane / G;
-  Cx<T>* xb = wbase + 2 * NPW * Q + pw * C::XB;
   const int Py = 2 * ny;
   if (threadIdx.x == 0) {
-    for (int i = 0; i < 2 * C::WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    for (int i = 0; i < 3 * C::WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -538,54 +570,72 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
   auto issue = [&](int task, int stage) {
     mbar_expect_tx(bars + stage, NPW * C::pencil_bytes);
     for (int p = 0; p < NPW; ++p)
-      bulk_load(wbase + (stage * NPW + p) * Q, pencil_ptr(task, p), C::pencil_bytes, bars + stage);
+      bulk_load(pbase + (stage * NPW + p) * Q, pencil_ptr(task, p), C::pencil_bytes, bars + stage);
   };
-  if (lane == 0 && gw < ntask) issue(gw, 0);
+  // table rows of a task: ky = i for mirror pair i; the pair i = 0 (always the first of its
+  // task) is (ky = 0, ky = ny) and needs the row ky = ny as well, in the extra slot
+  auto issue_table = [&](int task) {
+    const int pair0 = task * (NPW / 2);
+    const int plane = pair0 / ny, i0 = pair0 - plane * ny;
+    const T* rows = tab + ((size_t)(kx0 + plane) * (ny + 1)) * 6 * C::OZP;
+    mbar_expect_tx(bars + 2, (NPW / 2 + (i0 == 0 ? 1 : 0)) * C::table_bytes);
+    for (int pp = 0; pp < NPW / 2; ++pp)
+      bulk_load(tbase + pp * 6 * C::OZP, rows + (size_t)(i0 + pp) * 6 * C::OZP, C::table_bytes, bars + 2);
+    if (i0 == 0)
+      bulk_load(tbase + (NPW / 2) * 6 * C::OZP, rows + (size_t)ny * 6 * C::OZP, C::table_bytes, bars + 2);
+  };
+  if (lane == 0 && gw < ntask) { issue(gw, 0); issue_table(gw); }
   int it = 0;
   for (int task = gw; task < ntask; task += stride, ++it) {
     const int stage = it & 1;
+    const bool more = task + stride < ntask;
     if (lane == 0) {
       bulk_wait_read0();  // the previous task's store has finished reading the other stage
-      if (task + stride < ntask) issue(task + stride, stage ^ 1);
+      if (more) issue(task + stride, stage ^ 1);
     }
     __syncwarp();
     mbar_wait(bars + stage, (it >> 1) & 1);
-    Cx<T>* pen = wbase + (stage * NPW + pw) * Q;
-    // ---- forward
+    Cx<T>* pen = pbase + (stage * NPW + pw) * Q;
     Cx<T> X[3][16];
+    {
+      Cx<T> a[3][8];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) zp_forward<T, G>(pen, xb, tw, t, c, X[c]);
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[c][j] = pen[(t + G * j) * 3 + c];
+      __syncwarp();  // every sample is in registers: the pencil buffer becomes the exchange buffer
+#pragma unroll
+      for (int c = 0; c < 3; ++c) zp_forward<T, G>(a[c], pen, tw, t, X[c]);
+    }
     // ---- tensor multiply
     {
       const int pair = task * (NPW / 2) + (pw >> 1);
-      const int plane = pair / ny, i = pair - plane * ny;
-      const int kyo = (pw & 1) ? (i == 0 ? ny : i) : i;
+      const int i = pair % ny;
+      // the odd pencil of pair i is ky = Py - i (row i, odd components negated), of pair 0 ky = ny
+      const bool nyq = (pw & 1) && i == 0;
       const T sy = ((pw & 1) && i != 0) ? (T)-1 : (T)1;
-      const T* nrow = tab + ((size_t)(kx0 + plane) * (ny + 1) + kyo) * 6 * (nz + 1);
-#pragma unroll
-      for (int f = 0; f < 16; ++f) {
-        const int kz = C::NSUB * t + (f / G) + 16 * (f % G);
-        const bool mir = kz > nz;
-        const int idx = mir ? Pz - kz : kz;
-        const T sz = mir ? (T)-1 : (T)1;
-        const T nxx = __ldg(nrow + idx), nyy = __ldg(nrow + (nz + 1) + idx),
-                nzz = __ldg(nrow + 2 * (nz + 1) + idx), nxy = sy * __ldg(nrow + 3 * (nz + 1) + idx),
-                nxz = sz * __ldg(nrow + 4 * (nz + 1) + idx),
-                nyz = sy * sz * __ldg(nrow + 5 * (nz + 1) + idx);
-        const Cx<T> a = X[0][f], b = X[1][f], c = X[2][f];
-        X[0][f] = mk<T>(nxx * a.x + nxy * b.x + nxz * c.x, nxx * a.y + nxy * b.y + nxz * c.y);
-        X[1][f] = mk<T>(nxy * a.x + nyy * b.x + nyz * c.x, nxy * a.y + nyy * b.y + nyz * c.y);
-        X[2][f] = mk<T>(nxz * a.x + nyz * b.x + nzz * c.x, nxz * a.y + nyz * b.y + nzz * c.y);
-      }
+      mbar_wait(bars + 2, it & 1);
+      const T* trow = tbase + (nyq ? NPW / 2 : (pw >> 1)) * 6 * C::OZP;
+      zp_multiply<T, G>(trow, t, sy, X[0], X[1], X[2]);
+      __syncwarp();
+      if (lane == 0 && more) issue_table(task + stride);
     }
-    // ---- inverse, in place in the staged pencil
+    // ---- inverse; the truncated samples go back into the staged pencil
+    {
+      Cx<T> r[3][8];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) zp_inverse<T, G>(pen, xb, tw, t, c, X[c]);
+      for (int c = 0; c < 3; ++c) zp_inverse<T, G>(r[c], pen, tw, t, X[c]);
+      __syncwarp();  // the last exchange has been read
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) pen[(t + G * j) * 3 + c] = r[c][j];
+    }
     fence_async_smem();
     __syncwarp();
     if (lane == 0) {
       for (int p = 0; p < NPW; ++p)
-        bulk_store(pencil_ptr(task, p), wbase + (stage * NPW + p) * Q, C::pencil_bytes);
+        bulk_store(pencil_ptr(task, p), pbase + (stage * NPW + p) * Q, C::pencil_bytes);
       bulk_commit();
     }
   }

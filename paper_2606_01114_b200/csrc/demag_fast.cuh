@@ -15,6 +15,7 @@ struct FastGeom {
   int Px, Py, Pz;  // 2 n_d
   int Q;           // complex columns per (kx, y) row: 3 nz
   int kchunk;      // kx planes per launch of K2..K4 (0 = all nx + 1 planes at once)
+  int variant;     // kernel variant bits (experiments; MM_FAST_VARIANT): 1 = K3 with rotated loops
 };
 
 // true if the fast kernels cover this mesh (otherwise the generic path of demag_passes.cu runs)
@@ -26,7 +27,7 @@ template <typename T> struct FastBufs {
   const Cx<T>* Wz;        // ... / Pz
   const uint16_t* posx;   // shared-memory row (swizzled) of x frequency k in the K1/K5 tile, k < Px
   const uint16_t* posy;   // row of y frequency k in A2, k < Py
-  const T* table;         // Nhat[kx <= nx][ky <= ny][6][kz <= nz], scaled by -1/(Px Py Pz) parity sign
+  const T* table;         // Nhat[kx <= nx][ky <= ny][6][ozp] (kz <= nz used), scaled by 1/(Px Py Pz), parity sign folded
   Cx<T>* A1;              // [nx + 1][ny][Q]
   Cx<T>* A2;              // [kchunk planes][Py][Q] (rows in digit-reversed ky order), reused by every chunk
 };

@@ -174,7 +174,8 @@ __global__ void unpack_table_kernel(int comp, InitGeom g, const T* __restrict__ 
   out[e] = (T)((double)v * unscale);
 }
 
-// Fast path (demag_fast.cu): the natural-order octant itself, T[kx][ky][6][kz], with the
+// Fast path (demag_fast.cu): the natural-order octant itself, T[kx][ky][6][ozp] (kz < oz used,
+// the pitch ozp keeps every (kx, ky) row a multiple of 16 bytes for bulk copies), with the
 // (-i)^2 of the two odd axes and the normalisation folded in; the mirror signs are applied
 // by the z pass.
 template <typename T>
@@ -186,7 +187,9 @@ __global__ void pack_fast_kernel(int comp, InitGeom g, const double* __restrict_
   const int kz = (int)(e % g.oz);
   const size_t xy = e / g.oz;
   const double v = comp >= 3 ? -oct[e] : oct[e];
-  table[(xy * 6 + comp) * g.oz + kz] = (T)(v * scale);
+  table[(xy * 6 + comp) * g.ozp + kz] = (T)(v * scale);
+  if (kz == g.oz - 1)
+    for (int z = g.oz; z < g.ozp; ++z) table[(xy * 6 + comp) * g.ozp + z] = (T)0;  // pitch padding
 }
 template <typename T>
 __global__ void unpack_fast_kernel(int comp, InitGeom g, const T* __restrict__ table,
@@ -196,7 +199,7 @@ __global__ void unpack_fast_kernel(int comp, InitGeom g, const T* __restrict__ t
   if (e >= total) return;
   const int kz = (int)(e % g.oz);
   const size_t xy = e / g.oz;
-  out[e] = (T)((double)table[(xy * 6 + comp) * g.oz + kz] * unscale);
+  out[e] = (T)((double)table[(xy * 6 + comp) * g.ozp + kz] * unscale);
 }
 
 static unsigned blocks_for(size_t n, int t) { return (unsigned)((n + t - 1) / t); }

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -95,6 +96,7 @@ static void plan_layout(mm_ctx* c) {
   ig.ox = c->nx == 1 ? 1 : c->nx + 1;
   ig.oy = c->ny == 1 ? 1 : c->ny + 1;
   ig.oz = c->nz == 1 ? 1 : c->nz + 1;
+  ig.ozp = (ig.oz + 1) / 2 * 2;
   ig.Bk = g.Bk;
   c->fast = c->path_pref != 1 && fast_supported(c->nx, c->ny, c->nz, c->es);
   FastGeom& fg = c->fgeom;
@@ -102,10 +104,11 @@ static void plan_layout(mm_ctx* c) {
   fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;
   fg.Q = 3 * c->nz;
   fg.kchunk = (c->kchunk > 0 && c->kchunk < c->nx + 1) ? c->kchunk : 0;
+  { const char* v = getenv("MM_FAST_VARIANT"); fg.variant = v ? atoi(v) : 0; }
   // persistent
   size_t o = 0;
   c->off_table = o;
-  o += c->fast ? align256((size_t)ig.ox * ig.oy * ig.oz * 6 * c->es)
+  o += c->fast ? align256((size_t)ig.ox * ig.oy * ig.ozp * 6 * c->es)
                : align256((size_t)g.Kz * g.Py * g.Px * 6 * c->es);
   c->off_wx = o; o += align256((size_t)g.Px * cs);
   c->off_wy = o; o += align256((size_t)g.Py * cs);
