@@ -50,15 +50,15 @@ def test_create_validates_arguments(lib):
 
 def test_workspace_sizes_match_design(lib):
     """Config 4 fp32.  Generic passes: table 6*129*1024*1024*4 B, spectra 3*129*(512+1024)*512*8 B.
-    Fast path (selected automatically): octant table 6*513*513*129*4 B, A1 513*512*384*8 B,
+    Fast path (selected automatically): octant table 6*513*513*130*4 B (kz pitch nz+2: 16-byte rows for bulk copies), A1 513*512*384*8 B,
     A2 = kchunk (or 513) planes of 1024*384*8 B."""
     fields = 6 * 512 * 512 * 128 * 3 * 4
     p, s = C.c_size_t(), C.c_size_t()
     fast, kc = C.c_int(), C.c_int()
     for path, kchunk, table, spectra in (
             (1, 0, 6 * 129 * 1024 * 1024 * 4, 3 * 129 * (512 + 1024) * 512 * 8),
-            (0, 0, 6 * 513 * 513 * 129 * 4, 513 * 512 * 384 * 8 + 513 * 1024 * 384 * 8),
-            (2, 16, 6 * 513 * 513 * 129 * 4, 513 * 512 * 384 * 8 + 16 * 1024 * 384 * 8)):
+            (0, 0, 6 * 513 * 513 * 130 * 4, 513 * 512 * 384 * 8 + 513 * 1024 * 384 * 8),
+            (2, 16, 6 * 513 * 513 * 130 * 4, 513 * 512 * 384 * 8 + 16 * 1024 * 384 * 8)):
         h = C.c_void_p()
         assert lib.mm_ctx_create(512, 512, 128, 4e-9, 4e-9, 4e-9, 0, C.byref(h)) == 0
         assert lib.mm_ctx_set_path(h, path, kchunk) == 0
