@@ -734,9 +734,14 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
                               cudaStream_t st, unsigned long long* launches, Prof* prof) {
   cudaError_t e = cudaSuccess;
   prof->mark(0, st);
+  if (b.two_x) {
+    if constexpr (sizeof(T) == 4) e = strided2_launch<T>(0, g, b, m, H, scale, 0, 0, st);
+    else e = cudaErrorInvalidValue;
+  } else {
 #define CALL_XF(L) launch_xf<T, L>(g, b, m, st)
-  MM_DISPATCH_L(g.nx, CALL_XF)
+    MM_DISPATCH_L(g.nx, CALL_XF)
 #undef CALL_XF
+  }
   if (e != cudaSuccess) return e;
   ++*launches;
   const int nplanes = g.nx + 1;
@@ -744,24 +749,39 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   for (int k0 = 0; k0 < nplanes; k0 += kc) {
     const int nk = nplanes - k0 < kc ? nplanes - k0 : kc;
     prof->mark(1, st);
+    if (b.two_y) {
+      if constexpr (sizeof(T) == 4) e = strided2_launch<T>(1, g, b, m, H, scale, k0, nk, st);
+      else e = cudaErrorInvalidValue;
+    } else {
 #define CALL_YF(L) launch_yf<T, L>(g, b, k0, nk, st)
-    MM_DISPATCH_L(g.ny, CALL_YF)
+      MM_DISPATCH_L(g.ny, CALL_YF)
 #undef CALL_YF
+    }
     if (e != cudaSuccess) return e;
     prof->mark(2, st);
     e = g.nz == 128 ? launch_zp<T, 16>(g, b, k0, nk, st) : launch_zp<T, 8>(g, b, k0, nk, st);
     if (e != cudaSuccess) return e;
     prof->mark(3, st);
+    if (b.two_y) {
+      if constexpr (sizeof(T) == 4) e = strided2_launch<T>(3, g, b, m, H, scale, k0, nk, st);
+      else e = cudaErrorInvalidValue;
+    } else {
 #define CALL_YI(L) launch_yi<T, L>(g, b, k0, nk, st)
-    MM_DISPATCH_L(g.ny, CALL_YI)
+      MM_DISPATCH_L(g.ny, CALL_YI)
 #undef CALL_YI
+    }
     if (e != cudaSuccess) return e;
     *launches += 3;
   }
   prof->mark(4, st);
+  if (b.two_x) {
+    if constexpr (sizeof(T) == 4) e = strided2_launch<T>(4, g, b, m, H, scale, 0, 0, st);
+    else e = cudaErrorInvalidValue;
+  } else {
 #define CALL_XI(L) launch_xi<T, L>(g, b, H, scale, st)
-  MM_DISPATCH_L(g.nx, CALL_XI)
+    MM_DISPATCH_L(g.nx, CALL_XI)
 #undef CALL_XI
+  }
   if (e != cudaSuccess) return e;
   ++*launches;
   prof->mark(-1, st);

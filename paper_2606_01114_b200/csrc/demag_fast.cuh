@@ -27,6 +27,9 @@ template <typename T> struct FastBufs {
   const Cx<T>* Wz;        // ... / Pz
   const uint16_t* posx;   // shared-memory row (swizzled) of x frequency k in the K1/K5 tile, k < Px
   const uint16_t* posy;   // row of y frequency k in A2, k < Py
+  const Cx<T>* T2x;       // two-stage plan of the x axis: T2x[bf K1 + k1] = exp(-2 pi i bf k1 / Px) (or unused)
+  const Cx<T>* T2y;       // ... of the y axis
+  bool two_x, two_y;      // the axis runs the two-stage kernels of demag_fast2.cu (natural frequency order)
   const T* table;         // Nhat[kx <= nx][ky <= ny][6][ozp] (kz <= nz used), scaled by 1/(Px Py Pz), parity sign folded
   Cx<T>* A1;              // [nx + 1][ny][Q]
   Cx<T>* A2;              // [kchunk planes][Py][Q] (rows in digit-reversed ky order), reused by every chunk
@@ -36,6 +39,14 @@ template <typename T> struct FastBufs {
 template <typename T>
 cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
                               cudaStream_t st, unsigned long long* launches, Prof* prof);
+
+// Two-stage strided passes (demag_fast2.cu).  which: 0 = K1 (x forward), 1 = K2 (y forward),
+// 3 = K4 (y inverse), 4 = K5 (x inverse); k0, nk: first plane and plane count for K2 / K4.
+template <typename T>
+cudaError_t strided2_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
+                            int k0, int nk, cudaStream_t st);
+bool fast_two_stage(int L, size_t real_bytes);   // the two-stage kernels cover length L in this precision
+void fast2_plan(int L, int* K1, int* K2);        // P = 2L = K1 K2
 
 // Host helpers for the tables above (plan order of the fast kernels).
 int fast_pos_logical(int L, int k);   // row of frequency k < 2L in the [even half | odd half] layout

@@ -1,0 +1,376 @@
+// Two-stage strided passes of the fast demag path (K1, K2, K4, K5 of demag_fast.cu for
+// transform lengths L <= 512).
+//
+// The pruned length-P transform (P = 2L = K1 K2, L non-zero inputs; "zero-padding
+// and ... FFT") is split as
+//     X[k1 + K1 k2] = sum_bf w_K2^(bf k2) . w_P^(bf k1) . sum_{s < K1/2} a[bf + K2 s] w_K1^(s k1)
+// stage A: one thread per (bf, column): K1/2 inputs straight from global memory, pruned
+//          radix-K1 butterfly with compile-time roots, twiddle w_P^(bf k1), to shared memory;
+// stage B: one thread per (k1, column): radix-K2 butterfly, K2 outputs straight to global
+//          memory in NATURAL frequency order (row k1 + K1 k2).
+// The inverse is the mirror image with the truncation folded into stage A' (only the L wanted
+// samples are computed).  One exchange through shared memory per transform instead of two:
+// the passes are bound by L1/shared-memory wavefronts, not by HBM (profiles/r01_v1_*.md).
+//
+// K1/K5 (x axis, r2c / c2r): two real columns (q, q+1) ride as one complex column Z = a + i b.
+// The Hermitian separation A[k] = (Z[k] + conj Z[-k]) / 2, B[k] = (Z[k] - conj Z[-k]) / 2i needs
+// Z[-k], which sits in the stage-B thread of k1' = K1 - k1 at k2' = K2 - 1 - k2.  Stage-B slots
+// are ordered so that k1 and K1 - k1 are neighbours (slots 2p, 2p + 1) and hence B lanes apart
+// in the same warp: the halves are swapped with warp shuffles, no extra pass through shared
+// memory.  (The factor 1/2 is applied in K5's output scale.)
+#include "demag_fast.cuh"
+#include "fft_core.cuh"
+
+namespace mm {
+
+template <int L> struct Plan2;
+template <> struct Plan2<64> { static constexpr int K1 = 16, K2 = 8; };
+template <> struct Plan2<128> { static constexpr int K1 = 16, K2 = 16; };
+template <> struct Plan2<256> { static constexpr int K1 = 32, K2 = 16; };
+template <> struct Plan2<512> { static constexpr int K1 = 32, K2 = 32; };
+
+bool fast_two_stage(int L, size_t real_bytes) {
+  return real_bytes == 4 && (L == 64 || L == 128 || L == 256 || L == 512);
+}
+
+template <typename T, int L> struct Tile2 {
+  using P = Plan2<L>;
+  static constexpr int K1 = P::K1, K2 = P::K2, A = K1 / 2, H = K2 / 2;
+  static constexpr int B = 64 / (int)sizeof(Cx<T>);  // lanes along the batch (64-byte rows)
+  static constexpr int tasksA = K2 * B, tasksB = K1 * B;
+  static constexpr int NT = tasksA > tasksB ? tasksA : tasksB;
+  static constexpr int smem_bytes = K1 * K2 * 64;
+  static constexpr int min_blocks = smem_bytes >= 32 * 1024 ? 3 : 4;
+  static_assert(K1 * K2 == 2 * L && NT <= 256 && tasksB % 32 == 0, "plan");
+};
+
+// Shared-memory element (k1, bf, lane): sm[(k1 K2 + (bf ^ odd(k1))) B + lane], odd(k1) = k1 >= K1/2:
+// the two k1 of a stage-B half warp (slots 2p, 2p + 1) read rows of opposite parity, i.e.
+// different 64-byte halves of the banks.
+template <int K1> __device__ __forceinline__ int slot_k1(int slot) {
+  const int p = slot >> 1, odd = slot & 1;
+  return p == 0 ? (odd ? K1 / 2 : 0) : (odd ? K1 - p : p);
+}
+
+template <typename T, int K1, int... I>
+__device__ __forceinline__ void rot_fwd(const Cx<T>* v, Cx<T>* o, std::integer_sequence<int, I...>) {
+  ((o[I] = mul_root<T, K1, I, false>(v[I])), ...);
+}
+template <typename T, int K1, int... I>
+__device__ __forceinline__ void rot_inv_add(Cx<T>* e, const Cx<T>* o, std::integer_sequence<int, I...>) {
+  ((e[I] = cadd(e[I], mul_root<T, K1, I, true>(o[I]))), ...);
+}
+
+// two adjacent complex values as one vector access where the type allows it
+template <typename T> struct Vec2;
+template <> struct Vec2<float> {
+  static __device__ __forceinline__ void st(float2* p, float2 a, float2 b) {
+    *reinterpret_cast<float4*>(p) = make_float4(a.x, a.y, b.x, b.y);
+  }
+  static __device__ __forceinline__ void ld(const float2* p, float2& a, float2& b) {
+    const float4 t = *reinterpret_cast<const float4*>(p);
+    a = make_float2(t.x, t.y);
+    b = make_float2(t.z, t.w);
+  }
+  static __device__ __forceinline__ void ldg(const float2* p, float2& a, float2& b) {
+    const float4 t = __ldg(reinterpret_cast<const float4*>(p));
+    a = make_float2(t.x, t.y);
+    b = make_float2(t.z, t.w);
+  }
+};
+template <> struct Vec2<double> {
+  static __device__ __forceinline__ void st(double2* p, double2 a, double2 b) { p[0] = a; p[1] = b; }
+  static __device__ __forceinline__ void ld(const double2* p, double2& a, double2& b) { a = p[0]; b = p[1]; }
+  static __device__ __forceinline__ void ldg(const double2* p, double2& a, double2& b) {
+    a = __ldg(p); b = __ldg(p + 1);
+  }
+};
+
+// ---- stage A, forward: v[s] = a[bf + K2 s] (s < K1/2) -> shared memory
+template <typename T, int L>
+__device__ __forceinline__ void fwdA(Cx<T>* sm, const Cx<T>* __restrict__ Wt, int lane, int bf, Cx<T>* v) {
+  using TL = Tile2<T, L>;
+  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B;
+  Cx<T> o[A];
+  rot_fwd<T, K1>(v, o, std::make_integer_sequence<int, A>{});
+  Dft<T, A, false>::run(v);   // even outputs k1 = 2u
+  Dft<T, A, false>::run(o);   // odd outputs  k1 = 2u + 1
+  const Cx<T>* tw = Wt + bf * K1;
+  Cx<T>* lo = sm + bf * B + lane;          // rows of k1 <  K1/2: (k1 K2 + bf)
+  Cx<T>* hi = sm + (bf ^ 1) * B + lane;    // rows of k1 >= K1/2: (k1 K2 + (bf ^ 1))
+#pragma unroll
+  for (int u = 0; u < A; ++u) {
+    Cx<T> w0, w1;
+    Vec2<T>::ldg(tw + 2 * u, w0, w1);
+    Cx<T>* dst = (2 * u >= K1 / 2) ? hi : lo;
+    dst[(2 * u) * K2 * B] = u ? cmul(v[u], w0) : v[0];
+    dst[(2 * u + 1) * K2 * B] = cmul(o[u], w1);
+  }
+}
+
+// ---- stage B, forward: t[k2] = X[k1 + K1 k2]
+template <typename T, int L>
+__device__ __forceinline__ void fwdB(const Cx<T>* sm, int lane, int k1, Cx<T>* t) {
+  using TL = Tile2<T, L>;
+  constexpr int K1 = TL::K1, K2 = TL::K2, B = TL::B;
+  const int odd = k1 >= K1 / 2 ? 1 : 0;
+  const Cx<T>* base = sm + k1 * K2 * B + lane;
+  const Cx<T>* pe = base + odd * B;   // even bf: row bf + odd
+  const Cx<T>* po = base - odd * B;   // odd bf:  row bf - odd
+#pragma unroll
+  for (int bf = 0; bf < K2; ++bf) t[bf] = ((bf & 1) ? po : pe)[bf * B];
+  Dft<T, K2, false>::run(t);
+}
+
+// ---- stage B', inverse: t[k2] = X[k1 + K1 k2] on entry
+template <typename T, int L>
+__device__ __forceinline__ void invB(Cx<T>* sm, int lane, int k1, Cx<T>* t) {
+  using TL = Tile2<T, L>;
+  constexpr int K1 = TL::K1, K2 = TL::K2, B = TL::B;
+  Dft<T, K2, true>::run(t);
+  const int odd = k1 >= K1 / 2 ? 1 : 0;
+  Cx<T>* base = sm + k1 * K2 * B + lane;
+  Cx<T>* pe = base + odd * B;
+  Cx<T>* po = base - odd * B;
+#pragma unroll
+  for (int bf = 0; bf < K2; ++bf) ((bf & 1) ? po : pe)[bf * B] = t[bf];
+}
+
+// ---- stage A', inverse with truncation: v[s] = x[bf + K2 s], s < K1/2
+template <typename T, int L>
+__device__ __forceinline__ void invA(const Cx<T>* sm, const Cx<T>* __restrict__ Wt, int lane, int bf, Cx<T>* v) {
+  using TL = Tile2<T, L>;
+  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B;
+  Cx<T> o[A];
+  const Cx<T>* tw = Wt + bf * K1;
+  const Cx<T>* lo = sm + bf * B + lane;
+  const Cx<T>* hi = sm + (bf ^ 1) * B + lane;
+#pragma unroll
+  for (int u = 0; u < A; ++u) {
+    Cx<T> w0, w1;
+    Vec2<T>::ldg(tw + 2 * u, w0, w1);
+    const Cx<T>* src = (2 * u >= K1 / 2) ? hi : lo;
+    const Cx<T> a = src[(2 * u) * K2 * B], b = src[(2 * u + 1) * K2 * B];
+    v[u] = u ? cmulc(a, w0) : a;
+    o[u] = cmulc(b, w1);
+  }
+  Dft<T, A, true>::run(v);
+  Dft<T, A, true>::run(o);
+  rot_inv_add<T, K1>(v, o, std::make_integer_sequence<int, A>{});
+}
+
+#define MM_T2_PROLOGUE                                                     \
+  extern __shared__ __align__(16) unsigned char smem_raw[];                \
+  Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);                          \
+  using TL = Tile2<T, L>;                                                  \
+  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, H = TL::H, B = TL::B; \
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B;                \
+  (void)H; (void)A;
+
+// ---------------------------------------------------------------- K2: forward y
+// grid (Q / B, planes); A1, A2 point at the first plane of the launch.
+template <typename T, int L>
+__global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
+yf2_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>* __restrict__ Wt, int Q) {
+  MM_T2_PROLOGUE
+  const size_t col = (size_t)blockIdx.x * B + lane;
+  const Cx<T>* in = A1 + (size_t)blockIdx.y * L * Q + col;
+  Cx<T>* out = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
+  if (slot < K2) {
+    Cx<T> v[A];
+#pragma unroll
+    for (int s = 0; s < A; ++s) v[s] = in[(size_t)(slot + K2 * s) * Q];
+    fwdA<T, L>(sm, Wt, lane, slot, v);
+  }
+  __syncthreads();
+  if (slot < K1) {
+    const int k1 = slot_k1<K1>(slot);
+    Cx<T> t[K2];
+    fwdB<T, L>(sm, lane, k1, t);
+#pragma unroll
+    for (int k2 = 0; k2 < K2; ++k2) out[(size_t)(k1 + K1 * k2) * Q] = t[k2];
+  }
+}
+
+// ---------------------------------------------------------------- K4: inverse y
+template <typename T, int L>
+__global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
+yi2_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ Wt, int Q) {
+  MM_T2_PROLOGUE
+  const size_t col = (size_t)blockIdx.x * B + lane;
+  const Cx<T>* in = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
+  Cx<T>* out = A1 + (size_t)blockIdx.y * L * Q + col;
+  if (slot < K1) {
+    const int k1 = slot_k1<K1>(slot);
+    Cx<T> t[K2];
+#pragma unroll
+    for (int k2 = 0; k2 < K2; ++k2) t[k2] = in[(size_t)(k1 + K1 * k2) * Q];
+    invB<T, L>(sm, lane, k1, t);
+  }
+  __syncthreads();
+  if (slot < K2) {
+    Cx<T> v[A];
+    invA<T, L>(sm, Wt, lane, slot, v);
+#pragma unroll
+    for (int s = 0; s < A; ++s) out[(size_t)(slot + K2 * s) * Q] = v[s];
+  }
+}
+
+template <typename T> __device__ __forceinline__ Cx<T> shfl_xor_cx(Cx<T> v, int m) {
+  Cx<T> r;
+  r.x = __shfl_xor_sync(0xffffffffu, v.x, m);
+  r.y = __shfl_xor_sync(0xffffffffu, v.y, m);
+  return r;
+}
+
+// ---------------------------------------------------------------- K1: forward x, r2c
+// m [x][y][q] real, read as complex pairs (q, q+1); npairs = ny Q / 2 pairs per x row; the
+// spectrum rows k <= nx of A1 hold (A[k], B[k]) at complex columns (2 pair, 2 pair + 1).
+template <typename T, int L>
+__global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
+xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ Wt, size_t npairs) {
+  MM_T2_PROLOGUE
+  const size_t pair = (size_t)blockIdx.x * B + lane;
+  const Cx<T>* in = mp + pair;
+  if (slot < K2) {
+    Cx<T> v[A];
+#pragma unroll
+    for (int s = 0; s < A; ++s) v[s] = in[(size_t)(slot + K2 * s) * npairs];
+    fwdA<T, L>(sm, Wt, lane, slot, v);
+  }
+  __syncthreads();
+  if (slot < K1) {   // whole warps: K1 B is a multiple of 32
+    const int k1 = slot_k1<K1>(slot);
+    const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
+    Cx<T> t[K2];
+    fwdB<T, L>(sm, lane, k1, t);
+    Cx<T>* out = A1 + 2 * pair;
+    const size_t rowc = 2 * npairs;
+#pragma unroll
+    for (int j = 0; j < H; ++j) {
+      // Z[-k] for k = k1 + K1 j: the partner's t[K2 - 1 - j]; own t for the self-paired k1
+      const Cx<T> r = shfl_xor_cx<T>(t[K2 - 1 - j], B);
+      const Cx<T> own = odd ? t[K2 - 1 - j] : t[(K2 - j) % K2];
+      const Cx<T> z = t[j], zm = cconj(pair0 ? own : r);
+      const Cx<T> s = cadd(z, zm), d = csub(z, zm);
+      Vec2<T>::st(out + (size_t)(k1 + K1 * j) * rowc, s, mk<T>(d.y, -d.x));
+    }
+    if (k1 == 0) {  // k = L, its own mirror
+      const Cx<T> z = t[H];
+      Vec2<T>::st(out + (size_t)L * rowc, mk<T>(2 * z.x, (T)0), mk<T>(2 * z.y, (T)0));
+    }
+  }
+}
+
+// ---------------------------------------------------------------- K5: inverse x, c2r
+// Z[k] = A[k] + i B[k], Z[P - k] = conj A[k] + i conj B[k]; the truncated inverse gives
+// h_q(x) + i h_{q+1}(x), written as the real pair (q, q+1) of H, times scale.
+template <typename T, int L>
+__global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
+xi2_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>* __restrict__ Wt, size_t npairs,
+           T scale) {
+  MM_T2_PROLOGUE
+  const size_t pair = (size_t)blockIdx.x * B + lane;
+  if (slot < K1) {
+    const int k1 = slot_k1<K1>(slot);
+    const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
+    const Cx<T>* in = A1 + 2 * pair;
+    const size_t rowc = 2 * npairs;
+    Cx<T> t[K2];
+    Cx<T> a[H], b[H];
+#pragma unroll
+    for (int j = 0; j < H; ++j) Vec2<T>::ld(in + (size_t)(k1 + K1 * j) * rowc, a[j], b[j]);
+#pragma unroll
+    for (int j = 0; j < H; ++j) t[K2 - 1 - j] = mk<T>((T)0, (T)0);
+    if (k1 == 0) {
+      Cx<T> aL, bL;
+      Vec2<T>::ld(in + (size_t)L * rowc, aL, bL);
+      t[H] = mk<T>(aL.x - bL.y, aL.y + bL.x);
+    }
+#pragma unroll
+    for (int j = 0; j < H; ++j) {
+      t[j] = mk<T>(a[j].x - b[j].y, a[j].y + b[j].x);
+      const Cx<T> S = mk<T>(a[j].x + b[j].y, b[j].x - a[j].y);
+      const Cx<T> r = shfl_xor_cx<T>(S, B);
+      if (!pair0) t[K2 - 1 - j] = r;
+      else if (odd) t[K2 - 1 - j] = S;
+      else if (j >= 1) t[K2 - j] = S;
+    }
+    invB<T, L>(sm, lane, k1, t);
+  }
+  __syncthreads();
+  if (slot < K2) {
+    Cx<T> v[A];
+    invA<T, L>(sm, Wt, lane, slot, v);
+    Cx<T>* out = Hp + pair;
+#pragma unroll
+    for (int s = 0; s < A; ++s)
+      out[(size_t)(slot + K2 * s) * npairs] = mk<T>(scale * v[s].x, scale * v[s].y);
+  }
+}
+
+// ---------------------------------------------------------------- host side
+
+template <typename K> static cudaError_t opt_in(K kernel, int bytes) {
+  if (bytes <= 48 * 1024) return cudaSuccess;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+template <typename T, int L>
+static cudaError_t launch2(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
+                           int k0, int nk, cudaStream_t st) {
+  using TL = Tile2<T, L>;
+  const size_t npairs = (size_t)g.ny * g.Q / 2;
+  cudaError_t e;
+  switch (which) {
+    case 0:
+      if ((e = opt_in(xf2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
+      xf2_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
+          reinterpret_cast<const Cx<T>*>(m), b.A1, b.T2x, npairs);
+      break;
+    case 1:
+      if ((e = opt_in(yf2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
+      yf2_kernel<T, L><<<dim3(g.Q / TL::B, nk), TL::NT, TL::smem_bytes, st>>>(
+          b.A1 + (size_t)k0 * g.ny * g.Q, b.A2, b.T2y, g.Q);
+      break;
+    case 3:
+      if ((e = opt_in(yi2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
+      yi2_kernel<T, L><<<dim3(g.Q / TL::B, nk), TL::NT, TL::smem_bytes, st>>>(
+          b.A2, b.A1 + (size_t)k0 * g.ny * g.Q, b.T2y, g.Q);
+      break;
+    default:
+      if ((e = opt_in(xi2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
+      xi2_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
+          b.A1, reinterpret_cast<Cx<T>*>(H), b.T2x, npairs, (T)0.5 * scale);
+      break;
+  }
+  return cudaSuccess;
+}
+
+template <typename T>
+cudaError_t strided2_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
+                            int k0, int nk, cudaStream_t st) {
+  const int L = (which == 0 || which == 4) ? g.nx : g.ny;
+  switch (L) {
+    case 64: return launch2<T, 64>(which, g, b, m, H, scale, k0, nk, st);
+    case 128: return launch2<T, 128>(which, g, b, m, H, scale, k0, nk, st);
+    case 256: return launch2<T, 256>(which, g, b, m, H, scale, k0, nk, st);
+    case 512: return launch2<T, 512>(which, g, b, m, H, scale, k0, nk, st);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+template cudaError_t strided2_launch<float>(int, const FastGeom&, const FastBufs<float>&, const float*,
+                                            float*, float, int, int, cudaStream_t);
+
+// Host: table Wt[bf K1 + k1] = exp(-2 pi i bf k1 / P) of the length-L plan (P = 2L entries).
+void fast2_plan(int L, int* K1, int* K2) {
+  switch (L) {
+    case 64: *K1 = 16; *K2 = 8; break;
+    case 128: *K1 = 16; *K2 = 16; break;
+    case 256: *K1 = 32; *K2 = 16; break;
+    default: *K1 = 32; *K2 = 32; break;
+  }
+}
+
+}  // namespace mm

@@ -46,7 +46,7 @@ struct mm_ctx {
   size_t pers_bytes = 0, scr_bytes = 0;
   bool demag_ready = false;
   // persistent offsets
-  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, pers_need;
+  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, pers_need;
   // scratch offsets
   size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, scr_need;
   unsigned long long launches = 0;
@@ -118,6 +118,8 @@ static void plan_layout(mm_ctx* c) {
   c->off_fy = o; o += align256((size_t)g.Py * 2);
   c->off_posx = o; o += align256((size_t)g.Px * 2);
   c->off_posy = o; o += align256((size_t)g.Py * 2);
+  c->off_t2x = o; o += align256((size_t)g.Px * cs);
+  c->off_t2y = o; o += align256((size_t)g.Py * cs);
   c->pers_need = o;
   // scratch
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
@@ -328,6 +330,20 @@ template <typename T> static void fill_twiddles(std::vector<unsigned char>& buf,
   }
 }
 
+// Wt[bf K1 + k1] = exp(-2 pi i bf k1 / P) of the two-stage plan of length L = P / 2 (demag_fast2.cu).
+template <typename T> static void fill_twiddles2(std::vector<unsigned char>& buf, size_t off, int L) {
+  int K1, K2;
+  fast2_plan(L, &K1, &K2);
+  const int P = 2 * L;
+  Cx<T>* w = reinterpret_cast<Cx<T>*>(buf.data() + off);
+  for (int bf = 0; bf < K2; ++bf)
+    for (int k1 = 0; k1 < K1; ++k1) {
+      const int q = (bf * k1) % P;
+      const long double ph = -2.0L * 3.14159265358979323846264338327950288L * (long double)q / (long double)P;
+      w[bf * K1 + k1] = mk<T>((T)cosl(ph), (T)sinl(ph));
+    }
+}
+
 template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   const DemagGeom& g = c->geom;
   // small tables: twiddles and digit-reversal maps, built on the host, uploaded once
@@ -336,6 +352,9 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   fill_twiddles<T>(host, c->off_wx - small_off, g.Px);
   fill_twiddles<T>(host, c->off_wy - small_off, g.Py);
   fill_twiddles<T>(host, c->off_wz - small_off, g.Pz);
+  const bool two_x = c->fast && fast_two_stage(c->nx, c->es), two_y = c->fast && fast_two_stage(c->ny, c->es);
+  if (two_x) fill_twiddles2<T>(host, c->off_t2x - small_off, c->nx);
+  if (two_y) fill_twiddles2<T>(host, c->off_t2y - small_off, c->ny);
   auto u16 = [&](size_t off) { return reinterpret_cast<uint16_t*>(host.data() + (off - small_off)); };
   for (int k = 0; k < g.Pz; ++k) u16(c->off_posz)[k] = (uint16_t)pos_of_freq(g.pz, k);
   for (int k = 0; k < g.Px; ++k) {
@@ -345,7 +364,7 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   }
   for (int k = 0; k < g.Py; ++k) {
     const int p = pos_of_freq(g.py, k);
-    u16(c->off_posy)[k] = (uint16_t)(c->fast ? fast_pos_logical(c->ny, k) : p);
+    u16(c->off_posy)[k] = (uint16_t)(c->fast ? (two_y ? k : fast_pos_logical(c->ny, k)) : p);
     u16(c->off_fy)[p] = (uint16_t)k;
   }
   cudaError_t e = cudaMemcpyAsync(c->pers + small_off, host.data(), small_bytes,
@@ -411,6 +430,10 @@ template <typename T> static FastBufs<T> fast_bufs_of(mm_ctx* c) {
   b.Wz = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wz);
   b.posx = reinterpret_cast<const uint16_t*>(c->pers + c->off_posx);
   b.posy = reinterpret_cast<const uint16_t*>(c->pers + c->off_posy);
+  b.T2x = reinterpret_cast<const Cx<T>*>(c->pers + c->off_t2x);
+  b.T2y = reinterpret_cast<const Cx<T>*>(c->pers + c->off_t2y);
+  b.two_x = fast_two_stage(c->nx, c->es);
+  b.two_y = fast_two_stage(c->ny, c->es);
   b.table = reinterpret_cast<const T*>(c->pers + c->off_table);
   b.A1 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a1);
   b.A2 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a2);
