@@ -423,14 +423,20 @@ template <typename T, int G> struct ZpCfg {
   static constexpr int NSUB = 16 / G;       // second-stage sub-transforms per lane
   static constexpr int PITCH = G + 1;       // exchange row pitch (conflict-free transposition)
   static constexpr int XB = 16 * PITCH;     // exchange elements per pencil (aliases the pencil)
-  static constexpr int WARPS = sizeof(T) == 4 ? 4 : 2;
-  static constexpr int MINB = 3;
+  // One persistent CTA per SM holding every warp the register file and shared memory admit
+  // (fp32: 12 x 164 registers, 12 x 18.1 KB): warps of one CTA start together and stay close
+  // in the 70 KB instruction stream, which three independent 4-warp CTAs did not (1.06 -> 0.93 ms
+  // at config 4, profiles/r01_v3_*.md).  fp64: 3 CTAs of 2 warps (36.3 KB per warp).
+  static constexpr int WARPS = sizeof(T) == 4 ? 12 : 2;
+  static constexpr int MINB = sizeof(T) == 4 ? 1 : 3;
   static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
   static constexpr int table_bytes = 6 * OZP * (int)sizeof(T);  // one (kx, ky) row, 16 B multiple
   // per warp: two stages of NPW pencils + the table rows of the NPW / 2 mirror pairs + one slot
   // for the row ky = ny (the partner of ky = 0, the only pair that does not share its row)
   static constexpr int warp_bytes = 2 * NPW * pencil_bytes + (NPW / 2 + 1) * table_bytes;
-  static constexpr int smem_bytes = 128 + WARPS * warp_bytes;
+  static constexpr int hdr_for(int warps) { return (3 * warps * 8 + 127) / 128 * 128; }  // mbarriers
+  static constexpr int smem_for(int warps) { return hdr_for(warps) + warps * warp_bytes; }
+  static constexpr int smem_bytes = smem_for(WARPS);
   static_assert(XB <= Q, "exchange buffer must fit in the pencil it aliases");
   static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0, "bulk copies need 16 B multiples");
 };
@@ -500,13 +506,13 @@ __device__ __forceinline__ void zp_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw,
   Dft<T, 8, true>::run(e);
   Dft<T, 8, true>::run(o);
   r[0] = cadd(e[0], o[0]);
-  r[1] = cadd(e[1], mul_root<T, 16, 1, true>(o[1]));
-  r[2] = cadd(e[2], mul_root<T, 16, 2, true>(o[2]));
-  r[3] = cadd(e[3], mul_root<T, 16, 3, true>(o[3]));
-  r[4] = cadd(e[4], mul_root<T, 16, 4, true>(o[4]));
-  r[5] = cadd(e[5], mul_root<T, 16, 5, true>(o[5]));
-  r[6] = cadd(e[6], mul_root<T, 16, 6, true>(o[6]));
-  r[7] = cadd(e[7], mul_root<T, 16, 7, true>(o[7]));
+  r[1] = add_root<T, 16, 1, true>(e[1], o[1]);
+  r[2] = add_root<T, 16, 2, true>(e[2], o[2]);
+  r[3] = add_root<T, 16, 3, true>(e[3], o[3]);
+  r[4] = add_root<T, 16, 4, true>(e[4], o[4]);
+  r[5] = add_root<T, 16, 5, true>(e[5], o[5]);
+  r[6] = add_root<T, 16, 6, true>(e[6], o[6]);
+  r[7] = add_root<T, 16, 7, true>(e[7], o[7]);
 }
 
 // Hhat = Nhat mhat at the 16 frequencies of this lane.  trow: the (kx, ky) table row in shared
@@ -519,12 +525,17 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T sy, Cx<T>* X
 #pragma unroll
   for (int f = 0; f < 16; ++f) {
     const int kz = C::NSUB * t + (f / G) + 16 * (f % G);
-    const bool mir = kz > C::nz;
+    // kz > nz (the mirrored half, where N_xz and N_yz change sign) is known at compile time
+    // except for the one block of frequencies that straddles kz = nz
+    bool mir;
+    if ((f % G) < G / 2) mir = false;
+    else if ((f % G) > G / 2) mir = true;
+    else mir = kz > C::nz;
     const int idx = mir ? C::Pz - kz : kz;
-    const T sz = mir ? (T)-1 : (T)1;
     const T nxx = trow[idx], nyy = trow[C::OZP + idx], nzz = trow[2 * C::OZP + idx],
-            nxy = sy * trow[3 * C::OZP + idx], nxz = sz * trow[4 * C::OZP + idx],
-            nyz = sy * sz * trow[5 * C::OZP + idx];
+            nxy = sy * trow[3 * C::OZP + idx];
+    T nxz = trow[4 * C::OZP + idx], nyz = sy * trow[5 * C::OZP + idx];
+    if (mir) { nxz = -nxz; nyz = -nyz; }
     const Cx<T> a = X0[f], b = X1[f], c = X2[f];
     X0[f] = mk<T>(nxx * a.x + nxy * b.x + nxz * c.x, nxx * a.y + nxy * b.y + nxz * c.y);
     X1[f] = mk<T>(nxy * a.x + nyy * b.x + nyz * c.x, nxy * a.y + nyy * b.y + nyz * c.y);
@@ -536,8 +547,8 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T sy, Cx<T>* X
 // NPW/2 mirror pairs (ky, Py - ky) of one plane, which share their Nhat rows.  Pencils and
 // table rows arrive by bulk asynchronous copies one task ahead; the pencil's own buffer is
 // the exchange buffer of its transforms once its samples sit in registers.
-template <typename T, int G>
-__global__ void __launch_bounds__(ZpCfg<T, G>::WARPS * 32, ZpCfg<T, G>::MINB)
+template <typename T, int G, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB)
 zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
                const uint16_t* __restrict__ posy, int ny, int kx0, int ntask) {
   using C = ZpCfg<T, G>;
@@ -545,13 +556,13 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 3 * warp;  // stage 0, stage 1, table
-  unsigned char* wraw = smem_raw + 128 + (size_t)warp * C::warp_bytes;
+  unsigned char* wraw = smem_raw + C::hdr_for(WARPS) + (size_t)warp * C::warp_bytes;
   Cx<T>* pbase = reinterpret_cast<Cx<T>*>(wraw);
   T* tbase = reinterpret_cast<T*>(wraw + 2 * NPW * C::pencil_bytes);
   const int t = lane % G, pw = lane / G;
   const int Py = 2 * ny;
   if (threadIdx.x == 0) {
-    for (int i = 0; i < 3 * C::WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    for (int i = 0; i < 3 * WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -560,7 +571,7 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
   for (int u = 1; u < 16; ++u) tw[u] = __ldg(Wz + t * u);
   tw[0] = mk<T>(1, 0);
 
-  const int gw = blockIdx.x * C::WARPS + warp, stride = gridDim.x * C::WARPS;
+  const int gw = blockIdx.x * WARPS + warp, stride = gridDim.x * WARPS;
   auto pencil_ptr = [&](int task, int p) -> Cx<T>* {
     const int pair = task * (NPW / 2) + (p >> 1);
     const int plane = pair / ny, i = pair - plane * ny;
@@ -586,6 +597,9 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
   };
   if (lane == 0 && gw < ntask) { issue(gw, 0); issue_table(gw); }
   int it = 0;
+  // not unrolled: the body is ~2,300 instructions and two copies of it (the compiler's choice,
+  // to make `stage` a constant) overflow the instruction cache
+#pragma unroll 1
   for (int task = gw; task < ntask; task += stride, ++it) {
     const int stage = it & 1;
     const bool more = task + stride < ntask;
@@ -709,12 +723,13 @@ static cudaError_t launch_yi(const FastGeom& g, const FastBufs<T>& b, int k0, in
 template <typename T, int G>
 static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
   using C = ZpCfg<T, G>;
-  cudaError_t e = opt_in_smem(zp_fast_kernel<T, G>, C::smem_bytes);
+  constexpr int WARPS = C::WARPS, MINB = C::MINB;
+  cudaError_t e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB>, C::smem_bytes);
   if (e != cudaSuccess) return e;
   const int ntask = (int)((size_t)nk * g.ny * 2 / C::NPW);
-  int grid = sm_count() * C::MINB;
-  if (grid * C::WARPS > ntask) grid = (ntask + C::WARPS - 1) / C::WARPS;
-  zp_fast_kernel<T, G><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(
+  int grid = sm_count() * MINB;
+  if (grid * WARPS > ntask) grid = (ntask + WARPS - 1) / WARPS;
+  zp_fast_kernel<T, G, WARPS, MINB><<<grid, WARPS * 32, C::smem_bytes, st>>>(
       b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask);
   return cudaSuccess;
 }

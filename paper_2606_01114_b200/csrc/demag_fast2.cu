@@ -18,6 +18,9 @@
 // are ordered so that k1 and K1 - k1 are neighbours (slots 2p, 2p + 1) and hence B lanes apart
 // in the same warp: the halves are swapped with warp shuffles, no extra pass through shared
 // memory.  (The factor 1/2 is applied in K5's output scale.)
+// scalar fp32 complex add/subtract here: the two-wide form (mm_common.cuh) measured slower in these
+// memory-latency-bound passes (K2 0.497 -> 0.528 ms at config 4) and faster only in K3
+#define MM_NO_PACKED_F32
 #include "demag_fast.cuh"
 #include "fft_core.cuh"
 
@@ -58,7 +61,7 @@ __device__ __forceinline__ void rot_fwd(const Cx<T>* v, Cx<T>* o, std::integer_s
 }
 template <typename T, int K1, int... I>
 __device__ __forceinline__ void rot_inv_add(Cx<T>* e, const Cx<T>* o, std::integer_sequence<int, I...>) {
-  ((e[I] = cadd(e[I], mul_root<T, K1, I, true>(o[I]))), ...);
+  ((e[I] = add_root<T, K1, I, true>(e[I], o[I])), ...);
 }
 
 // two adjacent complex values as one vector access where the type allows it

@@ -11,6 +11,9 @@
 // Pruning: a length-2L transform with only L non-zero inputs is two length-L transforms
 // (even outputs: a_j; odd outputs: a_j w_2L^j); the zero half is never read or stored.
 // Truncation on the way back is the mirror image.
+// scalar fp32 complex add/subtract here: the two-wide form (mm_common.cuh) measured slower in these
+// memory-latency-bound passes (K2 0.497 -> 0.528 ms at config 4) and faster only in K3
+#define MM_NO_PACKED_F32
 #include "demag_passes.cuh"
 
 #include "fft_core.cuh"

@@ -52,18 +52,53 @@ template <typename T, int R, int S, bool INV> __device__ __forceinline__ Cx<T> m
     return mk<T>(-v.x, -v.y);
   } else if constexpr (4 * s == 3 * R) {  // +i (forward)
     return INV ? mk<T>(v.y, -v.x) : mk<T>(-v.y, v.x);
-  } else if constexpr (8 * s == R) {  // (1 - i)/sqrt2 (forward)
+  } else if constexpr (8 * s == R) {  // (1 - i)/sqrt2 (forward); one multiply + two fused multiply-adds
     constexpr T h = (T)0.70710678118654752440;
-    return INV ? mk<T>((v.x - v.y) * h, (v.x + v.y) * h) : mk<T>((v.x + v.y) * h, (v.y - v.x) * h);
+    if constexpr (INV) { const T t = v.x * h; return mk<T>(fma(-v.y, h, t), fma(v.y, h, t)); }
+    else { const T t = v.y * h; return mk<T>(fma(v.x, h, t), fma(-v.x, h, t)); }
   } else if constexpr (8 * s == 3 * R) {  // (-1 - i)/sqrt2 (forward)
     constexpr T h = (T)0.70710678118654752440;
-    return INV ? mk<T>((-v.x - v.y) * h, (v.x - v.y) * h) : mk<T>((v.y - v.x) * h, (-v.x - v.y) * h);
+    if constexpr (INV) { const T t = v.x * h; return mk<T>(fma(-v.y, h, -t), fma(-v.y, h, t)); }
+    else { const T t = v.y * h; return mk<T>(fma(-v.x, h, t), fma(-v.x, h, -t)); }
   } else {
     constexpr T c = (T)root_cos<R, s>();
     constexpr T sn = (T)root_sin<R, s>();
     // forward: (c - i sn); inverse: (c + i sn)
     return INV ? mk<T>(v.x * c - v.y * sn, v.y * c + v.x * sn)
                : mk<T>(v.x * c + v.y * sn, v.y * c - v.x * sn);
+  }
+}
+
+// e + o * w_R^S with the products contracted into the sums (two fused multiply-adds per real).
+template <typename T, int R, int S, bool INV> __device__ __forceinline__ Cx<T> add_root(Cx<T> e, Cx<T> o) {
+  constexpr int s = S % R;
+  if constexpr (s == 0) {
+    return cadd(e, o);
+  } else if constexpr (4 * s == R) {  // -i (forward)
+    return INV ? mk<T>(e.x - o.y, e.y + o.x) : mk<T>(e.x + o.y, e.y - o.x);
+  } else if constexpr (2 * s == R) {
+    return csub(e, o);
+  } else if constexpr (4 * s == 3 * R) {  // +i (forward)
+    return INV ? mk<T>(e.x + o.y, e.y - o.x) : mk<T>(e.x - o.y, e.y + o.x);
+  } else {
+    constexpr T c = (T)root_cos<R, s>();
+    constexpr T sn = (T)root_sin<R, s>();
+    return INV ? mk<T>(fma(o.x, c, fma(-o.y, sn, e.x)), fma(o.y, c, fma(o.x, sn, e.y)))
+               : mk<T>(fma(o.x, c, fma(o.y, sn, e.x)), fma(o.y, c, fma(-o.x, sn, e.y)));
+  }
+}
+
+// (a - b) * w_R^S.  The quarter-turn roots swap the two halves of the complex value: the
+// difference is then taken half by half into the swapped positions, so the packed two-wide
+// arithmetic of cadd/csub downstream never needs a register shuffle.
+template <typename T, int R, int S, bool INV> __device__ __forceinline__ Cx<T> sub_root(Cx<T> a, Cx<T> b) {
+  constexpr int s = S % R;
+  if constexpr (4 * s == R) {  // -i (forward): (d.y, -d.x)
+    return INV ? mk<T>(b.y - a.y, a.x - b.x) : mk<T>(a.y - b.y, b.x - a.x);
+  } else if constexpr (4 * s == 3 * R) {  // +i (forward): (-d.y, d.x)
+    return INV ? mk<T>(a.y - b.y, b.x - a.x) : mk<T>(b.y - a.y, a.x - b.x);
+  } else {
+    return mul_root<T, R, S, INV>(csub(a, b));
   }
 }
 
@@ -74,7 +109,7 @@ template <typename T, int R, bool INV> struct Dft {
   static __device__ __forceinline__ void split(const Cx<T>* v, Cx<T>* a, Cx<T>* b,
                                                std::integer_sequence<int, I...>) {
     ((a[I] = cadd(v[I], v[I + R / 2])), ...);
-    ((b[I] = mul_root<T, R, I, INV>(csub(v[I], v[I + R / 2]))), ...);
+    ((b[I] = sub_root<T, R, I, INV>(v[I], v[I + R / 2])), ...);
   }
   static __device__ __forceinline__ void run(Cx<T>* v) {
     Cx<T> a[R / 2], b[R / 2];
