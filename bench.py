@@ -327,6 +327,79 @@ def run_ours(args, cfg):
     return 0
 
 
+def run_sweep(args):
+    """Config 5 of BASELINE.json: H_demag and H_eff+LLG throughput over the sweep meshes, fp32 and
+    fp64, one JSON line per (mesh, dtype); the CPU oracle's FFT path is timed at the sizes it
+    finishes in about a minute (--no-cpu skips it).  Not the driver's bench line: a report."""
+    import torch
+    from paper_2606_01114_b200 import Context, build
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    build.build()
+    cfg5 = w.get_config(5)
+    peak, peak_src = measured_peak()
+    steps = max(3, min(args.steps, 30))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps
+
+    for n in w.SWEEP_MESHES:
+        cfg = cfg5.with_mesh(n, name="cfg5_sweep_%dx%dx%d" % n)
+        for dt in ("f32", "f64"):
+            s = 4 if dt == "f32" else 8
+            tdt = torch.float32 if dt == "f32" else torch.float64
+            ctx = Context(cfg.n, cfg.d, dtype=tdt, device="cuda:0")
+            ctx.set_material(cfg.Ms, cfg.Aex, cfg.Ku, cfg.axis, cfg.alpha, cfg.gamma)
+            ctx.set_terms(cfg.terms)
+            t0 = time.time()
+            ctx.demag_init()
+            torch.cuda.synchronize()
+            t_init = time.time() - t0
+            m = torch.from_numpy(w.random_unit_vectors(cfg.seed, cfg.n).astype(
+                np.float32 if dt == "f32" else np.float64)).cuda()
+            out = torch.empty_like(m)
+            ms_d = timed(lambda: ctx.demag_field(m, out))
+            ms_r = timed(lambda: ctx.llg_rhs(m, out))
+            kb, total = byte_model(cfg.n, s, fast=ctx.path[0])
+            demag_bytes = total - kb["S6_pointwise"]
+            line = {"sweep": cfg.name, "dtype": dt, "cells": cfg.ncell,
+                    "path": "fast (x-first)" if ctx.path[0] else "generic (z-first)",
+                    "demag": {"ms": ms_d, "cell_updates_per_s": cfg.ncell / ms_d * 1e3,
+                              "frac_hbm_measured": demag_bytes / ms_d / 1e6 / peak,
+                              "frac_hbm_8TBps": demag_bytes / ms_d / 1e6 / 8000.0},
+                    "heff_llg": {"ms": ms_r, "cell_updates_per_s": cfg.ncell / ms_r * 1e3,
+                                 "frac_hbm_measured": total / ms_r / 1e6 / peak,
+                                 "frac_hbm_8TBps": total / ms_r / 1e6 / 8000.0},
+                    "init_s": t_init, "peak_GBps": peak}
+            ctx.close()
+            del m, out, ctx
+            torch.cuda.empty_cache()
+            if dt == "f64" and not args.no_cpu and cfg.ncell <= 128 ** 3:
+                from oracle import oracle as o
+                o.build()
+                P = o.Problem(n=cfg.n, d=cfg.d, Ms=cfg.Ms, Aex=cfg.Aex, alpha=cfg.alpha, gamma=cfg.gamma,
+                              terms=cfg.terms).prepare()
+                mh = w.random_unit_vectors(cfg.seed, cfg.n)
+                P.llg_rhs(mh)
+                t = time.perf_counter()
+                P.llg_rhs(mh)
+                dtc = time.perf_counter() - t
+                line["cpu_oracle"] = {"cell_updates_per_s": cfg.ncell / dtc, "ms": 1e3 * dtc,
+                                      "cores": o.num_threads(), "what": "oracle FFT path, H_eff+LLG, fp64"}
+            print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -338,7 +411,10 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic passes, 2 fast kernels (experiments)")
     ap.add_argument("--kchunk", type=int, default=0, help="kx planes per y/z/y launch group (experiments)")
     ap.add_argument("--mesh", default=None, help="override mesh, e.g. 256x256x64 (experiments)")
+    ap.add_argument("--sweep", action="store_true", help="config 5: one line per sweep mesh and dtype")
     args = ap.parse_args()
+    if args.sweep:
+        return run_sweep(args)
     cfg = w.get_config(4)
     if args.mesh:
         cfg = cfg.with_mesh(tuple(int(v) for v in args.mesh.split("x")),

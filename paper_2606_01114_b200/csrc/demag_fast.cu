@@ -656,11 +656,246 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
   if (lane == 0) bulk_wait0();
 }
 
+// ---------------------------------------------------------------- K3 for nz = 256 (fp32)
+// Pz = 512 = 16 x 32: all 32 lanes of a warp own ONE pencil, 16 frequencies x 3 components per
+// lane as above.  The second stage is a radix-32 transform per first-stage output k1 (16 of
+// them): it is split over the lane pair (k1, h): h = 0 computes its even outputs (radix 16 of
+// b[s] + b[s + 16]), h = 1 its odd outputs (radix 16 of (b[s] - b[s + 16]) w32^s), both reading
+// all 32 exchanged values.  Lane t = k1 + 16 h then holds the spectrum at kz = t + 32 u, u < 16.
+// The way back mirrors it: each lane writes g[s] = IDFT16(X)[s] (h = 1: times conj w32^s) to slot
+// s + 16 h, and the first-stage reader combines b[tp] = g[tp & 15] +- g[(tp & 15) + 16].
+// Pencils are processed one at a time (the two pencils of a mirror pair (ky, Py - ky) in turn,
+// sharing one staged Nhat row), double buffered by bulk copies as in zp_fast_kernel.
+template <typename T> struct ZwCfg {
+  static constexpr int nz = 256, Pz = 512, Q = 3 * nz, OZP = nz + 2, PITCH = 33;
+  static constexpr int WARPS = 12;
+  static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
+  static constexpr int table_bytes = 6 * OZP * (int)sizeof(T);
+  static constexpr int warp_bytes = 2 * pencil_bytes + table_bytes;
+  static constexpr int hdr_bytes = (3 * WARPS * 8 + 127) / 128 * 128;
+  static constexpr int smem_bytes = hdr_bytes + WARPS * warp_bytes;
+  static_assert(16 * PITCH <= Q, "exchange buffer must fit in the pencil it aliases");
+  static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0, "bulk copies need 16 B multiples");
+};
+
+template <typename T, int... S>
+__device__ __forceinline__ void zw_half_fwd(const Cx<T>* row, T sgn, bool h, Cx<T>* c,
+                                            std::integer_sequence<int, S...>) {
+  ((c[S] = [&] {
+     const Cx<T> lo = row[S], hi = row[S + 16];
+     const Cx<T> d = mk<T>(fma(sgn, hi.x, lo.x), fma(sgn, hi.y, lo.y));
+     const Cx<T> r = mul_root<T, 32, S, false>(d);
+     return h ? r : d;
+   }()),
+   ...);
+}
+template <typename T, int... S>
+__device__ __forceinline__ void zw_half_inv(Cx<T>* row, bool h, const Cx<T>* c,
+                                            std::integer_sequence<int, S...>) {
+  ((row[S] = h ? mul_root<T, 32, S, true>(c[S]) : c[S]), ...);
+}
+
+// a[j] = sample z = t + 32 j (j < 8)  ->  X[u] = spectrum at kz = t + 32 u
+template <typename T>
+__device__ __forceinline__ void zw_forward(const Cx<T>* a, Cx<T>* xb, const Cx<T>* tw, int t, Cx<T>* X) {
+  using C = ZwCfg<T>;
+  Cx<T> e[8], o[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) e[j] = a[j];
+  o[0] = e[0];
+  o[1] = mul_root<T, 16, 1, false>(e[1]);
+  o[2] = mul_root<T, 16, 2, false>(e[2]);
+  o[3] = mul_root<T, 16, 3, false>(e[3]);
+  o[4] = mul_root<T, 16, 4, false>(e[4]);
+  o[5] = mul_root<T, 16, 5, false>(e[5]);
+  o[6] = mul_root<T, 16, 6, false>(e[6]);
+  o[7] = mul_root<T, 16, 7, false>(e[7]);
+  Dft<T, 8, false>::run(e);
+  Dft<T, 8, false>::run(o);
+  xb[t] = e[0];
+#pragma unroll
+  for (int v = 0; v < 8; ++v) {
+    if (v) xb[(2 * v) * C::PITCH + t] = cmul(e[v], tw[2 * v]);
+    xb[(2 * v + 1) * C::PITCH + t] = cmul(o[v], tw[2 * v + 1]);
+  }
+  __syncwarp();
+  const bool h = t >= 16;
+  zw_half_fwd<T>(xb + (t & 15) * C::PITCH, h ? (T)-1 : (T)1, h, X, std::make_integer_sequence<int, 16>{});
+  Dft<T, 16, false>::run(X);
+  __syncwarp();
+}
+
+template <typename T>
+__device__ __forceinline__ void zw_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw, int t, const Cx<T>* X) {
+  using C = ZwCfg<T>;
+  const bool h = t >= 16;
+  {
+    Cx<T> c[16];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) c[u] = X[u];
+    Dft<T, 16, true>::run(c);
+    zw_half_inv<T>(xb + (t & 15) * C::PITCH + (h ? 16 : 0), h, c, std::make_integer_sequence<int, 16>{});
+  }
+  __syncwarp();
+  const T sgn = h ? (T)-1 : (T)1;
+  const Cx<T>* col = xb + (t & 15);
+  Cx<T> e[8], o[8];
+#pragma unroll
+  for (int v = 0; v < 8; ++v) {
+    const Cx<T> l0 = col[(2 * v) * C::PITCH], h0 = col[(2 * v) * C::PITCH + 16];
+    const Cx<T> l1 = col[(2 * v + 1) * C::PITCH], h1 = col[(2 * v + 1) * C::PITCH + 16];
+    const Cx<T> b0 = mk<T>(fma(sgn, h0.x, l0.x), fma(sgn, h0.y, l0.y));
+    const Cx<T> b1 = mk<T>(fma(sgn, h1.x, l1.x), fma(sgn, h1.y, l1.y));
+    e[v] = v ? cmulc(b0, tw[2 * v]) : b0;
+    o[v] = cmulc(b1, tw[2 * v + 1]);
+  }
+  __syncwarp();
+  Dft<T, 8, true>::run(e);
+  Dft<T, 8, true>::run(o);
+  r[0] = cadd(e[0], o[0]);
+  r[1] = add_root<T, 16, 1, true>(e[1], o[1]);
+  r[2] = add_root<T, 16, 2, true>(e[2], o[2]);
+  r[3] = add_root<T, 16, 3, true>(e[3], o[3]);
+  r[4] = add_root<T, 16, 4, true>(e[4], o[4]);
+  r[5] = add_root<T, 16, 5, true>(e[5], o[5]);
+  r[6] = add_root<T, 16, 6, true>(e[6], o[6]);
+  r[7] = add_root<T, 16, 7, true>(e[7], o[7]);
+}
+
+template <typename T>
+__device__ __forceinline__ void zw_multiply(const T* trow, int t, T sy, Cx<T>* X0, Cx<T>* X1, Cx<T>* X2) {
+  using C = ZwCfg<T>;
+#pragma unroll
+  for (int u = 0; u < 16; ++u) {
+    const int kz = t + 32 * u;
+    bool mir;
+    if (u < 8) mir = false;
+    else if (u > 8) mir = true;
+    else mir = t > 0;
+    const int idx = mir ? C::Pz - kz : kz;
+    const T nxx = trow[idx], nyy = trow[C::OZP + idx], nzz = trow[2 * C::OZP + idx],
+            nxy = sy * trow[3 * C::OZP + idx];
+    T nxz = trow[4 * C::OZP + idx], nyz = sy * trow[5 * C::OZP + idx];
+    if (mir) { nxz = -nxz; nyz = -nyz; }
+    const Cx<T> a = X0[u], b = X1[u], c = X2[u];
+    X0[u] = mk<T>(nxx * a.x + nxy * b.x + nxz * c.x, nxx * a.y + nxy * b.y + nxz * c.y);
+    X1[u] = mk<T>(nxy * a.x + nyy * b.x + nyz * c.x, nxy * a.y + nyy * b.y + nyz * c.y);
+    X2[u] = mk<T>(nxz * a.x + nyz * b.x + nzz * c.x, nxz * a.y + nyz * b.y + nzz * c.y);
+  }
+}
+
+// A2 points at the first plane of the launch (kx = kx0).  A warp walks mirror pairs
+// pair = plane ny + i -> pencils ky = i and ky = (i == 0 ? ny : Py - i), one pencil per step.
+template <typename T>
+__global__ void __launch_bounds__(ZwCfg<T>::WARPS * 32, 1)
+zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
+               const uint16_t* __restrict__ posy, int ny, int kx0, int npair) {
+  using C = ZwCfg<T>;
+  constexpr int Q = C::Q;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, t = threadIdx.x & 31;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 3 * warp;  // pencil buffer 0, 1, table
+  unsigned char* wraw = smem_raw + C::hdr_bytes + (size_t)warp * C::warp_bytes;
+  Cx<T>* pbase = reinterpret_cast<Cx<T>*>(wraw);
+  T* trow = reinterpret_cast<T*>(wraw + 2 * C::pencil_bytes);
+  const int Py = 2 * ny;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 3 * C::WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  Cx<T> tw[16];
+#pragma unroll
+  for (int u = 1; u < 16; ++u) tw[u] = __ldg(Wz + t * u);
+  tw[0] = mk<T>(1, 0);
+
+  const int gw = blockIdx.x * C::WARPS + warp, stride = gridDim.x * C::WARPS;
+  const int mine = gw < npair ? (npair - gw + stride - 1) / stride : 0;  // pairs of this warp
+  const int nsteps = 2 * mine;
+  auto pencil_ptr = [&](int step) -> Cx<T>* {
+    const int pair = gw + (step >> 1) * stride;
+    const int plane = pair / ny, i = pair - plane * ny;
+    const int ky = (step & 1) ? (i == 0 ? ny : Py - i) : i;
+    return A2 + ((size_t)plane * Py + posy[ky]) * Q;
+  };
+  // Nhat row of a step; -1 if it is the row already staged (second pencil of a pair i != 0)
+  auto table_row = [&](int step) -> long long {
+    const int pair = gw + (step >> 1) * stride;
+    const int plane = pair / ny, i = pair - plane * ny;
+    if ((step & 1) && i != 0) return -1;
+    return ((long long)(kx0 + plane) * (ny + 1) + ((step & 1) ? ny : i));
+  };
+  if (t == 0 && nsteps > 0) {
+    mbar_expect_tx(bars + 0, C::pencil_bytes);
+    bulk_load(pbase, pencil_ptr(0), C::pencil_bytes, bars + 0);
+    mbar_expect_tx(bars + 2, C::table_bytes);
+    bulk_load(trow, tab + (size_t)table_row(0) * 6 * C::OZP, C::table_bytes, bars + 2);
+  }
+  int tphase = 0;
+#pragma unroll 1
+  for (int step = 0; step < nsteps; ++step) {
+    const int buf = step & 1;
+    if (t == 0) {
+      bulk_wait_read0();  // the previous step's store has finished reading the other buffer
+      if (step + 1 < nsteps) {
+        mbar_expect_tx(bars + (buf ^ 1), C::pencil_bytes);
+        bulk_load(pbase + (buf ^ 1) * Q, pencil_ptr(step + 1), C::pencil_bytes, bars + (buf ^ 1));
+      }
+    }
+    __syncwarp();
+    mbar_wait(bars + buf, (step >> 1) & 1);
+    Cx<T>* pen = pbase + buf * Q;
+    Cx<T> X[3][16];
+    {
+      Cx<T> a[3][8];
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[c][j] = pen[(t + 32 * j) * 3 + c];
+      __syncwarp();  // every sample is in registers: the pencil buffer becomes the exchange buffer
+#pragma unroll
+      for (int c = 0; c < 3; ++c) zw_forward<T>(a[c], pen, tw, t, X[c]);
+    }
+    {
+      const int pair = gw + (step >> 1) * stride;
+      const int i = pair % ny;
+      const T sy = ((step & 1) && i != 0) ? (T)-1 : (T)1;
+      if (table_row(step) >= 0) { mbar_wait(bars + 2, tphase); tphase ^= 1; }
+      zw_multiply<T>(trow, t, sy, X[0], X[1], X[2]);
+      __syncwarp();
+      if (t == 0 && step + 1 < nsteps) {
+        const long long row = table_row(step + 1);
+        if (row >= 0) {
+          mbar_expect_tx(bars + 2, C::table_bytes);
+          bulk_load(trow, tab + (size_t)row * 6 * C::OZP, C::table_bytes, bars + 2);
+        }
+      }
+    }
+    {
+      Cx<T> r[3][8];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) zw_inverse<T>(r[c], pen, tw, t, X[c]);
+      __syncwarp();  // the last exchange has been read
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) pen[(t + 32 * j) * 3 + c] = r[c][j];
+    }
+    fence_async_smem();
+    __syncwarp();
+    if (t == 0) {
+      bulk_store(pencil_ptr(step), pen, C::pencil_bytes);
+      bulk_commit();
+    }
+  }
+  if (t == 0) bulk_wait0();
+}
+
 // ---------------------------------------------------------------- host side
 
-bool fast_supported(int nx, int ny, int nz, size_t /*real_bytes*/) {
+bool fast_supported(int nx, int ny, int nz, size_t real_bytes) {
   auto okxy = [](int n) { return n == 64 || n == 128 || n == 256 || n == 512 || n == 1024; };
-  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128);
+  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128 || (nz == 256 && real_bytes == 4));
 }
 
 template <typename K> static cudaError_t opt_in_smem(K kernel, int bytes) {
@@ -734,6 +969,18 @@ static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, in
   return cudaSuccess;
 }
 
+template <typename T>
+static cudaError_t launch_zw(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
+  using C = ZwCfg<T>;
+  cudaError_t e = opt_in_smem(zw_fast_kernel<T>, C::smem_bytes);
+  if (e != cudaSuccess) return e;
+  const int npair = nk * g.ny;
+  int grid = sm_count();
+  if (grid * C::WARPS > npair) grid = (npair + C::WARPS - 1) / C::WARPS;
+  zw_fast_kernel<T><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair);
+  return cudaSuccess;
+}
+
 #define MM_DISPATCH_L(L, CALL)                       \
   switch (L) {                                       \
     case 64: e = CALL(64); break;                    \
@@ -774,7 +1021,12 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
     }
     if (e != cudaSuccess) return e;
     prof->mark(2, st);
-    e = g.nz == 128 ? launch_zp<T, 16>(g, b, k0, nk, st) : launch_zp<T, 8>(g, b, k0, nk, st);
+    if (g.nz == 256) {
+      if constexpr (sizeof(T) == 4) e = launch_zw<T>(g, b, k0, nk, st);
+      else e = cudaErrorInvalidValue;
+    } else {
+      e = g.nz == 128 ? launch_zp<T, 16>(g, b, k0, nk, st) : launch_zp<T, 8>(g, b, k0, nk, st);
+    }
     if (e != cudaSuccess) return e;
     prof->mark(3, st);
     if (b.two_y) {

@@ -101,7 +101,7 @@ def test_config3_dense_heff_and_rhs(oracle):
     ctx.close()
 
 
-@pytest.mark.parametrize("n", [(64, 64, 64), (128, 128, 128), (1024, 1024, 64)])
+@pytest.mark.parametrize("n", [(64, 64, 64), (128, 128, 128), (256, 256, 256), (1024, 1024, 64)])
 def test_sweep_meshes_sparse(oracle, n):
     """Config 5 sweep sizes (incl. the 1024-point axes): sparse-source parity, fp32."""
     cfg = w.get_config(5).with_mesh(n)
