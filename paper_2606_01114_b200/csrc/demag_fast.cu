@@ -72,7 +72,10 @@ template <typename T, int L> struct Tile {
   static constexpr int R1 = P::R1, R2 = P::R2, R3 = P::R3;
   static constexpr int q1 = R2 * R3, q2 = R3;
   static constexpr int B = 64 / (int)sizeof(Cx<T>);   // lanes along the batch (64-byte rows)
-  static constexpr int NS = kStrideThreads / B;       // task slots
+  static constexpr int smem_bytes_ = 2 * L * 64;
+  // threads per CTA: the 128 KB tile of L = 1024 admits one CTA per SM, which then gets 16 warps (fp32)
+  static constexpr int NT = (smem_bytes_ > 110 * 1024 && sizeof(T) == 4) ? 2 * kStrideThreads : kStrideThreads;
+  static constexpr int NS = NT / B;                   // task slots
   static constexpr int LOG3 = ilog2c(R3);
   static constexpr int smem_bytes = 2 * L * 64;
   // resident CTAs per SM the kernels are compiled for (shared memory and registers)
@@ -235,7 +238,7 @@ template <> struct Pair2<double> {
 // ---------------------------------------------------------------- K2: forward y (S2)
 // grid (Q / B, planes).  A1, A2 point at the first plane of the launch.
 template <typename T, int L>
-__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+__global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 yf_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>* __restrict__ W, int Q) {
   MM_TILE_PROLOGUE
   const size_t col = (size_t)blockIdx.x * B + lane;
@@ -262,7 +265,7 @@ yf_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>
 
 // ---------------------------------------------------------------- K4: inverse y (S4)
 template <typename T, int L>
-__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+__global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 yi_fast_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W, int Q) {
   MM_TILE_PROLOGUE
   const size_t col = (size_t)blockIdx.x * B + lane;
@@ -292,7 +295,7 @@ yi_fast_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>
 // signals, separated afterwards with A[k] = (Z[k] + conj Z[-k])/2, B[k] = (Z[k] - conj Z[-k])/(2i)
 // for k <= nx.  grid (ny Q / 2 / B).  npairs = ny Q / 2 (pairs per x row); rowc = ny Q.
 template <typename T, int L>
-__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+__global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 xf_fast_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W,
                const uint16_t* __restrict__ pos, size_t npairs) {
   MM_TILE_PROLOGUE
@@ -333,7 +336,7 @@ xf_fast_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>
 // Z[k] = A[k] + i B[k], Z[Px - k] = conj A[k] + i conj B[k]; the truncated inverse gives
 // h_q(x) + i h_{q+1}(x), written as the real pair (q, q+1) of H, times scale (-Ms).
 template <typename T, int L>
-__global__ void __launch_bounds__(kStrideThreads, Tile<T, L>::min_blocks)
+__global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 xi_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>* __restrict__ W,
                const uint16_t* __restrict__ pos, size_t npairs, T scale) {
   MM_TILE_PROLOGUE
@@ -921,7 +924,7 @@ static cudaError_t launch_xf(const FastGeom& g, const FastBufs<T>& b, const T* m
   cudaError_t e = opt_in_smem(xf_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
   const size_t npairs = (size_t)g.ny * g.Q / 2;
-  xf_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), kStrideThreads, TL::smem_bytes, st>>>(
+  xf_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
       reinterpret_cast<const Cx<T>*>(m), b.A1, b.Wx, b.posx, npairs);
   return cudaSuccess;
 }
@@ -931,7 +934,7 @@ static cudaError_t launch_xi(const FastGeom& g, const FastBufs<T>& b, T* H, T sc
   cudaError_t e = opt_in_smem(xi_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
   const size_t npairs = (size_t)g.ny * g.Q / 2;
-  xi_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), kStrideThreads, TL::smem_bytes, st>>>(
+  xi_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
       b.A1, reinterpret_cast<Cx<T>*>(H), b.Wx, b.posx, npairs, scale);
   return cudaSuccess;
 }
@@ -941,7 +944,7 @@ static cudaError_t launch_yf(const FastGeom& g, const FastBufs<T>& b, int k0, in
   cudaError_t e = opt_in_smem(yf_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
   dim3 grid(g.Q / TL::B, nk);
-  yf_fast_kernel<T, L><<<grid, kStrideThreads, TL::smem_bytes, st>>>(
+  yf_fast_kernel<T, L><<<grid, TL::NT, TL::smem_bytes, st>>>(
       b.A1 + (size_t)k0 * g.ny * g.Q, b.A2, b.Wy, g.Q);
   return cudaSuccess;
 }
@@ -951,7 +954,7 @@ static cudaError_t launch_yi(const FastGeom& g, const FastBufs<T>& b, int k0, in
   cudaError_t e = opt_in_smem(yi_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
   dim3 grid(g.Q / TL::B, nk);
-  yi_fast_kernel<T, L><<<grid, kStrideThreads, TL::smem_bytes, st>>>(
+  yi_fast_kernel<T, L><<<grid, TL::NT, TL::smem_bytes, st>>>(
       b.A2, b.A1 + (size_t)k0 * g.ny * g.Q, b.Wy, g.Q);
   return cudaSuccess;
 }
