@@ -21,6 +21,9 @@
  *   O7 orc_anisotropy/zeeman PAPER.md:30 (uniaxial, reading Q7), PAPER.md:140-143 (B/mu0)
  *   O8 orc_llg_rhs           PAPER.md:25 eq. 1 on unit m (reading Q4)
  *   O9 orc_rk4_step          classic RK4 + renormalise (reading Q14)
+ *   O10 orc_rkf45_step       Runge-Kutta-Fehlberg 4(5) attempt + max-error step control
+ *                            (the paper names the method and the max-error reduction; tableau, error
+ *                            norm and controller are readings Q23-Q26 of DESIGN.md)
  *
  * Pins: tests/test_oracle_*.py (closed forms, survey/mpmath values in tests/golden/,
  * Gauss-Legendre quadrature of the defining integral, direct-sum vs DFT vs FFT, invariants).
@@ -569,5 +572,80 @@ int orc_rk4_step(const orc_problem *p, double *m, double dt) {
     }
   }
   free(k1); free(ms);
+  return rc;
+}
+
+/* O10.  One attempted step of the Runge-Kutta-Fehlberg 4(5) pair ("only the
+ * Runge-Kutta-Fehlberg Method (RKF45) is supported"; "globally reduces the maximum
+ * error before computing the next step size").  Fehlberg's 1969 tableau, written out:
+ *   c = 0, 1/4, 3/8, 12/13, 1, 1/2
+ *   k1 = f(m)
+ *   k2 = f(m + dt (1/4 k1))
+ *   k3 = f(m + dt (3/32 k1 + 9/32 k2))
+ *   k4 = f(m + dt (1932/2197 k1 - 7200/2197 k2 + 7296/2197 k3))
+ *   k5 = f(m + dt (439/216 k1 - 8 k2 + 3680/513 k3 - 845/4104 k4))
+ *   k6 = f(m + dt (-8/27 k1 + 2 k2 - 3544/2565 k3 + 1859/4104 k4 - 11/40 k5))
+ *   m4 = m + dt (25/216 k1 + 1408/2565 k3 + 2197/4104 k4 - 1/5 k5)
+ *   m5 = m + dt (16/135 k1 + 6656/12825 k3 + 28561/56430 k4 - 9/50 k5 + 2/55 k6)
+ * Readings (Q23-Q26): err = max over cells and components of |m5 - m4|; the step is
+ * accepted iff err <= tol; an accepted step continues with the 5th-order value, renormalised per
+ * cell (m <- m5/|m5|), stage vectors are not renormalised; the next step size, after an accepted
+ * and after a rejected attempt alike, is dt * min(5, max(0.2, 0.9 (tol/err)^(1/5))) clamped to
+ * [dt_min, dt_max] (err = 0 -> factor 5).
+ * m is updated in place only if the step is accepted.  Outputs: *err, *accepted (0/1), *dt_next. */
+int orc_rkf45_step(const orc_problem *p, double *m, double dt, double tol, double dt_min,
+                   double dt_max, double *err, int *accepted, double *dt_next) {
+  static const double A[6][5] = {
+      {0, 0, 0, 0, 0},
+      {1.0 / 4.0, 0, 0, 0, 0},
+      {3.0 / 32.0, 9.0 / 32.0, 0, 0, 0},
+      {1932.0 / 2197.0, -7200.0 / 2197.0, 7296.0 / 2197.0, 0, 0},
+      {439.0 / 216.0, -8.0, 3680.0 / 513.0, -845.0 / 4104.0, 0},
+      {-8.0 / 27.0, 2.0, -3544.0 / 2565.0, 1859.0 / 4104.0, -11.0 / 40.0}};
+  static const double B4[6] = {25.0 / 216.0, 0, 1408.0 / 2565.0, 2197.0 / 4104.0, -1.0 / 5.0, 0};
+  static const double B5[6] = {16.0 / 135.0, 0, 6656.0 / 12825.0, 28561.0 / 56430.0, -9.0 / 50.0,
+                               2.0 / 55.0};
+  const size_t n3 = (size_t)p->nx * p->ny * p->nz * 3;
+  double *k = malloc(6 * n3 * sizeof(double)), *ms = malloc(n3 * sizeof(double));
+  if (!k || !ms) { free(k); free(ms); return 2; }
+  int rc = 0;
+  for (int i = 0; i < 6 && !rc; ++i) {
+    for (size_t q = 0; q < n3; ++q) {
+      double s = 0.0;
+      for (int j = 0; j < i; ++j) s += A[i][j] * k[(size_t)j * n3 + q];
+      ms[q] = m[q] + dt * s;
+    }
+    rc = orc_llg_rhs(p, ms, k + (size_t)i * n3);
+  }
+  if (!rc) {
+    double e = 0.0;
+    for (size_t q = 0; q < n3; ++q) {
+      double s4 = 0.0, s5 = 0.0;
+      for (int j = 0; j < 6; ++j) {
+        s4 += B4[j] * k[(size_t)j * n3 + q];
+        s5 += B5[j] * k[(size_t)j * n3 + q];
+      }
+      const double m4 = m[q] + dt * s4, m5 = m[q] + dt * s5;
+      ms[q] = m5;
+      const double d = fabs(m5 - m4);
+      if (d > e) e = d;
+    }
+    *err = e;
+    *accepted = e <= tol ? 1 : 0;
+    double fac = e > 0.0 ? 0.9 * pow(tol / e, 0.2) : 5.0;
+    if (fac > 5.0) fac = 5.0;
+    if (fac < 0.2) fac = 0.2;
+    double dn = dt * fac;
+    if (dn < dt_min) dn = dt_min;
+    if (dn > dt_max) dn = dt_max;
+    *dt_next = dn;
+    if (*accepted) {
+      for (size_t q = 0; q < n3; q += 3) {
+        const double nrm = sqrt(ms[q] * ms[q] + ms[q + 1] * ms[q + 1] + ms[q + 2] * ms[q + 2]);
+        m[q] = ms[q] / nrm; m[q + 1] = ms[q + 1] / nrm; m[q + 2] = ms[q + 2] / nrm;
+      }
+    }
+  }
+  free(k); free(ms);
   return rc;
 }

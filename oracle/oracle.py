@@ -222,6 +222,16 @@ class Problem:
         _chk(lib().orc_llg_rhs(C.byref(self._c()), _p(m), _p(out)), "llg_rhs")
         return out
 
+    def rkf45_step(self, m, dt, tol, dt_min=0.0, dt_max=1.0):
+        """O10; one attempted RKF45 step.  Returns (m_new, err, accepted, dt_next); m_new is the
+        input when the attempt is rejected."""
+        m = _f64(m).copy()
+        err, acc, dtn = C.c_double(), C.c_int(), C.c_double()
+        _chk(lib().orc_rkf45_step(C.byref(self._c()), _p(m), C.c_double(dt), C.c_double(tol),
+                                  C.c_double(dt_min), C.c_double(dt_max), C.byref(err),
+                                  C.byref(acc), C.byref(dtn)), "rkf45_step")
+        return m, err.value, bool(acc.value), dtn.value
+
     def rk4_step(self, m, dt):
         """O9; returns the new m (input untouched)."""
         m = _f64(m).copy()

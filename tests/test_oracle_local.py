@@ -122,3 +122,85 @@ def test_rk4_conserves_norm_full_problem(oracle):
     m1 = P.rk4_step(m, c.dt)
     assert np.allclose(np.linalg.norm(m1, axis=-1), 1.0, atol=2e-16)
     assert 0 < np.max(np.abs(m1 - m)) < 0.5
+
+
+# ---------------------------------------------------------------- O10: RKF45
+
+def _precession_problem(oracle, alpha, Hz=1e6):
+    return oracle.Problem(n=(2, 1, 1), d=(1e-9,) * 3, Ms=8e5, alpha=alpha, Hext=(0, 0, Hz),
+                          terms=oracle.TERM_ZEEMAN)
+
+
+def test_rkf45_linear_precession_matches_stability_polynomials(oracle):
+    """alpha = 0, uniform m in H = H z: m_x + i m_y obeys y' = i g H y, a linear test equation.
+    One RKF45 step multiplies y by the pair's stability polynomials (Hairer-Norsett-Wanner, Fehlberg
+    4(5)): R5(z) = 1 + z + z^2/2 + z^3/6 + z^4/24 + z^5/120 + z^6/2080 and
+    R4(z) = 1 + ... + z^4/24 + z^5/104, z = i g H dt.  So the accepted state has azimuth arg R5(z)
+    (renormalisation only rescales), m_z unchanged, and the error estimate is
+    s max(|Re|, |Im|) of (R5 - R4)(z) = s max(|z|^6/2080, |z|^5 (1/104 - 1/120))."""
+    P = _precession_problem(oracle, 0.0)
+    th = 0.9
+    s, mz = np.sin(th), np.cos(th)
+    m0 = np.tile(np.array([s, 0.0, mz]), (2, 1, 1, 1))
+    for dt in (2e-12, 1e-12, 3e-13):
+        x = 2.211e5 * 1e6 * dt
+        z = 1j * x
+        R5 = 1 + z + z**2 / 2 + z**3 / 6 + z**4 / 24 + z**5 / 120 + z**6 / 2080
+        m1, err, acc, _ = P.rkf45_step(m0, dt, tol=1.0, dt_min=0.0, dt_max=1.0)
+        assert acc
+        y = s * R5
+        want = np.array([y.real, y.imag, mz])
+        want /= np.linalg.norm(want)
+        assert np.allclose(m1[0, 0, 0], want, rtol=0, atol=3e-16)
+        est = s * max(x**6 / 2080, x**5 * (1 / 104 - 1 / 120))
+        assert abs(err - est) <= 1e-12 * est + 2e-16, (dt, err, est)
+
+
+def test_rkf45_macrospin_fifth_order_and_estimate_scaling(oracle):
+    """Damped macrospin (closed form as for RK4): with the step held fixed the propagated
+    5th-order solution has global error falling 32x when dt halves, and the error estimate of a
+    single step (a 4th-order local error) falls 32x as well."""
+    P = _precession_problem(oracle, 0.1)
+    m0 = np.array([np.sin(1.0), 0.0, np.cos(1.0)])
+    g, Hz, alpha = 2.211e5, 1e6, 0.1
+
+    def run(dt, steps):
+        m = np.tile(m0, (2, 1, 1, 1))
+        for _ in range(steps):
+            m, _, acc, dtn = P.rkf45_step(m, dt, tol=1.0, dt_min=dt, dt_max=dt)
+            assert acc and dtn == dt
+        T = dt * steps
+        mz = np.tanh(alpha * g * Hz * T / (1 + alpha**2) + np.arctanh(m0[2]))
+        phi = g * Hz * T / (1 + alpha**2)
+        sxy = np.sqrt(1 - mz * mz)
+        return np.max(np.abs(m[0, 0, 0] - np.array([sxy * np.cos(phi), sxy * np.sin(phi), mz])))
+
+    e4, e2, e1 = run(4e-12, 10), run(2e-12, 20), run(1e-12, 40)
+    assert e1 < 5e-6 and e4 < 2e-3
+    assert 24 < e4 / e2 < 40 and 24 < e2 / e1 < 40, (e4, e2, e1)
+    m = np.tile(m0, (2, 1, 1, 1))
+    errs = [P.rkf45_step(m, dt, tol=1.0)[1] for dt in (4e-12, 2e-12, 1e-12)]
+    assert 24 < errs[0] / errs[1] < 40 and 24 < errs[1] / errs[2] < 40, errs
+
+
+def test_rkf45_step_control(oracle):
+    """Readings Q23-Q26: accept iff err <= tol; a rejected attempt leaves m untouched; the factor
+    0.9 (tol/err)^(1/5) is clamped to [0.2, 5] and dt to [dt_min, dt_max]."""
+    c = w.get_config(1)
+    P = oracle.Problem(n=c.n, d=c.d, Ms=c.Ms, Aex=c.Aex, alpha=c.alpha, terms=c.terms).prepare()
+    m = c.initial_m()
+    dt = 2e-13
+    m1, err, acc, dtn = P.rkf45_step(m, dt, tol=1.0)
+    assert acc and err > 0 and dtn == 5 * dt                        # huge tol: factor clamp 5
+    assert np.allclose(np.linalg.norm(m1, axis=-1), 1.0, atol=2e-16)
+    m2, err2, acc2, dtn2 = P.rkf45_step(m, dt, tol=err * 1e-9)
+    assert not acc2 and err2 == err and np.array_equal(m2, m)      # rejected: m untouched
+    assert dtn2 == 0.2 * dt                                         # factor clamp 0.2
+    _, _, acc3, dtn3 = P.rkf45_step(m, dt, tol=err)                # err == tol is accepted
+    assert acc3 and abs(dtn3 - 0.9 * dt) < 1e-12 * dt
+    _, _, acc4, dtn4 = P.rkf45_step(m, dt, tol=err / 2)
+    assert not acc4 and abs(dtn4 - 0.9 * 0.5**0.2 * dt) < 1e-12 * dt
+    assert P.rkf45_step(m, dt, tol=1.0, dt_max=3 * dt)[3] == 3 * dt
+    assert P.rkf45_step(m, dt, tol=err * 1e-9, dt_min=0.5 * dt)[3] == 0.5 * dt
+    # against RK4 (a different 4th-order method): same state to the size of the error estimate
+    assert np.max(np.abs(m1 - P.rk4_step(m, dt))) < 50 * err
