@@ -101,6 +101,21 @@ mm_status mm_llg_rhs(mm_ctx *ctx, const void *m, void *dmdt);
  * (fixed-step stand-in for the paper's RKF45; reading Q14). */
 mm_status mm_rk_step(mm_ctx *ctx, void *m_inout, double dt);
 
+/* Adaptive Runge-Kutta-Fehlberg 4(5) stepping (the integrator the paper supports;
+ * the maximum error is reduced before the next step size is computed).  The controller state
+ * (t, dt, tolerance, counters) lives on the DEVICE: mm_rkf45_step enqueues one ATTEMPT -- six
+ * H_eff + LLG evaluations, the 5th-order candidate, err = max over cells and components of
+ * |m5 - m4|, accept iff err <= tol, next dt = dt * min(5, max(0.2, 0.9 (tol/err)^(1/5))) clamped to
+ * [dt_min, dt_max], and, if accepted, m := m5/|m5| per cell and t += dt -- without any host
+ * synchronisation (CUDA-graph capturable).  A rejected attempt leaves m untouched.  Readings
+ * Q23-Q26 of DESIGN.md.  mm_rkf45_init (re)sets the state; mm_rkf45_state synchronises the
+ * stream and reads it back (any output pointer may be NULL). */
+mm_status mm_rkf45_init(mm_ctx *ctx, double t0, double dt0, double tol, double dt_min, double dt_max);
+mm_status mm_rkf45_step(mm_ctx *ctx, void *m_inout);
+mm_status mm_rkf45_state(mm_ctx *ctx, double *t, double *dt_next, double *err_last, double *dt_last,
+                         int *accepted_last, unsigned long long *n_accepted,
+                         unsigned long long *n_rejected);
+
 /* Same operations on HOST buffers (pageable or pinned): copies m host->device into scratch
  * staging, runs the device path, copies the result device->host, synchronises.  These are
  * what bench.py's end-to-end leg times. */

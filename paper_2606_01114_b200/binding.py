@@ -57,6 +57,10 @@ def load_library():
         "mm_heff": [vp, vp, vp],
         "mm_llg_rhs": [vp, vp, vp],
         "mm_rk_step": [vp, vp, dbl],
+        "mm_rkf45_init": [vp, dbl, dbl, dbl, dbl, dbl],
+        "mm_rkf45_step": [vp, vp],
+        "mm_rkf45_state": [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl),
+                           C.POINTER(i32), C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)],
         "mm_demag_field_host": [vp, vp, vp],
         "mm_heff_host": [vp, vp, vp],
         "mm_llg_rhs_host": [vp, vp, vp],
@@ -214,6 +218,24 @@ class Context:
         self._check(m)
         self._call("mm_rk_step", m.data_ptr(), float(dt))
         return m
+
+    def rkf45_init(self, t0=0.0, dt0=1e-13, tol=1e-6, dt_min=0.0, dt_max=1.0):
+        self._call("mm_rkf45_init", float(t0), float(dt0), float(tol), float(dt_min), float(dt_max))
+
+    def rkf45_step(self, m):
+        """Enqueues one attempted RKF45 step (accept/reject and the next dt are decided on the device)."""
+        self._check(m)
+        self._call("mm_rkf45_step", m.data_ptr())
+        return m
+
+    def rkf45_state(self):
+        """Synchronises; dict(t, dt_next, err, dt_last, accepted, n_accepted, n_rejected)."""
+        t, dn, er, dl = C.c_double(), C.c_double(), C.c_double(), C.c_double()
+        acc, na, nr = C.c_int(), C.c_ulonglong(), C.c_ulonglong()
+        self._call("mm_rkf45_state", C.byref(t), C.byref(dn), C.byref(er), C.byref(dl), C.byref(acc),
+                   C.byref(na), C.byref(nr))
+        return {"t": t.value, "dt_next": dn.value, "err": er.value, "dt_last": dl.value,
+                "accepted": bool(acc.value), "n_accepted": na.value, "n_rejected": nr.value}
 
     def nhat_export(self):
         o = tuple(1 if v == 1 else v + 1 for v in self.n)

@@ -15,6 +15,7 @@
 #include "demag_passes.cuh"
 #include "fft_core.cuh"
 #include "pointwise.cuh"
+#include "rkf45.cuh"
 
 using namespace mm;
 
@@ -46,9 +47,11 @@ struct mm_ctx {
   size_t pers_bytes = 0, scr_bytes = 0;
   bool demag_ready = false;
   // persistent offsets
-  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, pers_need;
+  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, pers_need;
   // scratch offsets
-  size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, scr_need;
+  size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, scr_need;
+  RkfState rk_host{};
+  bool rk_ready = false;
   unsigned long long launches = 0;
   Prof prof;
   double prof_ms[Prof::kKinds] = {0};
@@ -120,6 +123,7 @@ static void plan_layout(mm_ctx* c) {
   c->off_posy = o; o += align256((size_t)g.Py * 2);
   c->off_t2x = o; o += align256((size_t)g.Px * cs);
   c->off_t2y = o; o += align256((size_t)g.Py * cs);
+  c->off_rkstate = o; o += align256(sizeof(RkfState));
   c->pers_need = o;
   // scratch
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
@@ -139,6 +143,7 @@ static void plan_layout(mm_ctx* c) {
   c->off_acc = o; o += align256(n3);
   c->off_sin = o; o += align256(n3);
   c->off_sout = o; o += align256(n3);
+  c->off_rkf = o; o += 6 * align256(n3);   // RKF45: k_1..k_6, n3 reals apart (stage state and candidate reuse msa, msb)
   (void)spectra;
   const size_t init_need = demag_init_scratch_bytes(ig);  // aliases the start of scratch
   c->scr_need = o > init_need ? o : init_need;
@@ -242,6 +247,7 @@ mm_status mm_ctx_set_workspace(mm_ctx* ctx, void* persistent, size_t pbytes, voi
   ctx->pers_bytes = pbytes;
   ctx->scr_bytes = sbytes;
   ctx->demag_ready = false;
+  ctx->rk_ready = false;
   return MM_OK;
 }
 
@@ -558,6 +564,76 @@ mm_status mm_rk_step(mm_ctx* ctx, void* m_inout, double dt) {
   if (!(dt > 0)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_rk_step: dt must be positive");
   if ((s = need_ready(ctx, "mm_rk_step", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
   return ctx->dtype == MM_F32 ? rk_t<float>(ctx, m_inout, dt) : rk_t<double>(ctx, m_inout, dt);
+}
+
+}  // extern "C"
+
+// ---- adaptive RKF45 (rkf45.cu)
+
+template <typename T> static mm_status rkf_step_t(mm_ctx* c, void* m) {
+  const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3;
+  // K_1..K_6 contiguous, n3 reals apart; the stage state and the 5th-order candidate reuse the RK4 buffers
+  T* K = reinterpret_cast<T*>(c->scr + c->off_rkf);
+  RkfState* sd = reinterpret_cast<RkfState*>(c->pers + c->off_rkstate);
+  T* stage = reinterpret_cast<T*>(c->scr + c->off_msa);
+  T* cand = reinterpret_cast<T*>(c->scr + c->off_msb);
+  const PwParams<T> p = pw_of<T>(c, c->terms);
+  mm_status s = eval_t<T>(c, PW_RHS, m, K, nullptr, p);
+  for (int i = 1; i <= 5 && s == MM_OK; ++i) {
+    cudaError_t e = rkf_combine_launch<T>(sd, static_cast<const T*>(m), K, n3, i, rkf_row(i), stage, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, "mm_rkf45_step: stage combination", e);
+    ++c->launches;
+    s = eval_t<T>(c, PW_RHS, stage, K + (size_t)i * n3, nullptr, p);
+  }
+  if (s != MM_OK) return s;
+  cudaError_t e = rkf_finish_launch<T>(sd, static_cast<T*>(m), K, n3, cand, c->stream, &c->launches);
+  return e == cudaSuccess ? MM_OK : cuda_fail(c, "mm_rkf45_step: finish", e);
+}
+
+extern "C" {
+
+mm_status mm_rkf45_init(mm_ctx* ctx, double t0, double dt0, double tol, double dt_min, double dt_max) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!ctx->pers) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_rkf45_init: mm_ctx_set_workspace not called");
+  if (!(dt0 > 0) || !(tol > 0) || dt_min < 0 || !(dt_max >= dt_min) || dt0 < dt_min || dt0 > dt_max)
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_rkf45_init: need tol > 0 and 0 <= dt_min <= dt0 <= dt_max, dt0 > 0");
+  RkfState& h = ctx->rk_host;
+  h = RkfState{};
+  h.t = t0; h.dt = dt0; h.tol = tol; h.dt_min = dt_min; h.dt_max = dt_max;
+  cudaError_t e = cudaMemcpyAsync(ctx->pers + ctx->off_rkstate, &h, sizeof(RkfState), cudaMemcpyHostToDevice,
+                                  ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, "mm_rkf45_init", e);
+  ctx->rk_ready = true;
+  return MM_OK;
+}
+
+mm_status mm_rkf45_step(mm_ctx* ctx, void* m_inout) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_rkf45_step", m_inout, m_inout)) != MM_OK) return s;
+  if ((s = need_ready(ctx, "mm_rkf45_step", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
+  if (!ctx->rk_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_rkf45_step: mm_rkf45_init not called");
+  return ctx->dtype == MM_F32 ? rkf_step_t<float>(ctx, m_inout) : rkf_step_t<double>(ctx, m_inout);
+}
+
+mm_status mm_rkf45_state(mm_ctx* ctx, double* t, double* dt_next, double* err_last, double* dt_last,
+                         int* accepted_last, unsigned long long* n_accepted, unsigned long long* n_rejected) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!ctx->rk_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_rkf45_state: mm_rkf45_init not called");
+  RkfState h;
+  cudaError_t e = cudaMemcpyAsync(&h, ctx->pers + ctx->off_rkstate, sizeof(RkfState), cudaMemcpyDeviceToHost,
+                                  ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, "mm_rkf45_state", e);
+  if (t) *t = h.t;
+  if (dt_next) *dt_next = h.dt;
+  if (err_last) *err_last = h.err;
+  if (dt_last) *dt_last = h.dt_last;
+  if (accepted_last) *accepted_last = h.accept;
+  if (n_accepted) *n_accepted = h.n_acc;
+  if (n_rejected) *n_rejected = h.n_rej;
+  return MM_OK;
 }
 
 // ---- host-buffer variants: H2D, device path, D2H, synchronise
