@@ -16,7 +16,8 @@
  *   O2 sign/scale            PAPER.md:45 eq. 4, reading Q2: H = -Ms * sum N(r-r') m(r')
  *   O3 orc_demag_direct*     eq. 4 written out as the O(n^2) real-space sum (ground truth)
  *   O4 orc_demag_dft         the zero-padded circular convolution of PAPER.md:47 by literal DFT
- *   O5 orc_demag_fft*        the same by an own radix-2 FFT, z then y then x
+ *   O5 orc_demag_fft*        the same by an own radix-2 FFT, z then y then x; period 2n,
+ *                            or the next power of two above 2n when n is not one (reading Q27)
  *   O6 orc_exchange          PAPER.md:32 eq. 2, 6-point stencil, Neumann boundary (reading Q5)
  *   O7 orc_anisotropy/zeeman PAPER.md:30 (uniaxial, reading Q7), PAPER.md:140-143 (B/mu0)
  *   O8 orc_llg_rhs           PAPER.md:25 eq. 1 on unit m (reading Q4)
@@ -227,16 +228,19 @@ int orc_demag_direct_sampled(int nx, int ny, int nz, const double *N, double Ms,
 
 static int padded(int n) { return n == 1 ? 1 : 2 * n; } /* reading Q10 */
 
-/* Mirror the octant table onto the padded grid: offset -i sits at index P-i, index n
- * (distance +-n, never needed) is 0 (reading Q11).  out[Px][Py][Pz] for one component. */
-static void mirror_fill(const double *N, int nx, int ny, int nz, int comp, double complex *out) {
-  const int Px = padded(nx), Py = padded(ny), Pz = padded(nz);
+/* Mirror the octant table onto the padded (periodic) grid of period Px x Py x Pz >= 2n (or 1):
+ * offset -i sits at index P-i, the unused indices (distance >= n, never needed) are 0
+ * (reading Q11).  out[Px][Py][Pz] for one component. */
+static void mirror_fill(const double *N, int nx, int ny, int nz, int Px, int Py, int Pz, int comp,
+                        double complex *out) {
   for (int a = 0; a < Px; ++a)
     for (int b = 0; b < Py; ++b)
       for (int c = 0; c < Pz; ++c) {
         const int di = a < nx ? a : a - Px, dj = b < ny ? b : b - Py, dk = c < nz ? c : c - Pz;
         double v = 0.0;
-        if (!(Px > 1 && a == nx) && !(Py > 1 && b == ny) && !(Pz > 1 && c == nz)) {
+        /* offsets of magnitude >= n never occur between two cells of the mesh: 0 (for P = 2n
+         * that is the single index n; for a longer period the whole gap n .. P-n) */
+        if (abs(di) < nx && abs(dj) < ny && abs(dk) < nz) {
           const int r = comp < 3 ? comp : (comp == 5 ? 1 : 0);
           const int cc = comp < 3 ? comp : (comp == 3 ? 1 : 2);
           v = newell_lookup(N, nx, ny, nz, r, cc, di, dj, dk);
@@ -259,7 +263,7 @@ int orc_demag_dft(int nx, int ny, int nz, const double *N, double Ms, const doub
   double complex *mk = malloc(3 * P * sizeof(double complex));
   double complex *hk = malloc(3 * P * sizeof(double complex));
   if (!Nr || !Nk || !mr || !mk || !hk) return 2;
-  for (int comp = 0; comp < 6; ++comp) mirror_fill(N, nx, ny, nz, comp, Nr + comp * P);
+  for (int comp = 0; comp < 6; ++comp) mirror_fill(N, nx, ny, nz, Px, Py, Pz, comp, Nr + comp * P);
   for (int x = 0; x < nx; ++x)
     for (int y = 0; y < ny; ++y)
       for (int z = 0; z < nz; ++z)
@@ -315,7 +319,17 @@ int orc_demag_dft(int nx, int ny, int nz, const double *N, double Ms, const doub
 
 /* ------------------------------------------------------------------ O5: own FFT path */
 
-static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
+/* Period of the FFT path along an axis of n cells: 2n when n is a power of two (the paper's
+ * zero-padding), else the next power of two above 2n.  A circular convolution of
+ * any period P >= 2n - 1 equals the linear convolution of eq. 4 on the n cells (the wrapped
+ * images fall on zero padding), so the field does not depend on this choice (DESIGN.md reading
+ * Q27); it keeps the oracle's FFT the textbook radix-2 one.  orc_fft_period exports it. */
+int orc_fft_period(int n) {
+  if (n == 1) return 1;
+  int P = 2;
+  while (P < 2 * n) P *= 2;
+  return P;
+}
 
 /* Textbook iterative radix-2 decimation-in-time FFT on a contiguous buffer of length n
  * (power of two).  sign = -1 forward, +1 inverse (unnormalised).  tw[q] = exp(sign 2 pi i q/n). */
@@ -376,14 +390,13 @@ static void fft_axis(double complex *A, int Px, int Py, int Pz, int axis, int si
  * Nhat[6][Px][Py][Pz] (the imaginary part is analytically zero; its measured max is
  * returned through max_imag if non-NULL). */
 int orc_demag_fft_nhat(int nx, int ny, int nz, const double *N, double *Nhat, double *max_imag) {
-  if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz)) return 1;
-  const int Px = padded(nx), Py = padded(ny), Pz = padded(nz);
+  const int Px = orc_fft_period(nx), Py = orc_fft_period(ny), Pz = orc_fft_period(nz);
   const size_t P = (size_t)Px * Py * Pz;
   double complex *A = malloc(P * sizeof(double complex));
   if (!A) return 2;
   double mi = 0.0;
   for (int comp = 0; comp < 6; ++comp) {
-    mirror_fill(N, nx, ny, nz, comp, A);
+    mirror_fill(N, nx, ny, nz, Px, Py, Pz, comp, A);
     fft_axis(A, Px, Py, Pz, 2, -1, Px, Py);
     fft_axis(A, Px, Py, Pz, 1, -1, Px, Pz);
     fft_axis(A, Px, Py, Pz, 0, -1, Py, Pz);
@@ -402,8 +415,7 @@ int orc_demag_fft_nhat(int nx, int ny, int nz, const double *N, double *Nhat, do
  * discarded (inverse) are skipped; that changes no value. */
 int orc_demag_fft(int nx, int ny, int nz, const double *Nhat, double Ms, const double *m,
                   double *H) {
-  if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz)) return 1;
-  const int Px = padded(nx), Py = padded(ny), Pz = padded(nz);
+  const int Px = orc_fft_period(nx), Py = orc_fft_period(ny), Pz = orc_fft_period(nz);
   const size_t P = (size_t)Px * Py * Pz;
   double complex *A = calloc(3 * P, sizeof(double complex));
   if (!A) return 2;

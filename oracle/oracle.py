@@ -119,13 +119,20 @@ def demag_dft(N, Ms, m):
 
 
 def padded(n):
+    """Period of the paper's zero-padding: 2n, or 1 for a one-cell axis (Q10)."""
     return 1 if n == 1 else 2 * n
+
+
+def fft_period(n):
+    """Period the oracle's radix-2 FFT path uses: 2n for powers of two, else the next power of
+    two above 2n (same linear convolution, reading Q27)."""
+    return int(lib().orc_fft_period(C.c_int(n)))
 
 
 def demag_fft_nhat(N, return_max_imag=False):
     """O5 set-up: real Fourier-space tensor Nhat[6, Px, Py, Pz]."""
     _, nx, ny, nz = N.shape
-    Nhat = np.zeros((6, padded(nx), padded(ny), padded(nz)))
+    Nhat = np.zeros((6, fft_period(nx), fft_period(ny), fft_period(nz)))
     mi = C.c_double(0.0)
     _chk(lib().orc_demag_fft_nhat(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(N), _p(Nhat),
                                   C.byref(mi)), "demag_fft_nhat")

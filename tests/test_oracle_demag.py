@@ -13,7 +13,11 @@ GOLD = os.path.join(os.path.dirname(__file__), "golden", "demag_film_survey_valu
 
 @pytest.mark.parametrize("n,d", [((16, 16, 2), (5e-9, 5e-9, 3e-9)), ((8, 4, 1), (3e-9, 4e-9, 5e-9)),
                                  ((4, 1, 8), (2e-9, 2e-9, 1e-9)), ((1, 1, 4), (1e-9, 2e-9, 3e-9)),
-                                 ((1, 1, 1), (1e-9, 2e-9, 3e-9))])
+                                 ((1, 1, 1), (1e-9, 2e-9, 3e-9)),
+                                 # not powers of two: O4 keeps the paper's period 2n, O5 pads to the next
+                                 # power of two (reading Q27); both must equal the direct sum
+                                 ((6, 5, 3), (3e-9, 4e-9, 5e-9)), ((7, 3, 2), (2e-9, 2e-9, 1e-9)),
+                                 ((12, 10, 1), (5e-9, 5e-9, 3e-9))])
 def test_direct_vs_dft_vs_fft(oracle, n, d):
     Ms = 8.0e5
     m = w.random_unit_vectors(77, n)
@@ -115,7 +119,17 @@ def test_sampled_equals_full_direct(oracle):
     assert np.array_equal(Hs, Hd[cells])
 
 
-def test_rejects_non_power_of_two(oracle):
-    N = oracle.newell_octant((3, 4, 1), (1, 1, 1))
-    with pytest.raises(RuntimeError):
-        oracle.demag_fft_nhat(N)
+def test_fft_period(oracle):
+    # powers of two keep the paper's 2n; other sizes pad to the next power of two above 2n
+    assert [oracle.fft_period(n) for n in (1, 2, 8, 3, 5, 100, 350, 90)] == [1, 4, 16, 8, 16, 256, 1024, 256]
+
+
+def test_fft_path_on_a_mesh_shaped_like_the_papers_sp4_grid(oracle):
+    # n = (100, 25, 1), 5 x 5 x 3 nm cells; sampled direct sum vs the FFT path
+    n, d, Ms = (100, 25, 1), (5e-9, 5e-9, 3e-9), 8.0e5
+    m = w.random_unit_vectors(5, n)
+    N = oracle.newell_octant(n, d)
+    H = oracle.demag_fft(oracle.demag_fft_nhat(N), Ms, m)
+    cells = np.array([0, 24, 99 * 25, 99 * 25 + 24, 50 * 25 + 12, 1234, 777])
+    Hs = oracle.demag_direct_sampled(N, Ms, m, cells)
+    assert np.max(np.abs(H.reshape(-1, 3)[cells] - Hs)) < 1e-13 * Ms
