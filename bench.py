@@ -353,8 +353,9 @@ def run_sweep(args):
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / steps
 
-    for n in w.SWEEP_MESHES:
-        cfg = cfg5.with_mesh(n, name="cfg5_sweep_%dx%dx%d" % n)
+    meshes = w.PAPER_MESHES if args.paper_meshes else w.SWEEP_MESHES
+    for n in meshes:
+        cfg = cfg5.with_mesh(n, name=("paper_mesh_%dx%dx%d" if args.paper_meshes else "cfg5_sweep_%dx%dx%d") % n)
         for dt in ("f32", "f64"):
             s = 4 if dt == "f32" else 8
             tdt = torch.float32 if dt == "f32" else torch.float64
@@ -381,6 +382,9 @@ def run_sweep(args):
                                  "frac_hbm_measured": total / ms_r / 1e6 / peak,
                                  "frac_hbm_8TBps": total / ms_r / 1e6 / 8000.0},
                     "init_s": t_init, "peak_GBps": peak}
+            if dt == "f64" and tuple(n) in w.PAPER_DEMAG_MS:
+                pms, src = w.PAPER_DEMAG_MS[tuple(n)]
+                line["paper_context"] = {"demag_ms": pms, "hardware": src, "ratio_demag": pms / ms_d}
             ctx.close()
             del m, out, ctx
             torch.cuda.empty_cache()
@@ -412,6 +416,8 @@ def main():
     ap.add_argument("--kchunk", type=int, default=0, help="kx planes per y/z/y launch group (experiments)")
     ap.add_argument("--mesh", default=None, help="override mesh, e.g. 256x256x64 (experiments)")
     ap.add_argument("--sweep", action="store_true", help="config 5: one line per sweep mesh and dtype")
+    ap.add_argument("--paper-meshes", action="store_true",
+                    help="with --sweep: the paper's own meshes (N = 100, 350, 400 cubes, 512x512x90)")
     args = ap.parse_args()
     if args.sweep:
         return run_sweep(args)

@@ -22,7 +22,7 @@
  *    the *_host calls synchronise the stream before returning.
  *  - Errors: every call returns mm_status; nothing is thrown across the ABI.  After a
  *    non-OK status mm_last_error(ctx) holds a one-line explanation.
- *  - Sizes: every n_d must be 1 or a power of two, nx, ny <= 1024, nz <= 512
+ *  - Sizes: every n_d must be of the form 2^a 3^b 5^c 7^d (1 included), nx, ny <= 1024, nz <= 512
  *    (MM_ERR_UNSUPPORTED_SIZE otherwise).  An axis with n_d = 1 is neither padded nor
  *    transformed (reading Q10 in DESIGN.md).
  */
@@ -42,7 +42,7 @@ typedef enum { MM_F32 = 0, MM_F64 = 1 } mm_dtype;
 typedef enum {
   MM_OK = 0,
   MM_ERR_INVALID_ARG = 1,      /* NULL / misaligned pointer, non-positive size or cell, H == m */
-  MM_ERR_UNSUPPORTED_SIZE = 2, /* n_d not 1 or a power of two, or above the planned maximum */
+  MM_ERR_UNSUPPORTED_SIZE = 2, /* n_d has a prime factor above 7, or is above the planned maximum */
   MM_ERR_NOT_INITIALISED = 3,  /* workspace, material or mm_demag_init missing */
   MM_ERR_WORKSPACE = 4,        /* workspace too small */
   MM_ERR_CUDA = 5,             /* CUDA runtime / launch error, text in mm_last_error */

@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(512) zf_kernel(DemagGeom g, const T* __restric
       a = mk<T>(z1.x, 0);
       b = mk<T>(z1.y, 0);
     } else {
-      const int p1 = posz[kz], p2 = posz[(Pz - kz) & (Pz - 1)];
+      const int p1 = posz[kz], p2 = posz[kz ? Pz - kz : 0];
       const Cx<T> z1 = sm[(size_t)(c * Pz + p1) * B + xl];
       const Cx<T> z2 = cconj(sm[(size_t)(c * Pz + p2) * B + xl]);
       const Cx<T> s = cadd(z1, z2), d = csub(z1, z2);
@@ -214,12 +214,19 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+// Threads per CTA: a whole number of threads per column (the in-place stages give thread
+// (col, tt) the butterflies tt, tt + NT, ... of its column).
 static int pick_threads(int B, int rows) {
   int want = B * (rows / 8 > 0 ? rows / 8 : 1);
-  int t = 64;
-  while (t < want && t < 512) t *= 2;
-  if (t < B) t = B;
-  return t;
+  if ((B & (B - 1)) == 0) {
+    int t = 64;
+    while (t < want && t < 512) t *= 2;
+    if (t < B) t = B;
+    return t;
+  }
+  int nt = want / B;
+  if (nt > 512 / B) nt = 512 / B;
+  return B * (nt > 0 ? nt : 1);
 }
 
 template <typename T>

@@ -127,6 +127,58 @@ template <typename T, bool INV> struct Dft<T, 1, INV> {
   static __device__ __forceinline__ void run(Cx<T>*) {}
 };
 
+// Odd prime radices 3, 5, 7 (meshes that are not powers of two: the paper's own workloads are
+// 100 x 25 x 1, N = 100, 350, 400 and 512 x 512 x 90 cells).  With
+// a_k = v_k + v_{R-k}, b_k = v_k - v_{R-k}:
+//   X_j, X_{R-j} = v_0 + sum_k cos(2 pi j k / R) a_k  -/+  i sum_k sin(2 pi j k / R) b_k   (forward).
+template <int R> constexpr double odd_cos(int m) {  // cos(2 pi m / R), m < R
+  const int h = m <= R / 2 ? m : R - m;
+  if (h == 0) return 1.0;
+  if (R == 3) return -0.5;
+  if (R == 5) return h == 1 ? 0.30901699437494742410 : -0.80901699437494742410;
+  return h == 1 ? 0.62348980185873353053 : (h == 2 ? -0.22252093395631440429 : -0.90096886790241912624);
+}
+template <int R> constexpr double odd_sin(int m) {  // sin(2 pi m / R), m < R
+  const int h = m <= R / 2 ? m : R - m;
+  const double sg = m <= R / 2 ? 1.0 : -1.0;
+  if (h == 0) return 0.0;
+  if (R == 3) return sg * 0.86602540378443864676;
+  if (R == 5) return sg * (h == 1 ? 0.95105651629515357212 : 0.58778525229247312917);
+  return sg * (h == 1 ? 0.78183148246802980871 : (h == 2 ? 0.97492791218182360702 : 0.43388373911755812048));
+}
+template <typename T, int R, bool INV> struct DftOdd {
+  static __device__ __forceinline__ void run(Cx<T>* v) {
+    constexpr int H = R / 2;
+    Cx<T> a[H], b[H], out[R];
+#pragma unroll
+    for (int k = 1; k <= H; ++k) {
+      a[k - 1] = mk<T>(v[k].x + v[R - k].x, v[k].y + v[R - k].y);
+      b[k - 1] = mk<T>(v[k].x - v[R - k].x, v[k].y - v[R - k].y);
+    }
+    out[0] = v[0];
+#pragma unroll
+    for (int k = 0; k < H; ++k) { out[0].x += a[k].x; out[0].y += a[k].y; }
+#pragma unroll
+    for (int j = 1; j <= H; ++j) {
+      Cx<T> r = v[0], s = mk<T>((T)0, (T)0);
+#pragma unroll
+      for (int k = 1; k <= H; ++k) {
+        const T c = (T)odd_cos<R>((j * k) % R), sn = (T)odd_sin<R>((j * k) % R);
+        r.x = fma(c, a[k - 1].x, r.x); r.y = fma(c, a[k - 1].y, r.y);
+        s.x = fma(sn, b[k - 1].x, s.x); s.y = fma(sn, b[k - 1].y, s.y);
+      }
+      const Cx<T> lo = mk<T>(r.x + s.y, r.y - s.x), hi = mk<T>(r.x - s.y, r.y + s.x);  // r - i s, r + i s
+      out[j] = INV ? hi : lo;
+      out[R - j] = INV ? lo : hi;
+    }
+#pragma unroll
+    for (int k = 0; k < R; ++k) v[k] = out[k];
+  }
+};
+template <typename T, bool INV> struct Dft<T, 3, INV> : DftOdd<T, 3, INV> {};
+template <typename T, bool INV> struct Dft<T, 5, INV> : DftOdd<T, 5, INV> {};
+template <typename T, bool INV> struct Dft<T, 7, INV> : DftOdd<T, 7, INV> {};
+
 // One forward stage of span S (radix R) over a tile of N rows x B columns in shared memory,
 // row r of column c at sm[r * B + c].  Thread (col, tt) with NT threads per column.
 // W[q] = exp(-2 pi i q / P); wstep = P / S so that w_S^(t u) = W[t u wstep].
@@ -182,6 +234,9 @@ __device__ __forceinline__ void run_stages_fwd(Cx<T>* sm, int B, int col, int tt
     switch (R) {
       case 16: stage_fwd<T, 16>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 8: stage_fwd<T, 8>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 7: stage_fwd<T, 7>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 5: stage_fwd<T, 5>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 3: stage_fwd<T, 3>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 4: stage_fwd<T, 4>(sm, B, col, tt, NT, N, S, W, wstep); break;
       default: stage_fwd<T, 2>(sm, B, col, tt, NT, N, S, W, wstep); break;
     }
@@ -201,6 +256,9 @@ __device__ __forceinline__ void run_stages_inv(Cx<T>* sm, int B, int col, int tt
     switch (R) {
       case 16: stage_inv<T, 16>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 8: stage_inv<T, 8>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 7: stage_inv<T, 7>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 5: stage_inv<T, 5>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 3: stage_inv<T, 3>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 4: stage_inv<T, 4>(sm, B, col, tt, NT, N, S, W, wstep); break;
       default: stage_inv<T, 2>(sm, B, col, tt, NT, N, S, W, wstep); break;
     }
@@ -224,14 +282,25 @@ inline int pos_of_freq(const FftPlan& pl, int k) {
   return pos;
 }
 
+// n = 2^a 3^b 5^c 7^d: radix-8 stages (then 4 or 2) for the power of two, then the odd primes.
+// nstages = -1 if n has another prime factor or needs more than MM_MAX_STAGES stages.
 inline FftPlan make_plan(int n) {
   FftPlan pl{};
   pl.L = n;
   pl.P = n == 1 ? 1 : 2 * n;
   pl.nstages = 0;
-  int rem = n;
-  while (rem >= 8) { pl.radix[pl.nstages++] = 8; rem /= 8; }
-  if (rem > 1) pl.radix[pl.nstages++] = rem;
+  int p2 = 1, odd = n;
+  while (odd % 2 == 0) { odd /= 2; p2 *= 2; }
+  while (p2 >= 8) { pl.radix[pl.nstages++] = 8; p2 /= 8; }
+  if (p2 > 1) pl.radix[pl.nstages++] = p2;
+  const int primes[3] = {7, 5, 3};
+  for (int f : primes)
+    while (odd % f == 0) {
+      if (pl.nstages == MM_MAX_STAGES) { pl.nstages = -1; return pl; }
+      pl.radix[pl.nstages++] = f;
+      odd /= f;
+    }
+  if (odd != 1) pl.nstages = -1;
   return pl;
 }
 

@@ -72,11 +72,16 @@ static bool pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
 static size_t align256(size_t v) { return (v + 255) / 256 * 256; }
 static int padded(int n) { return n == 1 ? 1 : 2 * n; }
 
-static int pick_tile(int limit, size_t bytes_per_col, size_t budget, int cap) {
-  int b = 1;
-  while (b * 2 <= limit && b * 2 <= cap && (size_t)(b * 2) * bytes_per_col <= budget) b *= 2;
-  return b;
+// Tile width: the largest divisor of `extent` (the tiled axis: tiles are never ragged) that is
+// at most `cap` and fits the shared-memory budget.  Powers of two give a power of two.
+static int pick_tile(int extent, size_t bytes_per_col, size_t budget, int cap) {
+  int best = 1;
+  for (int b = 2; b <= extent && b <= cap && (size_t)b * bytes_per_col <= budget; ++b)
+    if (extent % b == 0) best = b;
+  return best;
 }
+// n = 2^a 3^b 5^c 7^d (the radices of fft_core.cuh)
+static bool smooth7(int n) { return n >= 1 && make_plan(n).nstages >= 0; }
 
 // Tile widths and workspace layout; called at create and again if tiles change.
 static void plan_layout(mm_ctx* c) {
@@ -159,9 +164,9 @@ mm_status mm_ctx_create(int nx, int ny, int nz, double dx, double dy, double dz,
     return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: sizes and cell lengths must be positive");
   if (dtype != MM_F32 && dtype != MM_F64)
     return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: unknown dtype %d", (int)dtype);
-  if (!pow2(nx) || !pow2(ny) || !pow2(nz) || nx > 1024 || ny > 1024 || nz > 512)
+  if (!smooth7(nx) || !smooth7(ny) || !smooth7(nz) || nx > 1024 || ny > 1024 || nz > 512)
     return fail(nullptr, MM_ERR_UNSUPPORTED_SIZE,
-                "mm_ctx_create: %dx%dx%d unsupported (each n must be 1 or a power of two, "
+                "mm_ctx_create: %dx%dx%d unsupported (each n must be of the form 2^a 3^b 5^c 7^d, "
                 "nx,ny <= 1024, nz <= 512)", nx, ny, nz);
   mm_ctx* c = new (std::nothrow) mm_ctx();
   if (!c) return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: out of host memory");
@@ -192,6 +197,8 @@ mm_status mm_ctx_set_tiles(mm_ctx* ctx, int bz, int by, int bk) {
   for (int i = 0; i < 3; ++i)
     if (v[i] < 0 || (v[i] > 0 && !pow2(v[i])) || v[i] > 64)
       return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: tile widths must be 0 or a power of two <= 64");
+  if ((bz && ctx->nx % bz) || (by && ctx->nx % by) || (bk && padded(ctx->ny) % bk))
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: bz, by must divide nx and bk must divide the padded ny");
   ctx->want_bz = bz; ctx->want_by = by; ctx->want_bk = bk;
   plan_layout(ctx);
   const size_t cs = 2 * ctx->es;

@@ -40,8 +40,10 @@ def test_create_validates_arguments(lib):
     assert b"workspace" in lib.mm_last_error(h)
     assert lib.mm_set_terms(h, 64) == 1
     assert lib.mm_ctx_destroy(h) == 0
-    assert lib.mm_ctx_create(12, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 2     # not a power of two
-    assert b"power of two" in lib.mm_last_error(None)
+    assert lib.mm_ctx_create(11, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 2     # prime factor 11
+    assert b"2^a 3^b 5^c 7^d" in lib.mm_last_error(None)
+    assert lib.mm_ctx_create(12, 350, 90, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 0   # mixed radix sizes are fine
+    assert lib.mm_ctx_destroy(h) == 0
     assert lib.mm_ctx_create(2048, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 2   # above the plan
     assert lib.mm_ctx_create(16, 16, 2, 0.0, 5e-9, 3e-9, 1, C.byref(h)) == 1
     assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 7, C.byref(h)) == 1

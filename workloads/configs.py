@@ -73,6 +73,14 @@ CONFIGS = {
 SWEEP_MESHES = [(64, 64, 64), (128, 128, 128), (256, 256, 256), (512, 512, 64),
                 (1024, 1024, 64), (1024, 1024, 128)]
 
+# The paper's own benchmark meshes, none a power of two (cubes of side N = 100, 350, 400:
+# PAPER.md:217, 225, 240; the 512 x 512 x 90 multilayer: PAPER.md:250).  "paper_ms": the paper's
+# published demag time per evaluation in fp64 where it prints one for a single device
+# (context, other hardware).
+PAPER_MESHES = [(100, 100, 100), (350, 350, 350), (400, 400, 400), (512, 512, 90)]
+PAPER_DEMAG_MS = {(350, 350, 350): (164.9, "1x H100 HBM3, fp64, PAPER.md:217"),
+                  (100, 100, 100): (29.8, "2x Xeon 8490H, 8 MPI ranks NUMA-pinned, fp64, PAPER.md:240")}
+
 
 def get_config(i: int) -> Config:
     return CONFIGS[i]
