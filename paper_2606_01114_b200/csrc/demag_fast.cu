@@ -429,16 +429,19 @@ template <typename T, int G> struct ZpCfg {
   // One persistent CTA per SM holding every warp the register file and shared memory admit
   // (fp32: 12 x 164 registers, 12 x 18.1 KB): warps of one CTA start together and stay close
   // in the 70 KB instruction stream, which three independent 4-warp CTAs did not (1.06 -> 0.93 ms
-  // at config 4, profiles/r01_v3_*.md).  fp64: 3 CTAs of 2 warps (36.3 KB per warp).
-  static constexpr int WARPS = sizeof(T) == 4 ? 12 : 2;
-  static constexpr int MINB = sizeof(T) == 4 ? 1 : 3;
+  // at config 4, profiles/r01_v3_*.md).  fp64: 6 warps (36.3 KB per warp, 255 registers).
+  static constexpr int WARPS = sizeof(T) == 4 ? 12 : 6;
+  static constexpr int MINB = 1;
+  // fp64: the 15 inter-stage roots of a lane (60 registers) live in shared memory, [u][t]
+  static constexpr int TWS = sizeof(T) == 4 ? 1 : G;
+  static constexpr int tw_bytes = sizeof(T) == 4 ? 0 : 16 * G * (int)sizeof(Cx<T>);
   static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
   static constexpr int table_bytes = 6 * OZP * (int)sizeof(T);  // one (kx, ky) row, 16 B multiple
   // per warp: two stages of NPW pencils + the table rows of the NPW / 2 mirror pairs + one slot
   // for the row ky = ny (the partner of ky = 0, the only pair that does not share its row)
   static constexpr int warp_bytes = 2 * NPW * pencil_bytes + (NPW / 2 + 1) * table_bytes;
   static constexpr int hdr_for(int warps) { return (3 * warps * 8 + 127) / 128 * 128; }  // mbarriers
-  static constexpr int smem_for(int warps) { return hdr_for(warps) + warps * warp_bytes; }
+  static constexpr int smem_for(int warps) { return hdr_for(warps) + warps * warp_bytes + tw_bytes; }
   static constexpr int smem_bytes = smem_for(WARPS);
   static_assert(XB <= Q, "exchange buffer must fit in the pencil it aliases");
   static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0, "bulk copies need 16 B multiples");
@@ -467,8 +470,8 @@ __device__ __forceinline__ void zp_forward(const Cx<T>* a, Cx<T>* xb, const Cx<T
   xb[t] = e[0];
 #pragma unroll
   for (int v = 0; v < 8; ++v) {
-    if (v) xb[(2 * v) * C::PITCH + t] = cmul(e[v], tw[2 * v]);
-    xb[(2 * v + 1) * C::PITCH + t] = cmul(o[v], tw[2 * v + 1]);
+    if (v) xb[(2 * v) * C::PITCH + t] = cmul(e[v], tw[(2 * v) * C::TWS]);
+    xb[(2 * v + 1) * C::PITCH + t] = cmul(o[v], tw[(2 * v + 1) * C::TWS]);
   }
   __syncwarp();
 #pragma unroll
@@ -502,8 +505,8 @@ __device__ __forceinline__ void zp_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw,
   e[0] = xb[t];
 #pragma unroll
   for (int v = 0; v < 8; ++v) {
-    if (v) e[v] = cmulc(xb[(2 * v) * C::PITCH + t], tw[2 * v]);
-    o[v] = cmulc(xb[(2 * v + 1) * C::PITCH + t], tw[2 * v + 1]);
+    if (v) e[v] = cmulc(xb[(2 * v) * C::PITCH + t], tw[(2 * v) * C::TWS]);
+    o[v] = cmulc(xb[(2 * v + 1) * C::PITCH + t], tw[(2 * v + 1) * C::TWS]);
   }
   __syncwarp();
   Dft<T, 8, true>::run(e);
@@ -568,11 +571,20 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     for (int i = 0; i < 3 * WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if constexpr (sizeof(T) == 8) {
+    Cx<T>* tws = reinterpret_cast<Cx<T>*>(smem_raw + C::hdr_for(WARPS) + (size_t)WARPS * C::warp_bytes);
+    for (int i = threadIdx.x; i < 16 * G; i += WARPS * 32) tws[i] = __ldg(Wz + (i % G) * (i / G));
+  }
   __syncthreads();
-  Cx<T> tw[16];
+  Cx<T> twr[sizeof(T) == 4 ? 16 : 1];
+  const Cx<T>* tw = twr;
+  if constexpr (sizeof(T) == 4) {
 #pragma unroll
-  for (int u = 1; u < 16; ++u) tw[u] = __ldg(Wz + t * u);
-  tw[0] = mk<T>(1, 0);
+    for (int u = 1; u < 16; ++u) twr[u] = __ldg(Wz + t * u);
+    twr[0] = mk<T>(1, 0);
+  } else {
+    tw = reinterpret_cast<const Cx<T>*>(smem_raw + C::hdr_for(WARPS) + (size_t)WARPS * C::warp_bytes) + t;
+  }
 
   const int gw = blockIdx.x * WARPS + warp, stride = gridDim.x * WARPS;
   auto pencil_ptr = [&](int task, int p) -> Cx<T>* {
@@ -1000,8 +1012,7 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   cudaError_t e = cudaSuccess;
   prof->mark(0, st);
   if (b.two_x) {
-    if constexpr (sizeof(T) == 4) e = strided2_launch<T>(0, g, b, m, H, scale, 0, 0, st);
-    else e = cudaErrorInvalidValue;
+    e = strided2_launch<T>(0, g, b, m, H, scale, 0, 0, st);
   } else {
 #define CALL_XF(L) launch_xf<T, L>(g, b, m, st)
     MM_DISPATCH_L(g.nx, CALL_XF)
@@ -1015,8 +1026,7 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
     const int nk = nplanes - k0 < kc ? nplanes - k0 : kc;
     prof->mark(1, st);
     if (b.two_y) {
-      if constexpr (sizeof(T) == 4) e = strided2_launch<T>(1, g, b, m, H, scale, k0, nk, st);
-      else e = cudaErrorInvalidValue;
+      e = strided2_launch<T>(1, g, b, m, H, scale, k0, nk, st);
     } else {
 #define CALL_YF(L) launch_yf<T, L>(g, b, k0, nk, st)
       MM_DISPATCH_L(g.ny, CALL_YF)
@@ -1033,8 +1043,7 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
     if (e != cudaSuccess) return e;
     prof->mark(3, st);
     if (b.two_y) {
-      if constexpr (sizeof(T) == 4) e = strided2_launch<T>(3, g, b, m, H, scale, k0, nk, st);
-      else e = cudaErrorInvalidValue;
+      e = strided2_launch<T>(3, g, b, m, H, scale, k0, nk, st);
     } else {
 #define CALL_YI(L) launch_yi<T, L>(g, b, k0, nk, st)
       MM_DISPATCH_L(g.ny, CALL_YI)
@@ -1045,8 +1054,7 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   }
   prof->mark(4, st);
   if (b.two_x) {
-    if constexpr (sizeof(T) == 4) e = strided2_launch<T>(4, g, b, m, H, scale, 0, 0, st);
-    else e = cudaErrorInvalidValue;
+    e = strided2_launch<T>(4, g, b, m, H, scale, 0, 0, st);
   } else {
 #define CALL_XI(L) launch_xi<T, L>(g, b, H, scale, st)
     MM_DISPATCH_L(g.nx, CALL_XI)

@@ -2,7 +2,7 @@
 // (eq. 2, Neumann boundary), uniaxial anisotropy, Zeeman
 // (PAPER.md:140-143), adds H_demag, forms the LLG right-hand side (eq. 1) and
 // applies the RK4 stage arithmetic, so H_eff and k_i are never written to HBM.
-// HBM-bound: 128-bit loads/stores, 4 consecutive z cells (12 reals) per thread; the six
+// HBM-bound: 128-bit loads/stores, 4 (fp32) or 2 (fp64) consecutive z cells per thread; the six
 // neighbours come from L1/L2.
 #include "pointwise.cuh"
 
@@ -10,35 +10,39 @@
 
 namespace mm {
 
-template <typename T> struct V12;  // 12 consecutive reals, 16-byte aligned
-template <> struct V12<float> {
-  static __device__ __forceinline__ void ld(const float* p, float (&v)[12]) {
+// NR consecutive reals, 16-byte aligned, moved by 128-bit accesses.  A thread owns CPT consecutive
+// z cells: 4 in fp32 (12 reals = 3 float4), 2 in fp64 (6 reals = 3 double2; with 4 cells the
+// fp64 kernel held 60 doubles per thread and ran at 56 % of the HBM rate).
+template <typename T> struct Cpt { static constexpr int value = sizeof(T) == 4 ? 4 : 2; };
+template <typename T, int NR> struct VN;
+template <int NR> struct VN<float, NR> {
+  static __device__ __forceinline__ void ld(const float* p, float (&v)[NR]) {
     const float4* q = reinterpret_cast<const float4*>(p);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) {
+    for (int i = 0; i < NR / 4; ++i) {
       const float4 t = q[i];
       v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
     }
   }
-  static __device__ __forceinline__ void st(float* p, const float (&v)[12]) {
+  static __device__ __forceinline__ void st(float* p, const float (&v)[NR]) {
     float4* q = reinterpret_cast<float4*>(p);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) q[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+    for (int i = 0; i < NR / 4; ++i) q[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
   }
 };
-template <> struct V12<double> {
-  static __device__ __forceinline__ void ld(const double* p, double (&v)[12]) {
+template <int NR> struct VN<double, NR> {
+  static __device__ __forceinline__ void ld(const double* p, double (&v)[NR]) {
     const double2* q = reinterpret_cast<const double2*>(p);
 #pragma unroll
-    for (int i = 0; i < 6; ++i) {
+    for (int i = 0; i < NR / 2; ++i) {
       const double2 t = q[i];
       v[2 * i] = t.x; v[2 * i + 1] = t.y;
     }
   }
-  static __device__ __forceinline__ void st(double* p, const double (&v)[12]) {
+  static __device__ __forceinline__ void st(double* p, const double (&v)[NR]) {
     double2* q = reinterpret_cast<double2*>(p);
 #pragma unroll
-    for (int i = 0; i < 6; ++i) q[i] = make_double2(v[2 * i], v[2 * i + 1]);
+    for (int i = 0; i < NR / 2; ++i) q[i] = make_double2(v[2 * i], v[2 * i + 1]);
   }
 };
 
@@ -103,12 +107,14 @@ __device__ __forceinline__ void cell_update(const PwParams<T>& p, const T* mc, c
   }
 }
 
-// Vector path: nz % 4 == 0.  Thread = 4 consecutive z cells of one (x, y) line.
+// Vector path: nz % CPT == 0.  Thread = CPT consecutive z cells of one (x, y) line.
 template <typename T, int MODE>
 __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __restrict__ m,
                                                      const T* __restrict__ Hd, T* __restrict__ out,
                                                      T* __restrict__ m0, T* __restrict__ acc) {
-  const int nzq = p.nz >> 2;
+  constexpr int CPT = Cpt<T>::value, NR = 3 * CPT;
+  using V = VN<T, NR>;
+  const int nzq = p.nz / CPT;
   const size_t total = (size_t)p.nx * p.ny * nzq;
   const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= total) return;
@@ -116,30 +122,30 @@ __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __r
   const int y = (int)((g / nzq) % p.ny);
   const int x = (int)(g / ((size_t)nzq * p.ny));
   const size_t sy = (size_t)p.nz * 3, sx = sy * p.ny;
-  const size_t base = (size_t)x * sx + (size_t)y * sy + (size_t)zq * 12;
+  const size_t base = (size_t)x * sx + (size_t)y * sy + (size_t)zq * NR;
   const bool need_lap = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE;
 
-  T mc[12], lap[12];
-  V12<T>::ld(m + base, mc);
+  T mc[NR], lap[NR];
+  V::ld(m + base, mc);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) lap[i] = 0;
+  for (int i = 0; i < NR; ++i) lap[i] = 0;
   if (need_lap) {
-    T nb[12];
+    T nb[NR];
     if (p.nx > 1) {
-      V12<T>::ld(m + (x > 0 ? base - sx : base), nb);
+      V::ld(m + (x > 0 ? base - sx : base), nb);
 #pragma unroll
-      for (int i = 0; i < 12; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
-      V12<T>::ld(m + (x + 1 < p.nx ? base + sx : base), nb);
+      for (int i = 0; i < NR; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
+      V::ld(m + (x + 1 < p.nx ? base + sx : base), nb);
 #pragma unroll
-      for (int i = 0; i < 12; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
+      for (int i = 0; i < NR; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
     }
     if (p.ny > 1) {
-      V12<T>::ld(m + (y > 0 ? base - sy : base), nb);
+      V::ld(m + (y > 0 ? base - sy : base), nb);
 #pragma unroll
-      for (int i = 0; i < 12; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
-      V12<T>::ld(m + (y + 1 < p.ny ? base + sy : base), nb);
+      for (int i = 0; i < NR; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
+      V::ld(m + (y + 1 < p.ny ? base + sy : base), nb);
 #pragma unroll
-      for (int i = 0; i < 12; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
+      for (int i = 0; i < NR; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
     }
     {
       T lo[3], hi[3];
@@ -147,35 +153,35 @@ __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __r
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         lo[c] = has_lo ? m[base - 3 + c] : mc[c];
-        hi[c] = has_hi ? m[base + 12 + c] : mc[9 + c];
+        hi[c] = has_hi ? m[base + NR + c] : mc[NR - 3 + c];
       }
 #pragma unroll
-      for (int j = 0; j < 4; ++j)
+      for (int j = 0; j < CPT; ++j)
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
           const T below = j == 0 ? lo[c] : mc[3 * (j - 1) + c];
-          const T above = j == 3 ? hi[c] : mc[3 * (j + 1) + c];
+          const T above = j == CPT - 1 ? hi[c] : mc[3 * (j + 1) + c];
           lap[3 * j + c] += p.ex[2] * ((below - mc[3 * j + c]) + (above - mc[3 * j + c]));
         }
     }
   }
-  T hd[12], m0v[12], accv[12], o[12];
+  T hd[NR], m0v[NR], accv[NR], o[NR];
 #pragma unroll
-  for (int i = 0; i < 12; ++i) hd[i] = m0v[i] = accv[i] = 0;
-  if (MODE != PW_EXCHANGE && (p.terms & MM_TERM_DEMAG)) V12<T>::ld(Hd + base, hd);
+  for (int i = 0; i < NR; ++i) hd[i] = m0v[i] = accv[i] = 0;
+  if (MODE != PW_EXCHANGE && (p.terms & MM_TERM_DEMAG)) V::ld(Hd + base, hd);
   if (MODE == PW_RK_STAGE || MODE == PW_RK_FINAL) {
-    V12<T>::ld(m0 + base, m0v);
-    if (!(MODE == PW_RK_STAGE && p.first)) V12<T>::ld(acc + base, accv);
+    V::ld(m0 + base, m0v);
+    if (!(MODE == PW_RK_STAGE && p.first)) V::ld(acc + base, accv);
   }
 #pragma unroll
-  for (int j = 0; j < 4; ++j)
+  for (int j = 0; j < CPT; ++j)
     cell_update<T, MODE>(p, mc + 3 * j, lap + 3 * j, hd + 3 * j, m0v + 3 * j, accv + 3 * j,
                          o + 3 * j);
-  if (MODE == PW_RK_STAGE) V12<T>::st(acc + base, accv);
-  V12<T>::st((MODE == PW_RK_FINAL ? m0 : out) + base, o);
+  if (MODE == PW_RK_STAGE) V::st(acc + base, accv);
+  V::st((MODE == PW_RK_FINAL ? m0 : out) + base, o);
 }
 
-// Scalar path for nz in {1, 2} (thin films): thread = one cell.
+// Scalar path for the other nz (thin films, odd nz): thread = one cell.
 template <typename T, int MODE>
 __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __restrict__ m,
                                                       const T* __restrict__ Hd, T* __restrict__ out,
@@ -227,8 +233,8 @@ __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __
 template <typename T, int MODE>
 static void launch_mode(const PwParams<T>& p, const T* m, const T* Hd, T* out, T* m0, T* acc,
                         cudaStream_t st) {
-  if (p.nz % 4 == 0) {
-    const size_t total = (size_t)p.nx * p.ny * (p.nz / 4);
+  if (p.nz % Cpt<T>::value == 0) {
+    const size_t total = (size_t)p.nx * p.ny * (p.nz / Cpt<T>::value);
     pw_vec_kernel<T, MODE><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
   } else {
     const size_t total = (size_t)p.nx * p.ny * p.nz;
