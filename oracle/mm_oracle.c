@@ -22,6 +22,9 @@
  *   O7 orc_anisotropy/zeeman PAPER.md:30 (uniaxial, reading Q7), PAPER.md:140-143 (B/mu0)
  *   O8 orc_llg_rhs           PAPER.md:25 eq. 1 on unit m (reading Q4)
  *   O9 orc_rk4_step          classic RK4 + renormalise (reading Q14)
+ *   O11 orc_dmi              PAPER.md:34-39 eq. 3, central differences, boundary rule of the exchange stencil (Q28)
+ *   O12 orc_stt              spin-transfer torque as a local effective field a_damp (m x p) + a_field p
+ *                            (PAPER.md:30 names the term; amplitudes are inputs, reading Q29)
  *   O10 orc_rkf45_step       Runge-Kutta-Fehlberg 4(5) attempt + max-error step control
  *                            (the paper names the method and the max-error reduction; tableau, error
  *                            norm and controller are readings Q23-Q26 of DESIGN.md)
@@ -46,7 +49,8 @@ typedef __float128 quad;
 
 #define ORC_MU0 (4.0e-7 * M_PI) /* reading Q8: 4 pi 1e-7 T m / A */
 
-enum { ORC_TERM_DEMAG = 1, ORC_TERM_EXCHANGE = 2, ORC_TERM_ANISOTROPY = 4, ORC_TERM_ZEEMAN = 8 };
+enum { ORC_TERM_DEMAG = 1, ORC_TERM_EXCHANGE = 2, ORC_TERM_ANISOTROPY = 4, ORC_TERM_ZEEMAN = 8,
+       ORC_TERM_DMI = 16, ORC_TERM_STT = 32 };
 
 int orc_num_threads(void) {
 #ifdef _OPENMP
@@ -497,6 +501,57 @@ int orc_anisotropy(size_t ncell, double Ms, double Ku, const double u[3], const 
   return 0;
 }
 
+/* O11 DMI (eq. 3): H = 2D/(mu0 Ms) sum_{k=x,y,z} e_k^DMI x dm/dk, with the three
+ * DMI vectors e_k^DMI given as e[k][0..2] (interfacial: e_x = (0,1,0), e_y = (-1,0,0), e_z = 0;
+ * bulk: e_k = unit vector k).  dm/dk is the central difference
+ * (m(i+e_k) - m(i-e_k)) / (2 D_k); a neighbour outside the mesh is replaced by the cell itself
+ * (the rule of the exchange stencil, reading Q5; reading Q28), so an axis with
+ * n_k = 1 contributes 0. */
+int orc_dmi(int nx, int ny, int nz, double dx, double dy, double dz, double Ms, double D,
+            const double e[9], const double *m, double *H) {
+  const double pref = 2.0 * D / (ORC_MU0 * Ms);
+  const double h[3] = {dx, dy, dz};
+  const int n[3] = {nx, ny, nz};
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int x = 0; x < nx; ++x)
+    for (int y = 0; y < ny; ++y)
+      for (int z = 0; z < nz; ++z) {
+        const int idx[3] = {x, y, z};
+        const size_t i0 = (((size_t)x * ny + y) * nz + z) * 3;
+        double acc[3] = {0, 0, 0};
+        for (int k = 0; k < 3; ++k) {
+          int ip[3] = {x, y, z}, im[3] = {x, y, z};
+          ip[k] = idx[k] + 1 < n[k] ? idx[k] + 1 : idx[k];
+          im[k] = idx[k] - 1 >= 0 ? idx[k] - 1 : idx[k];
+          double dm[3];
+          for (int c = 0; c < 3; ++c)
+            dm[c] = (m[(((size_t)ip[0] * ny + ip[1]) * nz + ip[2]) * 3 + c] -
+                     m[(((size_t)im[0] * ny + im[1]) * nz + im[2]) * 3 + c]) / (2.0 * h[k]);
+          const double *ek = e + 3 * k;
+          acc[0] += ek[1] * dm[2] - ek[2] * dm[1];
+          acc[1] += ek[2] * dm[0] - ek[0] * dm[2];
+          acc[2] += ek[0] * dm[1] - ek[1] * dm[0];
+        }
+        for (int c = 0; c < 3; ++c) H[i0 + c] = pref * acc[c];
+      }
+  return 0;
+}
+
+/* O12 spin-transfer torque as an effective field (PAPER.md:30 names the Slonczewski torque as a
+ * local term; its prefactors are not printed): H = a_damp (m x p) + a_field p with a unit
+ * polarisation p and the two amplitudes in A/m given by the caller (reading Q29).
+ * Under eq. 1 the first part gives the damping-like torque ~ m x (m x p), the second the
+ * field-like torque ~ m x p. */
+int orc_stt(size_t ncell, const double pvec[3], double a_damp, double a_field, const double *m, double *H) {
+  for (size_t i = 0; i < ncell; ++i) {
+    const double *mi = m + 3 * i;
+    H[3 * i + 0] = a_damp * (mi[1] * pvec[2] - mi[2] * pvec[1]) + a_field * pvec[0];
+    H[3 * i + 1] = a_damp * (mi[2] * pvec[0] - mi[0] * pvec[2]) + a_field * pvec[1];
+    H[3 * i + 2] = a_damp * (mi[0] * pvec[1] - mi[1] * pvec[0]) + a_field * pvec[2];
+  }
+  return 0;
+}
+
 /* ------------------------------------------------------------------ problem + O8, O9 */
 
 typedef struct {
@@ -505,6 +560,8 @@ typedef struct {
   double Ms, Aex, Ku, axis[3], alpha, gamma, Hext[3];
   unsigned terms;
   const double *Nhat; /* from orc_demag_fft_nhat; required if DEMAG is enabled */
+  double D, edmi[9];                      /* DMI constant (J/m^2) and the three DMI vectors */
+  double stt_p[3], stt_damp, stt_field;   /* spin-torque field: unit polarisation, amplitudes (A/m) */
 } orc_problem;
 
 /* H_eff = sum of enabled terms. */
@@ -530,6 +587,14 @@ int orc_heff(const orc_problem *p, const double *m, double *H) {
   if (p->terms & ORC_TERM_ZEEMAN)
     for (size_t i = 0; i < n; ++i)
       for (int c = 0; c < 3; ++c) H[3 * i + c] += p->Hext[c];
+  if (p->terms & ORC_TERM_DMI) {
+    orc_dmi(p->nx, p->ny, p->nz, p->dx, p->dy, p->dz, p->Ms, p->D, p->edmi, m, T);
+    for (size_t i = 0; i < 3 * n; ++i) H[i] += T[i];
+  }
+  if (p->terms & ORC_TERM_STT) {
+    orc_stt(n, p->stt_p, p->stt_damp, p->stt_field, m, T);
+    for (size_t i = 0; i < 3 * n; ++i) H[i] += T[i];
+  }
   free(T);
   return 0;
 }

@@ -22,7 +22,11 @@ _LIB = os.path.join(_HERE, "libmm_oracle.so")
 
 MU0 = 4.0e-7 * np.pi  # reading Q8
 
-TERM_DEMAG, TERM_EXCHANGE, TERM_ANISOTROPY, TERM_ZEEMAN = 1, 2, 4, 8
+TERM_DEMAG, TERM_EXCHANGE, TERM_ANISOTROPY, TERM_ZEEMAN, TERM_DMI, TERM_STT = 1, 2, 4, 8, 16, 32
+
+# DMI vectors e_k^DMI of PAPER.md:39, rows k = x, y, z
+DMI_INTERFACIAL = ((0.0, 1.0, 0.0), (-1.0, 0.0, 0.0), (0.0, 0.0, 0.0))
+DMI_BULK = ((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0))
 
 
 def build(force: bool = False) -> str:
@@ -42,7 +46,9 @@ class _Problem(C.Structure):
                 ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
                 ("Ms", C.c_double), ("Aex", C.c_double), ("Ku", C.c_double),
                 ("axis", C.c_double * 3), ("alpha", C.c_double), ("gamma", C.c_double),
-                ("Hext", C.c_double * 3), ("terms", C.c_uint), ("Nhat", C.c_void_p)]
+                ("Hext", C.c_double * 3), ("terms", C.c_uint), ("Nhat", C.c_void_p),
+                ("D", C.c_double), ("edmi", C.c_double * 9),
+                ("stt_p", C.c_double * 3), ("stt_damp", C.c_double), ("stt_field", C.c_double)]
 
 
 def lib():
@@ -170,6 +176,27 @@ def anisotropy(Ms, Ku, axis, m):
     return H
 
 
+def dmi(d, Ms, D, e, m):
+    """O11: DMI field of eq. 3 for the DMI vectors e[k] (3 x 3)."""
+    m = _f64(m)
+    nx, ny, nz = m.shape[:3]
+    ev = _f64(np.asarray(e).reshape(9))
+    H = np.zeros_like(m)
+    _chk(lib().orc_dmi(C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_double(d[0]), C.c_double(d[1]),
+                       C.c_double(d[2]), C.c_double(Ms), C.c_double(D), _p(ev), _p(m), _p(H)), "dmi")
+    return H
+
+
+def stt(p, a_damp, a_field, m):
+    """O12: spin-torque effective field a_damp (m x p) + a_field p."""
+    m = _f64(m)
+    pv = _f64(p)
+    H = np.zeros_like(m)
+    _chk(lib().orc_stt(C.c_size_t(m.size // 3), _p(pv), C.c_double(a_damp), C.c_double(a_field),
+                       _p(m), _p(H)), "stt")
+    return H
+
+
 def llg_torque(alpha, gamma, m, H):
     """O8 on a given field."""
     m = _f64(m)
@@ -194,6 +221,11 @@ class Problem:
     gamma: float = 2.211e5
     Hext: tuple = (0.0, 0.0, 0.0)
     terms: int = TERM_DEMAG | TERM_EXCHANGE
+    D: float = 0.0
+    edmi: tuple = DMI_INTERFACIAL
+    stt_p: tuple = (0.0, 0.0, 1.0)
+    stt_damp: float = 0.0
+    stt_field: float = 0.0
     N: np.ndarray | None = field(default=None, repr=False)
     Nhat: np.ndarray | None = field(default=None, repr=False)
 
@@ -215,6 +247,10 @@ class Problem:
         s.Hext[:] = list(self.Hext)
         s.terms = self.terms
         s.Nhat = self.Nhat.ctypes.data if self.Nhat is not None else None
+        s.D = self.D
+        s.edmi[:] = [float(v) for row in self.edmi for v in row]
+        s.stt_p[:] = list(self.stt_p)
+        s.stt_damp, s.stt_field = self.stt_damp, self.stt_field
         return s
 
     def heff(self, m):

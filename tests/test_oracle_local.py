@@ -204,3 +204,114 @@ def test_rkf45_step_control(oracle):
     assert P.rkf45_step(m, dt, tol=err * 1e-9, dt_min=0.5 * dt)[3] == 0.5 * dt
     # against RK4 (a different 4th-order method): same state to the size of the error estimate
     assert np.max(np.abs(m1 - P.rk4_step(m, dt))) < 50 * err
+
+
+# ------------------------------------------------------------------ O11 DMI (eq. 3)
+
+def _linear(n, axis, comp, slope, d):
+    """m_comp = slope * (coordinate along axis); the stencil is linear per component, so the test
+    input need not have unit length."""
+    m = np.zeros(n + (3,))
+    shape = [1, 1, 1]
+    shape[axis] = n[axis]
+    m[..., comp] = (slope * d[axis] * np.arange(n[axis])).reshape(shape)
+    return m
+
+
+def test_dmi_zero_for_uniform_and_single_cell_axes(oracle):
+    m = np.zeros((5, 4, 3, 3))
+    m[...] = np.array([0.6, 0.0, 0.8])
+    for e in (oracle.DMI_INTERFACIAL, oracle.DMI_BULK):
+        assert np.all(oracle.dmi((1e-9, 2e-9, 3e-9), 8e5, 3e-3, e, m) == 0.0)
+    mm = w.random_unit_vectors(4, (1, 1, 1))
+    assert np.all(oracle.dmi((1e-9,) * 3, 8e5, 3e-3, oracle.DMI_BULK, mm) == 0.0)
+
+
+def test_dmi_interfacial_is_the_textbook_field(oracle):
+    """e_x = e_y-hat, e_y = -e_x-hat:  sum_k e_k x d_k m =
+    (d_x m_z, d_y m_z, -d_x m_x - d_y m_y); interior cells see the exact slope, surface cells
+    half of it (missing neighbour := the cell itself)."""
+    n, d, Ms, D = (6, 5, 2), (2e-9, 3e-9, 1e-9), 8e5, 3e-3
+    pref = 2 * D / (MU0 * Ms)
+    cases = [((0, 2, 7e7), (0, 1.0)), ((1, 2, -4e7), (1, 1.0)), ((0, 0, 5e7), (2, -1.0)), ((1, 1, 6e7), (2, -1.0)),
+             ((0, 1, 5e7), None), ((1, 0, 5e7), None), ((2, 0, 5e7), None), ((2, 2, 5e7), None)]
+    for (axis, comp, slope), expect in cases:
+        H = oracle.dmi(d, Ms, D, oracle.DMI_INTERFACIAL, _linear(n, axis, comp, slope, d))
+        if expect is None:
+            assert np.all(H == 0.0), (axis, comp)
+            continue
+        oc, sign = expect
+        inner = [slice(None)] * 3
+        inner[axis] = slice(1, -1)
+        assert np.allclose(H[tuple(inner) + (oc,)], sign * pref * slope, rtol=1e-12)
+        edge = [slice(None)] * 3
+        edge[axis] = 0
+        assert np.allclose(H[tuple(edge) + (oc,)], 0.5 * sign * pref * slope, rtol=1e-12)
+        others = [c for c in range(3) if c != oc]
+        assert np.all(H[..., others] == 0.0)
+
+
+def test_dmi_bulk_is_the_curl(oracle):
+    """e_k = unit vector k: sum_k e_k x d_k m = curl m.  On m = (sin(q y), sin(q z), sin(q x)) the
+    central difference of sin is cos * sin(q D)/D exactly (interior cells)."""
+    n, d, Ms, D = (9, 8, 7), (1e-9, 1.5e-9, 2e-9), 1e6, 2e-3
+    q = 2.0e8
+    x = (np.arange(n[0]) * d[0]).reshape(-1, 1, 1)
+    y = (np.arange(n[1]) * d[1]).reshape(1, -1, 1)
+    z = (np.arange(n[2]) * d[2]).reshape(1, 1, -1)
+    m = np.zeros(n + (3,))
+    m[..., 0] = np.sin(q * y)
+    m[..., 1] = np.sin(q * z)
+    m[..., 2] = np.sin(q * x)
+    H = oracle.dmi(d, Ms, D, oracle.DMI_BULK, m)
+    pref = 2 * D / (MU0 * Ms)
+    fd = [np.sin(q * h) / h for h in d]
+    curl = np.zeros_like(m)
+    curl[..., 0] = 0 * x + 0 * y - np.cos(q * z) * fd[2]      # d_y m_z - d_z m_y
+    curl[..., 1] = 0 * y + 0 * z - np.cos(q * x) * fd[0]      # d_z m_x - d_x m_z
+    curl[..., 2] = 0 * x + 0 * z - np.cos(q * y) * fd[1]      # d_x m_y - d_y m_x
+    inner = (slice(1, -1),) * 3
+    assert np.allclose(H[inner], pref * curl[inner], rtol=1e-10, atol=1e-12 * pref * q)
+
+
+def test_dmi_general_vectors_match_numpy_cross(oracle):
+    """Arbitrary e_k on a random field: numpy's gradient-free restatement with np.cross and np.roll."""
+    n, d, Ms, D = (5, 4, 3), (1e-9, 2e-9, 3e-9), 8e5, 1e-3
+    rng = np.random.default_rng(3)
+    e = rng.normal(size=(3, 3))
+    m = w.random_unit_vectors(9, n)
+    H = oracle.dmi(d, Ms, D, e, m)
+    acc = np.zeros_like(m)
+    for k in range(3):
+        hi = np.concatenate([np.take(m, range(1, n[k]), axis=k), np.take(m, [n[k] - 1], axis=k)], axis=k)
+        lo = np.concatenate([np.take(m, [0], axis=k), np.take(m, range(0, n[k] - 1), axis=k)], axis=k)
+        acc += np.cross(e[k], (hi - lo) / (2 * d[k]))
+    assert np.allclose(H, 2 * D / (MU0 * Ms) * acc, rtol=1e-12, atol=1e-3)
+
+
+# ------------------------------------------------------------------ O12 spin-torque field
+
+def test_stt_field_closed_forms(oracle):
+    p = np.array([0.0, 0.0, 1.0])
+    m = np.zeros((3, 1, 1, 3))
+    m[0, 0, 0] = [1, 0, 0]
+    m[1, 0, 0] = [0, 1, 0]
+    m[2, 0, 0] = [0, 0, 1]
+    H = oracle.stt(p, 2.0e3, 5.0e2, m)
+    assert np.allclose(H[0, 0, 0], [0, -2.0e3, 5.0e2])     # x-hat x z-hat = -y-hat
+    assert np.allclose(H[1, 0, 0], [2.0e3, 0, 5.0e2])      # y-hat x z-hat = +x-hat
+    assert np.allclose(H[2, 0, 0], [0, 0, 5.0e2])          # m || p: only the field-like part
+    mm = w.random_unit_vectors(2, (4, 3, 2))
+    pp = np.array([1.0, 2.0, 2.0]) / 3.0
+    assert np.allclose(oracle.stt(pp, 7.0, -3.0, mm), 7.0 * np.cross(mm, pp) - 3.0 * pp, rtol=1e-13)
+
+
+def test_heff_adds_dmi_and_stt(oracle):
+    n, d = (6, 4, 2), (2e-9, 2e-9, 1e-9)
+    m = w.random_unit_vectors(5, n)
+    kw = dict(n=n, d=d, Ms=8e5, Aex=1.3e-11, alpha=0.1)
+    base = oracle.Problem(terms=2, **kw).heff(m)
+    full = oracle.Problem(terms=2 | 16 | 32, D=3e-3, edmi=oracle.DMI_INTERFACIAL, stt_p=(0, 0, 1),
+                          stt_damp=1e3, stt_field=2e2, **kw).heff(m)
+    want = base + oracle.dmi(d, 8e5, 3e-3, oracle.DMI_INTERFACIAL, m) + oracle.stt((0, 0, 1), 1e3, 2e2, m)
+    assert np.allclose(full, want, rtol=1e-13, atol=1e-6)
