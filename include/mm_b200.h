@@ -50,7 +50,8 @@ typedef enum {
 } mm_status;
 
 /* Field terms of H_eff (H_eff is a sum of terms). */
-enum { MM_TERM_DEMAG = 1, MM_TERM_EXCHANGE = 2, MM_TERM_ANISOTROPY = 4, MM_TERM_ZEEMAN = 8 };
+enum { MM_TERM_DEMAG = 1, MM_TERM_EXCHANGE = 2, MM_TERM_ANISOTROPY = 4, MM_TERM_ZEEMAN = 8,
+       MM_TERM_DMI = 16, MM_TERM_STT = 32 };
 
 /* Mesh of nx x ny x nz cells of size dx x dy x dz metres (Mesh(n, dx)). */
 mm_status mm_ctx_create(int nx, int ny, int nz, double dx, double dy, double dz, mm_dtype dtype,
@@ -73,6 +74,18 @@ mm_status mm_set_material(mm_ctx *ctx, double Ms, double Aex, double Ku, const d
                           double alpha, double gamma);
 /* Uniform external field in A/m (PAPER.md:140-143 ExternalField(B/mu0)). */
 mm_status mm_set_zeeman(mm_ctx *ctx, const double Hext[3]);
+/* Dzyaloshinskii-Moriya interaction (eq. 3):
+ *   H = 2D/(mu0 Ms) sum_{k=x,y,z} e_k^DMI x dm/dk,
+ * D in J/m^2, e[3 k + c] = component c of the DMI vector of direction k.  The paper's two
+ * choices: interfacial e_x = (0,1,0), e_y = (-1,0,0), e_z = 0; bulk e_k = unit vector k.
+ * dm/dk is the central difference over the two neighbours of the exchange stencil, a
+ * neighbour outside the mesh being the cell itself (reading Q28).  Needs
+ * mm_set_material first (Ms).  Enabled by MM_TERM_DMI. */
+mm_status mm_set_dmi(mm_ctx *ctx, double D, const double e[9]);
+/* Spin-transfer torque as a local effective field (reading Q29):
+ *   H = a_damp (m x p) + a_field p,  p normalised by the library, amplitudes in A/m.
+ * Enabled by MM_TERM_STT. */
+mm_status mm_set_stt(mm_ctx *ctx, const double p[3], double a_damp, double a_field);
 /* OR of MM_TERM_*; default DEMAG | EXCHANGE. */
 mm_status mm_set_terms(mm_ctx *ctx, unsigned term_mask);
 
@@ -94,6 +107,8 @@ mm_status mm_demag_field(mm_ctx *ctx, const void *m, void *H);
 mm_status mm_exchange_field(mm_ctx *ctx, const void *m, void *H);
 /* H := sum of the enabled terms. */
 mm_status mm_heff(mm_ctx *ctx, const void *m, void *H);
+/* H := H_DMI(m) alone (eq. 3); same argument rules as mm_exchange_field. */
+mm_status mm_dmi_field(mm_ctx *ctx, const void *m, void *H);
 /* dmdt := -gamma/(1+alpha^2) [m x H_eff + alpha m x (m x H_eff)]  (eq. 1);
  * H_eff is evaluated internally and not materialised. */
 mm_status mm_llg_rhs(mm_ctx *ctx, const void *m, void *dmdt);

@@ -16,7 +16,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmm_b200.so")
 
 MM_F32, MM_F64 = 0, 1
-TERM_DEMAG, TERM_EXCHANGE, TERM_ANISOTROPY, TERM_ZEEMAN = 1, 2, 4, 8
+TERM_DEMAG, TERM_EXCHANGE, TERM_ANISOTROPY, TERM_ZEEMAN, TERM_DMI, TERM_STT = 1, 2, 4, 8, 16, 32
+# DMI vectors e_k^DMI of PAPER.md:39 (rows k = x, y, z)
+DMI_INTERFACIAL = ((0.0, 1.0, 0.0), (-1.0, 0.0, 0.0), (0.0, 0.0, 0.0))
+DMI_BULK = ((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0))
 STATUS = {0: "MM_OK", 1: "MM_ERR_INVALID_ARG", 2: "MM_ERR_UNSUPPORTED_SIZE",
           3: "MM_ERR_NOT_INITIALISED", 4: "MM_ERR_WORKSPACE", 5: "MM_ERR_CUDA",
           6: "MM_ERR_NOT_IMPLEMENTED"}
@@ -49,12 +52,15 @@ def load_library():
         "mm_ctx_set_workspace": [vp, vp, sz, vp, sz],
         "mm_set_material": [vp, dbl, dbl, dbl, C.POINTER(dbl), dbl, dbl],
         "mm_set_zeeman": [vp, C.POINTER(dbl)],
+        "mm_set_dmi": [vp, dbl, C.POINTER(dbl)],
+        "mm_set_stt": [vp, C.POINTER(dbl), dbl, dbl],
         "mm_set_terms": [vp, C.c_uint],
         "mm_demag_init": [vp],
         "mm_demag_nhat_export": [vp, vp],
         "mm_demag_field": [vp, vp, vp],
         "mm_exchange_field": [vp, vp, vp],
         "mm_heff": [vp, vp, vp],
+        "mm_dmi_field": [vp, vp, vp],
         "mm_llg_rhs": [vp, vp, vp],
         "mm_rk_step": [vp, vp, dbl],
         "mm_rkf45_init": [vp, dbl, dbl, dbl, dbl, dbl],
@@ -158,6 +164,12 @@ class Context:
     def set_zeeman(self, Hext):
         self._call("mm_set_zeeman", (C.c_double * 3)(*Hext))
 
+    def set_dmi(self, D, e=DMI_INTERFACIAL):
+        self._call("mm_set_dmi", float(D), (C.c_double * 9)(*[float(v) for row in e for v in row]))
+
+    def set_stt(self, p, a_damp, a_field=0.0):
+        self._call("mm_set_stt", (C.c_double * 3)(*p), float(a_damp), float(a_field))
+
     def set_terms(self, mask):
         self._call("mm_set_terms", int(mask))
 
@@ -207,6 +219,9 @@ class Context:
 
     def exchange_field(self, m, out=None):
         return self._field("mm_exchange_field", m, out)
+
+    def dmi_field(self, m, out=None):
+        return self._field("mm_dmi_field", m, out)
 
     def heff(self, m, out=None):
         return self._field("mm_heff", m, out)

@@ -32,6 +32,8 @@ struct mm_ctx {
   bool have_material = false;
   double Ms = 0, Aex = 0, Ku = 0, axis[3] = {0, 0, 1}, alpha = 0, gamma = 2.211e5;
   double Hext[3] = {0, 0, 0};
+  double Ddmi = 0, edmi[9] = {0, 1, 0, -1, 0, 0, 0, 0, 0};   // interfacial vectors by default
+  double stt_p[3] = {0, 0, 1}, stt_damp = 0, stt_field = 0;
   unsigned terms = MM_TERM_DEMAG | MM_TERM_EXCHANGE;
   // plan
   DemagGeom geom{};
@@ -283,9 +285,30 @@ mm_status mm_set_zeeman(mm_ctx* ctx, const double Hext[3]) {
   return MM_OK;
 }
 
+mm_status mm_set_dmi(mm_ctx* ctx, double D, const double e[9]) {
+  if (!ctx || !e) return MM_ERR_INVALID_ARG;
+  for (int i = 0; i < 9; ++i)
+    if (!std::isfinite(e[i])) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_dmi: DMI vectors must be finite");
+  if (!std::isfinite(D)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_dmi: D must be finite");
+  ctx->Ddmi = D;
+  for (int i = 0; i < 9; ++i) ctx->edmi[i] = e[i];
+  return MM_OK;
+}
+
+mm_status mm_set_stt(mm_ctx* ctx, const double p[3], double a_damp, double a_field) {
+  if (!ctx || !p) return MM_ERR_INVALID_ARG;
+  const double n = std::sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2]);
+  if (!(n > 0) || !std::isfinite(n) || !std::isfinite(a_damp) || !std::isfinite(a_field))
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_stt: need a non-zero polarisation and finite amplitudes");
+  for (int i = 0; i < 3; ++i) ctx->stt_p[i] = p[i] / n;
+  ctx->stt_damp = a_damp;
+  ctx->stt_field = a_field;
+  return MM_OK;
+}
+
 mm_status mm_set_terms(mm_ctx* ctx, unsigned term_mask) {
   if (!ctx) return MM_ERR_INVALID_ARG;
-  if (term_mask & ~15u) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_terms: unknown term bits 0x%x", term_mask);
+  if (term_mask & ~63u) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_terms: unknown term bits 0x%x", term_mask);
   ctx->terms = term_mask;
   return MM_OK;
 }
@@ -417,6 +440,13 @@ template <typename T> static PwParams<T> pw_of(const mm_ctx* c, unsigned terms) 
   p.ex[2] = (T)(pe / (c->dz * c->dz));
   p.kan = (T)(2.0 * c->Ku / (kMu0 * c->Ms));
   for (int i = 0; i < 3; ++i) { p.u[i] = (T)c->axis[i]; p.hext[i] = (T)c->Hext[i]; }
+  const double pd = 2.0 * c->Ddmi / (kMu0 * c->Ms);
+  const double cell[3] = {c->dx, c->dy, c->dz};
+  const int nn[3] = {c->nx, c->ny, c->nz};
+  for (int k = 0; k < 3; ++k)
+    for (int i = 0; i < 3; ++i) p.dmi[k][i] = nn[k] > 1 ? (T)(pd * c->edmi[3 * k + i] / (2.0 * cell[k])) : (T)0;
+  for (int i = 0; i < 3; ++i) p.sp[i] = (T)c->stt_p[i];
+  p.sdamp = (T)c->stt_damp; p.sfield = (T)c->stt_field;
   p.pref = (T)(-c->gamma / (1.0 + c->alpha * c->alpha));
   p.alpha = (T)c->alpha;
   p.first = 0; p.wk = (T)1; p.a = (T)0;
@@ -544,6 +574,15 @@ mm_status mm_exchange_field(mm_ctx* ctx, const void* m, void* H) {
   if (m == H) return fail(ctx, MM_ERR_INVALID_ARG, "mm_exchange_field: H must not alias m");
   if (!ctx->have_material) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_exchange_field: mm_set_material not called");
   return dispatch_eval(ctx, PW_EXCHANGE, MM_TERM_EXCHANGE, m, H);
+}
+
+mm_status mm_dmi_field(mm_ctx* ctx, const void* m, void* H) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_dmi_field", m, H)) != MM_OK) return s;
+  if (m == H) return fail(ctx, MM_ERR_INVALID_ARG, "mm_dmi_field: H must not alias m");
+  if (!ctx->have_material) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_dmi_field: mm_set_material not called");
+  return dispatch_eval(ctx, PW_HEFF, MM_TERM_DMI, m, H);
 }
 
 mm_status mm_heff(mm_ctx* ctx, const void* m, void* H) {

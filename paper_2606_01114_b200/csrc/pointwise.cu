@@ -1,6 +1,8 @@
 // S6/S7: one pass over the mesh computes the 6-point exchange stencil
-// (eq. 2, Neumann boundary), uniaxial anisotropy, Zeeman
-// (PAPER.md:140-143), adds H_demag, forms the LLG right-hand side (eq. 1) and
+// (eq. 2, Neumann boundary), the DMI field from the same six neighbours
+// (eq. 3, central differences), uniaxial anisotropy and the spin-torque field
+// (PAPER.md:30), Zeeman, adds H_demag, forms the LLG right-hand side
+// (eq. 1) and
 // applies the RK4 stage arithmetic, so H_eff and k_i are never written to HBM.
 // HBM-bound: 128-bit loads/stores, 4 (fp32) or 2 (fp64) consecutive z cells per thread; the six
 // neighbours come from L1/L2.
@@ -50,9 +52,16 @@ template <int NR> struct VN<double, NR> {
 // mc: m at the cell; lap: exchange field already summed; hd: demag field (or 0);
 // m0v / accv: RK4 step-start state and running sum (only read in RK modes).
 // Returns through o[3] the value to store in `out` (or m0 for PW_RK_FINAL); accv is updated.
-template <typename T, int MODE>
+// hx += E x d  (one DMI direction: E = scaled DMI vector, d = m(i + e_k) - m(i - e_k))
+template <typename T> __device__ __forceinline__ void dmi_add(const T* E, const T* d, T* hx) {
+  hx[0] += E[1] * d[2] - E[2] * d[1];
+  hx[1] += E[2] * d[0] - E[0] * d[2];
+  hx[2] += E[0] * d[1] - E[1] * d[0];
+}
+
+template <typename T, int MODE, bool DMI>
 __device__ __forceinline__ void cell_update(const PwParams<T>& p, const T* mc, const T* lap,
-                                            const T* hd, const T* m0v, T* accv, T* o) {
+                                            const T* hx, const T* hd, const T* m0v, T* accv, T* o) {
   T h[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) h[c] = (p.terms & MM_TERM_EXCHANGE) ? lap[c] : (T)0;
@@ -73,6 +82,15 @@ __device__ __forceinline__ void cell_update(const PwParams<T>& p, const T* mc, c
   if (p.terms & MM_TERM_ZEEMAN) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) h[c] += p.hext[c];
+  }
+  if (DMI) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) h[c] += hx[c];
+  }
+  if (p.terms & MM_TERM_STT) {
+    h[0] += p.sdamp * (mc[1] * p.sp[2] - mc[2] * p.sp[1]) + p.sfield * p.sp[0];
+    h[1] += p.sdamp * (mc[2] * p.sp[0] - mc[0] * p.sp[2]) + p.sfield * p.sp[1];
+    h[2] += p.sdamp * (mc[0] * p.sp[1] - mc[1] * p.sp[0]) + p.sfield * p.sp[2];
   }
   if (MODE == PW_HEFF) {
 #pragma unroll
@@ -108,7 +126,7 @@ __device__ __forceinline__ void cell_update(const PwParams<T>& p, const T* mc, c
 }
 
 // Vector path: nz % CPT == 0.  Thread = CPT consecutive z cells of one (x, y) line.
-template <typename T, int MODE>
+template <typename T, int MODE, bool DMI>
 __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __restrict__ m,
                                                      const T* __restrict__ Hd, T* __restrict__ out,
                                                      T* __restrict__ m0, T* __restrict__ acc) {
@@ -123,29 +141,51 @@ __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __r
   const int x = (int)(g / ((size_t)nzq * p.ny));
   const size_t sy = (size_t)p.nz * 3, sx = sy * p.ny;
   const size_t base = (size_t)x * sx + (size_t)y * sy + (size_t)zq * NR;
-  const bool need_lap = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE;
+  const bool need_lap = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE || DMI;
 
-  T mc[NR], lap[NR];
+  T mc[NR], lap[NR], hx[DMI ? NR : 1];
   V::ld(m + base, mc);
 #pragma unroll
   for (int i = 0; i < NR; ++i) lap[i] = 0;
+#pragma unroll
+  for (int i = 0; i < (DMI ? NR : 1); ++i) hx[i] = 0;
   if (need_lap) {
-    T nb[NR];
+    T nb[NR], dd[DMI ? NR : 1];
     if (p.nx > 1) {
       V::ld(m + (x > 0 ? base - sx : base), nb);
 #pragma unroll
-      for (int i = 0; i < NR; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
+      for (int i = 0; i < NR; ++i) {
+        lap[i] += p.ex[0] * (nb[i] - mc[i]);
+        if (DMI) dd[i] = -nb[i];
+      }
       V::ld(m + (x + 1 < p.nx ? base + sx : base), nb);
 #pragma unroll
-      for (int i = 0; i < NR; ++i) lap[i] += p.ex[0] * (nb[i] - mc[i]);
+      for (int i = 0; i < NR; ++i) {
+        lap[i] += p.ex[0] * (nb[i] - mc[i]);
+        if (DMI) dd[i] += nb[i];
+      }
+      if (DMI) {
+#pragma unroll
+        for (int j = 0; j < CPT; ++j) dmi_add<T>(p.dmi[0], dd + 3 * j, hx + 3 * j);
+      }
     }
     if (p.ny > 1) {
       V::ld(m + (y > 0 ? base - sy : base), nb);
 #pragma unroll
-      for (int i = 0; i < NR; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
+      for (int i = 0; i < NR; ++i) {
+        lap[i] += p.ex[1] * (nb[i] - mc[i]);
+        if (DMI) dd[i] = -nb[i];
+      }
       V::ld(m + (y + 1 < p.ny ? base + sy : base), nb);
 #pragma unroll
-      for (int i = 0; i < NR; ++i) lap[i] += p.ex[1] * (nb[i] - mc[i]);
+      for (int i = 0; i < NR; ++i) {
+        lap[i] += p.ex[1] * (nb[i] - mc[i]);
+        if (DMI) dd[i] += nb[i];
+      }
+      if (DMI) {
+#pragma unroll
+        for (int j = 0; j < CPT; ++j) dmi_add<T>(p.dmi[1], dd + 3 * j, hx + 3 * j);
+      }
     }
     {
       T lo[3], hi[3];
@@ -162,7 +202,12 @@ __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __r
           const T below = j == 0 ? lo[c] : mc[3 * (j - 1) + c];
           const T above = j == CPT - 1 ? hi[c] : mc[3 * (j + 1) + c];
           lap[3 * j + c] += p.ex[2] * ((below - mc[3 * j + c]) + (above - mc[3 * j + c]));
+          if (DMI) dd[3 * j + c] = above - below;
         }
+      if (DMI) {
+#pragma unroll
+        for (int j = 0; j < CPT; ++j) dmi_add<T>(p.dmi[2], dd + 3 * j, hx + 3 * j);
+      }
     }
   }
   T hd[NR], m0v[NR], accv[NR], o[NR];
@@ -175,14 +220,14 @@ __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __r
   }
 #pragma unroll
   for (int j = 0; j < CPT; ++j)
-    cell_update<T, MODE>(p, mc + 3 * j, lap + 3 * j, hd + 3 * j, m0v + 3 * j, accv + 3 * j,
-                         o + 3 * j);
+    cell_update<T, MODE, DMI>(p, mc + 3 * j, lap + 3 * j, hx + (DMI ? 3 * j : 0), hd + 3 * j, m0v + 3 * j,
+                              accv + 3 * j, o + 3 * j);
   if (MODE == PW_RK_STAGE) V::st(acc + base, accv);
   V::st((MODE == PW_RK_FINAL ? m0 : out) + base, o);
 }
 
 // Scalar path for the other nz (thin films, odd nz): thread = one cell.
-template <typename T, int MODE>
+template <typename T, int MODE, bool DMI>
 __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __restrict__ m,
                                                       const T* __restrict__ Hd, T* __restrict__ out,
                                                       T* __restrict__ m0, T* __restrict__ acc) {
@@ -194,8 +239,8 @@ __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __
   const int x = (int)(g / ((size_t)p.nz * p.ny));
   const size_t sy = (size_t)p.nz * 3, sx = sy * p.ny;
   const size_t base = g * 3;
-  const bool need_lap = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE;
-  T mc[3], lap[3] = {0, 0, 0};
+  const bool need_lap = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE || DMI;
+  T mc[3], lap[3] = {0, 0, 0}, hx[3] = {0, 0, 0};
 #pragma unroll
   for (int c = 0; c < 3; ++c) mc[c] = m[base + c];
   if (need_lap) {
@@ -207,6 +252,10 @@ __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __
       const size_t hi = idx[d] + 1 < n[d] ? base + off[d] : base;
 #pragma unroll
       for (int c = 0; c < 3; ++c) lap[c] += p.ex[d] * ((m[lo + c] - mc[c]) + (m[hi + c] - mc[c]));
+      if (DMI) {
+        const T dd[3] = {m[hi] - m[lo], m[hi + 1] - m[lo + 1], m[hi + 2] - m[lo + 2]};
+        dmi_add<T>(p.dmi[d], dd, hx);
+      }
     }
   }
   T hd[3] = {0, 0, 0}, m0v[3] = {0, 0, 0}, accv[3] = {0, 0, 0}, o[3];
@@ -221,7 +270,7 @@ __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __
       if (!(MODE == PW_RK_STAGE && p.first)) accv[c] = acc[base + c];
     }
   }
-  cell_update<T, MODE>(p, mc, lap, hd, m0v, accv, o);
+  cell_update<T, MODE, DMI>(p, mc, lap, hx, hd, m0v, accv, o);
   T* dst = MODE == PW_RK_FINAL ? m0 : out;
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
@@ -230,16 +279,22 @@ __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __
   }
 }
 
+template <typename T, int MODE, bool DMI>
+static void launch_mode_dmi(const PwParams<T>& p, const T* m, const T* Hd, T* out, T* m0, T* acc,
+                            cudaStream_t st) {
+  if (p.nz % Cpt<T>::value == 0) {
+    const size_t total = (size_t)p.nx * p.ny * (p.nz / Cpt<T>::value);
+    pw_vec_kernel<T, MODE, DMI><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
+  } else {
+    const size_t total = (size_t)p.nx * p.ny * p.nz;
+    pw_cell_kernel<T, MODE, DMI><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
+  }
+}
 template <typename T, int MODE>
 static void launch_mode(const PwParams<T>& p, const T* m, const T* Hd, T* out, T* m0, T* acc,
                         cudaStream_t st) {
-  if (p.nz % Cpt<T>::value == 0) {
-    const size_t total = (size_t)p.nx * p.ny * (p.nz / Cpt<T>::value);
-    pw_vec_kernel<T, MODE><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
-  } else {
-    const size_t total = (size_t)p.nx * p.ny * p.nz;
-    pw_cell_kernel<T, MODE><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
-  }
+  if (MODE != PW_EXCHANGE && (p.terms & MM_TERM_DMI)) launch_mode_dmi<T, MODE, true>(p, m, Hd, out, m0, acc, st);
+  else launch_mode_dmi<T, MODE, false>(p, m, Hd, out, m0, acc, st);
 }
 
 template <typename T>

@@ -18,6 +18,8 @@ template <typename T> struct PwParams {
   T ex[3];            // 2A/(mu0 Ms) / d_d^2
   T kan, u[3];        // 2Ku/(mu0 Ms), unit axis
   T hext[3];          // A/m
+  T dmi[3][3];        // DMI vectors e_k^DMI times 2D/(mu0 Ms) / (2 d_k); row k = 0 if n_k = 1
+  T sp[3], sdamp, sfield;  // spin-torque field a_damp (m x p) + a_field p: unit p, amplitudes in A/m
   T pref, alpha;      // -gamma/(1+alpha^2), alpha
   // RK4 bookkeeping
   int first;          // stage 1: acc is written, not accumulated
