@@ -25,6 +25,8 @@
  *   O11 orc_dmi              PAPER.md:34-39 eq. 3, central differences, boundary rule of the exchange stencil (Q28)
  *   O12 orc_stt              spin-transfer torque as a local effective field a_damp (m x p) + a_field p
  *                            (PAPER.md:30 names the term; amplitudes are inputs, reading Q29)
+ *   O13 orc_bb_step          Barzilai-Borwein energy minimiser iteration, PAPER.md:55, 146-148 (named only;
+ *                            step rule, update and stop criterion are reading Q30)
  *   O10 orc_rkf45_step       Runge-Kutta-Fehlberg 4(5) attempt + max-error step control
  *                            (the paper names the method and the max-error reduction; tableau, error
  *                            norm and controller are readings Q23-Q26 of DESIGN.md)
@@ -727,4 +729,72 @@ int orc_rkf45_step(const orc_problem *p, double *m, double dt, double tol, doubl
   }
   free(k); free(ms);
   return rc;
+}
+
+/* O13.  One iteration of the Barzilai-Borwein energy minimiser ("The
+ * Barzikai-Borwein algorithm for minimising the system energy ... all ranks terminate together
+ * after the convergence criteria are met"; PAPER.md:146-148 minimizer.minimize(state)).  The
+ * paper names the algorithm only; the scheme is DESIGN.md reading Q30 (steepest descent on the
+ * unit sphere with Barzilai-Borwein step lengths and a norm-preserving update):
+ *   H_n = H_eff(m_n),   g_n = m_n x (m_n x H_n)            (the tangential energy gradient, A/m)
+ *   n = 0:  tau = tau0
+ *   n > 0:  s = m_n - m_{n-1},  y = g_n - g_{n-1}, sums over all cells and components,
+ *           tau = (s.s)/(s.y) for odd n,  (s.y)/(y.y) for even n;
+ *           if s.y <= 0 (or the quotient is not finite) tau = tau0; then clamp to [tau_min, tau_max]
+ *   m_{n+1} = [ (1 - tau^2 |g_n|^2 / 4) m_n - tau g_n ] / (1 + tau^2 |g_n|^2 / 4)   per cell
+ *           (|g| = |m x H| for unit m: the update is a rotation of m towards H, |m_{n+1}| = 1)
+ *   dm_max = max over cells and components of |m_{n+1} - m_n|;  converged iff dm_max <= tol.
+ * State carried between calls: n, m_prev, g_prev (caller-owned arrays of the size of m).
+ * Outputs: *tau_used, *dm_max, *converged.  A call on a converged state is a no-op. */
+typedef struct {
+  long n;              /* iterations done */
+  double tau0, tau_min, tau_max, tol;
+  double tau, dm_max;  /* of the last iteration */
+  int converged;
+  double *m_prev, *g_prev;
+} orc_bb_state;
+
+int orc_bb_step(const orc_problem *p, double *m, orc_bb_state *st) {
+  if (st->converged) return 0;
+  const size_t n3 = (size_t)p->nx * p->ny * p->nz * 3;
+  double *H = malloc(n3 * sizeof(double)), *g = malloc(n3 * sizeof(double));
+  if (!H || !g) { free(H); free(g); return 2; }
+  int rc = orc_heff(p, m, H);
+  if (rc) { free(H); free(g); return rc; }
+  for (size_t i = 0; i < n3; i += 3) {
+    double mxh[3];
+    cross3(m + i, H + i, mxh);
+    cross3(m + i, mxh, g + i);
+  }
+  double tau = st->tau0;
+  if (st->n > 0) {
+    long double ss = 0.0L, sy = 0.0L, yy = 0.0L;
+    for (size_t i = 0; i < n3; ++i) {
+      const double s = m[i] - st->m_prev[i], y = g[i] - st->g_prev[i];
+      ss += (long double)s * s; sy += (long double)s * y; yy += (long double)y * y;
+    }
+    const double q = (st->n & 1) ? (double)(ss / sy) : (double)(sy / yy);
+    tau = (sy > 0.0L && isfinite(q)) ? q : st->tau0;
+  }
+  if (tau < st->tau_min) tau = st->tau_min;
+  if (tau > st->tau_max) tau = st->tau_max;
+  double dm = 0.0;
+  for (size_t i = 0; i < n3; i += 3) {
+    const double g2 = g[i] * g[i] + g[i + 1] * g[i + 1] + g[i + 2] * g[i + 2];
+    const double a = 0.25 * tau * tau * g2;
+    for (int c = 0; c < 3; ++c) {
+      const double mn = ((1.0 - a) * m[i + c] - tau * g[i + c]) / (1.0 + a);
+      const double d = fabs(mn - m[i + c]);
+      if (d > dm) dm = d;
+      st->m_prev[i + c] = m[i + c];
+      st->g_prev[i + c] = g[i + c];
+      m[i + c] = mn;
+    }
+  }
+  st->n += 1;
+  st->tau = tau;
+  st->dm_max = dm;
+  st->converged = dm <= st->tol ? 1 : 0;
+  free(H); free(g);
+  return 0;
 }

@@ -207,6 +207,33 @@ def llg_torque(alpha, gamma, m, H):
     return out
 
 
+class _BBState(C.Structure):
+    _fields_ = [("n", C.c_long), ("tau0", C.c_double), ("tau_min", C.c_double), ("tau_max", C.c_double),
+                ("tol", C.c_double), ("tau", C.c_double), ("dm_max", C.c_double), ("converged", C.c_int),
+                ("m_prev", C.c_void_p), ("g_prev", C.c_void_p)]
+
+
+class BBMinimizer:
+    """O13: Barzilai-Borwein minimiser state around orc_bb_step (reading Q30)."""
+
+    def __init__(self, problem, m, tau0=1e-6, tau_min=1e-9, tau_max=1e-3, tol=1e-8):
+        self.problem = problem
+        self.m = _f64(m).copy()
+        self._mp = np.zeros_like(self.m)
+        self._gp = np.zeros_like(self.m)
+        self.st = _BBState(0, tau0, tau_min, tau_max, tol, 0.0, 0.0, 0, self._mp.ctypes.data,
+                           self._gp.ctypes.data)
+
+    def step(self):
+        _chk(lib().orc_bb_step(C.byref(self.problem._c()), _p(self.m), C.byref(self.st)), "bb_step")
+        return self.st.tau, self.st.dm_max, bool(self.st.converged)
+
+    def minimize(self, max_iter=10000):
+        while self.st.n < max_iter and not self.st.converged:
+            self.step()
+        return self.m, int(self.st.n), bool(self.st.converged)
+
+
 @dataclass
 class Problem:
     """Mesh + material + enabled terms; mirrors the paper's state.material / field-term list
