@@ -131,6 +131,26 @@ mm_status mm_rkf45_state(mm_ctx *ctx, double *t, double *dt_next, double *err_la
                          int *accepted_last, unsigned long long *n_accepted,
                          unsigned long long *n_rejected);
 
+/* Barzilai-Borwein energy minimiser (PAPER.md:55, 146-148 minimizer.minimize(state); the paper
+ * names the algorithm, the scheme is DESIGN.md reading Q30): steepest descent on the unit sphere,
+ *   g = m x (m x H_eff);  tau = tau0 first, then (s.s)/(s.y) on odd and (s.y)/(y.y) on even
+ *   iterations (s = m_n - m_{n-1}, y = g_n - g_{n-1}, summed over the mesh), tau0 when s.y <= 0,
+ *   clamped to [tau_min, tau_max] (m/A);  m <- [(1 - tau^2 g^2/4) m - tau g]/(1 + tau^2 g^2/4);
+ *   converged iff max |m_{n+1} - m_n| <= tol.
+ * The state lives on the DEVICE: mm_minimize_step enqueues ONE iteration (one H_eff evaluation,
+ * deterministic fixed-order sums, controller, update) without host synchronisation; once
+ * converged, further iterations leave m and the state untouched.  mm_minimize_state
+ * synchronises and reads the state back (any output pointer may be NULL).  mm_minimize runs up
+ * to max_iter iterations, reading the state back every check_every iterations (the coordinated
+ * stop of PAPER.md:55).  The minimiser reuses the RKF45 stage buffers: do not interleave it
+ * with mm_rkf45_step on the same context without re-initialising. */
+mm_status mm_minimize_init(mm_ctx *ctx, double tau0, double tau_min, double tau_max, double tol);
+mm_status mm_minimize_step(mm_ctx *ctx, void *m_inout);
+mm_status mm_minimize_state(mm_ctx *ctx, unsigned long long *iterations, double *tau_last, double *dm_max,
+                            int *converged);
+mm_status mm_minimize(mm_ctx *ctx, void *m_inout, int max_iter, int check_every,
+                      unsigned long long *iterations, int *converged);
+
 /* Same operations on HOST buffers (pageable or pinned): copies m host->device into scratch
  * staging, runs the device path, copies the result device->host, synchronises.  These are
  * what bench.py's end-to-end leg times. */

@@ -67,6 +67,10 @@ def load_library():
         "mm_rkf45_step": [vp, vp],
         "mm_rkf45_state": [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl),
                            C.POINTER(i32), C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)],
+        "mm_minimize_init": [vp, dbl, dbl, dbl, dbl],
+        "mm_minimize_step": [vp, vp],
+        "mm_minimize_state": [vp, C.POINTER(C.c_ulonglong), C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i32)],
+        "mm_minimize": [vp, vp, i32, i32, C.POINTER(C.c_ulonglong), C.POINTER(i32)],
         "mm_demag_field_host": [vp, vp, vp],
         "mm_heff_host": [vp, vp, vp],
         "mm_llg_rhs_host": [vp, vp, vp],
@@ -251,6 +255,26 @@ class Context:
                    C.byref(na), C.byref(nr))
         return {"t": t.value, "dt_next": dn.value, "err": er.value, "dt_last": dl.value,
                 "accepted": bool(acc.value), "n_accepted": na.value, "n_rejected": nr.value}
+
+    def minimize_init(self, tau0=1e-6, tau_min=1e-9, tau_max=1e-3, tol=1e-8):
+        self._call("mm_minimize_init", tau0, tau_min, tau_max, tol)
+
+    def minimize_step(self, m):
+        self._check(m)
+        self._call("mm_minimize_step", m.data_ptr())
+
+    def minimize_state(self):
+        """(iterations, tau_last, dm_max, converged); synchronises."""
+        n, tau, dm, cv = C.c_ulonglong(), C.c_double(), C.c_double(), C.c_int()
+        self._call("mm_minimize_state", C.byref(n), C.byref(tau), C.byref(dm), C.byref(cv))
+        return n.value, tau.value, dm.value, bool(cv.value)
+
+    def minimize(self, m, max_iter=10000, check_every=10):
+        """Runs the minimiser in place; returns (iterations, converged)."""
+        self._check(m)
+        n, cv = C.c_ulonglong(), C.c_int()
+        self._call("mm_minimize", m.data_ptr(), int(max_iter), int(check_every), C.byref(n), C.byref(cv))
+        return n.value, bool(cv.value)
 
     def nhat_export(self):
         o = tuple(1 if v == 1 else v + 1 for v in self.n)

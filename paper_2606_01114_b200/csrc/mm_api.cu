@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "../../include/mm_b200.h"
+#include "bb.cuh"
 #include "demag_fast.cuh"
 #include "demag_init.cuh"
 #include "demag_passes.cuh"
@@ -49,11 +50,12 @@ struct mm_ctx {
   size_t pers_bytes = 0, scr_bytes = 0;
   bool demag_ready = false;
   // persistent offsets
-  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, pers_need;
+  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, off_bbstate, off_bbpart, pers_need;
   // scratch offsets
   size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, scr_need;
   RkfState rk_host{};
   bool rk_ready = false;
+  bool bb_ready = false;
   unsigned long long launches = 0;
   Prof prof;
   double prof_ms[Prof::kKinds] = {0};
@@ -131,6 +133,8 @@ static void plan_layout(mm_ctx* c) {
   c->off_t2x = o; o += align256((size_t)g.Px * cs);
   c->off_t2y = o; o += align256((size_t)g.Py * cs);
   c->off_rkstate = o; o += align256(sizeof(RkfState));
+  c->off_bbstate = o; o += align256(sizeof(BbState));
+  c->off_bbpart = o; o += align256((size_t)kBbMaxBlocks * 3 * sizeof(double));
   c->pers_need = o;
   // scratch
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
@@ -257,6 +261,7 @@ mm_status mm_ctx_set_workspace(mm_ctx* ctx, void* persistent, size_t pbytes, voi
   ctx->scr_bytes = sbytes;
   ctx->demag_ready = false;
   ctx->rk_ready = false;
+  ctx->bb_ready = false;
   return MM_OK;
 }
 
@@ -614,6 +619,21 @@ mm_status mm_rk_step(mm_ctx* ctx, void* m_inout, double dt) {
 
 }  // extern "C"
 
+// ---- Barzilai-Borwein minimiser iteration (bb.cu)
+
+template <typename T> static mm_status bb_step_t(mm_ctx* c, void* m) {
+  const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3;
+  const size_t pitch = align256(n3 * c->es) / c->es;       // the RKF45 stage buffers, reused (never both at once)
+  T* K = reinterpret_cast<T*>(c->scr + c->off_rkf);
+  T* g = K, *gp = K + pitch, *mp = K + 2 * pitch;
+  mm_status s = eval_t<T>(c, PW_MIN_G, m, g, nullptr, pw_of<T>(c, c->terms));
+  if (s != MM_OK) return s;
+  cudaError_t e = bb_iterate_launch<T>(reinterpret_cast<BbState*>(c->pers + c->off_bbstate), static_cast<T*>(m), g,
+                                       mp, gp, reinterpret_cast<double*>(c->pers + c->off_bbpart), n3, c->stream,
+                                       &c->launches);
+  return e == cudaSuccess ? MM_OK : cuda_fail(c, "mm_minimize_step", e);
+}
+
 // ---- adaptive RKF45 (rkf45.cu)
 
 template <typename T> static mm_status rkf_step_t(mm_ctx* c, void* m) {
@@ -680,6 +700,68 @@ mm_status mm_rkf45_state(mm_ctx* ctx, double* t, double* dt_next, double* err_la
   if (n_accepted) *n_accepted = h.n_acc;
   if (n_rejected) *n_rejected = h.n_rej;
   return MM_OK;
+}
+
+// ---- Barzilai-Borwein minimiser (bb.cu)
+
+mm_status mm_minimize_init(mm_ctx* ctx, double tau0, double tau_min, double tau_max, double tol) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!ctx->pers) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_minimize_init: mm_ctx_set_workspace not called");
+  if (!(tau0 > 0) || tau_min < 0 || !(tau_max >= tau_min) || tol < 0 || !std::isfinite(tau0) || !std::isfinite(tau_max))
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_minimize_init: need tau0 > 0, 0 <= tau_min <= tau_max, tol >= 0");
+  BbState h{};
+  h.tau0 = tau0; h.tau_min = tau_min; h.tau_max = tau_max; h.tol = tol;
+  cudaError_t e = cudaMemcpyAsync(ctx->pers + ctx->off_bbstate, &h, sizeof(BbState), cudaMemcpyHostToDevice,
+                                  ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, "mm_minimize_init", e);
+  ctx->bb_ready = true;
+  return MM_OK;
+}
+
+mm_status mm_minimize_step(mm_ctx* ctx, void* m_inout) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_minimize_step", m_inout, m_inout)) != MM_OK) return s;
+  if ((s = need_ready(ctx, "mm_minimize_step", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
+  if (!ctx->bb_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_minimize_step: mm_minimize_init not called");
+  return ctx->dtype == MM_F32 ? bb_step_t<float>(ctx, m_inout) : bb_step_t<double>(ctx, m_inout);
+}
+
+mm_status mm_minimize_state(mm_ctx* ctx, unsigned long long* iterations, double* tau_last, double* dm_max,
+                            int* converged) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (!ctx->bb_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_minimize_state: mm_minimize_init not called");
+  BbState h;
+  cudaError_t e = cudaMemcpyAsync(&h, ctx->pers + ctx->off_bbstate, sizeof(BbState), cudaMemcpyDeviceToHost,
+                                  ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, "mm_minimize_state", e);
+  if (iterations) *iterations = h.n;
+  if (tau_last) *tau_last = h.tau;
+  if (dm_max) *dm_max = h.dm_max;
+  if (converged) *converged = h.converged;
+  return MM_OK;
+}
+
+mm_status mm_minimize(mm_ctx* ctx, void* m_inout, int max_iter, int check_every, unsigned long long* iterations,
+                      int* converged) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (max_iter < 0 || check_every < 1)
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_minimize: need max_iter >= 0 and check_every >= 1");
+  unsigned long long n = 0;
+  int conv = 0;
+  mm_status s = mm_minimize_state(ctx, &n, nullptr, nullptr, &conv);
+  const unsigned long long n0 = n;
+  while (s == MM_OK && !conv && n - n0 < (unsigned long long)max_iter) {
+    unsigned long long todo = (unsigned long long)max_iter - (n - n0);
+    if (todo > (unsigned long long)check_every) todo = check_every;
+    for (unsigned long long i = 0; i < todo && s == MM_OK; ++i) s = mm_minimize_step(ctx, m_inout);
+    if (s == MM_OK) s = mm_minimize_state(ctx, &n, nullptr, nullptr, &conv);   // the only synchronisation
+  }
+  if (iterations) *iterations = n;
+  if (converged) *converged = conv;
+  return s;
 }
 
 // ---- host-buffer variants: H2D, device path, D2H, synchronise

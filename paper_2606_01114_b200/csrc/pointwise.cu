@@ -104,6 +104,10 @@ __device__ __forceinline__ void cell_update(const PwParams<T>& p, const T* mc, c
   const T d0 = mc[1] * t2 - mc[2] * t1;
   const T d1 = mc[2] * t0 - mc[0] * t2;
   const T d2 = mc[0] * t1 - mc[1] * t0;
+  if (MODE == PW_MIN_G) {
+    o[0] = d0; o[1] = d1; o[2] = d2;
+    return;
+  }
   T k[3] = {p.pref * (t0 + p.alpha * d0), p.pref * (t1 + p.alpha * d1),
             p.pref * (t2 + p.alpha * d2)};
   if (MODE == PW_RHS) {
@@ -307,6 +311,7 @@ cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T
     case PW_HEFF: launch_mode<T, PW_HEFF>(p, m, Hd, out, m0, acc, st); break;
     case PW_RHS: launch_mode<T, PW_RHS>(p, m, Hd, out, m0, acc, st); break;
     case PW_RK_STAGE: launch_mode<T, PW_RK_STAGE>(p, m, Hd, out, m0, acc, st); break;
+    case PW_MIN_G: launch_mode<T, PW_MIN_G>(p, m, Hd, out, m0, acc, st); break;
     default: launch_mode<T, PW_RK_FINAL>(p, m, Hd, out, m0, acc, st); break;
   }
   ++*launches;

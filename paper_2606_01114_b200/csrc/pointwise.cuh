@@ -9,7 +9,8 @@ enum PwMode {
   PW_HEFF = 1,      // out := sum of enabled terms (Hd added when the demag term is on)
   PW_RHS = 2,       // out := LLG right-hand side at H_eff
   PW_RK_STAGE = 3,  // k := RHS; acc := (first ? k : acc + wk k); out := m0 + a k
-  PW_RK_FINAL = 4   // k := RHS; m0 := normalise(m0 + b (acc + k))
+  PW_RK_FINAL = 4,  // k := RHS; m0 := normalise(m0 + b (acc + k))
+  PW_MIN_G = 5      // out := m x (m x H_eff), the minimiser's tangential gradient (bb.cuh)
 };
 
 template <typename T> struct PwParams {
