@@ -206,7 +206,8 @@ def run_ours(args, cfg):
 
     tdt = torch.float32 if args.dtype == "f32" else torch.float64
     s = 4 if args.dtype == "f32" else 8
-    ctx = Context(cfg.n, cfg.d, dtype=tdt, device=f"cuda:{local}", path=args.path, kchunk=args.kchunk)
+    tiles = tuple(int(v) for v in args.tiles.split(",")) if args.tiles else None
+    ctx = Context(cfg.n, cfg.d, dtype=tdt, device=f"cuda:{local}", path=args.path, kchunk=args.kchunk, tiles=tiles)
     ctx.set_material(cfg.Ms, cfg.Aex, cfg.Ku, cfg.axis, cfg.alpha, cfg.gamma)
     ctx.set_zeeman(cfg.Hext)
     ctx.set_terms(cfg.terms)
@@ -273,7 +274,7 @@ def run_ours(args, cfg):
         return 0
 
     ncell = cfg.ncell
-    kbytes, total_bytes = byte_model(cfg.n, s, fast=ctx.path[0])
+    kbytes, total_bytes = byte_model(cfg.n, s, fast=ctx.path_name != "generic")
     peak, peak_src = measured_peak()
     per_kernel = {}
     for k, (tot, cnt) in ktimes.items():
@@ -371,10 +372,10 @@ def run_sweep(args):
             out = torch.empty_like(m)
             ms_d = timed(lambda: ctx.demag_field(m, out))
             ms_r = timed(lambda: ctx.llg_rhs(m, out))
-            kb, total = byte_model(cfg.n, s, fast=ctx.path[0])
+            kb, total = byte_model(cfg.n, s, fast=ctx.path_name != "generic")
             demag_bytes = total - kb["S6_pointwise"]
             line = {"sweep": cfg.name, "dtype": dt, "cells": cfg.ncell,
-                    "path": "fast (x-first)" if ctx.path[0] else "generic (z-first)",
+                    "path": {"fast": "fast (x-first)", "mixed": "mixed-radix (x-first)", "generic": "generic (z-first)"}[ctx.path_name],
                     "demag": {"ms": ms_d, "cell_updates_per_s": cfg.ncell / ms_d * 1e3,
                               "frac_hbm_measured": demag_bytes / ms_d / 1e6 / peak,
                               "frac_hbm_8TBps": demag_bytes / ms_d / 1e6 / 8000.0},
@@ -414,6 +415,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic passes, 2 fast kernels (experiments)")
     ap.add_argument("--kchunk", type=int, default=0, help="kx planes per y/z/y launch group (experiments)")
+    ap.add_argument("--tiles", default=None, help="generic passes: tile widths bz,by,bk (experiments)")
     ap.add_argument("--mesh", default=None, help="override mesh, e.g. 256x256x64 (experiments)")
     ap.add_argument("--sweep", action="store_true", help="config 5: one line per sweep mesh and dtype")
     ap.add_argument("--paper-meshes", action="store_true",

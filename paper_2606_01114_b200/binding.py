@@ -182,10 +182,17 @@ class Context:
 
     @property
     def path(self):
-        """(fast, kchunk): whether the x-first fast kernels are selected, planes per chunk."""
+        """(fast, kchunk): whether the power-of-two x-first kernels are selected, planes per chunk."""
         f, k = C.c_int(), C.c_int()
         self._call("mm_ctx_path", C.byref(f), C.byref(k))
-        return bool(f.value), k.value
+        return f.value == 1, k.value
+
+    @property
+    def path_name(self):
+        """'generic' (z-first passes), 'fast' (power-of-two x-first) or 'mixed' (mixed-radix x-first)."""
+        f, k = C.c_int(), C.c_int()
+        self._call("mm_ctx_path", C.byref(f), C.byref(k))
+        return ("generic", "fast", "mixed")[f.value]
 
     @property
     def launch_count(self):

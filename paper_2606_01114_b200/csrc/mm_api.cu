@@ -13,6 +13,7 @@
 #include "bb.cuh"
 #include "demag_fast.cuh"
 #include "demag_init.cuh"
+#include "demag_mixed.cuh"
 #include "demag_passes.cuh"
 #include "fft_core.cuh"
 #include "pointwise.cuh"
@@ -41,6 +42,8 @@ struct mm_ctx {
   InitGeom igeom{};
   FastGeom fgeom{};
   bool fast = false;     // the x-first kernels of demag_fast.cu cover this mesh and are selected
+  bool mixed = false;    // the mixed-radix x-first kernels of demag_mixed.cu are selected
+  bool xfirst() const { return fast || mixed; }   // x-first spectra and the octant table
   int path_pref = 0;     // 0 auto, 1 generic (demag_passes.cu), 2 fast required
   int kchunk = 0;        // kx planes per K2..K4 launch group (0 = all)
   int want_bz = 0, want_by = 0, want_bk = 0;
@@ -50,7 +53,7 @@ struct mm_ctx {
   size_t pers_bytes = 0, scr_bytes = 0;
   bool demag_ready = false;
   // persistent offsets
-  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, off_bbstate, off_bbpart, pers_need;
+  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, off_bbstate, off_bbpart, pers_need;
   // scratch offsets
   size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, scr_need;
   RkfState rk_host{};
@@ -72,7 +75,6 @@ static mm_status fail(mm_ctx* c, mm_status s, const char* fmt, ...) {
   return s;
 }
 
-static bool pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
 static size_t align256(size_t v) { return (v + 255) / 256 * 256; }
 static int padded(int n) { return n == 1 ? 1 : 2 * n; }
 
@@ -110,7 +112,8 @@ static void plan_layout(mm_ctx* c) {
   ig.oz = c->nz == 1 ? 1 : c->nz + 1;
   ig.ozp = (ig.oz + 1) / 2 * 2;
   ig.Bk = g.Bk;
-  c->fast = c->path_pref != 1 && fast_supported(c->nx, c->ny, c->nz, c->es);
+  c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->nx, c->ny, c->nz, c->es);
+  c->mixed = !c->fast && c->path_pref != 1 && mixed_supported(c->nx, c->ny, c->nz, c->es);
   FastGeom& fg = c->fgeom;
   fg.nx = c->nx; fg.ny = c->ny; fg.nz = c->nz;
   fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;
@@ -120,12 +123,13 @@ static void plan_layout(mm_ctx* c) {
   // persistent
   size_t o = 0;
   c->off_table = o;
-  o += c->fast ? align256((size_t)ig.ox * ig.oy * ig.ozp * 6 * c->es)
+  o += c->xfirst() ? align256((size_t)ig.ox * ig.oy * ig.ozp * 6 * c->es)
                : align256((size_t)g.Kz * g.Py * g.Px * 6 * c->es);
   c->off_wx = o; o += align256((size_t)g.Px * cs);
   c->off_wy = o; o += align256((size_t)g.Py * cs);
   c->off_wz = o; o += align256((size_t)g.Pz * cs);
   c->off_posz = o; o += align256((size_t)g.Pz * 2);
+  c->off_fz = o; o += align256((size_t)g.Pz * 2);
   c->off_fx = o; o += align256((size_t)g.Px * 2);
   c->off_fy = o; o += align256((size_t)g.Py * 2);
   c->off_posx = o; o += align256((size_t)g.Px * 2);
@@ -139,8 +143,8 @@ static void plan_layout(mm_ctx* c) {
   // scratch
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
   o = 0;
-  if (c->fast) {
-    const size_t planes2 = fg.kchunk ? fg.kchunk : c->nx + 1;
+  if (c->xfirst()) {
+    const size_t planes2 = (c->fast && fg.kchunk) ? fg.kchunk : c->nx + 1;
     c->off_a1 = o; o += align256((size_t)(c->nx + 1) * g.ny * fg.Q * cs);
     c->off_a2 = o; o += align256(planes2 * g.Py * fg.Q * cs);
   } else {
@@ -201,8 +205,8 @@ mm_status mm_ctx_set_tiles(mm_ctx* ctx, int bz, int by, int bk) {
   if (ctx->pers) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: call before mm_ctx_set_workspace");
   const int v[3] = {bz, by, bk};
   for (int i = 0; i < 3; ++i)
-    if (v[i] < 0 || (v[i] > 0 && !pow2(v[i])) || v[i] > 64)
-      return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: tile widths must be 0 or a power of two <= 64");
+    if (v[i] < 0 || v[i] > 64)
+      return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: tile widths must be in 0 .. 64");
   if ((bz && ctx->nx % bz) || (by && ctx->nx % by) || (bk && padded(ctx->ny) % bk))
     return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_tiles: bz, by must divide nx and bk must divide the padded ny");
   ctx->want_bz = bz; ctx->want_by = by; ctx->want_bk = bk;
@@ -222,8 +226,11 @@ mm_status mm_ctx_set_tiles(mm_ctx* ctx, int bz, int by, int bk) {
 mm_status mm_ctx_set_path(mm_ctx* ctx, int path, int kchunk) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (ctx->pers) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: call before mm_ctx_set_workspace");
-  if (path < 0 || path > 2 || kchunk < 0)
-    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: path must be 0, 1 or 2 and kchunk >= 0");
+  if (path < 0 || path > 3 || kchunk < 0)
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: path must be 0 .. 3 and kchunk >= 0");
+  if (path == 3 && !mixed_supported(ctx->nx, ctx->ny, ctx->nz, ctx->es))
+    return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_path: the mixed-radix x-first kernels do not cover %dx%dx%d",
+                ctx->nx, ctx->ny, ctx->nz);
   if (path == 2 && !fast_supported(ctx->nx, ctx->ny, ctx->nz, ctx->es))
     return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_path: the fast kernels do not cover %dx%dx%d",
                 ctx->nx, ctx->ny, ctx->nz);
@@ -235,7 +242,7 @@ mm_status mm_ctx_set_path(mm_ctx* ctx, int path, int kchunk) {
 
 mm_status mm_ctx_path(const mm_ctx* ctx, int* fast, int* kchunk) {
   if (!ctx || !fast || !kchunk) return MM_ERR_INVALID_ARG;
-  *fast = ctx->fast ? 1 : 0;
+  *fast = ctx->fast ? 1 : (ctx->mixed ? 2 : 0);
   *kchunk = ctx->fgeom.kchunk;
   return MM_OK;
 }
@@ -397,7 +404,11 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   if (two_x) fill_twiddles2<T>(host, c->off_t2x - small_off, c->nx);
   if (two_y) fill_twiddles2<T>(host, c->off_t2y - small_off, c->ny);
   auto u16 = [&](size_t off) { return reinterpret_cast<uint16_t*>(host.data() + (off - small_off)); };
-  for (int k = 0; k < g.Pz; ++k) u16(c->off_posz)[k] = (uint16_t)pos_of_freq(g.pz, k);
+  for (int k = 0; k < g.Pz; ++k) {
+    const int p = pos_of_freq(g.pz, k);
+    u16(c->off_posz)[k] = (uint16_t)p;
+    u16(c->off_fz)[p] = (uint16_t)k;
+  }
   for (int k = 0; k < g.Px; ++k) {
     const int p = pos_of_freq(g.px, k);
     u16(c->off_posx)[k] = (uint16_t)(c->fast ? fast_swizzle(c->nx, fast_pos_logical(c->nx, k)) : p);
@@ -414,7 +425,7 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   e = demag_init_launch<T>(c->igeom, c->dx, c->dy, c->dz, c->scr,
                            reinterpret_cast<const uint16_t*>(c->pers + c->off_fx),
                            reinterpret_cast<const uint16_t*>(c->pers + c->off_fy),
-                           reinterpret_cast<T*>(c->pers + c->off_table), c->fast ? 1 : 0, c->stream,
+                           reinterpret_cast<T*>(c->pers + c->off_table), c->xfirst() ? 1 : 0, c->stream,
                            &c->launches);
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: launch", e);
   e = cudaStreamSynchronize(c->stream);  // also keeps `host` alive until the copy is done
@@ -488,7 +499,27 @@ template <typename T> static FastBufs<T> fast_bufs_of(mm_ctx* c) {
   return b;
 }
 
+template <typename T> static MixedBufs<T> mixed_bufs_of(mm_ctx* c) {
+  MixedBufs<T> b;
+  b.Wx = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wx);
+  b.Wy = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wy);
+  b.Wz = reinterpret_cast<const Cx<T>*>(c->pers + c->off_wz);
+  b.posx = reinterpret_cast<const uint16_t*>(c->pers + c->off_posx);
+  b.posy = reinterpret_cast<const uint16_t*>(c->pers + c->off_posy);
+  b.fz = reinterpret_cast<const uint16_t*>(c->pers + c->off_fz);
+  b.table = reinterpret_cast<const T*>(c->pers + c->off_table);
+  b.A1 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a1);
+  b.A2 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a2);
+  return b;
+}
+
 template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H) {
+  if (c->mixed) {
+    const MixedPlans pl{c->geom.px, c->geom.py, c->geom.pz};
+    cudaError_t e = demag_mixed_launch<T>(c->fgeom, pl, mixed_bufs_of<T>(c), static_cast<const T*>(m),
+                                          static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches, &c->prof);
+    return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag (mixed-radix path) launch", e);
+  }
   if (c->fast) {
     cudaError_t e = demag_fast_launch<T>(c->fgeom, fast_bufs_of<T>(c), static_cast<const T*>(m),
                                          static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches,
@@ -554,11 +585,11 @@ mm_status mm_demag_nhat_export(mm_ctx* ctx, void* out) {
   cudaError_t e;
   if (ctx->dtype == MM_F32)
     e = demag_export_launch<float>(ctx->igeom, reinterpret_cast<const float*>(ctx->pers + ctx->off_table),
-                                   posx, posy, static_cast<float*>(out), ctx->fast ? 1 : 0, ctx->stream,
+                                   posx, posy, static_cast<float*>(out), ctx->xfirst() ? 1 : 0, ctx->stream,
                                    &ctx->launches);
   else
     e = demag_export_launch<double>(ctx->igeom, reinterpret_cast<const double*>(ctx->pers + ctx->off_table),
-                                    posx, posy, static_cast<double*>(out), ctx->fast ? 1 : 0, ctx->stream,
+                                    posx, posy, static_cast<double*>(out), ctx->xfirst() ? 1 : 0, ctx->stream,
                                     &ctx->launches);
   return e == cudaSuccess ? MM_OK : cuda_fail(ctx, "mm_demag_nhat_export", e);
 }

@@ -131,3 +131,37 @@ def test_paper_meshes_fullsize(oracle, n, dt):
     err = float((tot - 1.0).abs().max())
     assert err <= (1e-11 if dt == "f64" else 2e-5), err
     ctx.close()
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n", [(16, 16, 2), (32, 16, 8), (64, 64, 64), (128, 64, 32), (25, 14, 6), (10, 6, 90),
+                               (2, 2, 2), (70, 3, 4)])
+def test_mixed_radix_xfirst_kernels_explicitly(oracle, n, dt):
+    """path = 3 forces demag_mixed.cu (also on power-of-two meshes): N-hat export, field vs the oracle
+    FFT path, agreement with the generic z-first passes, determinism."""
+    cfg = cfg_for(n, (4e-9, 3e-9, 2e-9))
+    m, m64 = round_input(w.random_unit_vectors(313, n), dt)
+    P = make_problem(oracle, cfg, terms=1)
+    ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
+    ctx = make_ctx(cfg, dt, terms=1, path=3)
+    assert ctx.path_name == "mixed"
+    got = ctx.demag_field(to_dev(m)).cpu().numpy()
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+    assert np.array_equal(got, ctx.demag_field(to_dev(m)).cpu().numpy())
+    nh = ctx.nhat_export().cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(nh - mirrored_nhat(oracle, n, cfg.d))) < (5e-14 if dt == "f64" else 2e-7)
+    gen = make_ctx(cfg, dt, terms=1, path=1)
+    assert gen.path_name == "generic"
+    l2, mx = w.field_errors(gen.demag_field(to_dev(m)).cpu().numpy(), got)
+    assert l2 <= TOL[dt], (l2, mx)
+
+
+def test_mixed_radix_selection():
+    from paper_2606_01114_b200 import MMError
+    assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0).path_name == "mixed"
+    assert make_ctx(cfg_for((512, 512, 128), (4e-9,) * 3), "f32", terms=0).path_name == "fast"
+    assert make_ctx(cfg_for((100, 25, 1), (5e-9, 5e-9, 3e-9)), "f64", terms=0).path_name == "generic"
+    assert make_ctx(cfg_for((9, 15, 5), (1e-9,) * 3), "f64", terms=0).path_name == "generic"   # ny 3 nz odd
+    with pytest.raises(MMError):
+        make_ctx(cfg_for((100, 25, 1), (5e-9, 5e-9, 3e-9)), "f64", terms=0, path=3)
