@@ -30,7 +30,7 @@ template <typename T> struct MixB { static constexpr int value = 64 / (int)sizeo
 // ---------------------------------------------------------------- K2: forward y
 // grid (ceil(Q / B), planes)
 template <typename T>
-__global__ void __launch_bounds__(512) yf_mixed_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2,
+__global__ void __launch_bounds__(256, 2) yf_mixed_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2,
                                                        const Cx<T>* __restrict__ W, FftPlan pl, int Q) {
   MM_MIXED_PROLOGUE
   const int col = blockIdx.x * B + lane;
@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(512) yf_mixed_kernel(const Cx<T>* __restrict__
 
 // ---------------------------------------------------------------- K4: inverse y
 template <typename T>
-__global__ void __launch_bounds__(512) yi_mixed_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1,
+__global__ void __launch_bounds__(256, 2) yi_mixed_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1,
                                                        const Cx<T>* __restrict__ W, FftPlan pl, int Q) {
   MM_MIXED_PROLOGUE
   const int col = blockIdx.x * B + lane;
@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(512) yi_mixed_kernel(const Cx<T>* __restrict__
 // separated with A[k] = (Z[k] + conj Z[-k]) / 2, B[k] = (Z[k] - conj Z[-k]) / 2i for k <= nx.
 // grid ceil(npairs / B); npairs = ny Q / 2 pairs per x row.
 template <typename T>
-__global__ void __launch_bounds__(512) xf_mixed_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1,
+__global__ void __launch_bounds__(256, 2) xf_mixed_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1,
                                                        const Cx<T>* __restrict__ W, const uint16_t* __restrict__ pos,
                                                        FftPlan pl, size_t npairs) {
   MM_MIXED_PROLOGUE
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(512) xf_mixed_kernel(const Cx<T>* __restrict__
 // Z[k] = A[k] + i B[k], Z[P - k] = conj A[k] + i conj B[k]; the truncated inverse gives
 // h_q(x) + i h_{q+1}(x), written as the real pair (q, q + 1) of H, times scale.
 template <typename T>
-__global__ void __launch_bounds__(512) xi_mixed_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp,
+__global__ void __launch_bounds__(256, 2) xi_mixed_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp,
                                                        const Cx<T>* __restrict__ W, const uint16_t* __restrict__ pos,
                                                        FftPlan pl, size_t npairs, T scale) {
   MM_MIXED_PROLOGUE
@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(512) xi_mixed_kernel(const Cx<T>* __restrict__
 // grid (ceil(ny / NPAIR), planes); block = C * NT threads, C = 6 NPAIR columns (3 components of
 // the 2 NPAIR pencils); shared memory Pz rows of pitch C + 1.
 template <typename T>
-__global__ void __launch_bounds__(512) zp_mixed_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab,
+__global__ void __launch_bounds__(256, 2) zp_mixed_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab,
                                                        const Cx<T>* __restrict__ Wz,
                                                        const uint16_t* __restrict__ posy,
                                                        const uint16_t* __restrict__ fz, FftPlan pl, int ny, int Q,
@@ -218,7 +218,7 @@ static int strided_threads(int P, int B) {
   int t = P / 4 * B;
   t = (t + 31) / 32 * 32;
   if (t < 64) t = 64;
-  if (t > 512) t = 512;
+  if (t > 256) t = 256;
   return t / B * B;
 }
 

@@ -179,26 +179,76 @@ template <typename T, bool INV> struct Dft<T, 3, INV> : DftOdd<T, 3, INV> {};
 template <typename T, bool INV> struct Dft<T, 5, INV> : DftOdd<T, 5, INV> {};
 template <typename T, bool INV> struct Dft<T, 7, INV> : DftOdd<T, 7, INV> {};
 
+// Radix 2 x Q (Q = 3, 5, 7) in registers, decimation in frequency: sums and differences of the
+// halves, the differences turned by w_R^n (compile-time roots), then two radix-Q transforms;
+// even outputs from the sums, odd outputs from the differences.
+template <int R> constexpr double comp_cos(int m) {   // cos(2 pi m / R), R = 6, 10, 14, m < R / 2
+  constexpr double c6[3] = {1.0, 0.5, -0.5};
+  constexpr double c10[5] = {1.0, 0.80901699437494742410, 0.30901699437494742410, -0.30901699437494742410,
+                             -0.80901699437494742410};
+  constexpr double c14[7] = {1.0, 0.90096886790241912624, 0.62348980185873353053, 0.22252093395631440429,
+                             -0.22252093395631440429, -0.62348980185873353053, -0.90096886790241912624};
+  return R == 6 ? c6[m] : (R == 10 ? c10[m] : c14[m]);
+}
+template <int R> constexpr double comp_sin(int m) {   // sin(2 pi m / R)
+  constexpr double s6[3] = {0.0, 0.86602540378443864676, 0.86602540378443864676};
+  constexpr double s10[5] = {0.0, 0.58778525229247312917, 0.95105651629515357212, 0.95105651629515357212,
+                             0.58778525229247312917};
+  constexpr double s14[7] = {0.0, 0.43388373911755812048, 0.78183148246802980871, 0.97492791218182360702,
+                             0.97492791218182360702, 0.78183148246802980871, 0.43388373911755812048};
+  return R == 6 ? s6[m] : (R == 10 ? s10[m] : s14[m]);
+}
+template <typename T, int R, bool INV> struct DftTwoOdd {
+  static __device__ __forceinline__ void run(Cx<T>* v) {
+    constexpr int Q = R / 2;
+    Cx<T> a[Q], b[Q];
+#pragma unroll
+    for (int n = 0; n < Q; ++n) {
+      a[n] = mk<T>(v[n].x + v[n + Q].x, v[n].y + v[n + Q].y);
+      const Cx<T> d = mk<T>(v[n].x - v[n + Q].x, v[n].y - v[n + Q].y);
+      const T c = (T)comp_cos<R>(n), sn = (T)comp_sin<R>(n);
+      // forward: d (c - i sn); inverse: d (c + i sn)
+      b[n] = n == 0 ? d
+                    : (INV ? mk<T>(d.x * c - d.y * sn, d.y * c + d.x * sn) : mk<T>(d.x * c + d.y * sn, d.y * c - d.x * sn));
+    }
+    Dft<T, Q, INV>::run(a);
+    Dft<T, Q, INV>::run(b);
+#pragma unroll
+    for (int k = 0; k < Q; ++k) {
+      v[2 * k] = a[k];
+      v[2 * k + 1] = b[k];
+    }
+  }
+};
+template <typename T, bool INV> struct Dft<T, 6, INV> : DftTwoOdd<T, 6, INV> {};
+template <typename T, bool INV> struct Dft<T, 10, INV> : DftTwoOdd<T, 10, INV> {};
+template <typename T, bool INV> struct Dft<T, 14, INV> : DftTwoOdd<T, 14, INV> {};
+
 // One forward stage of span S (radix R) over a tile of N rows x B columns in shared memory,
 // row r of column c at sm[r * B + c].  Thread (col, tt) with NT threads per column.
 // W[q] = exp(-2 pi i q / P); wstep = P / S so that w_S^(t u) = W[t u wstep].
 template <typename T, int R>
 __device__ __forceinline__ void stage_fwd(Cx<T>* sm, int B, int col, int tt, int NT, int N, int S,
                                           const Cx<T>* __restrict__ W, int wstep) {
-  const int q = S / R;
-  for (int b = tt; b < N / R; b += NT) {
-    const int blk = b / q, t = b - blk * q;
-    Cx<T>* p = sm + (size_t)(blk * S + t) * B + col;
+  const unsigned q = S / R, qB = q * B, nb = N / R;
+  for (unsigned b = tt; b < nb; b += NT) {
+    const unsigned blk = b / q, t = b - blk * q;
+    Cx<T>* p = sm + (blk * S + t) * B + col;
     Cx<T> v[R];
 #pragma unroll
-    for (int s = 0; s < R; ++s) v[s] = p[(size_t)s * q * B];
+    for (int s = 0; s < R; ++s) v[s] = p[s * qB];
     Dft<T, R, false>::run(v);
     if (q > 1) {
+      // w_S^(t u), u = 1 .. R - 1: the first from the table, the rest by successive products
+      // (R - 2 roundings: well inside the 1e-12 / 2e-5 bars) instead of R - 1 table loads
+      const Cx<T> w1 = __ldg(W + t * wstep);
+      Cx<T> w = w1;
+      v[1] = cmul(v[1], w);
 #pragma unroll
-      for (int u = 1; u < R; ++u) v[u] = cmul(v[u], __ldg(W + t * u * wstep));
+      for (int u = 2; u < R; ++u) { w = cmul(w, w1); v[u] = cmul(v[u], w); }
     }
 #pragma unroll
-    for (int u = 0; u < R; ++u) p[(size_t)u * q * B] = v[u];
+    for (int u = 0; u < R; ++u) p[u * qB] = v[u];
   }
 }
 
@@ -206,20 +256,23 @@ __device__ __forceinline__ void stage_fwd(Cx<T>* sm, int B, int col, int tt, int
 template <typename T, int R>
 __device__ __forceinline__ void stage_inv(Cx<T>* sm, int B, int col, int tt, int NT, int N, int S,
                                           const Cx<T>* __restrict__ W, int wstep) {
-  const int q = S / R;
-  for (int b = tt; b < N / R; b += NT) {
-    const int blk = b / q, t = b - blk * q;
-    Cx<T>* p = sm + (size_t)(blk * S + t) * B + col;
+  const unsigned q = S / R, qB = q * B, nb = N / R;
+  for (unsigned b = tt; b < nb; b += NT) {
+    const unsigned blk = b / q, t = b - blk * q;
+    Cx<T>* p = sm + (blk * S + t) * B + col;
     Cx<T> v[R];
 #pragma unroll
-    for (int u = 0; u < R; ++u) v[u] = p[(size_t)u * q * B];
+    for (int u = 0; u < R; ++u) v[u] = p[u * qB];
     if (q > 1) {
+      const Cx<T> w1 = __ldg(W + t * wstep);
+      Cx<T> w = w1;
+      v[1] = cmulc(v[1], w);
 #pragma unroll
-      for (int u = 1; u < R; ++u) v[u] = cmulc(v[u], __ldg(W + t * u * wstep));
+      for (int u = 2; u < R; ++u) { w = cmul(w, w1); v[u] = cmulc(v[u], w); }
     }
     Dft<T, R, true>::run(v);
 #pragma unroll
-    for (int s = 0; s < R; ++s) p[(size_t)s * q * B] = v[s];
+    for (int s = 0; s < R; ++s) p[s * qB] = v[s];
   }
 }
 
@@ -233,6 +286,9 @@ __device__ __forceinline__ void run_stages_fwd(Cx<T>* sm, int B, int col, int tt
     const int wstep = pl.P / S;
     switch (R) {
       case 16: stage_fwd<T, 16>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 14: stage_fwd<T, 14>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 10: stage_fwd<T, 10>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 6: stage_fwd<T, 6>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 8: stage_fwd<T, 8>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 7: stage_fwd<T, 7>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 5: stage_fwd<T, 5>(sm, B, col, tt, NT, N, S, W, wstep); break;
@@ -255,6 +311,9 @@ __device__ __forceinline__ void run_stages_inv(Cx<T>* sm, int B, int col, int tt
     const int wstep = pl.P / S;
     switch (R) {
       case 16: stage_inv<T, 16>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 14: stage_inv<T, 14>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 10: stage_inv<T, 10>(sm, B, col, tt, NT, N, S, W, wstep); break;
+      case 6: stage_inv<T, 6>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 8: stage_inv<T, 8>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 7: stage_inv<T, 7>(sm, B, col, tt, NT, N, S, W, wstep); break;
       case 5: stage_inv<T, 5>(sm, B, col, tt, NT, N, S, W, wstep); break;
@@ -292,8 +351,15 @@ inline FftPlan make_plan(int n) {
   int p2 = 1, odd = n;
   while (odd % 2 == 0) { odd /= 2; p2 *= 2; }
   while (p2 >= 8) { pl.radix[pl.nstages++] = 8; p2 /= 8; }
-  if (p2 > 1) pl.radix[pl.nstages++] = p2;
   const int primes[3] = {7, 5, 3};
+  // a remaining factor 2 (or each 2 of a remaining 4) joins an odd prime: radix 14, 10 or 6
+  for (int f : primes)
+    while (p2 > 1 && odd % f == 0) {
+      pl.radix[pl.nstages++] = 2 * f;
+      odd /= f;
+      p2 /= 2;
+    }
+  if (p2 > 1) pl.radix[pl.nstages++] = p2;
   for (int f : primes)
     while (odd % f == 0) {
       if (pl.nstages == MM_MAX_STAGES) { pl.nstages = -1; return pl; }

@@ -113,7 +113,9 @@ static void plan_layout(mm_ctx* c) {
   ig.ozp = (ig.oz + 1) / 2 * 2;
   ig.Bk = g.Bk;
   c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->nx, c->ny, c->nz, c->es);
-  c->mixed = !c->fast && c->path_pref != 1 && mixed_supported(c->nx, c->ny, c->nz, c->es);
+  // measured (profiles/r01_v4_mixed_meshes.md): the mixed-radix x-first kernels only tie with the generic
+  // z-first passes, so they are opt-in (path 3) until their stages move into registers
+  c->mixed = c->path_pref == 3 && mixed_supported(c->nx, c->ny, c->nz, c->es);
   FastGeom& fg = c->fgeom;
   fg.nx = c->nx; fg.ny = c->ny; fg.nz = c->nz;
   fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;

@@ -53,7 +53,7 @@ template <typename C> __device__ __forceinline__ C cconj(C a) { a.y = -a.y; retu
 
 constexpr int MM_MAX_STAGES = 8;
 
-// Radix plan of one in-place transform of length L = prod radix[i], radix[i] in {2, 3, 4, 5, 7, 8, 16}.
+// Radix plan of one in-place transform of length L = prod radix[i], radix[i] in {2, 3, 4, 5, 6, 7, 8, 10, 14, 16}.
 struct FftPlan {
   int L;        // sub-transform length (n_d); the padded length is P = 2L (or 1)
   int P;

@@ -91,12 +91,12 @@ def test_fast_wide_pencil_nz256_fp32(oracle, n):
 
 
 def test_fast_path_rejects_fp64_nz256():
-    """fp64 with nz = 256 is served by the mixed-radix x-first kernels; requiring the power-of-two
-    kernels fails loudly."""
+    """fp64 with nz = 256 is served by the generic passes; requiring the power-of-two kernels fails
+    loudly."""
     from paper_2606_01114_b200 import MMError
     with pytest.raises(MMError) as ei:
         make_ctx(cfg_for((64, 64, 256)), "f64", terms=1, path=2)
     assert ei.value.status == 2
     ctx = make_ctx(cfg_for((64, 64, 256)), "f64", terms=1, path=0)
-    assert ctx.path[0] is False and ctx.path_name == "mixed"
+    assert ctx.path[0] is False and ctx.path_name == "generic"
     ctx.close()

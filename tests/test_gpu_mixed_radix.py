@@ -159,7 +159,8 @@ def test_mixed_radix_xfirst_kernels_explicitly(oracle, n, dt):
 
 def test_mixed_radix_selection():
     from paper_2606_01114_b200 import MMError
-    assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0).path_name == "mixed"
+    assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0).path_name == "generic"
+    assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0, path=3).path_name == "mixed"
     assert make_ctx(cfg_for((512, 512, 128), (4e-9,) * 3), "f32", terms=0).path_name == "fast"
     assert make_ctx(cfg_for((100, 25, 1), (5e-9, 5e-9, 3e-9)), "f64", terms=0).path_name == "generic"
     assert make_ctx(cfg_for((9, 15, 5), (1e-9,) * 3), "f64", terms=0).path_name == "generic"   # ny 3 nz odd
