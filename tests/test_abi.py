@@ -74,5 +74,10 @@ def test_workspace_sizes_match_design(lib):
     h = C.c_void_p()
     assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 0, C.byref(h)) == 0
     assert lib.mm_ctx_set_path(h, 2, 0) == 2          # fast kernels do not cover thin films
-    assert lib.mm_ctx_set_path(h, 3, 0) == 1
+    assert lib.mm_ctx_set_path(h, 3, 0) == 0          # the mixed-radix x-first kernels do
+    assert lib.mm_ctx_path(h, C.byref(fast), C.byref(kc)) == 0 and fast.value == 2
+    assert lib.mm_ctx_set_path(h, 4, 0) == 1
+    lib.mm_ctx_destroy(h)
+    assert lib.mm_ctx_create(100, 25, 1, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 0
+    assert lib.mm_ctx_set_path(h, 3, 0) == 2          # one-cell axis: generic passes only
     lib.mm_ctx_destroy(h)
