@@ -375,7 +375,8 @@ def run_sweep(args):
             kb, total = byte_model(cfg.n, s, fast=ctx.path_name != "generic")
             demag_bytes = total - kb["S6_pointwise"]
             line = {"sweep": cfg.name, "dtype": dt, "cells": cfg.ncell,
-                    "path": {"fast": "fast (x-first)", "mixed": "mixed-radix (x-first)", "generic": "generic (z-first)"}[ctx.path_name],
+                    "path": {"fast": "fast (x-first)", "mixed": "mixed-radix (x-first)", "generic": "generic (z-first)",
+                             "embedded": "fast (x-first) on the enclosing power-of-two mesh"}[ctx.path_name],
                     "demag": {"ms": ms_d, "cell_updates_per_s": cfg.ncell / ms_d * 1e3,
                               "frac_hbm_measured": demag_bytes / ms_d / 1e6 / peak,
                               "frac_hbm_8TBps": demag_bytes / ms_d / 1e6 / 8000.0},

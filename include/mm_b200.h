@@ -180,10 +180,14 @@ mm_status mm_ctx_set_tiles(mm_ctx *ctx, int bz, int by, int bk);
 
 /* Demag path selection (experiments and tests).  path: 0 = automatic (the power-of-two x-first
  * kernels of demag_fast.cu where they cover the mesh: nx, ny in {64..1024}, nz in {64, 128, 256
- * (fp32)}; else the generic z-first passes), 1 = generic passes always, 2 = power-of-two kernels
+ * (fp32)}; else the same kernels on the enclosing power-of-two mesh when its extra cells cost less
+ * than the generic passes -- at most 3.0x (fp32) / 2.2x (fp64) the cells, e.g. 512 x 512 x 90 in
+ * 512 x 512 x 128: cells outside the mesh carry no magnetisation and add nothing to eq. 4; else
+ * the generic z-first passes), 1 = generic passes always, 2 = power-of-two kernels
  * required, 3 = the mixed-radix x-first kernels of demag_mixed.cu (every n_d >= 2 and ny * 3 nz
  * even; a quarter of the generic passes' table memory, same speed today)
- * (MM_ERR_UNSUPPORTED_SIZE if the required kernels do not cover the mesh).  mm_ctx_path reports 0 generic, 1 power-of-two, 2 mixed-radix.  kchunk: number of kx planes the
+ * (MM_ERR_UNSUPPORTED_SIZE if the required kernels do not cover the mesh).  mm_ctx_path reports
+ * 0 generic, 1 power-of-two, 2 mixed-radix, 3 power-of-two on the enclosing mesh.  kchunk: number of kx planes the
  * y/z/y passes of the fast path process per launch group through one reused (L2-sized)
  * buffer; 0 = all planes at once.  Changes the workspace sizes: call before
  * mm_ctx_workspace_bytes / mm_ctx_set_workspace.  mm_ctx_path reports what is selected. */

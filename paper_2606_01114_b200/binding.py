@@ -189,10 +189,11 @@ class Context:
 
     @property
     def path_name(self):
-        """'generic' (z-first passes), 'fast' (power-of-two x-first) or 'mixed' (mixed-radix x-first)."""
+        """'generic' (z-first passes), 'fast' (power-of-two x-first), 'mixed' (mixed-radix x-first) or
+        'embedded' (power-of-two x-first kernels on the enclosing power-of-two mesh)."""
         f, k = C.c_int(), C.c_int()
         self._call("mm_ctx_path", C.byref(f), C.byref(k))
-        return ("generic", "fast", "mixed")[f.value]
+        return ("generic", "fast", "mixed", "embedded")[f.value]
 
     @property
     def launch_count(self):

@@ -43,6 +43,8 @@ struct mm_ctx {
   FastGeom fgeom{};
   bool fast = false;     // the x-first kernels of demag_fast.cu cover this mesh and are selected
   bool mixed = false;    // the mixed-radix x-first kernels of demag_mixed.cu are selected
+  bool embed = false;    // the demag passes run on the enclosing power-of-two mesh dnx x dny x dnz
+  int dnx = 0, dny = 0, dnz = 0;   // mesh of the demag passes (= nx, ny, nz unless embedded)
   bool xfirst() const { return fast || mixed; }   // x-first spectra and the octant table
   int path_pref = 0;     // 0 auto, 1 generic (demag_passes.cu), 2 fast required
   int kchunk = 0;        // kx planes per K2..K4 launch group (0 = all)
@@ -55,7 +57,7 @@ struct mm_ctx {
   // persistent offsets
   size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, off_bbstate, off_bbpart, pers_need;
   // scratch offsets
-  size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, scr_need;
+  size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, off_emb_m, off_emb_h, scr_need;
   RkfState rk_host{};
   bool rk_ready = false;
   bool bb_ready = false;
@@ -90,37 +92,53 @@ static int pick_tile(int extent, size_t bytes_per_col, size_t budget, int cap) {
 static bool smooth7(int n) { return n >= 1 && make_plan(n).nstages >= 0; }
 
 // Tile widths and workspace layout; called at create and again if tiles change.
+// Embedding: a mesh the power-of-two kernels do not cover is placed in the corner of
+// the next mesh they do cover (cells outside carry no magnetisation and add nothing to eq. 4), when the
+// extra cells cost less than the slower generic passes.  Per-cell cost ratio generic / fast measured on
+// the paper's meshes (profiles/r01_v4_paper_meshes.md): about 4.6 in fp32, 3.1 in fp64.
+static bool embed_mesh(const mm_ctx* c, int* ex, int* ey, int* ez) {
+  auto up = [](int n, int cap) { int v = 64; while (v < n) v *= 2; return v <= cap ? v : 0; };
+  const int x = up(c->nx, 1024), y = up(c->ny, 1024), z = up(c->nz, c->es == 4 ? 256 : 128);
+  if (!x || !y || !z) return false;
+  const double r = (double)x * y * z / ((double)c->nx * c->ny * c->nz);
+  if (r > (c->es == 4 ? 3.0 : 2.2)) return false;
+  *ex = x; *ey = y; *ez = z;
+  return true;
+}
+
 static void plan_layout(mm_ctx* c) {
   DemagGeom& g = c->geom;
-  g.nx = c->nx; g.ny = c->ny; g.nz = c->nz;
-  g.Px = padded(c->nx); g.Py = padded(c->ny); g.Pz = padded(c->nz);
+  c->dnx = c->nx; c->dny = c->ny; c->dnz = c->nz;
+  c->embed = c->path_pref == 0 && !fast_supported(c->nx, c->ny, c->nz, c->es) && embed_mesh(c, &c->dnx, &c->dny, &c->dnz);
+  g.nx = c->dnx; g.ny = c->dny; g.nz = c->dnz;
+  g.Px = padded(c->dnx); g.Py = padded(c->dny); g.Pz = padded(c->dnz);
   g.Kz = g.Pz == 1 ? 1 : g.Pz / 2 + 1;
-  g.px = make_plan(c->nx); g.py = make_plan(c->ny); g.pz = make_plan(c->nz);
+  g.px = make_plan(c->dnx); g.py = make_plan(c->dny); g.pz = make_plan(c->dnz);
   const size_t cs = 2 * c->es;
   const size_t kMax = 200 * 1024;  // usable dynamic shared memory we plan for (227 KB limit)
-  g.Bz = c->want_bz ? c->want_bz : pick_tile(c->nx, 3 * g.Pz * cs, 100 * 1024, 32);
-  g.By = c->want_by ? c->want_by : pick_tile(c->nx, g.Py * cs, 100 * 1024, 32);
+  g.Bz = c->want_bz ? c->want_bz : pick_tile(c->dnx, 3 * g.Pz * cs, 100 * 1024, 32);
+  g.By = c->want_by ? c->want_by : pick_tile(c->dnx, g.Py * cs, 100 * 1024, 32);
   g.Bk = c->want_bk ? c->want_bk : pick_tile(g.Py, 3 * g.Px * cs, kMax, 32);
-  if (g.Bz > c->nx) g.Bz = c->nx;
-  if (g.By > c->nx) g.By = c->nx;
+  if (g.Bz > c->dnx) g.Bz = c->dnx;
+  if (g.By > c->dnx) g.By = c->dnx;
   if (g.Bk > g.Py) g.Bk = g.Py;
   InitGeom& ig = c->igeom;
-  ig.nx = c->nx; ig.ny = c->ny; ig.nz = c->nz;
+  ig.nx = c->dnx; ig.ny = c->dny; ig.nz = c->dnz;
   ig.Px = g.Px; ig.Py = g.Py; ig.Pz = g.Pz; ig.Kz = g.Kz;
-  ig.ox = c->nx == 1 ? 1 : c->nx + 1;
-  ig.oy = c->ny == 1 ? 1 : c->ny + 1;
-  ig.oz = c->nz == 1 ? 1 : c->nz + 1;
+  ig.ox = c->dnx == 1 ? 1 : c->dnx + 1;
+  ig.oy = c->dny == 1 ? 1 : c->dny + 1;
+  ig.oz = c->dnz == 1 ? 1 : c->dnz + 1;
   ig.ozp = (ig.oz + 1) / 2 * 2;
   ig.Bk = g.Bk;
-  c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->nx, c->ny, c->nz, c->es);
+  c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->dnx, c->dny, c->dnz, c->es);
   // measured (profiles/r01_v4_mixed_meshes.md): the mixed-radix x-first kernels only tie with the generic
   // z-first passes, so they are opt-in (path 3) until their stages move into registers
-  c->mixed = c->path_pref == 3 && mixed_supported(c->nx, c->ny, c->nz, c->es);
+  c->mixed = c->path_pref == 3 && mixed_supported(c->dnx, c->dny, c->dnz, c->es);
   FastGeom& fg = c->fgeom;
-  fg.nx = c->nx; fg.ny = c->ny; fg.nz = c->nz;
+  fg.nx = c->dnx; fg.ny = c->dny; fg.nz = c->dnz;
   fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;
-  fg.Q = 3 * c->nz;
-  fg.kchunk = (c->kchunk > 0 && c->kchunk < c->nx + 1) ? c->kchunk : 0;
+  fg.Q = 3 * c->dnz;
+  fg.kchunk = (c->kchunk > 0 && c->kchunk < c->dnx + 1) ? c->kchunk : 0;
   { const char* v = getenv("MM_FAST_VARIANT"); fg.variant = v ? atoi(v) : 0; }
   // persistent
   size_t o = 0;
@@ -146,8 +164,8 @@ static void plan_layout(mm_ctx* c) {
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
   o = 0;
   if (c->xfirst()) {
-    const size_t planes2 = (c->fast && fg.kchunk) ? fg.kchunk : c->nx + 1;
-    c->off_a1 = o; o += align256((size_t)(c->nx + 1) * g.ny * fg.Q * cs);
+    const size_t planes2 = (c->fast && fg.kchunk) ? fg.kchunk : c->dnx + 1;
+    c->off_a1 = o; o += align256((size_t)(c->dnx + 1) * g.ny * fg.Q * cs);
     c->off_a2 = o; o += align256(planes2 * g.Py * fg.Q * cs);
   } else {
     c->off_a1 = o; o += align256((size_t)3 * g.Kz * g.ny * g.nx * cs);
@@ -160,7 +178,10 @@ static void plan_layout(mm_ctx* c) {
   c->off_acc = o; o += align256(n3);
   c->off_sin = o; o += align256(n3);
   c->off_sout = o; o += align256(n3);
-  c->off_rkf = o; o += 6 * align256(n3);   // RKF45: k_1..k_6, n3 reals apart (stage state and candidate reuse msa, msb)
+  c->off_rkf = o; o += 6 * align256(n3);
+  const size_t e3 = c->embed ? (size_t)c->dnx * c->dny * c->dnz * 3 * c->es : 0;   // embedded m and H
+  c->off_emb_m = o; o += align256(e3);
+  c->off_emb_h = o; o += align256(e3);   // RKF45: k_1..k_6, n3 reals apart (stage state and candidate reuse msa, msb)
   (void)spectra;
   const size_t init_need = demag_init_scratch_bytes(ig);  // aliases the start of scratch
   c->scr_need = o > init_need ? o : init_need;
@@ -244,7 +265,7 @@ mm_status mm_ctx_set_path(mm_ctx* ctx, int path, int kchunk) {
 
 mm_status mm_ctx_path(const mm_ctx* ctx, int* fast, int* kchunk) {
   if (!ctx || !fast || !kchunk) return MM_ERR_INVALID_ARG;
-  *fast = ctx->fast ? 1 : (ctx->mixed ? 2 : 0);
+  *fast = ctx->fast ? (ctx->embed ? 3 : 1) : (ctx->mixed ? 2 : 0);
   *kchunk = ctx->fgeom.kchunk;
   return MM_OK;
 }
@@ -402,9 +423,9 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   fill_twiddles<T>(host, c->off_wx - small_off, g.Px);
   fill_twiddles<T>(host, c->off_wy - small_off, g.Py);
   fill_twiddles<T>(host, c->off_wz - small_off, g.Pz);
-  const bool two_x = c->fast && fast_two_stage(c->nx, c->es), two_y = c->fast && fast_two_stage(c->ny, c->es);
-  if (two_x) fill_twiddles2<T>(host, c->off_t2x - small_off, c->nx);
-  if (two_y) fill_twiddles2<T>(host, c->off_t2y - small_off, c->ny);
+  const bool two_x = c->fast && fast_two_stage(c->dnx, c->es), two_y = c->fast && fast_two_stage(c->dny, c->es);
+  if (two_x) fill_twiddles2<T>(host, c->off_t2x - small_off, c->dnx);
+  if (two_y) fill_twiddles2<T>(host, c->off_t2y - small_off, c->dny);
   auto u16 = [&](size_t off) { return reinterpret_cast<uint16_t*>(host.data() + (off - small_off)); };
   for (int k = 0; k < g.Pz; ++k) {
     const int p = pos_of_freq(g.pz, k);
@@ -413,12 +434,12 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   }
   for (int k = 0; k < g.Px; ++k) {
     const int p = pos_of_freq(g.px, k);
-    u16(c->off_posx)[k] = (uint16_t)(c->fast ? fast_swizzle(c->nx, fast_pos_logical(c->nx, k)) : p);
+    u16(c->off_posx)[k] = (uint16_t)(c->fast ? fast_swizzle(c->dnx, fast_pos_logical(c->dnx, k)) : p);
     u16(c->off_fx)[p] = (uint16_t)k;
   }
   for (int k = 0; k < g.Py; ++k) {
     const int p = pos_of_freq(g.py, k);
-    u16(c->off_posy)[k] = (uint16_t)(c->fast ? (two_y ? k : fast_pos_logical(c->ny, k)) : p);
+    u16(c->off_posy)[k] = (uint16_t)(c->fast ? (two_y ? k : fast_pos_logical(c->dny, k)) : p);
     u16(c->off_fy)[p] = (uint16_t)k;
   }
   cudaError_t e = cudaMemcpyAsync(c->pers + small_off, host.data(), small_bytes,
@@ -430,6 +451,9 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
                            reinterpret_cast<T*>(c->pers + c->off_table), c->xfirst() ? 1 : 0, c->stream,
                            &c->launches);
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: launch", e);
+  if (c->embed)   // the padding cells of the embedded m stay zero from here on (init's scratch use is over)
+    e = cudaMemsetAsync(c->scr + c->off_emb_m, 0, (size_t)c->dnx * c->dny * c->dnz * 3 * c->es, c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: clearing the embedded mesh", e);
   e = cudaStreamSynchronize(c->stream);  // also keeps `host` alive until the copy is done
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: execution", e);
   c->demag_ready = true;
@@ -493,8 +517,8 @@ template <typename T> static FastBufs<T> fast_bufs_of(mm_ctx* c) {
   b.posy = reinterpret_cast<const uint16_t*>(c->pers + c->off_posy);
   b.T2x = reinterpret_cast<const Cx<T>*>(c->pers + c->off_t2x);
   b.T2y = reinterpret_cast<const Cx<T>*>(c->pers + c->off_t2y);
-  b.two_x = fast_two_stage(c->nx, c->es);
-  b.two_y = fast_two_stage(c->ny, c->es);
+  b.two_x = fast_two_stage(c->dnx, c->es);
+  b.two_y = fast_two_stage(c->dny, c->es);
   b.table = reinterpret_cast<const T*>(c->pers + c->off_table);
   b.A1 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a1);
   b.A2 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a2);
@@ -521,6 +545,20 @@ template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H
     cudaError_t e = demag_mixed_launch<T>(c->fgeom, pl, mixed_bufs_of<T>(c), static_cast<const T*>(m),
                                           static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches, &c->prof);
     return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag (mixed-radix path) launch", e);
+  }
+  if (c->fast && c->embed) {
+    T* mE = reinterpret_cast<T*>(c->scr + c->off_emb_m);
+    T* HE = reinterpret_cast<T*>(c->scr + c->off_emb_h);
+    c->prof.mark(0, c->stream);
+    cudaError_t e = embed_copy_launch<T>(static_cast<const T*>(m), mE, c->nx, c->ny, c->nz, c->dny, c->dnz, 1, c->stream);
+    if (e == cudaSuccess)
+      e = demag_fast_launch<T>(c->fgeom, fast_bufs_of<T>(c), mE, HE, (T)(-c->Ms), c->stream, &c->launches, &c->prof);
+    c->prof.mark(4, c->stream);
+    if (e == cudaSuccess)
+      e = embed_copy_launch<T>(HE, static_cast<T*>(H), c->nx, c->ny, c->nz, c->dny, c->dnz, 0, c->stream);
+    c->prof.mark(-1, c->stream);
+    c->launches += 2;
+    return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag (embedded fast path) launch", e);
   }
   if (c->fast) {
     cudaError_t e = demag_fast_launch<T>(c->fgeom, fast_bufs_of<T>(c), static_cast<const T*>(m),
@@ -582,6 +620,10 @@ mm_status mm_demag_nhat_export(mm_ctx* ctx, void* out) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (!ctx->demag_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_demag_nhat_export: mm_demag_init not called");
   if (!out || ((uintptr_t)out & 15)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_demag_nhat_export: bad pointer");
+  if (ctx->embed)
+    return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_demag_nhat_export: this context holds the table of the enclosing "
+                "%dx%dx%d mesh; select the generic passes (mm_ctx_set_path 1) to export the mesh's own table",
+                ctx->dnx, ctx->dny, ctx->dnz);
   const uint16_t* posx = reinterpret_cast<const uint16_t*>(ctx->pers + ctx->off_posx);
   const uint16_t* posy = reinterpret_cast<const uint16_t*>(ctx->pers + ctx->off_posy);
   cudaError_t e;

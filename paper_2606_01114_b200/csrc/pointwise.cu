@@ -319,6 +319,25 @@ cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T
   return cudaGetLastError();
 }
 
+template <typename T>
+__global__ void __launch_bounds__(128) embed_copy_kernel(const T* __restrict__ src, T* __restrict__ dst, int ny, int nz,
+                                                         int eny, int enz, int embed) {
+  const int x = blockIdx.x / ny, y = blockIdx.x - x * ny;
+  const size_t small = ((size_t)x * ny + y) * nz * 3, big = ((size_t)x * eny + y) * enz * 3;
+  const T* s = src + (embed ? small : big);
+  T* d = dst + (embed ? big : small);
+  for (int q = threadIdx.x; q < 3 * nz; q += blockDim.x) d[q] = s[q];
+}
+
+template <typename T>
+cudaError_t embed_copy_launch(const T* src, T* dst, int nx, int ny, int nz, int eny, int enz, int embed,
+                              cudaStream_t st) {
+  embed_copy_kernel<T><<<(unsigned)(nx * ny), 128, 0, st>>>(src, dst, ny, nz, eny, enz, embed);
+  return cudaGetLastError();
+}
+template cudaError_t embed_copy_launch<float>(const float*, float*, int, int, int, int, int, int, cudaStream_t);
+template cudaError_t embed_copy_launch<double>(const double*, double*, int, int, int, int, int, int, cudaStream_t);
+
 template cudaError_t pointwise_launch<float>(int, const PwParams<float>&, const float*,
                                              const float*, float*, float*, float*, cudaStream_t,
                                              unsigned long long*, Prof*);

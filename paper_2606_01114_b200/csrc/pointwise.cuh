@@ -33,4 +33,11 @@ cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T
                              T* m0, T* acc, cudaStream_t st, unsigned long long* launches,
                              Prof* prof);
 
+// Copies between the mesh [nx][ny][nz][3] and its embedding in the corner of [..][eny][enz][3]
+// (mm_api.cu "Embedding").  embed != 0: mesh -> embedded array (padding cells untouched);
+// embed == 0: embedded array -> mesh.
+template <typename T>
+cudaError_t embed_copy_launch(const T* src, T* dst, int nx, int ny, int nz, int eny, int enz, int embed,
+                              cudaStream_t st);
+
 }  // namespace mm

@@ -166,3 +166,30 @@ def test_mixed_radix_selection():
     assert make_ctx(cfg_for((9, 15, 5), (1e-9,) * 3), "f64", terms=0).path_name == "generic"   # ny 3 nz odd
     with pytest.raises(MMError):
         make_ctx(cfg_for((100, 25, 1), (5e-9, 5e-9, 3e-9)), "f64", terms=0, path=3)
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+@pytest.mark.parametrize("n", [(60, 50, 40), (40, 64, 100), (100, 100, 100)])
+def test_embedding_in_the_enclosing_power_of_two_mesh(oracle, n, dt):
+    """Automatic selection places these meshes in the corner of 64^3 / 64 x 64 x 128 / 128^3 and runs the
+    power-of-two kernels there (cells outside carry no magnetisation): dense parity vs the oracle FFT
+    path, agreement with the generic passes, H_eff + LLG through the cropped field, determinism."""
+    cfg = cfg_for(n, (4e-9, 3e-9, 2e-9), terms=1 | 2 | 8, Hext=(1e4, 2e4, -3e4))
+    m, m64 = round_input(w.random_unit_vectors(414, n), dt)
+    P = make_problem(oracle, cfg)
+    ctx = make_ctx(cfg, dt)
+    assert ctx.path_name == "embedded"
+    md = to_dev(m)
+    got = ctx.demag_field(md).cpu().numpy()
+    l2, mx = w.field_errors(got, oracle.demag_fft(P.Nhat, cfg.Ms, m64))
+    assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+    assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
+    l2, mx = w.field_errors(ctx.llg_rhs(md).cpu().numpy(), P.llg_rhs(m64))
+    assert l2 <= TOL[dt], (l2, mx)
+    gen = make_ctx(cfg, dt, path=1)
+    assert gen.path_name == "generic"
+    l2, mx = w.field_errors(gen.demag_field(md).cpu().numpy(), got)
+    assert l2 <= TOL[dt], (l2, mx)
+    from paper_2606_01114_b200 import MMError
+    with pytest.raises(MMError):
+        ctx.nhat_export()
