@@ -139,6 +139,43 @@ def test_config2_first_100_steps(oracle, dt):
     assert worst <= TRAJ_TOL[dt], worst
 
 
+@pytest.mark.slow
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+def test_config2_full_run_average_magnetisation(oracle, dt):
+    """Config 2 as BASELINE.json states it: 10,000 RK4 steps at dt = 1e-13 s (1 ns) with demag + exchange +
+    Zeeman.  The CUDA path replays one captured step (CUDA graph); <m>(t) is compared with the oracle's
+    every 100 steps and the final state pointwise (reading Q18: no hard gate beyond step 100 is
+    stated in BASELINE, the bars here are what fp64 / fp32 round-off growth over 40,000 evaluations allows)."""
+    import torch
+    cfg = w.get_config(2)
+    m, m64 = round_input(cfg.initial_m(), dt)
+    P = make_problem(oracle, cfg)
+    ctx = make_ctx(cfg, dt)
+    md = to_dev(m)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        ctx.use_current_stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for _ in range(100):
+                ctx.rk_step(md, cfg.dt)
+        ref = m64
+        drift = 0.0
+        for block in range(100):
+            g.replay()
+            for _ in range(100):
+                ref = P.rk4_step(ref, cfg.dt)
+            s.synchronize()
+            avg = md.double().mean(dim=(0, 1, 2)).cpu().numpy()
+            drift = max(drift, float(np.max(np.abs(avg - ref.mean(axis=(0, 1, 2))))))
+        final = w.traj_error(md.cpu().numpy(), ref)
+    print(f"config 2, 10,000 steps, {dt}: max |<m> - <m>_oracle| = {drift:.3e}, final pointwise = {final:.3e}")
+    # the driven strip has switched: <m_x> went from ~ +1 to negative (PAPER.md:140-143 reversal field)
+    assert ref.mean(axis=(0, 1, 2))[0] < 0.0
+    assert drift <= (1e-9 if dt == "f64" else 5e-3) and final <= (1e-8 if dt == "f64" else 5e-2), (drift, final)
+
+
 def test_host_calls_match_device_calls(oracle):
     cfg = cfg_for((32, 16, 8), (4e-9, 3e-9, 2e-9))
     ctx = make_ctx(cfg, "f32")
