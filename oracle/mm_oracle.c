@@ -27,6 +27,7 @@
  *                            (PAPER.md:30 names the term; amplitudes are inputs, reading Q29)
  *   O13 orc_bb_step          Barzilai-Borwein energy minimiser iteration, PAPER.md:55, 146-148 (named only;
  *                            step rule, update and stop criterion are reading Q30)
+ *   O14 orc_heff (cells)     per-cell Ms and A (eq. 2 as div(A grad M)); discrete form = reading Q31
  *   O10 orc_rkf45_step       Runge-Kutta-Fehlberg 4(5) attempt + max-error step control
  *                            (the paper names the method and the max-error reduction; tableau, error
  *                            norm and controller are readings Q23-Q26 of DESIGN.md)
@@ -564,10 +565,93 @@ typedef struct {
   const double *Nhat; /* from orc_demag_fft_nhat; required if DEMAG is enabled */
   double D, edmi[9];                      /* DMI constant (J/m^2) and the three DMI vectors */
   double stt_p[3], stt_damp, stt_field;   /* spin-torque field: unit polarisation, amplitudes (A/m) */
+  const double *Ms_cells, *A_cells;       /* per-cell Ms (A/m) and A (J/m), [nx][ny][nz]; NULL = uniform Ms / Aex */
 } orc_problem;
+
+/* O14 inhomogeneous material parameters ("inhomogeneous material parameters"; eq. 2 is
+ * written as div(A grad M) for that reason; the discrete form is DESIGN.md reading Q31):
+ *   demag     H(i) = - sum_j N(i - j) Ms_j m_j                                   (M = Ms m, eq. 4)
+ *   exchange  H(i) = 2/(mu0 Ms_i) sum_{d, +-} A_ij (m_j - m_i) / D_d^2,  A_ij = 2 A_i A_j / (A_i + A_j)
+ *             (harmonic mean: the flux A dm/dx is continuous across the interface; 0 if either is 0),
+ *             a neighbour outside the mesh contributes nothing (Q5)
+ *   anisotropy, DMI: the homogeneous formulas with Ms_i; for DMI a neighbour with Ms_j = 0 counts as
+ *             outside the mesh (replaced by the cell itself, Q28)
+ *   a cell with Ms_i = 0 is vacuum: the terms with a 1/Ms_i prefactor vanish there and dm/dt = 0.
+ * Ms_i(p, i), A_i(p, i) read the arrays or fall back to the uniform values. */
+static double ms_at(const orc_problem *p, size_t i) { return p->Ms_cells ? p->Ms_cells[i] : p->Ms; }
+static double a_at(const orc_problem *p, size_t i) { return p->A_cells ? p->A_cells[i] : p->Aex; }
+
+static int orc_heff_cells(const orc_problem *p, const double *m, double *H) {
+  const int nx = p->nx, ny = p->ny, nz = p->nz;
+  const size_t n = (size_t)nx * ny * nz;
+  const double h[3] = {p->dx, p->dy, p->dz};
+  const int nn[3] = {nx, ny, nz};
+  memset(H, 0, 3 * n * sizeof(double));
+  if (p->terms & ORC_TERM_DEMAG) {
+    if (!p->Nhat) return 3;
+    double *Mm = malloc(3 * n * sizeof(double)), *T = malloc(3 * n * sizeof(double));
+    if (!Mm || !T) { free(Mm); free(T); return 2; }
+    for (size_t i = 0; i < n; ++i)
+      for (int c = 0; c < 3; ++c) Mm[3 * i + c] = ms_at(p, i) * m[3 * i + c];
+    int rc = orc_demag_fft(nx, ny, nz, p->Nhat, 1.0, Mm, T);   /* - sum N M */
+    if (!rc) for (size_t i = 0; i < 3 * n; ++i) H[i] += T[i];
+    free(Mm); free(T);
+    if (rc) return rc;
+  }
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int x = 0; x < nx; ++x)
+    for (int y = 0; y < ny; ++y)
+      for (int z = 0; z < nz; ++z) {
+        const int idx[3] = {x, y, z};
+        const size_t ci = ((size_t)x * ny + y) * nz + z, i0 = 3 * ci;
+        const double Msi = ms_at(p, ci), Ai = a_at(p, ci);
+        double acc[3] = {0, 0, 0};
+        if (Msi > 0.0) {
+          for (int d = 0; d < 3; ++d) {
+            double dm[3] = {0, 0, 0};   /* m(+) - m(-) with the boundary / vacuum rule, for DMI */
+            for (int sgn = -1; sgn <= 1; sgn += 2) {
+              int j[3] = {x, y, z};
+              j[d] += sgn;
+              const int inside = j[d] >= 0 && j[d] < nn[d];
+              const size_t cj = inside ? ((size_t)j[0] * ny + j[1]) * nz + j[2] : ci;
+              const double Msj = ms_at(p, cj), Aj = a_at(p, cj);
+              if ((p->terms & ORC_TERM_EXCHANGE) && inside && Ai + Aj > 0.0) {
+                const double Aij = 2.0 * Ai * Aj / (Ai + Aj);
+                for (int c = 0; c < 3; ++c)
+                  acc[c] += 2.0 / (ORC_MU0 * Msi) * Aij * (m[3 * cj + c] - m[i0 + c]) / (h[d] * h[d]);
+              }
+              const size_t cd = (inside && Msj > 0.0) ? cj : ci;
+              for (int c = 0; c < 3; ++c) dm[c] += sgn * m[3 * cd + c];
+            }
+            if (p->terms & ORC_TERM_DMI) {
+              const double *ek = p->edmi + 3 * d;
+              const double f = 2.0 * p->D / (ORC_MU0 * Msi) / (2.0 * h[d]);
+              acc[0] += f * (ek[1] * dm[2] - ek[2] * dm[1]);
+              acc[1] += f * (ek[2] * dm[0] - ek[0] * dm[2]);
+              acc[2] += f * (ek[0] * dm[1] - ek[1] * dm[0]);
+            }
+          }
+          if (p->terms & ORC_TERM_ANISOTROPY) {
+            const double dot = m[i0] * p->axis[0] + m[i0 + 1] * p->axis[1] + m[i0 + 2] * p->axis[2];
+            for (int c = 0; c < 3; ++c) acc[c] += 2.0 * p->Ku / (ORC_MU0 * Msi) * dot * p->axis[c];
+          }
+        }
+        if (p->terms & ORC_TERM_ZEEMAN)
+          for (int c = 0; c < 3; ++c) acc[c] += p->Hext[c];
+        if (p->terms & ORC_TERM_STT) {
+          const double *mi = m + i0, *pv = p->stt_p;
+          acc[0] += p->stt_damp * (mi[1] * pv[2] - mi[2] * pv[1]) + p->stt_field * pv[0];
+          acc[1] += p->stt_damp * (mi[2] * pv[0] - mi[0] * pv[2]) + p->stt_field * pv[1];
+          acc[2] += p->stt_damp * (mi[0] * pv[1] - mi[1] * pv[0]) + p->stt_field * pv[2];
+        }
+        for (int c = 0; c < 3; ++c) H[i0 + c] += acc[c];
+      }
+  return 0;
+}
 
 /* H_eff = sum of enabled terms. */
 int orc_heff(const orc_problem *p, const double *m, double *H) {
+  if (p->Ms_cells || p->A_cells) return orc_heff_cells(p, m, H);
   const size_t n = (size_t)p->nx * p->ny * p->nz;
   double *T = malloc(3 * n * sizeof(double));
   if (!T) return 2;
@@ -626,6 +710,9 @@ int orc_llg_rhs(const orc_problem *p, const double *m, double *dmdt) {
   if (!H) return 2;
   int rc = orc_heff(p, m, H);
   if (!rc) rc = orc_llg_torque(n, p->alpha, p->gamma, m, H, dmdt);
+  if (!rc && p->Ms_cells)   /* vacuum cells (Ms_i = 0) carry no magnetisation: dm/dt = 0 (O14) */
+    for (size_t i = 0; i < n; ++i)
+      if (!(p->Ms_cells[i] > 0.0)) dmdt[3 * i] = dmdt[3 * i + 1] = dmdt[3 * i + 2] = 0.0;
   free(H);
   return rc;
 }
@@ -647,7 +734,7 @@ int orc_rk4_step(const orc_problem *p, double *m, double dt) {
     for (size_t i = 0; i < n3; ++i) m[i] += dt / 6.0 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
     for (size_t i = 0; i < n3; i += 3) {
       const double nrm = sqrt(m[i] * m[i] + m[i + 1] * m[i + 1] + m[i + 2] * m[i + 2]);
-      m[i] /= nrm; m[i + 1] /= nrm; m[i + 2] /= nrm;
+      if (nrm > 0.0) { m[i] /= nrm; m[i + 1] /= nrm; m[i + 2] /= nrm; }   /* a zero vector (vacuum cell) stays zero */
     }
   }
   free(k1); free(ms);
@@ -723,7 +810,7 @@ int orc_rkf45_step(const orc_problem *p, double *m, double dt, double tol, doubl
     if (*accepted) {
       for (size_t q = 0; q < n3; q += 3) {
         const double nrm = sqrt(ms[q] * ms[q] + ms[q + 1] * ms[q + 1] + ms[q + 2] * ms[q + 2]);
-        m[q] = ms[q] / nrm; m[q + 1] = ms[q + 1] / nrm; m[q + 2] = ms[q + 2] / nrm;
+        if (nrm > 0.0) { m[q] = ms[q] / nrm; m[q + 1] = ms[q + 1] / nrm; m[q + 2] = ms[q + 2] / nrm; }
       }
     }
   }
@@ -765,6 +852,7 @@ int orc_bb_step(const orc_problem *p, double *m, orc_bb_state *st) {
     double mxh[3];
     cross3(m + i, H + i, mxh);
     cross3(m + i, mxh, g + i);
+    if (p->Ms_cells && !(p->Ms_cells[i / 3] > 0.0)) g[i] = g[i + 1] = g[i + 2] = 0.0;   /* vacuum cell (O14) */
   }
   double tau = st->tau0;
   if (st->n > 0) {

@@ -48,7 +48,8 @@ class _Problem(C.Structure):
                 ("axis", C.c_double * 3), ("alpha", C.c_double), ("gamma", C.c_double),
                 ("Hext", C.c_double * 3), ("terms", C.c_uint), ("Nhat", C.c_void_p),
                 ("D", C.c_double), ("edmi", C.c_double * 9),
-                ("stt_p", C.c_double * 3), ("stt_damp", C.c_double), ("stt_field", C.c_double)]
+                ("stt_p", C.c_double * 3), ("stt_damp", C.c_double), ("stt_field", C.c_double),
+                ("Ms_cells", C.c_void_p), ("A_cells", C.c_void_p)]
 
 
 def lib():
@@ -253,6 +254,8 @@ class Problem:
     stt_p: tuple = (0.0, 0.0, 1.0)
     stt_damp: float = 0.0
     stt_field: float = 0.0
+    Ms_cells: np.ndarray | None = field(default=None, repr=False)   # [nx, ny, nz] or None (uniform Ms)
+    A_cells: np.ndarray | None = field(default=None, repr=False)    # [nx, ny, nz] or None (uniform Aex)
     N: np.ndarray | None = field(default=None, repr=False)
     Nhat: np.ndarray | None = field(default=None, repr=False)
 
@@ -278,6 +281,12 @@ class Problem:
         s.edmi[:] = [float(v) for row in self.edmi for v in row]
         s.stt_p[:] = list(self.stt_p)
         s.stt_damp, s.stt_field = self.stt_damp, self.stt_field
+        if self.Ms_cells is not None:
+            self.Ms_cells = _f64(self.Ms_cells)
+            s.Ms_cells = self.Ms_cells.ctypes.data
+        if self.A_cells is not None:
+            self.A_cells = _f64(self.A_cells)
+            s.A_cells = self.A_cells.ctypes.data
         return s
 
     def heff(self, m):
