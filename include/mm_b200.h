@@ -74,6 +74,15 @@ mm_status mm_set_material(mm_ctx *ctx, double Ms, double Aex, double Ku, const d
                           double alpha, double gamma);
 /* Uniform external field in A/m (PAPER.md:140-143 ExternalField(B/mu0)). */
 mm_status mm_set_zeeman(mm_ctx *ctx, const double Hext[3]);
+/* Per-cell saturation magnetisation and exchange stiffness ("inhomogeneous material
+ * parameters"; eq. 2 is div(A grad M); discrete form: DESIGN.md reading Q31).  Ms_cells, A_cells:
+ * DEVICE arrays [nx][ny][nz] in the context's dtype (A/m, J/m), owned by the caller and read at
+ * every later call until replaced; either may be NULL (the uniform value of mm_set_material).
+ *   demag: M_j = Ms_j m_j;   exchange: 2/(mu0 Ms_i) sum A_ij (m_j - m_i)/d^2 with the harmonic mean
+ *   A_ij = 2 A_i A_j/(A_i + A_j);   anisotropy, DMI: with Ms_i (DMI: a neighbour with Ms_j = 0 counts
+ *   as outside the mesh);   Ms_i = 0 is vacuum: those terms vanish, dm/dt = 0, m is left alone.
+ * With arrays set the pointwise pass runs one cell per thread (no 128-bit vector path). */
+mm_status mm_set_material_cells(mm_ctx *ctx, const void *Ms_cells, const void *A_cells);
 /* Dzyaloshinskii-Moriya interaction (eq. 3):
  *   H = 2D/(mu0 Ms) sum_{k=x,y,z} e_k^DMI x dm/dk,
  * D in J/m^2, e[3 k + c] = component c of the DMI vector of direction k.  The paper's two

@@ -52,6 +52,7 @@ def load_library():
         "mm_ctx_set_workspace": [vp, vp, sz, vp, sz],
         "mm_set_material": [vp, dbl, dbl, dbl, C.POINTER(dbl), dbl, dbl],
         "mm_set_zeeman": [vp, C.POINTER(dbl)],
+        "mm_set_material_cells": [vp, vp, vp],
         "mm_set_dmi": [vp, dbl, C.POINTER(dbl)],
         "mm_set_stt": [vp, C.POINTER(dbl), dbl, dbl],
         "mm_set_terms": [vp, C.c_uint],
@@ -167,6 +168,16 @@ class Context:
 
     def set_zeeman(self, Hext):
         self._call("mm_set_zeeman", (C.c_double * 3)(*Hext))
+
+    def set_material_cells(self, Ms_cells=None, A_cells=None):
+        """Per-cell Ms / A as cuda tensors of shape n in the context dtype (kept alive by the context)."""
+        for t in (Ms_cells, A_cells):
+            if t is not None and not (t.is_cuda and t.dtype == self.dtype and t.is_contiguous()
+                                      and tuple(t.shape) == self.n):
+                raise ValueError(f"expected contiguous cuda {self.dtype} tensor of shape {self.n}")
+        self._cells = (Ms_cells, A_cells)
+        self._call("mm_set_material_cells", Ms_cells.data_ptr() if Ms_cells is not None else None,
+                   A_cells.data_ptr() if A_cells is not None else None)
 
     def set_dmi(self, D, e=DMI_INTERFACIAL):
         self._call("mm_set_dmi", float(D), (C.c_double * 9)(*[float(v) for row in e for v in row]))

@@ -36,6 +36,8 @@ struct mm_ctx {
   double Hext[3] = {0, 0, 0};
   double Ddmi = 0, edmi[9] = {0, 1, 0, -1, 0, 0, 0, 0, 0};   // interfacial vectors by default
   double stt_p[3] = {0, 0, 1}, stt_damp = 0, stt_field = 0;
+  const void* ms_cells = nullptr;   // per-cell Ms / A (device, ctx dtype, caller-owned), or NULL = uniform
+  const void* a_cells = nullptr;
   unsigned terms = MM_TERM_DEMAG | MM_TERM_EXCHANGE;
   // plan
   DemagGeom geom{};
@@ -57,7 +59,7 @@ struct mm_ctx {
   // persistent offsets
   size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, off_bbstate, off_bbpart, pers_need;
   // scratch offsets
-  size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, off_emb_m, off_emb_h, scr_need;
+  size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, off_emb_m, off_emb_h, off_mscaled, scr_need;
   RkfState rk_host{};
   bool rk_ready = false;
   bool bb_ready = false;
@@ -181,7 +183,8 @@ static void plan_layout(mm_ctx* c) {
   c->off_rkf = o; o += 6 * align256(n3);
   const size_t e3 = c->embed ? (size_t)c->dnx * c->dny * c->dnz * 3 * c->es : 0;   // embedded m and H
   c->off_emb_m = o; o += align256(e3);
-  c->off_emb_h = o; o += align256(e3);   // RKF45: k_1..k_6, n3 reals apart (stage state and candidate reuse msa, msb)
+  c->off_emb_h = o; o += align256(e3);
+  c->off_mscaled = o; o += align256(n3);   // M = Ms_i m when Ms varies per cell   // RKF45: k_1..k_6, n3 reals apart (stage state and candidate reuse msa, msb)
   (void)spectra;
   const size_t init_need = demag_init_scratch_bytes(ig);  // aliases the start of scratch
   c->scr_need = o > init_need ? o : init_need;
@@ -341,6 +344,15 @@ mm_status mm_set_stt(mm_ctx* ctx, const double p[3], double a_damp, double a_fie
   return MM_OK;
 }
 
+mm_status mm_set_material_cells(mm_ctx* ctx, const void* Ms_cells, const void* A_cells) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (((uintptr_t)Ms_cells & 15) || ((uintptr_t)A_cells & 15))
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_material_cells: device pointers must be 16-byte aligned");
+  ctx->ms_cells = Ms_cells;
+  ctx->a_cells = A_cells;
+  return MM_OK;
+}
+
 mm_status mm_set_terms(mm_ctx* ctx, unsigned term_mask) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (term_mask & ~63u) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_terms: unknown term bits 0x%x", term_mask);
@@ -487,6 +499,15 @@ template <typename T> static PwParams<T> pw_of(const mm_ctx* c, unsigned terms) 
   const int nn[3] = {c->nx, c->ny, c->nz};
   for (int k = 0; k < 3; ++k)
     for (int i = 0; i < 3; ++i) p.dmi[k][i] = nn[k] > 1 ? (T)(pd * c->edmi[3 * k + i] / (2.0 * cell[k])) : (T)0;
+  p.ms_cells = static_cast<const T*>(c->ms_cells);
+  p.a_cells = static_cast<const T*>(c->a_cells);
+  p.ms_ref = (T)c->Ms; p.a_ref = (T)c->Aex;
+  for (int k = 0; k < 3; ++k) {
+    p.exq[k] = (T)(2.0 / (kMu0 * cell[k] * cell[k]));
+    for (int i = 0; i < 3; ++i)
+      p.dmiq[k][i] = nn[k] > 1 ? (T)(2.0 * c->Ddmi / kMu0 * c->edmi[3 * k + i] / (2.0 * cell[k])) : (T)0;
+  }
+  p.kanq = (T)(2.0 * c->Ku / kMu0);
   for (int i = 0; i < 3; ++i) p.sp[i] = (T)c->stt_p[i];
   p.sdamp = (T)c->stt_damp; p.sfield = (T)c->stt_field;
   p.pref = (T)(-c->gamma / (1.0 + c->alpha * c->alpha));
@@ -539,7 +560,25 @@ template <typename T> static MixedBufs<T> mixed_bufs_of(mm_ctx* c) {
   return b;
 }
 
+template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H);
+
+// per-cell Ms: the passes transform M = Ms_i m and the final scale is -1 (eq. 4 with M = Ms m)
+template <typename T> static mm_status demag_cells_t(mm_ctx* c, const void* m, void* H) {
+  T* M = reinterpret_cast<T*>(c->scr + c->off_mscaled);
+  cudaError_t e = scale_by_ms_launch<T>(static_cast<const T*>(m), static_cast<const T*>(c->ms_cells), M,
+                                        (size_t)c->nx * c->ny * c->nz, c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, "demag (per-cell Ms) launch", e);
+  ++c->launches;
+  const double Ms = c->Ms;
+  const void* cells = c->ms_cells;
+  c->Ms = 1.0; c->ms_cells = nullptr;
+  const mm_status s = demag_t<T>(c, M, H);
+  c->Ms = Ms; c->ms_cells = cells;
+  return s;
+}
+
 template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H) {
+  if (c->ms_cells) return demag_cells_t<T>(c, m, H);
   if (c->mixed) {
     const MixedPlans pl{c->geom.px, c->geom.py, c->geom.pz};
     cudaError_t e = demag_mixed_launch<T>(c->fgeom, pl, mixed_bufs_of<T>(c), static_cast<const T*>(m),

@@ -283,6 +283,132 @@ __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __
   }
 }
 
+// Per-cell Ms and A (eq. 2 as div(A grad M); reading Q31): thread = one cell.
+//   exchange  2/(mu0 Ms_i) sum A_ij (m_j - m_i)/d^2, A_ij = 2 A_i A_j/(A_i + A_j), missing neighbour: no term
+//   DMI, anisotropy with Ms_i; for DMI a neighbour outside the mesh or with Ms_j = 0 is the cell itself
+//   Ms_i = 0: vacuum -- those terms vanish, dm/dt = 0, a zero vector is not renormalised
+template <typename T, int MODE>
+__global__ void __launch_bounds__(256) pw_inhom_kernel(PwParams<T> p, const T* __restrict__ m,
+                                                       const T* __restrict__ Hd, T* __restrict__ out,
+                                                       T* __restrict__ m0, T* __restrict__ acc) {
+  const size_t total = (size_t)p.nx * p.ny * p.nz;
+  const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= total) return;
+  const int z = (int)(g % p.nz);
+  const int y = (int)((g / p.nz) % p.ny);
+  const int x = (int)(g / ((size_t)p.nz * p.ny));
+  const size_t off[3] = {(size_t)p.nz * p.ny, (size_t)p.nz, 1};   // in cells
+  const int idx[3] = {x, y, z}, n[3] = {p.nx, p.ny, p.nz};
+  const size_t base = g * 3;
+  const T Msi = p.ms_cells ? p.ms_cells[g] : p.ms_ref, Ai = p.a_cells ? p.a_cells[g] : p.a_ref;
+  const bool mag = Msi > (T)0;
+  T mc[3] = {m[base], m[base + 1], m[base + 2]};
+  T lap[3] = {0, 0, 0}, hx[3] = {0, 0, 0};
+  const bool want_ex = (p.terms & MM_TERM_EXCHANGE) || MODE == PW_EXCHANGE;
+  const bool want_dmi = (p.terms & MM_TERM_DMI) && MODE != PW_EXCHANGE;
+  if (mag && (want_ex || want_dmi)) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      T dm[3] = {0, 0, 0};
+#pragma unroll
+      for (int sg = -1; sg <= 1; sg += 2) {
+        const bool inside = sg < 0 ? idx[d] > 0 : idx[d] + 1 < n[d];
+        const size_t cj = inside ? (sg < 0 ? g - off[d] : g + off[d]) : g;
+        const T Msj = p.ms_cells ? p.ms_cells[cj] : p.ms_ref, Aj = p.a_cells ? p.a_cells[cj] : p.a_ref;
+        const T mj[3] = {m[3 * cj], m[3 * cj + 1], m[3 * cj + 2]};
+        if (want_ex && inside && Ai + Aj > (T)0) {
+          const T w = p.exq[d] * ((T)2 * Ai * Aj / (Ai + Aj));
+#pragma unroll
+          for (int c = 0; c < 3; ++c) lap[c] += w * (mj[c] - mc[c]);
+        }
+        const bool use = inside && Msj > (T)0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) dm[c] += (T)sg * (use ? mj[c] : mc[c]);
+      }
+      if (want_dmi) dmi_add<T>(p.dmiq[d], dm, hx);
+    }
+  }
+  const T inv_ms = mag ? (T)1 / Msi : (T)0;
+  T h[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) h[c] = lap[c] * inv_ms;
+  T* dst = MODE == PW_RK_FINAL ? m0 : out;
+  if (MODE == PW_EXCHANGE) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dst[base + c] = h[c];
+    return;
+  }
+  if (!(p.terms & MM_TERM_EXCHANGE)) h[0] = h[1] = h[2] = (T)0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) h[c] += hx[c] * inv_ms;
+  if (p.terms & MM_TERM_ANISOTROPY) {
+    const T dot = p.kanq * inv_ms * (mc[0] * p.u[0] + mc[1] * p.u[1] + mc[2] * p.u[2]);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) h[c] += dot * p.u[c];
+  }
+  if (p.terms & MM_TERM_DEMAG) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) h[c] += Hd[base + c];
+  }
+  if (p.terms & MM_TERM_ZEEMAN) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) h[c] += p.hext[c];
+  }
+  if (p.terms & MM_TERM_STT) {
+    h[0] += p.sdamp * (mc[1] * p.sp[2] - mc[2] * p.sp[1]) + p.sfield * p.sp[0];
+    h[1] += p.sdamp * (mc[2] * p.sp[0] - mc[0] * p.sp[2]) + p.sfield * p.sp[1];
+    h[2] += p.sdamp * (mc[0] * p.sp[1] - mc[1] * p.sp[0]) + p.sfield * p.sp[2];
+  }
+  if (MODE == PW_HEFF) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dst[base + c] = h[c];
+    return;
+  }
+  const T t0 = mc[1] * h[2] - mc[2] * h[1];
+  const T t1 = mc[2] * h[0] - mc[0] * h[2];
+  const T t2 = mc[0] * h[1] - mc[1] * h[0];
+  T dd[3] = {mc[1] * t2 - mc[2] * t1, mc[2] * t0 - mc[0] * t2, mc[0] * t1 - mc[1] * t0};
+  T k[3] = {p.pref * (t0 + p.alpha * dd[0]), p.pref * (t1 + p.alpha * dd[1]), p.pref * (t2 + p.alpha * dd[2])};
+  if (!mag) { k[0] = k[1] = k[2] = (T)0; dd[0] = dd[1] = dd[2] = (T)0; }
+  if (MODE == PW_MIN_G) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dst[base + c] = dd[c];
+  } else if (MODE == PW_RHS) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dst[base + c] = k[c];
+  } else if (MODE == PW_RK_STAGE) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      acc[base + c] = p.first ? k[c] : acc[base + c] + p.wk * k[c];
+      dst[base + c] = m0[base + c] + p.a * k[c];
+    }
+  } else {  // PW_RK_FINAL
+    T v[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) v[c] = m0[base + c] + p.a * (acc[base + c] + k[c]);
+    const T nrm = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    const T inv = nrm > (T)0 ? (T)1 / nrm : (T)0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dst[base + c] = v[c] * inv;
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) scale_by_ms_kernel(const T* __restrict__ m, const T* __restrict__ ms,
+                                                          T* __restrict__ out, size_t ncell) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < 3 * ncell; q += stride) out[q] = ms[q / 3] * m[q];
+}
+template <typename T>
+cudaError_t scale_by_ms_launch(const T* m, const T* ms_cells, T* out, size_t ncell, cudaStream_t st) {
+  size_t b = (3 * ncell + 255) / 256;
+  if (b > 148 * 32) b = 148 * 32;
+  scale_by_ms_kernel<T><<<(unsigned)b, 256, 0, st>>>(m, ms_cells, out, ncell);
+  return cudaGetLastError();
+}
+template cudaError_t scale_by_ms_launch<float>(const float*, const float*, float*, size_t, cudaStream_t);
+template cudaError_t scale_by_ms_launch<double>(const double*, const double*, double*, size_t, cudaStream_t);
+
 template <typename T, int MODE, bool DMI>
 static void launch_mode_dmi(const PwParams<T>& p, const T* m, const T* Hd, T* out, T* m0, T* acc,
                             cudaStream_t st) {
@@ -297,6 +423,11 @@ static void launch_mode_dmi(const PwParams<T>& p, const T* m, const T* Hd, T* ou
 template <typename T, int MODE>
 static void launch_mode(const PwParams<T>& p, const T* m, const T* Hd, T* out, T* m0, T* acc,
                         cudaStream_t st) {
+  if (p.ms_cells || p.a_cells) {
+    const size_t total = (size_t)p.nx * p.ny * p.nz;
+    pw_inhom_kernel<T, MODE><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
+    return;
+  }
   if (MODE != PW_EXCHANGE && (p.terms & MM_TERM_DMI)) launch_mode_dmi<T, MODE, true>(p, m, Hd, out, m0, acc, st);
   else launch_mode_dmi<T, MODE, false>(p, m, Hd, out, m0, acc, st);
 }

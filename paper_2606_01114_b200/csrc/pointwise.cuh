@@ -21,6 +21,13 @@ template <typename T> struct PwParams {
   T hext[3];          // A/m
   T dmi[3][3];        // DMI vectors e_k^DMI times 2D/(mu0 Ms) / (2 d_k); row k = 0 if n_k = 1
   T sp[3], sdamp, sfield;  // spin-torque field a_damp (m x p) + a_field p: unit p, amplitudes in A/m
+  // per-cell material parameters (reading Q31); both NULL = uniform (the fields above)
+  const T* ms_cells;  // Ms_i [nx][ny][nz] in A/m, or NULL (ms_ref everywhere)
+  const T* a_cells;   // A_i in J/m, or NULL (a_ref everywhere)
+  T ms_ref, a_ref;
+  T exq[3];           // 2/(mu0 d_d^2)
+  T kanq;             // 2 Ku / mu0
+  T dmiq[3][3];       // DMI vectors times (2D/mu0) / (2 d_k); row k = 0 if n_k = 1
   T pref, alpha;      // -gamma/(1+alpha^2), alpha
   // RK4 bookkeeping
   int first;          // stage 1: acc is written, not accumulated
@@ -32,6 +39,10 @@ template <typename T>
 cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T* Hd, T* out,
                              T* m0, T* acc, cudaStream_t st, unsigned long long* launches,
                              Prof* prof);
+
+// out[i][c] = Ms_i m[i][c]: the magnetisation M = Ms m the demag passes transform when Ms varies per cell.
+template <typename T>
+cudaError_t scale_by_ms_launch(const T* m, const T* ms_cells, T* out, size_t ncell, cudaStream_t st);
 
 // Copies between the mesh [nx][ny][nz][3] and its embedding in the corner of [..][eny][enz][3]
 // (mm_api.cu "Embedding").  embed != 0: mesh -> embedded array (padding cells untouched);

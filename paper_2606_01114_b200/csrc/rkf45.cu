@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(256) rkf_commit_kernel(const RkfState* __restr
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncell; i += stride) {
     const T x = cand[3 * i], y = cand[3 * i + 1], z = cand[3 * i + 2];
     const T nrm = sqrt(x * x + y * y + z * z);
-    m[3 * i] = x / nrm; m[3 * i + 1] = y / nrm; m[3 * i + 2] = z / nrm;
+    if (nrm > (T)0) { m[3 * i] = x / nrm; m[3 * i + 1] = y / nrm; m[3 * i + 2] = z / nrm; }   // a vacuum cell stays zero
   }
 }
 

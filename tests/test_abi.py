@@ -54,8 +54,8 @@ def test_workspace_sizes_match_design(lib):
     """Config 4 fp32.  Generic passes: table 6*129*1024*1024*4 B, spectra 3*129*(512+1024)*512*8 B.
     Fast path (selected automatically): octant table 6*513*513*130*4 B (kz pitch nz+2: 16-byte rows for bulk copies), A1 513*512*384*8 B,
     A2 = kchunk (or 513) planes of 1024*384*8 B.  Field-sized scratch arrays: H_demag, two stage states,
-    RK4 accumulator, two host-call staging buffers, six RKF45 k arrays."""
-    fields = 12 * 512 * 512 * 128 * 3 * 4
+    RK4 accumulator, two host-call staging buffers, six RKF45 k arrays, M = Ms_i m for per-cell Ms."""
+    fields = 13 * 512 * 512 * 128 * 3 * 4
     p, s = C.c_size_t(), C.c_size_t()
     fast, kc = C.c_int(), C.c_int()
     for path, kchunk, table, spectra in (
