@@ -15,7 +15,6 @@ struct FastGeom {
   int Px, Py, Pz;  // 2 n_d
   int Q;           // complex columns per (kx, y) row: 3 nz
   int kchunk;      // kx planes per launch of K2..K4 (0 = all nx + 1 planes at once)
-  int variant;     // kernel variant bits (experiments; MM_FAST_VARIANT): 1 = K3 with rotated loops
 };
 
 // true if the fast kernels cover this mesh (otherwise the generic path of demag_passes.cu runs)

@@ -141,7 +141,6 @@ static void plan_layout(mm_ctx* c) {
   fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;
   fg.Q = 3 * c->dnz;
   fg.kchunk = (c->kchunk > 0 && c->kchunk < c->dnx + 1) ? c->kchunk : 0;
-  { const char* v = getenv("MM_FAST_VARIANT"); fg.variant = v ? atoi(v) : 0; }
   // persistent
   size_t o = 0;
   c->off_table = o;
