@@ -188,8 +188,8 @@ mm_status mm_ctx_kernel_times(mm_ctx *ctx, int reset, double ms_sum[8],
 mm_status mm_ctx_set_tiles(mm_ctx *ctx, int bz, int by, int bk);
 
 /* Demag path selection (experiments and tests).  path: 0 = automatic (the power-of-two x-first
- * kernels of demag_fast.cu where they cover the mesh: nx, ny in {64..1024}, nz in {64, 128, 256
- * (fp32)}; else the same kernels on the enclosing power-of-two mesh when its extra cells cost less
+ * kernels of demag_fast.cu where they cover the mesh: nx, ny in {64..1024}, nz in {64, 128, 256};
+ * else the same kernels on the enclosing power-of-two mesh when its extra cells cost less
  * than the generic passes -- at most 3.0x (fp32) / 2.2x (fp64) the cells, e.g. 512 x 512 x 90 in
  * 512 x 512 x 128: cells outside the mesh carry no magnetisation and add nothing to eq. 4; else
  * the generic z-first passes), 1 = generic passes always, 2 = power-of-two kernels

@@ -683,12 +683,16 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
 // sharing one staged Nhat row), double buffered by bulk copies as in zp_fast_kernel.
 template <typename T> struct ZwCfg {
   static constexpr int nz = 256, Pz = 512, Q = 3 * nz, OZP = nz + 2, PITCH = 33;
-  static constexpr int WARPS = 12;
+  static constexpr int WARPS = sizeof(T) == 4 ? 12 : 6;
   static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
   static constexpr int table_bytes = 6 * OZP * (int)sizeof(T);
   static constexpr int warp_bytes = 2 * pencil_bytes + table_bytes;
   static constexpr int hdr_bytes = (3 * WARPS * 8 + 127) / 128 * 128;
-  static constexpr int smem_bytes = hdr_bytes + WARPS * warp_bytes;
+  // fp64: the 15 inter-stage roots of a lane live in shared memory, [u][t] (as in zp_fast_kernel)
+  static constexpr int TWS = sizeof(T) == 4 ? 1 : 32;
+  static constexpr int tw_bytes = sizeof(T) == 4 ? 0 : 16 * 32 * (int)sizeof(Cx<T>);
+  static constexpr int smem_bytes = hdr_bytes + WARPS * warp_bytes + tw_bytes;
+  static_assert(smem_bytes <= 227 * 1024, "one CTA per SM");
   static_assert(16 * PITCH <= Q, "exchange buffer must fit in the pencil it aliases");
   static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0, "bulk copies need 16 B multiples");
 };
@@ -730,8 +734,8 @@ __device__ __forceinline__ void zw_forward(const Cx<T>* a, Cx<T>* xb, const Cx<T
   xb[t] = e[0];
 #pragma unroll
   for (int v = 0; v < 8; ++v) {
-    if (v) xb[(2 * v) * C::PITCH + t] = cmul(e[v], tw[2 * v]);
-    xb[(2 * v + 1) * C::PITCH + t] = cmul(o[v], tw[2 * v + 1]);
+    if (v) xb[(2 * v) * C::PITCH + t] = cmul(e[v], tw[(2 * v) * C::TWS]);
+    xb[(2 * v + 1) * C::PITCH + t] = cmul(o[v], tw[(2 * v + 1) * C::TWS]);
   }
   __syncwarp();
   const bool h = t >= 16;
@@ -761,8 +765,8 @@ __device__ __forceinline__ void zw_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw,
     const Cx<T> l1 = col[(2 * v + 1) * C::PITCH], h1 = col[(2 * v + 1) * C::PITCH + 16];
     const Cx<T> b0 = mk<T>(fma(sgn, h0.x, l0.x), fma(sgn, h0.y, l0.y));
     const Cx<T> b1 = mk<T>(fma(sgn, h1.x, l1.x), fma(sgn, h1.y, l1.y));
-    e[v] = v ? cmulc(b0, tw[2 * v]) : b0;
-    o[v] = cmulc(b1, tw[2 * v + 1]);
+    e[v] = v ? cmulc(b0, tw[(2 * v) * C::TWS]) : b0;
+    o[v] = cmulc(b1, tw[(2 * v + 1) * C::TWS]);
   }
   __syncwarp();
   Dft<T, 8, true>::run(e);
@@ -818,11 +822,20 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     for (int i = 0; i < 3 * C::WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if constexpr (sizeof(T) == 8) {
+    Cx<T>* tws = reinterpret_cast<Cx<T>*>(smem_raw + C::hdr_bytes + (size_t)C::WARPS * C::warp_bytes);
+    for (int i = threadIdx.x; i < 16 * 32; i += C::WARPS * 32) tws[i] = __ldg(Wz + (i % 32) * (i / 32));
+  }
   __syncthreads();
-  Cx<T> tw[16];
+  Cx<T> twr[sizeof(T) == 4 ? 16 : 1];
+  const Cx<T>* tw = twr;
+  if constexpr (sizeof(T) == 4) {
 #pragma unroll
-  for (int u = 1; u < 16; ++u) tw[u] = __ldg(Wz + t * u);
-  tw[0] = mk<T>(1, 0);
+    for (int u = 1; u < 16; ++u) twr[u] = __ldg(Wz + t * u);
+    twr[0] = mk<T>(1, 0);
+  } else {
+    tw = reinterpret_cast<const Cx<T>*>(smem_raw + C::hdr_bytes + (size_t)C::WARPS * C::warp_bytes) + t;
+  }
 
   const int gw = blockIdx.x * C::WARPS + warp, stride = gridDim.x * C::WARPS;
   const int mine = gw < npair ? (npair - gw + stride - 1) / stride : 0;  // pairs of this warp
@@ -910,7 +923,8 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
 
 bool fast_supported(int nx, int ny, int nz, size_t real_bytes) {
   auto okxy = [](int n) { return n == 64 || n == 128 || n == 256 || n == 512 || n == 1024; };
-  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128 || (nz == 256 && real_bytes == 4));
+  (void)real_bytes;
+  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128 || nz == 256);
 }
 
 template <typename K> static cudaError_t opt_in_smem(K kernel, int bytes) {
@@ -1035,8 +1049,7 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
     if (e != cudaSuccess) return e;
     prof->mark(2, st);
     if (g.nz == 256) {
-      if constexpr (sizeof(T) == 4) e = launch_zw<T>(g, b, k0, nk, st);
-      else e = cudaErrorInvalidValue;
+      e = launch_zw<T>(g, b, k0, nk, st);
     } else {
       e = g.nz == 128 ? launch_zp<T, 16>(g, b, k0, nk, st) : launch_zp<T, 8>(g, b, k0, nk, st);
     }

@@ -68,35 +68,35 @@ def test_fast_vs_direct_sum_sampled(oracle):
     assert l2 <= TOL["f64"], (l2, mx)
 
 
+@pytest.mark.parametrize("dt", ["f32", "f64"])
 @pytest.mark.parametrize("n", [(64, 64, 256), (128, 64, 256)])
-def test_fast_wide_pencil_nz256_fp32(oracle, n):
-    """nz = 256 (Pz = 512): the one-pencil-per-warp z kernel with the split second stage, fp32;
+def test_fast_wide_pencil_nz256(oracle, n, dt):
+    """nz = 256 (Pz = 512): the one-pencil-per-warp z kernel with the split second stage, fp32 and fp64;
     several planes and mirror pairs per warp, ragged last chunk."""
     cfg = cfg_for(n)
-    m, m64 = round_input(w.random_unit_vectors(606, n), "f32")
+    m, m64 = round_input(w.random_unit_vectors(606, n), dt)
     P = make_problem(oracle, cfg, terms=1)
     ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
     md = to_dev(m)
     results = []
     for kchunk in (0, 5):
-        ctx = make_ctx(cfg, "f32", terms=1, path=2, kchunk=kchunk)
+        ctx = make_ctx(cfg, dt, terms=1, path=2, kchunk=kchunk)
         assert ctx.path == (True, kchunk)
         got = ctx.demag_field(md).cpu().numpy()
         l2, mx = w.field_errors(got, ref)
-        assert l2 <= TOL["f32"] and mx <= 10 * TOL["f32"], (kchunk, l2, mx)
+        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (kchunk, l2, mx)
         assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
         results.append(got)
         ctx.close()
     assert np.array_equal(results[0], results[1])
 
 
-def test_fast_path_rejects_fp64_nz256():
-    """fp64 with nz = 256 is served by the generic passes; requiring the power-of-two kernels fails
-    loudly."""
+def test_fast_path_rejects_meshes_it_does_not_cover():
+    """nz = 32 is served by the generic passes; requiring the power-of-two kernels fails loudly."""
     from paper_2606_01114_b200 import MMError
     with pytest.raises(MMError) as ei:
-        make_ctx(cfg_for((64, 64, 256)), "f64", terms=1, path=2)
+        make_ctx(cfg_for((64, 64, 32)), "f64", terms=1, path=2)
     assert ei.value.status == 2
-    ctx = make_ctx(cfg_for((64, 64, 256)), "f64", terms=1, path=0)
-    assert ctx.path[0] is False and ctx.path_name == "generic"
+    ctx = make_ctx(cfg_for((64, 64, 32)), "f64", terms=1, path=0)
+    assert ctx.path[0] is False and ctx.path_name in ("generic", "embedded")
     ctx.close()
