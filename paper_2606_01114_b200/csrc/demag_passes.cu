@@ -216,16 +216,23 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
 
 // Threads per CTA: a whole number of threads per column (the in-place stages give thread
 // (col, tt) the butterflies tt, tt + NT, ... of its column).
-static int pick_threads(int B, int rows) {
+// The kernels hold up to 128 registers per thread, so 512 threads fill an SM's register file: when
+// the tile leaves room for several CTAs per SM the CTA shrinks accordingly (two or three CTAs whose
+// load, transform and store phases overlap instead of one that runs them back to back).
+static int pick_threads(int B, int rows, size_t smem_bytes) {
+  int ctas = (int)((size_t)(227 * 1024) / (smem_bytes + 1024));
+  if (ctas < 1) ctas = 1;
+  if (ctas > 4) ctas = 4;
+  const int cap = 512 / ctas;
   int want = B * (rows / 8 > 0 ? rows / 8 : 1);
   if ((B & (B - 1)) == 0) {
     int t = 64;
-    while (t < want && t < 512) t *= 2;
+    while (t < want && t * 2 <= cap) t *= 2;
     if (t < B) t = B;
     return t;
   }
   int nt = want / B;
-  if (nt > 512 / B) nt = 512 / B;
+  if (nt > cap / B) nt = cap / B;
   return B * (nt > 0 ? nt : 1);
 }
 
@@ -240,7 +247,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     if ((err = set_smem(zf_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.Bz, (g.ny + 1) / 2);
     prof->mark(0, st);
-    zf_kernel<T><<<grid, pick_threads(g.Bz, 3 * g.Pz), sb, st>>>(g, m, b.A1, b.Wz, b.posz);
+    zf_kernel<T><<<grid, pick_threads(g.Bz, 3 * g.Pz, sb), sb, st>>>(g, m, b.A1, b.Wz, b.posz);
     ++*launches;
   }
   if (g.Py > 1) {
@@ -248,7 +255,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     if ((err = set_smem(yf_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.By, g.Kz, 3);
     prof->mark(1, st);
-    yf_kernel<T><<<grid, pick_threads(g.By, g.Py), sb, st>>>(g, b.A1, b.A2, b.Wy);
+    yf_kernel<T><<<grid, pick_threads(g.By, g.Py, sb), sb, st>>>(g, b.A1, b.A2, b.Wy);
     ++*launches;
   }
   {
@@ -256,7 +263,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     if ((err = set_smem(xp_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.Py / g.Bk, g.Kz);
     prof->mark(2, st);
-    xp_kernel<T><<<grid, pick_threads(g.Bk, 3 * g.Px), sb, st>>>(g, A2, b.table, b.Wx);
+    xp_kernel<T><<<grid, pick_threads(g.Bk, 3 * g.Px, sb), sb, st>>>(g, A2, b.table, b.Wx);
     ++*launches;
   }
   if (g.Py > 1) {
@@ -264,7 +271,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     if ((err = set_smem(yi_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.By, g.Kz, 3);
     prof->mark(3, st);
-    yi_kernel<T><<<grid, pick_threads(g.By, g.Py), sb, st>>>(g, b.A2, b.A1, b.Wy);
+    yi_kernel<T><<<grid, pick_threads(g.By, g.Py, sb), sb, st>>>(g, b.A2, b.A1, b.Wy);
     ++*launches;
   }
   {
@@ -272,7 +279,7 @@ cudaError_t demag_field_launch(const DemagGeom& g, const DemagBufs<T>& b, const 
     if ((err = set_smem(zi_kernel<T>, sb)) != cudaSuccess) return err;
     dim3 grid(g.nx / g.Bz, (g.ny + 1) / 2);
     prof->mark(4, st);
-    zi_kernel<T><<<grid, pick_threads(g.Bz, 3 * g.Pz), sb, st>>>(g, b.A1, H, b.Wz, b.posz, scale);
+    zi_kernel<T><<<grid, pick_threads(g.Bz, 3 * g.Pz, sb), sb, st>>>(g, b.A1, H, b.Wz, b.posz, scale);
     ++*launches;
   }
   prof->mark(-1, st);
