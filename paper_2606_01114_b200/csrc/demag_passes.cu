@@ -36,6 +36,7 @@ __global__ void __launch_bounds__(512) zf_kernel(DemagGeom g, const T* __restric
   const bool has1 = (y0 + 1) < g.ny;
   const int nz = g.nz, Pz = g.Pz, Kz = g.Kz;
   const int line = nz * 3;
+#pragma unroll 4
   for (int e = tid; e < B * line; e += NTHR) {
     const int xl = e / line, rem = e - xl * line;
     const int z = rem / 3, c = rem - z * 3;
@@ -46,6 +47,7 @@ __global__ void __launch_bounds__(512) zf_kernel(DemagGeom g, const T* __restric
   }
   __syncthreads();
   run_stages_fwd<T>(sm, B, tid % B, tid / B, NTHR / B, 3 * Pz, g.pz, Wz);
+#pragma unroll 4
   for (int e = tid; e < 3 * Kz * B; e += NTHR) {
     const int xl = e % B, kz = (e / B) % Kz, c = e / (B * Kz);
     Cx<T> a, b;
@@ -79,6 +81,7 @@ __global__ void __launch_bounds__(512) yf_kernel(DemagGeom g, const Cx<T>* __res
   const int ny = g.ny, Py = g.Py;
   const Cx<T>* in = A1 + ((size_t)c * g.Kz + kz) * ny * g.nx + x0;
   Cx<T>* out = A2 + ((size_t)c * g.Kz + kz) * Py * g.nx + x0;
+#pragma unroll 4
   for (int e = tid; e < ny * B; e += NTHR) {
     const int xl = e % B, y = e / B;
     const Cx<T> v = in[(size_t)y * g.nx + xl];
@@ -87,6 +90,7 @@ __global__ void __launch_bounds__(512) yf_kernel(DemagGeom g, const Cx<T>* __res
   }
   __syncthreads();
   run_stages_fwd<T>(sm, B, tid % B, tid / B, NTHR / B, Py, g.py, Wy);
+#pragma unroll 4
   for (int e = tid; e < Py * B; e += NTHR) {
     const int xl = e % B, r = e / B;
     out[(size_t)r * g.nx + xl] = sm[(size_t)r * B + xl];
@@ -108,6 +112,7 @@ __global__ void __launch_bounds__(512) xp_kernel(DemagGeom g, Cx<T>* __restrict_
   const int blk = blockIdx.x, kz = blockIdx.y;
   const int nx = g.nx, Px = g.Px, Py = g.Py, Kz = g.Kz;
   const int ky0 = blk * B;
+#pragma unroll(sizeof(T) == 8 ? 8 : 4)
   for (int e = tid; e < 3 * B * nx; e += NTHR) {
     const int x = e % nx, p = (e / nx) % B, c = e / (nx * B);
     const Cx<T> v = A[(((size_t)c * Kz + kz) * Py + ky0 + p) * nx + x];
@@ -117,6 +122,7 @@ __global__ void __launch_bounds__(512) xp_kernel(DemagGeom g, Cx<T>* __restrict_
   __syncthreads();
   run_stages_fwd<T>(sm, B, tid % B, tid / B, NTHR / B, 3 * Px, g.px, Wx);
   const T* tb = table + ((size_t)kz * (Py / B) + blk) * Px * 6 * B;
+#pragma unroll(sizeof(T) == 8 ? 8 : 4)
   for (int e = tid; e < Px * B; e += NTHR) {
     const int p = e % B, r = e / B;
     const T* t6 = tb + (size_t)r * 6 * B + p;
@@ -132,6 +138,7 @@ __global__ void __launch_bounds__(512) xp_kernel(DemagGeom g, Cx<T>* __restrict_
   }
   __syncthreads();
   run_stages_inv<T>(sm, B, tid % B, tid / B, NTHR / B, 3 * Px, g.px, Wx);
+#pragma unroll(sizeof(T) == 8 ? 8 : 4)
   for (int e = tid; e < 3 * B * nx; e += NTHR) {
     const int x = e % nx, p = (e / nx) % B, c = e / (nx * B);
     Cx<T> v = sm[(size_t)(c * Px + x) * B + p];
@@ -152,12 +159,14 @@ __global__ void __launch_bounds__(512) yi_kernel(DemagGeom g, const Cx<T>* __res
   const int ny = g.ny, Py = g.Py;
   const Cx<T>* in = A2 + ((size_t)c * g.Kz + kz) * Py * g.nx + x0;
   Cx<T>* out = A1 + ((size_t)c * g.Kz + kz) * ny * g.nx + x0;
+#pragma unroll 4
   for (int e = tid; e < Py * B; e += NTHR) {
     const int xl = e % B, r = e / B;
     sm[(size_t)r * B + xl] = in[(size_t)r * g.nx + xl];
   }
   __syncthreads();
   run_stages_inv<T>(sm, B, tid % B, tid / B, NTHR / B, Py, g.py, Wy);
+#pragma unroll 4
   for (int e = tid; e < ny * B; e += NTHR) {
     const int xl = e % B, y = e / B;
     const Cx<T> v =
