@@ -343,7 +343,9 @@ xi_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>
   const size_t pair = (size_t)blockIdx.x * B + lane;
   const Cx<T>* in = A1 + 2 * pair;
   const size_t rowc = 2 * npairs;
-#pragma unroll 1
+  // four independent row loads in flight per thread (one at a time left this pass latency-bound: 0.26 of the
+  // roofline at L = 1024)
+#pragma unroll 4
   for (int k = slot; k <= L; k += NS) {
     Cx<T> a, b;
     Pair2<T>::ld(in + (size_t)k * rowc, a, b);
