@@ -271,7 +271,7 @@ yi_fast_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>
   const size_t col = (size_t)blockIdx.x * B + lane;
   const Cx<T>* in = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
   Cx<T>* out = A1 + (size_t)blockIdx.y * L * Q + col;
-#pragma unroll 1
+#pragma unroll 2
   for (int i = slot; i < 2 * R1 * R2; i += NS) {
     Cx<T> v[R3];
 #pragma unroll
@@ -322,7 +322,7 @@ xf_fast_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>
   __syncthreads();
   Cx<T>* out = A1 + 2 * pair;
   const size_t rowc = 2 * npairs;
-#pragma unroll 1
+#pragma unroll 4
   for (int k = slot; k <= L; k += NS) {
     const int p1 = pos[k], p2 = pos[(2 * L - k) & (2 * L - 1)];
     const Cx<T> z1 = sm[p1 * B + lane], z2 = cconj(sm[p2 * B + lane]);
