@@ -284,12 +284,15 @@ def run_ours(args, cfg):
                              "achieved_GBps": kbytes[k] / ms / 1e6, "frac": kbytes[k] / ms / 1e6 / peak}
     dom = max(per_kernel, key=lambda k: per_kernel[k]["ms"])
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
+    # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu --set full
+    # capture (profiles/dominant_kernel_traffic.csv; the command is in profiles/r01_v3_fast_path.md)
+    tp = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.csv")
     if os.path.exists(tp):
         try:
-            tj = json.load(open(tp))
-            if tj.get("kernel") == dom and tj.get("dtype") == args.dtype:
-                traffic = tj.get("dram_bytes_per_launch")
+            import csv
+            for row in csv.DictReader(open(tp)):
+                if row["kernel"] == dom and row["dtype"] == args.dtype and row["workload"] == "cfg4" and not args.mesh:
+                    traffic = int(row["dram_bytes_per_launch"])
         except Exception:
             pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": per_kernel[dom]["achieved_GBps"],
