@@ -135,7 +135,7 @@ static void plan_layout(mm_ctx* c) {
   ig.ozp = (ig.oz + 1) / 2 * 2;
   ig.Bk = g.Bk;
   c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->dnx, c->dny, c->dnz, c->es);
-  // measured (profiles/r01_v4_mixed_meshes.md): the mixed-radix x-first kernels only tie with the generic
+  // measured (profiles/r01_v4_paper_meshes.md): the mixed-radix x-first kernels only tie with the generic
   // z-first passes, so they are opt-in (path 3) until their stages move into registers
   c->mixed = c->path_pref == 3 && mixed_supported(c->dnx, c->dny, c->dnz, c->es);
   FastGeom& fg = c->fgeom;
