@@ -573,7 +573,7 @@ typedef struct {
  *   demag     H(i) = - sum_j N(i - j) Ms_j m_j                                   (M = Ms m, eq. 4)
  *   exchange  H(i) = 2/(mu0 Ms_i) sum_{d, +-} A_ij (m_j - m_i) / D_d^2,  A_ij = 2 A_i A_j / (A_i + A_j)
  *             (harmonic mean: the flux A dm/dx is continuous across the interface; 0 if either is 0),
- *             a neighbour outside the mesh contributes nothing (Q5)
+ *             a neighbour outside the mesh or in vacuum (Ms_j = 0) contributes nothing (Q5)
  *   anisotropy, DMI: the homogeneous formulas with Ms_i; for DMI a neighbour with Ms_j = 0 counts as
  *             outside the mesh (replaced by the cell itself, Q28)
  *   a cell with Ms_i = 0 is vacuum: the terms with a 1/Ms_i prefactor vanish there and dm/dt = 0.
@@ -615,7 +615,9 @@ static int orc_heff_cells(const orc_problem *p, const double *m, double *H) {
               const int inside = j[d] >= 0 && j[d] < nn[d];
               const size_t cj = inside ? ((size_t)j[0] * ny + j[1]) * nz + j[2] : ci;
               const double Msj = ms_at(p, cj), Aj = a_at(p, cj);
-              if ((p->terms & ORC_TERM_EXCHANGE) && inside && Ai + Aj > 0.0) {
+              /* a vacuum neighbour (Ms_j = 0) is outside the magnet: no exchange partner, whatever
+               * A_j and the frozen m_j stored there are (reading Q31: interface = mesh boundary) */
+              if ((p->terms & ORC_TERM_EXCHANGE) && inside && Msj > 0.0 && Ai + Aj > 0.0) {
                 const double Aij = 2.0 * Ai * Aj / (Ai + Aj);
                 for (int c = 0; c < 3; ++c)
                   acc[c] += 2.0 / (ORC_MU0 * Msi) * Aij * (m[3 * cj + c] - m[i0 + c]) / (h[d] * h[d]);

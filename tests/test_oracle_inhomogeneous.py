@@ -70,6 +70,14 @@ def test_vacuum_cells_do_not_source_the_demag_field_and_do_not_move(oracle):
     Hx = oracle.Problem(n=n, d=d, Ms=Ms0, Aex=1.3e-11, terms=2, Ms_cells=Ms, A_cells=A).heff(m)
     ref_x = oracle.exchange(d, Ms0, 1.3e-11, m[:4])
     assert np.max(np.abs(Hx[:4] - ref_x)) <= 1e-13 * np.max(np.abs(ref_x))
+    # the same holds with UNIFORM A (A_cells = None) and arbitrary non-zero vectors stored in the vacuum
+    # cells: a neighbour with Ms_j = 0 is no exchange partner (reading Q31), so the magnet's exchange
+    # field is that of the 4-cell-long mesh and does not depend on what the vacuum cells hold
+    mv = m.copy()
+    mv[4:] = w.random_unit_vectors(43, n)[4:]
+    Hu = oracle.Problem(n=n, d=d, Ms=Ms0, Aex=1.3e-11, terms=2, Ms_cells=Ms).heff(mv)
+    assert np.max(np.abs(Hu[:4] - ref_x)) <= 1e-13 * np.max(np.abs(ref_x))
+    assert np.all(Hu[4:] == 0.0)
 
 
 def test_demag_is_linear_in_Ms_cells_and_dmi_skips_vacuum_neighbours(oracle):
