@@ -18,8 +18,11 @@
  *    library never allocates or frees device memory (PyTorch does, in the binding).
  *    The context owns only small host-side plan data.
  *  - Execution: field/step calls enqueue kernels on the context's stream and return without
- *    synchronising (CUDA-graph capturable, deterministic: no atomics).  mm_demag_init and
- *    the *_host calls synchronise the stream before returning.
+ *    synchronising (CUDA-graph capturable).  Results are deterministic, bit-identical from run to
+ *    run: sums are reduced in a fixed order; the only atomics are atomicMax on the bit pattern of a
+ *    non-negative real (the RKF45 error and the minimiser's largest change), whose result does not
+ *    depend on the order of arrival.  mm_demag_init, the *_state and the *_host calls synchronise
+ *    the stream before returning.
  *  - Errors: every call returns mm_status; nothing is thrown across the ABI.  After a
  *    non-OK status mm_last_error(ctx) holds a one-line explanation.
  *  - Sizes: every n_d must be of the form 2^a 3^b 5^c 7^d (1 included), nx, ny <= 1024, nz <= 512
@@ -62,8 +65,13 @@ mm_status mm_ctx_destroy(mm_ctx *ctx);
 mm_status mm_ctx_set_stream(mm_ctx *ctx, void *cuda_stream);
 
 /* Bytes the caller must provide.  persistent: Fourier-space demag tensor, twiddle and index
- * tables (written by mm_demag_init, read afterwards).  scratch: padded spectra, H_demag,
- * RK4 stage buffers, host-call staging; contents are undefined between calls. */
+ * tables (written by mm_demag_init, read afterwards) and the RKF45 / minimiser controller records.
+ * scratch: padded spectra, H_demag, stage buffers, host-call staging.  Field and step calls
+ * leave nothing in scratch that a later call reads, with ONE exception: between mm_minimize_init
+ * and the last mm_minimize_step of a minimisation the previous iterate and gradient (m_{n-1},
+ * g_{n-1}) live there, so scratch must not be overwritten by anyone else during a minimisation.
+ * Two contexts may share one scratch buffer if their calls do not overlap in time and no
+ * minimisation is in flight; persistent workspaces are never shared. */
 mm_status mm_ctx_workspace_bytes(const mm_ctx *ctx, size_t *persistent, size_t *scratch);
 mm_status mm_ctx_set_workspace(mm_ctx *ctx, void *persistent, size_t pbytes, void *scratch,
                                size_t sbytes);
@@ -168,6 +176,11 @@ mm_status mm_heff_host(mm_ctx *ctx, const void *m_host, void *H_host);
 mm_status mm_llg_rhs_host(mm_ctx *ctx, const void *m_host, void *dmdt_host);
 mm_status mm_rk_step_host(mm_ctx *ctx, void *m_inout_host, double dt);
 
+/* ------------------------------------------------------------------------------------------
+ * Diagnostics and experiments.  Not part of the method's boundary: bench.py, the
+ * tests and profiling runs use them; a simulation never needs to.
+ * ------------------------------------------------------------------------------------------ */
+
 /* Number of kernel launches the library has enqueued on this context since creation
  * (bench.py reports the difference over its timed region as gpu_launches). */
 mm_status mm_ctx_launch_count(const mm_ctx *ctx, unsigned long long *count);
@@ -176,32 +189,33 @@ mm_status mm_ctx_launch_count(const mm_ctx *ctx, unsigned long long *count);
  * CUDA events on the context's stream around each kernel it enqueues (a few microseconds of
  * host time per launch; at most 8192 marks are kept between two reads).
  * mm_ctx_kernel_times synchronises the stream and returns, per kernel kind, the summed
- * duration in milliseconds and the number of launches since the last reset:
- *   0 S1 forward z   1 S2 forward y   2 S3 fused x pass   3 S4 inverse y   4 S5 inverse z
- *   5 S6/S7 fused pointwise pass      6, 7 unused */
+ * duration in milliseconds and the number of launches since the last reset.  Kinds, in the order
+ * the demag passes run (the transform axis depends on the path, see
+ * mm_ctx_kernel_name):
+ *   0 S1 first forward axis (r2c)   1 S2 forward y   2 S3 last axis fused with the tensor multiply
+ *   3 S4 inverse y   4 S5 first axis inverse (c2r)   5 S6/S7 fused pointwise pass   6, 7 unused */
 mm_status mm_ctx_set_profiling(mm_ctx *ctx, int enable);
 mm_status mm_ctx_kernel_times(mm_ctx *ctx, int reset, double ms_sum[8],
                               unsigned long long count[8]);
+/* Name of the __global__ function this context launches for kernel kind `kind` (e.g.
+ * "zp_fast_kernel<float,16>"), as it appears in an ncu launch list; "" for unused kinds.
+ * The returned string is static. */
+const char *mm_ctx_kernel_name(const mm_ctx *ctx, int kind);
 
-/* Tuning knobs for experiments (tile widths of the FFT passes); 0 keeps the default.
- * Applies to the generic passes.  Must be called before mm_ctx_set_workspace. */
+/* Tile widths of the generic z-first passes; 0 keeps the default.  Must be called before
+ * mm_ctx_set_workspace. */
 mm_status mm_ctx_set_tiles(mm_ctx *ctx, int bz, int by, int bk);
 
-/* Demag path selection (experiments and tests).  path: 0 = automatic (the power-of-two x-first
- * kernels of demag_fast.cu where they cover the mesh: nx, ny in {64..1024}, nz in {64, 128, 256};
- * else the same kernels on the enclosing power-of-two mesh when its extra cells cost less
- * than the generic passes -- at most 3.0x (fp32) / 2.2x (fp64) the cells, e.g. 512 x 512 x 90 in
- * 512 x 512 x 128: cells outside the mesh carry no magnetisation and add nothing to eq. 4; else
- * the generic z-first passes), 1 = generic passes always, 2 = power-of-two kernels
- * required, 3 = the mixed-radix x-first kernels of demag_mixed.cu (every n_d >= 2 and ny * 3 nz
- * even; a quarter of the generic passes' table memory, same speed today)
- * (MM_ERR_UNSUPPORTED_SIZE if the required kernels do not cover the mesh).  mm_ctx_path reports
- * 0 generic, 1 power-of-two, 2 mixed-radix, 3 power-of-two on the enclosing mesh.  kchunk: number of kx planes the
- * y/z/y passes of the fast path process per launch group through one reused (L2-sized)
- * buffer; 0 = all planes at once.  Changes the workspace sizes: call before
- * mm_ctx_workspace_bytes / mm_ctx_set_workspace.  mm_ctx_path reports what is selected. */
-mm_status mm_ctx_set_path(mm_ctx *ctx, int path, int kchunk);
-mm_status mm_ctx_path(const mm_ctx *ctx, int *fast, int *kchunk);
+/* Demag path selection.  path: 0 = automatic (the x-first register-stage
+ * kernels where they cover the mesh, else the same kernels on an enclosing mesh when its extra
+ * cells cost less than the generic passes, else the generic z-first passes), 1 = generic passes
+ * always, 2 = x-first register-stage kernels required, 3 = the shared-memory-stage mixed-radix
+ * x-first kernels of demag_mixed.cu (MM_ERR_UNSUPPORTED_SIZE if the required kernels do not
+ * cover the mesh).  Changes the workspace sizes: call before mm_ctx_workspace_bytes /
+ * mm_ctx_set_workspace.  mm_ctx_path reports what runs: 0 generic, 1 x-first register-stage
+ * kernels, 2 mixed-radix shared-memory stages, 3 x-first kernels on the enclosing mesh. */
+mm_status mm_ctx_set_path(mm_ctx *ctx, int path);
+mm_status mm_ctx_path(const mm_ctx *ctx, int *path);
 
 /* Last error text of this context (or of the last failed mm_ctx_create if ctx is NULL).
  * Not thread-safe. */

@@ -78,8 +78,8 @@ def load_library():
         "mm_rk_step_host": [vp, vp, dbl],
         "mm_ctx_launch_count": [vp, C.POINTER(C.c_ulonglong)],
         "mm_ctx_set_tiles": [vp, i32, i32, i32],
-        "mm_ctx_set_path": [vp, i32, i32],
-        "mm_ctx_path": [vp, C.POINTER(i32), C.POINTER(i32)],
+        "mm_ctx_set_path": [vp, i32],
+        "mm_ctx_path": [vp, C.POINTER(i32)],
         "mm_ctx_set_profiling": [vp, i32],
         "mm_ctx_kernel_times": [vp, i32, C.POINTER(dbl), C.POINTER(C.c_ulonglong)],
     }
@@ -89,6 +89,8 @@ def load_library():
         fn.restype = i32
     lib.mm_last_error.argtypes = [vp]
     lib.mm_last_error.restype = C.c_char_p
+    lib.mm_ctx_kernel_name.argtypes = [vp, i32]
+    lib.mm_ctx_kernel_name.restype = C.c_char_p
     _lib = lib
     return lib
 
@@ -105,8 +107,7 @@ class Context:
     """One mesh on one GPU (mm_ctx).  Mirrors Mesh(n, dx) + State.material + the field-term
     list of the paper's scripts."""
 
-    def __init__(self, n, d, dtype=torch.float32, device="cuda:0", tiles=None, allocate=True,
-                 path=0, kchunk=0):
+    def __init__(self, n, d, dtype=torch.float32, device="cuda:0", tiles=None, allocate=True, path=0):
         self.lib = load_library()
         self.n = tuple(int(v) for v in n)
         self.d = tuple(float(v) for v in d)
@@ -118,8 +119,8 @@ class Context:
             raise MMError(st, self.lib.mm_last_error(None).decode())
         if tiles is not None:
             self._call("mm_ctx_set_tiles", *[int(t) for t in tiles])
-        if path or kchunk:
-            self._call("mm_ctx_set_path", int(path), int(kchunk))
+        if path:
+            self._call("mm_ctx_set_path", int(path))
         self._ws = None
         if allocate:
             self.allocate()
@@ -191,20 +192,15 @@ class Context:
     def demag_init(self):
         self._call("mm_demag_init")
 
-    @property
-    def path(self):
-        """(fast, kchunk): whether the power-of-two x-first kernels are selected, planes per chunk."""
-        f, k = C.c_int(), C.c_int()
-        self._call("mm_ctx_path", C.byref(f), C.byref(k))
-        return f.value == 1, k.value
+    PATH_NAMES = ("generic", "fast", "mixed", "embedded")
 
     @property
     def path_name(self):
-        """'generic' (z-first passes), 'fast' (power-of-two x-first), 'mixed' (mixed-radix x-first) or
-        'embedded' (power-of-two x-first kernels on the enclosing power-of-two mesh)."""
-        f, k = C.c_int(), C.c_int()
-        self._call("mm_ctx_path", C.byref(f), C.byref(k))
-        return ("generic", "fast", "mixed", "embedded")[f.value]
+        """'generic' (z-first passes), 'fast' (x-first register-stage kernels), 'mixed' (mixed-radix x-first,
+        shared-memory stages) or 'embedded' (x-first kernels on an enclosing mesh)."""
+        f = C.c_int()
+        self._call("mm_ctx_path", C.byref(f))
+        return self.PATH_NAMES[f.value]
 
     @property
     def launch_count(self):
@@ -215,14 +211,18 @@ class Context:
     def set_profiling(self, on=True):
         self._call("mm_ctx_set_profiling", 1 if on else 0)
 
-    KERNEL_NAMES = ("S1_zf", "S2_yf", "S3_xp", "S4_yi", "S5_zi", "S6_pointwise")
+    KERNEL_KINDS = ("S1", "S2", "S3", "S4", "S5", "S6")   # mm_ctx_kernel_times kinds 0..5
+
+    def kernel_name(self, kind):
+        """__global__ function launched for kernel kind 0..5 (as in an ncu launch list)."""
+        return self.lib.mm_ctx_kernel_name(self._h, int(kind)).decode()
 
     def kernel_times(self, reset=True):
-        """{kernel: (total ms, launches)} since the last reset; synchronises."""
+        """{kind: (total ms, launches)} since the last reset, kinds 'S1'..'S6'; synchronises."""
         ms = (C.c_double * 8)()
         cnt = (C.c_ulonglong * 8)()
         self._call("mm_ctx_kernel_times", 1 if reset else 0, ms, cnt)
-        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_NAMES)}
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_KINDS)}
 
     # -- device calls
     def _check(self, t):

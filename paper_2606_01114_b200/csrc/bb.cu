@@ -91,7 +91,10 @@ __global__ void __launch_bounds__(256) bb_update_kernel(BbState* __restrict__ s,
     const T n0 = (((T)1 - a) * m0 - tau * g0) * inv;
     const T n1 = (((T)1 - a) * m1 - tau * g1) * inv;
     const T n2 = (((T)1 - a) * m2 - tau * g2) * inv;
-    dmax = fmax(dmax, fmax(fabs(n0 - m0), fmax(fabs(n1 - m1), fabs(n2 - m2))));
+    // a non-finite change (blown-up state) counts as +inf: never reported as converged
+    const T d0 = fabs(n0 - m0), d1 = fabs(n1 - m1), d2 = fabs(n2 - m2);
+    const T dd = (d0 == d0 && d1 == d1 && d2 == d2) ? fmax(d0, fmax(d1, d2)) : (T)INFINITY;
+    dmax = fmax(dmax, dd);
     mp[3 * i] = m0; mp[3 * i + 1] = m1; mp[3 * i + 2] = m2;
     gp[3 * i] = g0; gp[3 * i + 1] = g1; gp[3 * i + 2] = g2;
     m[3 * i] = n0; m[3 * i + 1] = n1; m[3 * i + 2] = n2;

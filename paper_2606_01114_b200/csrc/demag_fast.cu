@@ -25,6 +25,8 @@
 
 #include <cuda/std/cstdint>
 
+#include "demag_ztile.cuh"
+
 #include "fft_core.cuh"
 
 namespace mm {
@@ -33,38 +35,23 @@ constexpr int kStrideThreads = 256;
 
 constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v / 2); }
 
-// Radix plan of the length-L sub-transforms of the strided passes: L = R1 R2 R3.
+// Radix plan of the length-L sub-transforms of the three-stage strided passes: L = R1 R2 R3.  Only L = 1024
+// runs them: every L <= 512 runs the two-stage kernels of demag_fast2.cu (fast_two_stage).
 template <int L> struct FastPlan;
-template <> struct FastPlan<64> { static constexpr int R1 = 4, R2 = 4, R3 = 4; };
-template <> struct FastPlan<128> { static constexpr int R1 = 8, R2 = 4, R3 = 4; };
-template <> struct FastPlan<256> { static constexpr int R1 = 8, R2 = 8, R3 = 4; };
-template <> struct FastPlan<512> { static constexpr int R1 = 8, R2 = 8, R3 = 8; };
 template <> struct FastPlan<1024> { static constexpr int R1 = 16, R2 = 8, R3 = 8; };
 
-static void plan_of(int L, int& R1, int& R2, int& R3) {
-  switch (L) {
-    case 64: R1 = 4; R2 = 4; R3 = 4; break;
-    case 128: R1 = 8; R2 = 4; R3 = 4; break;
-    case 256: R1 = 8; R2 = 8; R3 = 4; break;
-    case 512: R1 = 8; R2 = 8; R3 = 8; break;
-    default: R1 = 16; R2 = 8; R3 = 8; break;
-  }
-}
-
-// k = h + 2 (u1 + R1 (u2 + R2 u3))  ->  row h L + u1 R2 R3 + u2 R3 + u3
+// k = h + 2 (u1 + R1 (u2 + R2 u3))  ->  row h L + u1 R2 R3 + u2 R3 + u3   (L = 1024)
 int fast_pos_logical(int L, int k) {
-  int R1, R2, R3;
-  plan_of(L, R1, R2, R3);
+  using P = FastPlan<1024>;
   const int h = k & 1;
   int kk = k >> 1;
-  const int u1 = kk % R1; kk /= R1;
-  const int u2 = kk % R2; kk /= R2;
-  return h * L + u1 * R2 * R3 + u2 * R3 + kk;
+  const int u1 = kk % P::R1; kk /= P::R1;
+  const int u2 = kk % P::R2; kk /= P::R2;
+  return h * L + u1 * P::R2 * P::R3 + u2 * P::R3 + kk;
 }
 int fast_swizzle(int L, int row) {
-  int R1, R2, R3;
-  plan_of(L, R1, R2, R3);
-  return row ^ ((row >> ilog2c(R3)) & 1);
+  (void)L;
+  return row ^ ((row >> ilog2c(FastPlan<1024>::R3)) & 1);
 }
 
 template <typename T, int L> struct Tile {
@@ -923,10 +910,12 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
 
 // ---------------------------------------------------------------- host side
 
-bool fast_supported(int nx, int ny, int nz, size_t real_bytes) {
-  auto okxy = [](int n) { return n == 64 || n == 128 || n == 256 || n == 512 || n == 1024; };
-  (void)real_bytes;
-  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128 || nz == 256);
+// x, y: a two-stage plan (plan2.cuh) or the three-stage L = 1024 kernels; z: the warp-per-pencil kernels
+// (64, 128, 256) or the tile pass of demag_ztile.cu.  K1 / K5 move the real arrays as complex pairs.
+bool fast_supported(int nx, int ny, int nz) {
+  auto okxy = [](int n) { return fast_two_stage(n) || n == 1024; };
+  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128 || nz == 256 || ztile_supported(nz)) &&
+         ((size_t)ny * 3 * nz) % 2 == 0;
 }
 
 template <typename K> static cudaError_t opt_in_smem(K kernel, int bytes) {
@@ -1012,71 +1001,30 @@ static cudaError_t launch_zw(const FastGeom& g, const FastBufs<T>& b, int k0, in
   return cudaSuccess;
 }
 
-#define MM_DISPATCH_L(L, CALL)                       \
-  switch (L) {                                       \
-    case 64: e = CALL(64); break;                    \
-    case 128: e = CALL(128); break;                  \
-    case 256: e = CALL(256); break;                  \
-    case 512: e = CALL(512); break;                  \
-    case 1024: e = CALL(1024); break;                \
-    default: e = cudaErrorInvalidValue; break;       \
-  }
-
 template <typename T>
 cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
                               cudaStream_t st, unsigned long long* launches, Prof* prof) {
   cudaError_t e = cudaSuccess;
-  prof->mark(0, st);
-  if (b.two_x) {
-    e = strided2_launch<T>(0, g, b, m, H, scale, 0, 0, st);
-  } else {
-#define CALL_XF(L) launch_xf<T, L>(g, b, m, st)
-    MM_DISPATCH_L(g.nx, CALL_XF)
-#undef CALL_XF
-  }
-  if (e != cudaSuccess) return e;
-  ++*launches;
   const int nplanes = g.nx + 1;
-  const int kc = g.kchunk > 0 ? g.kchunk : nplanes;
-  for (int k0 = 0; k0 < nplanes; k0 += kc) {
-    const int nk = nplanes - k0 < kc ? nplanes - k0 : kc;
-    prof->mark(1, st);
-    if (b.two_y) {
-      e = strided2_launch<T>(1, g, b, m, H, scale, k0, nk, st);
-    } else {
-#define CALL_YF(L) launch_yf<T, L>(g, b, k0, nk, st)
-      MM_DISPATCH_L(g.ny, CALL_YF)
-#undef CALL_YF
-    }
-    if (e != cudaSuccess) return e;
-    prof->mark(2, st);
-    if (g.nz == 256) {
-      e = launch_zw<T>(g, b, k0, nk, st);
-    } else {
-      e = g.nz == 128 ? launch_zp<T, 16>(g, b, k0, nk, st) : launch_zp<T, 8>(g, b, k0, nk, st);
-    }
-    if (e != cudaSuccess) return e;
-    prof->mark(3, st);
-    if (b.two_y) {
-      e = strided2_launch<T>(3, g, b, m, H, scale, k0, nk, st);
-    } else {
-#define CALL_YI(L) launch_yi<T, L>(g, b, k0, nk, st)
-      MM_DISPATCH_L(g.ny, CALL_YI)
-#undef CALL_YI
-    }
-    if (e != cudaSuccess) return e;
-    *launches += 3;
-  }
-  prof->mark(4, st);
-  if (b.two_x) {
-    e = strided2_launch<T>(4, g, b, m, H, scale, 0, 0, st);
-  } else {
-#define CALL_XI(L) launch_xi<T, L>(g, b, H, scale, st)
-    MM_DISPATCH_L(g.nx, CALL_XI)
-#undef CALL_XI
-  }
+  prof->mark(0, st);
+  e = b.two_x ? strided2_launch<T>(0, g, b, m, H, scale, st) : launch_xf<T, 1024>(g, b, m, st);
   if (e != cudaSuccess) return e;
-  ++*launches;
+  prof->mark(1, st);
+  e = b.two_y ? strided2_launch<T>(1, g, b, m, H, scale, st) : launch_yf<T, 1024>(g, b, 0, nplanes, st);
+  if (e != cudaSuccess) return e;
+  prof->mark(2, st);
+  if (g.nz == 256) e = launch_zw<T>(g, b, 0, nplanes, st);
+  else if (g.nz == 128) e = launch_zp<T, 16>(g, b, 0, nplanes, st);
+  else if (g.nz == 64) e = launch_zp<T, 8>(g, b, 0, nplanes, st);
+  else e = ztile_launch<T>(g, b, st);
+  if (e != cudaSuccess) return e;
+  prof->mark(3, st);
+  e = b.two_y ? strided2_launch<T>(3, g, b, m, H, scale, st) : launch_yi<T, 1024>(g, b, 0, nplanes, st);
+  if (e != cudaSuccess) return e;
+  prof->mark(4, st);
+  e = b.two_x ? strided2_launch<T>(4, g, b, m, H, scale, st) : launch_xi<T, 1024>(g, b, H, scale, st);
+  if (e != cudaSuccess) return e;
+  *launches += 5;
   prof->mark(-1, st);
   return cudaGetLastError();
 }

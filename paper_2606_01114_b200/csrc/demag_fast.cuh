@@ -14,11 +14,10 @@ struct FastGeom {
   int nx, ny, nz;
   int Px, Py, Pz;  // 2 n_d
   int Q;           // complex columns per (kx, y) row: 3 nz
-  int kchunk;      // kx planes per launch of K2..K4 (0 = all nx + 1 planes at once)
 };
 
 // true if the fast kernels cover this mesh (otherwise the generic path of demag_passes.cu runs)
-bool fast_supported(int nx, int ny, int nz, size_t real_bytes);
+bool fast_supported(int nx, int ny, int nz);
 
 template <typename T> struct FastBufs {
   const Cx<T>* Wx;        // Wx[q] = exp(-2 pi i q / Px), q < Px
@@ -28,10 +27,12 @@ template <typename T> struct FastBufs {
   const uint16_t* posy;   // row of y frequency k in A2, k < Py
   const Cx<T>* T2x;       // two-stage plan of the x axis: T2x[bf K1 + k1] = exp(-2 pi i bf k1 / Px) (or unused)
   const Cx<T>* T2y;       // ... of the y axis
+  const Cx<T>* T2z;       // ... of the z axis (tile pass of demag_ztile.cu; unused by the warp-per-pencil kernels)
   bool two_x, two_y;      // the axis runs the two-stage kernels of demag_fast2.cu (natural frequency order)
   const T* table;         // Nhat[kx <= nx][ky <= ny][6][ozp] (kz <= nz used), scaled by 1/(Px Py Pz), parity sign folded
   Cx<T>* A1;              // [nx + 1][ny][Q]
-  Cx<T>* A2;              // [kchunk planes][Py][Q] (rows in digit-reversed ky order), reused by every chunk
+  Cx<T>* A2;              // [nx + 1][Py][Q]; ky rows in natural order (two-stage y pass) or in the three-stage
+                          // plan's order (L = 1024; K3 finds row ky through posy)
 };
 
 // Enqueues K1..K5: H := scale * crop(IFFT(table . FFT(pad(m)))).
@@ -40,12 +41,12 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
                               cudaStream_t st, unsigned long long* launches, Prof* prof);
 
 // Two-stage strided passes (demag_fast2.cu).  which: 0 = K1 (x forward), 1 = K2 (y forward),
-// 3 = K4 (y inverse), 4 = K5 (x inverse); k0, nk: first plane and plane count for K2 / K4.
+// 3 = K4 (y inverse), 4 = K5 (x inverse).
 template <typename T>
 cudaError_t strided2_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
-                            int k0, int nk, cudaStream_t st);
-bool fast_two_stage(int L, size_t real_bytes);   // the two-stage kernels cover length L in this precision
-void fast2_plan(int L, int* K1, int* K2);        // P = 2L = K1 K2
+                            cudaStream_t st);
+bool fast_two_stage(int L);                      // the two-stage kernels cover length L (both precisions)
+void fast2_plan(int L, int* K1, int* K2);        // P = 2L = K1 K2 (plan2.cuh; 0, 0 if L has no plan)
 
 // Host helpers for the tables above (plan order of the fast kernels).
 int fast_pos_logical(int L, int k);   // row of frequency k < 2L in the [even half | odd half] layout

@@ -1,7 +1,9 @@
-// Two-stage strided passes of the fast demag path (K1, K2, K4, K5 of demag_fast.cu for
-// transform lengths L <= 512).
+// Two-stage strided passes of the x-first demag path (K1, K2, K4, K5) for every
+// transform length with a plan in plan2.cuh: the powers of two 64 .. 512 and the paper's own sides
+// L = 100, 350, 400, whose padded lengths are 200 = 20 x 10, 700 = 28 x 25
+// and 800 = 32 x 25.
 //
-// The pruned length-P transform (P = 2L = K1 K2, L non-zero inputs; "zero-padding
+// The pruned length-P transform (P = 2L = K1 K2, K1 even, L non-zero inputs; "zero-padding
 // and ... FFT") is split as
 //     X[k1 + K1 k2] = sum_bf w_K2^(bf k2) . w_P^(bf k1) . sum_{s < K1/2} a[bf + K2 s] w_K1^(s k1)
 // stage A: one thread per (bf, column): K1/2 inputs straight from global memory, pruned
@@ -10,7 +12,8 @@
 //          memory in NATURAL frequency order (row k1 + K1 k2).
 // The inverse is the mirror image with the truncation folded into stage A' (only the L wanted
 // samples are computed).  One exchange through shared memory per transform instead of two:
-// the passes are bound by L1/shared-memory wavefronts, not by HBM (profiles/r01_v1_*.md).
+// the passes are bound by L1/shared-memory wavefronts, not by HBM (profiles/r01_v2_fast_path.md).
+// Radix 25 runs as 5 x 5, radix 14 / 10 as 2 x 7 / 2 x 5 in registers (fft_core.cuh).
 //
 // K1/K5 (x axis, r2c / c2r): two real columns (q, q+1) ride as one complex column Z = a + i b.
 // The Hermitian separation A[k] = (Z[k] + conj Z[-k]) / 2, B[k] = (Z[k] - conj Z[-k]) / 2i needs
@@ -18,37 +21,50 @@
 // are ordered so that k1 and K1 - k1 are neighbours (slots 2p, 2p + 1) and hence B lanes apart
 // in the same warp: the halves are swapped with warp shuffles, no extra pass through shared
 // memory.  (The factor 1/2 is applied in K5's output scale.)
+//
+// Columns beyond the end of a row (3 nz and ny 3 nz / 2 need not be multiples of the 64-byte row of a
+// tile) are loaded from column 0 and never stored.
 // scalar fp32 complex add/subtract here: the two-wide form (mm_common.cuh) measured slower in these
 // memory-latency-bound passes (K2 0.497 -> 0.528 ms at config 4) and faster only in K3
 #define MM_NO_PACKED_F32
 #include "demag_fast.cuh"
 #include "fft_core.cuh"
+#include "plan2.cuh"
 
 namespace mm {
 
-template <int L> struct Plan2;
-template <> struct Plan2<64> { static constexpr int K1 = 16, K2 = 8; };
-template <> struct Plan2<128> { static constexpr int K1 = 16, K2 = 16; };
-template <> struct Plan2<256> { static constexpr int K1 = 32, K2 = 16; };
-template <> struct Plan2<512> { static constexpr int K1 = 32, K2 = 32; };
-
-bool fast_two_stage(int L, size_t real_bytes) {
-  (void)real_bytes;  // fp32 and fp64 (fp64: K1 0.79 -> 0.69 ms, K5 0.96 -> 0.57 ms at config 4)
-  return L == 64 || L == 128 || L == 256 || L == 512;
+// fp32 and fp64 (fp64: K1 0.79 -> 0.69 ms, K5 0.96 -> 0.57 ms at config 4 against the three-stage kernels)
+bool fast_two_stage(int L) {
+  switch (L) {
+#define MM_PLAN2_CASE(LL) case LL: return true;
+    MM_PLAN2_LENGTHS(MM_PLAN2_CASE)
+#undef MM_PLAN2_CASE
+    default: return false;
+  }
 }
 
 template <typename T, int L> struct Tile2 {
   using P = Plan2<L>;
-  static constexpr int K1 = P::K1, K2 = P::K2, A = K1 / 2, H = K2 / 2;
+  static constexpr int K1 = P::K1, K2 = P::K2, A = K1 / 2;
+  static constexpr int K2P = (K2 + 1) / 2 * 2;       // row pitch of a k1 block: even, so that bf ^ 1 stays inside it
+  static constexpr int JN = K2 / 2 + 1;              // k2 values of a stage-B thread that can hold a k <= L
   static constexpr int B = 64 / (int)sizeof(Cx<T>);  // lanes along the batch (64-byte rows)
   static constexpr int tasksA = K2 * B, tasksB = K1 * B;
-  static constexpr int NT = tasksA > tasksB ? tasksA : tasksB;
-  static constexpr int smem_bytes = K1 * K2 * 64;
+  static constexpr int NT = ((tasksA > tasksB ? tasksA : tasksB) + 31) / 32 * 32;
+  static constexpr int slotsB = (tasksB + 31) / 32 * 32 / B;   // stage-B slots rounded up to whole warps
+  // Does the stage-B thread of slot (pair0, odd) hold a row k = k1 + K1 j <= L in its slot j < JN?  Even K2:
+  // every j < K2/2 (the slot j = K2/2 is k = L of k1 = 0, handled apart).  Odd K2: k1 <= K1/2 (even slots and
+  // the self-paired k1 = K1/2) holds j <= (K2-1)/2, k1 > K1/2 (odd slots of the other pairs) one row less.
+  static __device__ __forceinline__ bool has_row(int j, bool pair0, bool odd) {
+    if (K2 % 2 == 0) return j < K2 / 2;
+    return j < K2 / 2 || (j == K2 / 2 && (pair0 || !odd));
+  }
+  static constexpr int smem_bytes = K1 * K2P * 64;
   static constexpr int min_blocks = sizeof(T) == 8 ? 2 : (smem_bytes >= 32 * 1024 ? 3 : 4);
-  static_assert(K1 * K2 == 2 * L && NT <= 256 && tasksB % 32 == 0, "plan");
+  static_assert(K1 * K2 == 2 * L && K1 % 2 == 0 && NT <= 256, "plan");
 };
 
-// Shared-memory element (k1, bf, lane): sm[(k1 K2 + (bf ^ odd(k1))) B + lane], odd(k1) = k1 >= K1/2:
+// Shared-memory element (k1, bf, lane): sm[(k1 K2P + (bf ^ odd(k1))) B + lane], odd(k1) = k1 >= K1/2:
 // the two k1 of a stage-B half warp (slots 2p, 2p + 1) read rows of opposite parity, i.e.
 // different 64-byte halves of the banks.
 template <int K1> __device__ __forceinline__ int slot_k1(int slot) {
@@ -94,21 +110,20 @@ template <> struct Vec2<double> {
 template <typename T, int L>
 __device__ __forceinline__ void fwdA(Cx<T>* sm, const Cx<T>* __restrict__ Wt, int lane, int bf, Cx<T>* v) {
   using TL = Tile2<T, L>;
-  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B;
+  constexpr int K1 = TL::K1, K2P = TL::K2P, A = TL::A, B = TL::B;
   Cx<T> o[A];
   rot_fwd<T, K1>(v, o, std::make_integer_sequence<int, A>{});
   Dft<T, A, false>::run(v);   // even outputs k1 = 2u
   Dft<T, A, false>::run(o);   // odd outputs  k1 = 2u + 1
   const Cx<T>* tw = Wt + bf * K1;
-  Cx<T>* lo = sm + bf * B + lane;          // rows of k1 <  K1/2: (k1 K2 + bf)
-  Cx<T>* hi = sm + (bf ^ 1) * B + lane;    // rows of k1 >= K1/2: (k1 K2 + (bf ^ 1))
+  Cx<T>* lo = sm + bf * B + lane;          // rows of k1 <  K1/2: (k1 K2P + bf)
+  Cx<T>* hi = sm + (bf ^ 1) * B + lane;    // rows of k1 >= K1/2: (k1 K2P + (bf ^ 1))
 #pragma unroll
   for (int u = 0; u < A; ++u) {
     Cx<T> w0, w1;
     Vec2<T>::ldg(tw + 2 * u, w0, w1);
-    Cx<T>* dst = (2 * u >= K1 / 2) ? hi : lo;
-    dst[(2 * u) * K2 * B] = u ? cmul(v[u], w0) : v[0];
-    dst[(2 * u + 1) * K2 * B] = cmul(o[u], w1);
+    (2 * u >= K1 / 2 ? hi : lo)[(2 * u) * K2P * B] = u ? cmul(v[u], w0) : v[0];
+    (2 * u + 1 >= K1 / 2 ? hi : lo)[(2 * u + 1) * K2P * B] = cmul(o[u], w1);
   }
 }
 
@@ -116,9 +131,9 @@ __device__ __forceinline__ void fwdA(Cx<T>* sm, const Cx<T>* __restrict__ Wt, in
 template <typename T, int L>
 __device__ __forceinline__ void fwdB(const Cx<T>* sm, int lane, int k1, Cx<T>* t) {
   using TL = Tile2<T, L>;
-  constexpr int K1 = TL::K1, K2 = TL::K2, B = TL::B;
+  constexpr int K1 = TL::K1, K2 = TL::K2, K2P = TL::K2P, B = TL::B;
   const int odd = k1 >= K1 / 2 ? 1 : 0;
-  const Cx<T>* base = sm + k1 * K2 * B + lane;
+  const Cx<T>* base = sm + k1 * K2P * B + lane;
   const Cx<T>* pe = base + odd * B;   // even bf: row bf + odd
   const Cx<T>* po = base - odd * B;   // odd bf:  row bf - odd
 #pragma unroll
@@ -130,10 +145,10 @@ __device__ __forceinline__ void fwdB(const Cx<T>* sm, int lane, int k1, Cx<T>* t
 template <typename T, int L>
 __device__ __forceinline__ void invB(Cx<T>* sm, int lane, int k1, Cx<T>* t) {
   using TL = Tile2<T, L>;
-  constexpr int K1 = TL::K1, K2 = TL::K2, B = TL::B;
+  constexpr int K1 = TL::K1, K2 = TL::K2, K2P = TL::K2P, B = TL::B;
   Dft<T, K2, true>::run(t);
   const int odd = k1 >= K1 / 2 ? 1 : 0;
-  Cx<T>* base = sm + k1 * K2 * B + lane;
+  Cx<T>* base = sm + k1 * K2P * B + lane;
   Cx<T>* pe = base + odd * B;
   Cx<T>* po = base - odd * B;
 #pragma unroll
@@ -144,7 +159,7 @@ __device__ __forceinline__ void invB(Cx<T>* sm, int lane, int k1, Cx<T>* t) {
 template <typename T, int L>
 __device__ __forceinline__ void invA(const Cx<T>* sm, const Cx<T>* __restrict__ Wt, int lane, int bf, Cx<T>* v) {
   using TL = Tile2<T, L>;
-  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B;
+  constexpr int K1 = TL::K1, K2P = TL::K2P, A = TL::A, B = TL::B;
   Cx<T> o[A];
   const Cx<T>* tw = Wt + bf * K1;
   const Cx<T>* lo = sm + bf * B + lane;
@@ -153,8 +168,8 @@ __device__ __forceinline__ void invA(const Cx<T>* sm, const Cx<T>* __restrict__ 
   for (int u = 0; u < A; ++u) {
     Cx<T> w0, w1;
     Vec2<T>::ldg(tw + 2 * u, w0, w1);
-    const Cx<T>* src = (2 * u >= K1 / 2) ? hi : lo;
-    const Cx<T> a = src[(2 * u) * K2 * B], b = src[(2 * u + 1) * K2 * B];
+    const Cx<T> a = (2 * u >= K1 / 2 ? hi : lo)[(2 * u) * K2P * B];
+    const Cx<T> b = (2 * u + 1 >= K1 / 2 ? hi : lo)[(2 * u + 1) * K2P * B];
     v[u] = u ? cmulc(a, w0) : a;
     o[u] = cmulc(b, w1);
   }
@@ -167,17 +182,19 @@ __device__ __forceinline__ void invA(const Cx<T>* sm, const Cx<T>* __restrict__ 
   extern __shared__ __align__(16) unsigned char smem_raw[];                \
   Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);                          \
   using TL = Tile2<T, L>;                                                  \
-  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, H = TL::H, B = TL::B; \
+  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, JN = TL::JN, B = TL::B; \
   const int lane = threadIdx.x % B, slot = threadIdx.x / B;                \
-  (void)H; (void)A;
+  (void)JN; (void)A;
 
 // ---------------------------------------------------------------- K2: forward y
-// grid (Q / B, planes); A1, A2 point at the first plane of the launch.
+// grid (ceil(Q / B), planes)
 template <typename T, int L>
 __global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
 yf2_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>* __restrict__ Wt, int Q) {
   MM_T2_PROLOGUE
-  const size_t col = (size_t)blockIdx.x * B + lane;
+  const int colq = blockIdx.x * B + lane;
+  const bool ok = colq < Q;
+  const size_t col = ok ? colq : 0;
   const Cx<T>* in = A1 + (size_t)blockIdx.y * L * Q + col;
   Cx<T>* out = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
   if (slot < K2) {
@@ -191,8 +208,10 @@ yf2_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>* __
     const int k1 = slot_k1<K1>(slot);
     Cx<T> t[K2];
     fwdB<T, L>(sm, lane, k1, t);
+    if (ok) {
 #pragma unroll
-    for (int k2 = 0; k2 < K2; ++k2) out[(size_t)(k1 + K1 * k2) * Q] = t[k2];
+      for (int k2 = 0; k2 < K2; ++k2) out[(size_t)(k1 + K1 * k2) * Q] = t[k2];
+    }
   }
 }
 
@@ -201,7 +220,9 @@ template <typename T, int L>
 __global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
 yi2_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ Wt, int Q) {
   MM_T2_PROLOGUE
-  const size_t col = (size_t)blockIdx.x * B + lane;
+  const int colq = blockIdx.x * B + lane;
+  const bool ok = colq < Q;
+  const size_t col = ok ? colq : 0;
   const Cx<T>* in = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
   Cx<T>* out = A1 + (size_t)blockIdx.y * L * Q + col;
   if (slot < K1) {
@@ -212,7 +233,7 @@ yi2_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>* __
     invB<T, L>(sm, lane, k1, t);
   }
   __syncthreads();
-  if (slot < K2) {
+  if (slot < K2 && ok) {
     Cx<T> v[A];
     invA<T, L>(sm, Wt, lane, slot, v);
 #pragma unroll
@@ -230,11 +251,17 @@ template <typename T> __device__ __forceinline__ Cx<T> shfl_xor_cx(Cx<T> v, int 
 // ---------------------------------------------------------------- K1: forward x, r2c
 // m [x][y][q] real, read as complex pairs (q, q+1); npairs = ny Q / 2 pairs per x row; the
 // spectrum rows k <= nx of A1 hold (A[k], B[k]) at complex columns (2 pair, 2 pair + 1).
+// Stage-B thread k1 holds Z[k1 + K1 j] and stores the rows k = k1 + K1 j <= L.  Z[-k] is the partner
+// thread's t[K2 - 1 - j] (k1' = K1 - k1), the thread's own t[K2 - 1 - j] for the self-paired k1 = K1/2
+// and its own t[(K2 - j) % K2] for k1 = 0.  Every lane of a warp takes part in the shuffles (threads
+// past the last slot with dummy values).
 template <typename T, int L>
 __global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
 xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ Wt, size_t npairs) {
   MM_T2_PROLOGUE
-  const size_t pair = (size_t)blockIdx.x * B + lane;
+  const size_t pairq = (size_t)blockIdx.x * B + lane;
+  const bool ok = pairq < npairs;
+  const size_t pair = ok ? pairq : 0;
   const Cx<T>* in = mp + pair;
   if (slot < K2) {
     Cx<T> v[A];
@@ -243,67 +270,84 @@ xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __
     fwdA<T, L>(sm, Wt, lane, slot, v);
   }
   __syncthreads();
-  if (slot < K1) {   // whole warps: K1 B is a multiple of 32
-    const int k1 = slot_k1<K1>(slot);
+  if (slot < TL::slotsB) {   // whole warps: every lane takes part in the shuffles
+    const bool live = TL::slotsB == K1 || slot < K1;
+    const int k1 = slot_k1<K1>(live ? slot : 0);
     const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
     Cx<T> t[K2];
     fwdB<T, L>(sm, lane, k1, t);
     Cx<T>* out = A1 + 2 * pair;
     const size_t rowc = 2 * npairs;
 #pragma unroll
-    for (int j = 0; j < H; ++j) {
-      // Z[-k] for k = k1 + K1 j: the partner's t[K2 - 1 - j]; own t for the self-paired k1
-      const Cx<T> r = shfl_xor_cx<T>(t[K2 - 1 - j], B);
-      const Cx<T> own = odd ? t[K2 - 1 - j] : t[(K2 - j) % K2];
-      const Cx<T> z = t[j], zm = cconj(pair0 ? own : r);
-      const Cx<T> s = cadd(z, zm), d = csub(z, zm);
-      Vec2<T>::st(out + (size_t)(k1 + K1 * j) * rowc, s, mk<T>(d.y, -d.x));
-    }
-    if (k1 == 0) {  // k = L, its own mirror
-      const Cx<T> z = t[H];
-      Vec2<T>::st(out + (size_t)L * rowc, mk<T>(2 * z.x, (T)0), mk<T>(2 * z.y, (T)0));
+    for (int j = 0; j < JN; ++j) {
+      if (K2 % 2 == 0 && j == K2 / 2) {   // even K2: the last j holds only k = L (k1 = 0), its own mirror
+        if (live && ok && k1 == 0) {
+          const Cx<T> z = t[j % K2];
+          Vec2<T>::st(out + (size_t)L * rowc, mk<T>(2 * z.x, (T)0), mk<T>(2 * z.y, (T)0));
+        }
+        continue;
+      }
+      const Cx<T> r = shfl_xor_cx<T>(t[(2 * K2 - 1 - j) % K2], B);
+      const Cx<T> own = odd ? t[(2 * K2 - 1 - j) % K2] : t[(K2 - j) % K2];
+      if (live && ok && TL::has_row(j, pair0, odd)) {
+        const Cx<T> z = t[j % K2], zm = cconj(pair0 ? own : r);
+        const Cx<T> s = cadd(z, zm), d = csub(z, zm);
+        Vec2<T>::st(out + (size_t)(k1 + K1 * j) * rowc, s, mk<T>(d.y, -d.x));
+      }
     }
   }
 }
 
 // ---------------------------------------------------------------- K5: inverse x, c2r
 // Z[k] = A[k] + i B[k], Z[P - k] = conj A[k] + i conj B[k]; the truncated inverse gives
-// h_q(x) + i h_{q+1}(x), written as the real pair (q, q+1) of H, times scale.
+// h_q(x) + i h_{q+1}(x), written as the real pair (q, q+1) of H, times scale.  A stage-B' thread loads
+// its rows k = k1 + K1 j <= L, keeps Z[k] in t[j] and hands S = conj A + i conj B = Z[P - k] to the
+// thread that owns P - k: the partner's (or, for k1 = K1/2, its own) slot K2 - 1 - j, for k1 = 0 its own
+// slot (K2 - j) % K2.  The self-mirrored rows k = 0 and k = L keep Z[k].
 template <typename T, int L>
 __global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
 xi2_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>* __restrict__ Wt, size_t npairs,
            T scale) {
   MM_T2_PROLOGUE
-  const size_t pair = (size_t)blockIdx.x * B + lane;
-  if (slot < K1) {
-    const int k1 = slot_k1<K1>(slot);
+  const size_t pairq = (size_t)blockIdx.x * B + lane;
+  const bool ok = pairq < npairs;
+  const size_t pair = ok ? pairq : 0;
+  if (slot < TL::slotsB) {   // whole warps: every lane takes part in the shuffles
+    const bool live = TL::slotsB == K1 || slot < K1;
+    const int k1 = slot_k1<K1>(live ? slot : 0);
     const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
     const Cx<T>* in = A1 + 2 * pair;
     const size_t rowc = 2 * npairs;
     Cx<T> t[K2];
-    Cx<T> a[H], b[H];
+    Cx<T> a[JN], b[JN];
 #pragma unroll
-    for (int j = 0; j < H; ++j) Vec2<T>::ld(in + (size_t)(k1 + K1 * j) * rowc, a[j], b[j]);
-#pragma unroll
-    for (int j = 0; j < H; ++j) t[K2 - 1 - j] = mk<T>((T)0, (T)0);
-    if (k1 == 0) {
-      Cx<T> aL, bL;
-      Vec2<T>::ld(in + (size_t)L * rowc, aL, bL);
-      t[H] = mk<T>(aL.x - bL.y, aL.y + bL.x);
+    for (int j = 0; j < JN; ++j) {
+      const bool last_even = K2 % 2 == 0 && j == K2 / 2;   // only k = L of k1 = 0
+      if (live && (last_even ? k1 == 0 : TL::has_row(j, pair0, odd)))
+        Vec2<T>::ld(in + (size_t)(k1 + K1 * j) * rowc, a[j], b[j]);
+      else a[j] = b[j] = mk<T>((T)0, (T)0);
     }
 #pragma unroll
-    for (int j = 0; j < H; ++j) {
-      t[j] = mk<T>(a[j].x - b[j].y, a[j].y + b[j].x);
+    for (int k2 = 0; k2 < K2; ++k2) t[k2] = mk<T>((T)0, (T)0);
+#pragma unroll
+    for (int j = 0; j < JN; ++j) {
+      if (K2 % 2 == 0 && j == K2 / 2) {   // k = L (k1 = 0): its own mirror
+        if (k1 == 0) t[j % K2] = mk<T>(a[j].x - b[j].y, a[j].y + b[j].x);
+        continue;
+      }
       const Cx<T> S = mk<T>(a[j].x + b[j].y, b[j].x - a[j].y);
       const Cx<T> r = shfl_xor_cx<T>(S, B);
-      if (!pair0) t[K2 - 1 - j] = r;
-      else if (odd) t[K2 - 1 - j] = S;
-      else if (j >= 1) t[K2 - j] = S;
+      // the mirror Z[P - k] of row k goes to the partner's (k1 = K1/2: the thread's own) slot K2 - 1 - j, for
+      // k1 = 0 to its own slot (K2 - j) % K2; the self-mirrored rows k = 0 and k = L keep Z[k]
+      if (!pair0) { if (TL::has_row(j, false, !odd)) t[(2 * K2 - 1 - j) % K2] = r; }
+      else if (odd) { if (!(K2 % 2 == 1 && j == K2 / 2)) t[(2 * K2 - 1 - j) % K2] = S; }
+      else if (j >= 1) t[(K2 - j) % K2] = S;
+      if (TL::has_row(j, pair0, odd)) t[j % K2] = mk<T>(a[j].x - b[j].y, a[j].y + b[j].x);
     }
-    invB<T, L>(sm, lane, k1, t);
+    if (live) invB<T, L>(sm, lane, k1, t);
   }
   __syncthreads();
-  if (slot < K2) {
+  if (slot < K2 && ok) {
     Cx<T> v[A];
     invA<T, L>(sm, Wt, lane, slot, v);
     Cx<T>* out = Hp + pair;
@@ -322,30 +366,29 @@ template <typename K> static cudaError_t opt_in(K kernel, int bytes) {
 
 template <typename T, int L>
 static cudaError_t launch2(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
-                           int k0, int nk, cudaStream_t st) {
+                           cudaStream_t st) {
   using TL = Tile2<T, L>;
   const size_t npairs = (size_t)g.ny * g.Q / 2;
+  const unsigned gx = (unsigned)((npairs + TL::B - 1) / TL::B), gq = (unsigned)((g.Q + TL::B - 1) / TL::B);
+  const int nk = g.nx + 1;
   cudaError_t e;
   switch (which) {
     case 0:
       if ((e = opt_in(xf2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
-      xf2_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
-          reinterpret_cast<const Cx<T>*>(m), b.A1, b.T2x, npairs);
+      xf2_kernel<T, L><<<gx, TL::NT, TL::smem_bytes, st>>>(reinterpret_cast<const Cx<T>*>(m), b.A1, b.T2x, npairs);
       break;
     case 1:
       if ((e = opt_in(yf2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
-      yf2_kernel<T, L><<<dim3(g.Q / TL::B, nk), TL::NT, TL::smem_bytes, st>>>(
-          b.A1 + (size_t)k0 * g.ny * g.Q, b.A2, b.T2y, g.Q);
+      yf2_kernel<T, L><<<dim3(gq, nk), TL::NT, TL::smem_bytes, st>>>(b.A1, b.A2, b.T2y, g.Q);
       break;
     case 3:
       if ((e = opt_in(yi2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
-      yi2_kernel<T, L><<<dim3(g.Q / TL::B, nk), TL::NT, TL::smem_bytes, st>>>(
-          b.A2, b.A1 + (size_t)k0 * g.ny * g.Q, b.T2y, g.Q);
+      yi2_kernel<T, L><<<dim3(gq, nk), TL::NT, TL::smem_bytes, st>>>(b.A2, b.A1, b.T2y, g.Q);
       break;
     default:
       if ((e = opt_in(xi2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
-      xi2_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
-          b.A1, reinterpret_cast<Cx<T>*>(H), b.T2x, npairs, (T)0.5 * scale);
+      xi2_kernel<T, L><<<gx, TL::NT, TL::smem_bytes, st>>>(b.A1, reinterpret_cast<Cx<T>*>(H), b.T2x, npairs,
+                                                           (T)0.5 * scale);
       break;
   }
   return cudaSuccess;
@@ -353,30 +396,23 @@ static cudaError_t launch2(int which, const FastGeom& g, const FastBufs<T>& b, c
 
 template <typename T>
 cudaError_t strided2_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
-                            int k0, int nk, cudaStream_t st) {
+                            cudaStream_t st) {
   const int L = (which == 0 || which == 4) ? g.nx : g.ny;
   switch (L) {
-    case 64: return launch2<T, 64>(which, g, b, m, H, scale, k0, nk, st);
-    case 128: return launch2<T, 128>(which, g, b, m, H, scale, k0, nk, st);
-    case 256: return launch2<T, 256>(which, g, b, m, H, scale, k0, nk, st);
-    case 512: return launch2<T, 512>(which, g, b, m, H, scale, k0, nk, st);
+#define MM_PLAN2_CASE(LL) case LL: return launch2<T, LL>(which, g, b, m, H, scale, st);
+    MM_PLAN2_LENGTHS(MM_PLAN2_CASE)
+#undef MM_PLAN2_CASE
     default: return cudaErrorInvalidValue;
   }
 }
 
 template cudaError_t strided2_launch<float>(int, const FastGeom&, const FastBufs<float>&, const float*,
-                                            float*, float, int, int, cudaStream_t);
+                                            float*, float, cudaStream_t);
 template cudaError_t strided2_launch<double>(int, const FastGeom&, const FastBufs<double>&, const double*,
-                                             double*, double, int, int, cudaStream_t);
+                                             double*, double, cudaStream_t);
 
-// Host: table Wt[bf K1 + k1] = exp(-2 pi i bf k1 / P) of the length-L plan (P = 2L entries).
 void fast2_plan(int L, int* K1, int* K2) {
-  switch (L) {
-    case 64: *K1 = 16; *K2 = 8; break;
-    case 128: *K1 = 16; *K2 = 16; break;
-    case 256: *K1 = 32; *K2 = 16; break;
-    default: *K1 = 32; *K2 = 32; break;
-  }
+  if (!plan2_of(L, K1, K2)) { *K1 = 0; *K2 = 0; }
 }
 
 }  // namespace mm

@@ -26,19 +26,62 @@ constexpr double kCos32[9] = {1.0,
                                          0.19509032201612826785,
                                          0.0};
 
+// cos / sin of 2 pi num / den at compile time for any den (the radices of the mixed-radix plans: 28, 25,
+// 20, 18, ...).  The angle is reduced to the first octant in exact integer arithmetic, then a Taylor
+// series in double (|x| <= pi / 4: 13 terms leave < 1e-17); the result is within a few 1e-16 of the
+// correctly rounded value, far inside the 1e-12 parity bar.
+constexpr double kPi = 3.14159265358979323846264338327950288;
+constexpr double small_sin(double x) {
+  double term = x, sum = x;
+  for (int i = 1; i <= 13; ++i) { term *= -x * x / ((2.0 * i) * (2.0 * i + 1.0)); sum += term; }
+  return sum;
+}
+constexpr double small_cos(double x) {
+  double term = 1.0, sum = 1.0;
+  for (int i = 1; i <= 13; ++i) { term *= -x * x / ((2.0 * i - 1.0) * (2.0 * i)); sum += term; }
+  return sum;
+}
+constexpr double sin_turn(long long num, long long den);
+constexpr double cos_turn(long long num, long long den) {   // cos(2 pi num / den), 0 <= num < den
+  if (2 * num > den) return cos_turn(den - num, den);
+  if (4 * num > den) return -cos_turn(den - 2 * num, 2 * den);
+  if (8 * num > den) return sin_turn(den - 4 * num, 4 * den);
+  return small_cos(2.0 * kPi * (double)num / (double)den);
+}
+constexpr double sin_turn(long long num, long long den) {   // sin(2 pi num / den), 0 <= num < den
+  if (2 * num > den) return -sin_turn(den - num, den);
+  if (4 * num > den) return sin_turn(den - 2 * num, 2 * den);
+  if (8 * num > den) return cos_turn(den - 4 * num, 4 * den);
+  return small_sin(2.0 * kPi * (double)num / (double)den);
+}
+
+constexpr bool near_enough(double a, double b) { return a - b < 4e-16 && b - a < 4e-16; }
+static_assert(near_enough(cos_turn(1, 5), 0.30901699437494742410) && near_enough(sin_turn(1, 7), 0.78183148246802980871) &&
+                  near_enough(cos_turn(3, 8), -0.70710678118654752440) && near_enough(sin_turn(11, 25), 0.36812455268467795916) &&
+                  near_enough(cos_turn(13, 28), -0.97492791218182360702) && near_enough(sin_turn(27, 28), -0.22252093395631440429),
+              "compile-time trigonometry");
+
 template <int R, int S> constexpr double root_cos() {
-  constexpr int a = (S % R) * (32 / R);  // angle in 1/32 turns, 0..31
-  if (a <= 8) return kCos32[a];
-  if (a <= 16) return -kCos32[16 - a];
-  if (a <= 24) return -kCos32[a - 16];
-  return kCos32[32 - a];
+  if constexpr (32 % R != 0) {
+    return cos_turn(S % R, R);
+  } else {
+    constexpr int a = (S % R) * (32 / R);  // angle in 1/32 turns, 0..31
+    if (a <= 8) return kCos32[a];
+    if (a <= 16) return -kCos32[16 - a];
+    if (a <= 24) return -kCos32[a - 16];
+    return kCos32[32 - a];
+  }
 }
 template <int R, int S> constexpr double root_sin() {
-  constexpr int a = (S % R) * (32 / R);
-  if (a <= 8) return kCos32[8 - a];
-  if (a <= 16) return kCos32[a - 8];
-  if (a <= 24) return -kCos32[24 - a];
-  return -kCos32[a - 24];
+  if constexpr (32 % R != 0) {
+    return sin_turn(S % R, R);
+  } else {
+    constexpr int a = (S % R) * (32 / R);
+    if (a <= 8) return kCos32[8 - a];
+    if (a <= 16) return kCos32[a - 8];
+    if (a <= 24) return -kCos32[24 - a];
+    return -kCos32[a - 24];
+  }
 }
 
 // v * w_R^S with w_R = exp(-2 pi i / R) (forward) or its conjugate (INV).
@@ -224,6 +267,42 @@ template <typename T, bool INV> struct Dft<T, 6, INV> : DftTwoOdd<T, 6, INV> {};
 template <typename T, bool INV> struct Dft<T, 10, INV> : DftTwoOdd<T, 10, INV> {};
 template <typename T, bool INV> struct Dft<T, 14, INV> : DftTwoOdd<T, 14, INV> {};
 
+// Composite radix N = RA x RB in registers (Cooley-Tukey, compile-time roots): with n = RB n1 + n2 and
+// k = k1 + RA k2,  X[k] = sum_n2 w_RB^(n2 k2) . w_N^(n2 k1) . sum_n1 w_RA^(n1 k1) x[RB n1 + n2].
+// Used for 25 = 5 x 5, 9 = 3 x 3, 15 = 5 x 3, 12 = 4 x 3 of the two-stage mixed-radix plans.
+template <typename T, int RA, int RB, bool INV> struct DftCT {
+  static constexpr int N = RA * RB;
+  template <int N2, int... K1>
+  static __device__ __forceinline__ void inner(const Cx<T>* v, Cx<T>* t, std::integer_sequence<int, K1...>) {
+    Cx<T> y[RA];
+#pragma unroll
+    for (int n1 = 0; n1 < RA; ++n1) y[n1] = v[RB * n1 + N2];
+    Dft<T, RA, INV>::run(y);
+    ((t[N2 * RA + K1] = mul_root<T, N, N2 * K1, INV>(y[K1])), ...);
+  }
+  template <int... N2>
+  static __device__ __forceinline__ void first(const Cx<T>* v, Cx<T>* t, std::integer_sequence<int, N2...>) {
+    (inner<N2>(v, t, std::make_integer_sequence<int, RA>{}), ...);
+  }
+  static __device__ __forceinline__ void run(Cx<T>* v) {
+    Cx<T> t[N];
+    first(v, t, std::make_integer_sequence<int, RB>{});
+#pragma unroll
+    for (int k1 = 0; k1 < RA; ++k1) {
+      Cx<T> z[RB];
+#pragma unroll
+      for (int n2 = 0; n2 < RB; ++n2) z[n2] = t[n2 * RA + k1];
+      Dft<T, RB, INV>::run(z);
+#pragma unroll
+      for (int k2 = 0; k2 < RB; ++k2) v[k1 + RA * k2] = z[k2];
+    }
+  }
+};
+template <typename T, bool INV> struct Dft<T, 25, INV> : DftCT<T, 5, 5, INV> {};
+template <typename T, bool INV> struct Dft<T, 9, INV> : DftCT<T, 3, 3, INV> {};
+template <typename T, bool INV> struct Dft<T, 15, INV> : DftCT<T, 5, 3, INV> {};
+template <typename T, bool INV> struct Dft<T, 12, INV> : DftCT<T, 4, 3, INV> {};
+
 // One forward stage of span S (radix R) over a tile of N rows x B columns in shared memory,
 // row r of column c at sm[r * B + c].  Thread (col, tt) with NT threads per column.
 // W[q] = exp(-2 pi i q / P); wstep = P / S so that w_S^(t u) = W[t u wstep].
@@ -349,23 +428,28 @@ inline FftPlan make_plan(int n) {
   pl.P = n == 1 ? 1 : 2 * n;
   pl.nstages = 0;
   int p2 = 1, odd = n;
+  bool full = false;   // more than MM_MAX_STAGES stages: unsupported, never written past radix[]
+  auto push = [&](int r) {
+    if (pl.nstages == MM_MAX_STAGES) { full = true; return; }
+    pl.radix[pl.nstages++] = r;
+  };
   while (odd % 2 == 0) { odd /= 2; p2 *= 2; }
-  while (p2 >= 8) { pl.radix[pl.nstages++] = 8; p2 /= 8; }
+  while (p2 >= 8) { push(8); p2 /= 8; }
   const int primes[3] = {7, 5, 3};
   // a remaining factor 2 (or each 2 of a remaining 4) joins an odd prime: radix 14, 10 or 6
   for (int f : primes)
     while (p2 > 1 && odd % f == 0) {
-      pl.radix[pl.nstages++] = 2 * f;
+      push(2 * f);
       odd /= f;
       p2 /= 2;
     }
-  if (p2 > 1) pl.radix[pl.nstages++] = p2;
+  if (p2 > 1) push(p2);
   for (int f : primes)
     while (odd % f == 0) {
-      if (pl.nstages == MM_MAX_STAGES) { pl.nstages = -1; return pl; }
-      pl.radix[pl.nstages++] = f;
+      push(f);
       odd /= f;
     }
+  if (full) { pl.nstages = -1; return pl; }
   if (odd != 1) pl.nstages = -1;
   return pl;
 }

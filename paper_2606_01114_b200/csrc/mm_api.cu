@@ -15,6 +15,7 @@
 #include "demag_init.cuh"
 #include "demag_mixed.cuh"
 #include "demag_passes.cuh"
+#include "demag_ztile.cuh"
 #include "fft_core.cuh"
 #include "pointwise.cuh"
 #include "rkf45.cuh"
@@ -49,7 +50,6 @@ struct mm_ctx {
   int dnx = 0, dny = 0, dnz = 0;   // mesh of the demag passes (= nx, ny, nz unless embedded)
   bool xfirst() const { return fast || mixed; }   // x-first spectra and the octant table
   int path_pref = 0;     // 0 auto, 1 generic (demag_passes.cu), 2 fast required
-  int kchunk = 0;        // kx planes per K2..K4 launch group (0 = all)
   int want_bz = 0, want_by = 0, want_bk = 0;
   // workspaces
   unsigned char* pers = nullptr;
@@ -57,7 +57,7 @@ struct mm_ctx {
   size_t pers_bytes = 0, scr_bytes = 0;
   bool demag_ready = false;
   // persistent offsets
-  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_rkstate, off_bbstate, off_bbpart, pers_need;
+  size_t off_table, off_wx, off_wy, off_wz, off_posz, off_fz, off_fx, off_fy, off_posx, off_posy, off_t2x, off_t2y, off_t2z, off_rkstate, off_bbstate, off_bbpart, pers_need;
   // scratch offsets
   size_t off_a1, off_a2, off_hd, off_msa, off_msb, off_acc, off_sin, off_sout, off_rkf, off_emb_m, off_emb_h, off_mscaled, scr_need;
   RkfState rk_host{};
@@ -99,9 +99,11 @@ static bool smooth7(int n) { return n >= 1 && make_plan(n).nstages >= 0; }
 // extra cells cost less than the slower generic passes.  Per-cell cost ratio generic / fast measured on
 // the paper's meshes (profiles/r01_v4_paper_meshes.md): about 4.6 in fp32, 3.1 in fp64.
 static bool embed_mesh(const mm_ctx* c, int* ex, int* ey, int* ez) {
-  auto up = [](int n, int cap) { int v = 64; while (v < n) v *= 2; return v <= cap ? v : 0; };
-  const int x = up(c->nx, 1024), y = up(c->ny, 1024), z = up(c->nz, 256);
-  if (!x || !y || !z) return false;
+  // smallest length the x-first kernels cover that holds n (0: none)
+  static const int kxy[] = {64, 100, 128, 256, 350, 400, 512, 1024}, kz[] = {64, 90, 100, 128, 256, 350, 400};
+  auto up = [](int n, const int* list, int count) { for (int i = 0; i < count; ++i) if (list[i] >= n) return list[i]; return 0; };
+  const int x = up(c->nx, kxy, 8), y = up(c->ny, kxy, 8), z = up(c->nz, kz, 7);
+  if (!x || !y || !z || !fast_supported(x, y, z)) return false;
   const double r = (double)x * y * z / ((double)c->nx * c->ny * c->nz);
   // fp64 with nz' = 256 runs the wide-pencil K3 at 0.34 of the roofline: a smaller margin
   if (r > (c->es == 4 ? 3.0 : (z == 256 ? 1.7 : 2.2))) return false;
@@ -112,7 +114,7 @@ static bool embed_mesh(const mm_ctx* c, int* ex, int* ey, int* ez) {
 static void plan_layout(mm_ctx* c) {
   DemagGeom& g = c->geom;
   c->dnx = c->nx; c->dny = c->ny; c->dnz = c->nz;
-  c->embed = c->path_pref == 0 && !fast_supported(c->nx, c->ny, c->nz, c->es) && embed_mesh(c, &c->dnx, &c->dny, &c->dnz);
+  c->embed = c->path_pref == 0 && !fast_supported(c->nx, c->ny, c->nz) && embed_mesh(c, &c->dnx, &c->dny, &c->dnz);
   g.nx = c->dnx; g.ny = c->dny; g.nz = c->dnz;
   g.Px = padded(c->dnx); g.Py = padded(c->dny); g.Pz = padded(c->dnz);
   g.Kz = g.Pz == 1 ? 1 : g.Pz / 2 + 1;
@@ -134,7 +136,7 @@ static void plan_layout(mm_ctx* c) {
   ig.oz = c->dnz == 1 ? 1 : c->dnz + 1;
   ig.ozp = (ig.oz + 1) / 2 * 2;
   ig.Bk = g.Bk;
-  c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->dnx, c->dny, c->dnz, c->es);
+  c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->dnx, c->dny, c->dnz);
   // measured (profiles/r01_v4_paper_meshes.md): the mixed-radix x-first kernels only tie with the generic
   // z-first passes, so they are opt-in (path 3) until their stages move into registers
   c->mixed = c->path_pref == 3 && mixed_supported(c->dnx, c->dny, c->dnz, c->es);
@@ -142,7 +144,6 @@ static void plan_layout(mm_ctx* c) {
   fg.nx = c->dnx; fg.ny = c->dny; fg.nz = c->dnz;
   fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;
   fg.Q = 3 * c->dnz;
-  fg.kchunk = (c->kchunk > 0 && c->kchunk < c->dnx + 1) ? c->kchunk : 0;
   // persistent
   size_t o = 0;
   c->off_table = o;
@@ -159,6 +160,7 @@ static void plan_layout(mm_ctx* c) {
   c->off_posy = o; o += align256((size_t)g.Py * 2);
   c->off_t2x = o; o += align256((size_t)g.Px * cs);
   c->off_t2y = o; o += align256((size_t)g.Py * cs);
+  c->off_t2z = o; o += align256((size_t)g.Pz * cs);
   c->off_rkstate = o; o += align256(sizeof(RkfState));
   c->off_bbstate = o; o += align256(sizeof(BbState));
   c->off_bbpart = o; o += align256((size_t)kBbMaxBlocks * 3 * sizeof(double));
@@ -167,7 +169,7 @@ static void plan_layout(mm_ctx* c) {
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
   o = 0;
   if (c->xfirst()) {
-    const size_t planes2 = (c->fast && fg.kchunk) ? fg.kchunk : c->dnx + 1;
+    const size_t planes2 = c->dnx + 1;
     c->off_a1 = o; o += align256((size_t)(c->dnx + 1) * g.ny * fg.Q * cs);
     c->off_a2 = o; o += align256(planes2 * g.Py * fg.Q * cs);
   } else {
@@ -201,7 +203,7 @@ mm_status mm_ctx_create(int nx, int ny, int nz, double dx, double dy, double dz,
     return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: sizes and cell lengths must be positive");
   if (dtype != MM_F32 && dtype != MM_F64)
     return fail(nullptr, MM_ERR_INVALID_ARG, "mm_ctx_create: unknown dtype %d", (int)dtype);
-  if (!smooth7(nx) || !smooth7(ny) || !smooth7(nz) || nx > 1024 || ny > 1024 || nz > 512)
+  if (nx > 1024 || ny > 1024 || nz > 512 || !smooth7(nx) || !smooth7(ny) || !smooth7(nz))
     return fail(nullptr, MM_ERR_UNSUPPORTED_SIZE,
                 "mm_ctx_create: %dx%dx%d unsupported (each n must be of the form 2^a 3^b 5^c 7^d, "
                 "nx,ny <= 1024, nz <= 512)", nx, ny, nz);
@@ -250,27 +252,25 @@ mm_status mm_ctx_set_tiles(mm_ctx* ctx, int bz, int by, int bk) {
   return MM_OK;
 }
 
-mm_status mm_ctx_set_path(mm_ctx* ctx, int path, int kchunk) {
+mm_status mm_ctx_set_path(mm_ctx* ctx, int path) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (ctx->pers) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: call before mm_ctx_set_workspace");
-  if (path < 0 || path > 3 || kchunk < 0)
-    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: path must be 0 .. 3 and kchunk >= 0");
+  if (path < 0 || path > 3)
+    return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_path: path must be 0 .. 3");
   if (path == 3 && !mixed_supported(ctx->nx, ctx->ny, ctx->nz, ctx->es))
     return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_path: the mixed-radix x-first kernels do not cover %dx%dx%d",
                 ctx->nx, ctx->ny, ctx->nz);
-  if (path == 2 && !fast_supported(ctx->nx, ctx->ny, ctx->nz, ctx->es))
+  if (path == 2 && !fast_supported(ctx->nx, ctx->ny, ctx->nz))
     return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_path: the fast kernels do not cover %dx%dx%d",
                 ctx->nx, ctx->ny, ctx->nz);
   ctx->path_pref = path;
-  ctx->kchunk = kchunk;
   plan_layout(ctx);
   return MM_OK;
 }
 
-mm_status mm_ctx_path(const mm_ctx* ctx, int* fast, int* kchunk) {
-  if (!ctx || !fast || !kchunk) return MM_ERR_INVALID_ARG;
-  *fast = ctx->fast ? (ctx->embed ? 3 : 1) : (ctx->mixed ? 2 : 0);
-  *kchunk = ctx->fgeom.kchunk;
+mm_status mm_ctx_path(const mm_ctx* ctx, int* path) {
+  if (!ctx || !path) return MM_ERR_INVALID_ARG;
+  *path = ctx->fast ? (ctx->embed ? 3 : 1) : (ctx->mixed ? 2 : 0);
   return MM_OK;
 }
 
@@ -369,6 +369,28 @@ mm_status mm_ctx_launch_count(const mm_ctx* ctx, unsigned long long* count) {
 
 const char* mm_last_error(const mm_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
 
+const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
+  if (!ctx || kind < 0 || kind > 5) return "";
+  if (kind == 5) {
+    if (ctx->ms_cells || ctx->a_cells) return "pw_inhom_kernel";
+    return ctx->nz % (ctx->es == 4 ? 4 : 2) == 0 ? "pw_vec_kernel" : "pw_cell_kernel";
+  }
+  if (ctx->fast) {
+    const bool two_x = fast_two_stage(ctx->dnx), two_y = fast_two_stage(ctx->dny);
+    switch (kind) {
+      case 0: return two_x ? "xf2_kernel" : "xf_fast_kernel";
+      case 1: return two_y ? "yf2_kernel" : "yf_fast_kernel";
+      case 2: return ctx->dnz == 256 ? "zw_fast_kernel" : (ztile_supported(ctx->dnz) ? "zt_kernel" : "zp_fast_kernel");
+      case 3: return two_y ? "yi2_kernel" : "yi_fast_kernel";
+      default: return two_x ? "xi2_kernel" : "xi_fast_kernel";
+    }
+  }
+  static const char* const mixed[5] = {"xf_mixed_kernel", "yf_mixed_kernel", "zp_mixed_kernel", "yi_mixed_kernel",
+                                       "xi_mixed_kernel"};
+  static const char* const generic[5] = {"zf_kernel", "yf_kernel", "xp_kernel", "yi_kernel", "zi_kernel"};
+  return ctx->mixed ? mixed[kind] : generic[kind];
+}
+
 mm_status mm_ctx_set_profiling(mm_ctx* ctx, int enable) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   ctx->prof.on = enable != 0;
@@ -430,15 +452,18 @@ template <typename T> static void fill_twiddles2(std::vector<unsigned char>& buf
 
 template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   const DemagGeom& g = c->geom;
-  // small tables: twiddles and digit-reversal maps, built on the host, uploaded once
-  const size_t small_off = c->off_wx, small_bytes = c->pers_need - c->off_wx;
+  // small tables: twiddles and digit-reversal maps, built on the host, uploaded once.  The upload stops
+  // short of the RKF45 / minimiser controller records, which mm_rkf45_init / mm_minimize_init own and
+  // may have written already (the header does not fix the order of the init calls).
+  const size_t small_off = c->off_wx, small_bytes = c->off_rkstate - c->off_wx;
   std::vector<unsigned char> host(small_bytes, 0);
   fill_twiddles<T>(host, c->off_wx - small_off, g.Px);
   fill_twiddles<T>(host, c->off_wy - small_off, g.Py);
   fill_twiddles<T>(host, c->off_wz - small_off, g.Pz);
-  const bool two_x = c->fast && fast_two_stage(c->dnx, c->es), two_y = c->fast && fast_two_stage(c->dny, c->es);
+  const bool two_x = c->fast && fast_two_stage(c->dnx), two_y = c->fast && fast_two_stage(c->dny);
   if (two_x) fill_twiddles2<T>(host, c->off_t2x - small_off, c->dnx);
   if (two_y) fill_twiddles2<T>(host, c->off_t2y - small_off, c->dny);
+  if (c->fast && ztile_supported(c->dnz)) fill_twiddles2<T>(host, c->off_t2z - small_off, c->dnz);
   auto u16 = [&](size_t off) { return reinterpret_cast<uint16_t*>(host.data() + (off - small_off)); };
   for (int k = 0; k < g.Pz; ++k) {
     const int p = pos_of_freq(g.pz, k);
@@ -464,9 +489,6 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
                            reinterpret_cast<T*>(c->pers + c->off_table), c->xfirst() ? 1 : 0, c->stream,
                            &c->launches);
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: launch", e);
-  if (c->embed)   // the padding cells of the embedded m stay zero from here on (init's scratch use is over)
-    e = cudaMemsetAsync(c->scr + c->off_emb_m, 0, (size_t)c->dnx * c->dny * c->dnz * 3 * c->es, c->stream);
-  if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: clearing the embedded mesh", e);
   e = cudaStreamSynchronize(c->stream);  // also keeps `host` alive until the copy is done
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: execution", e);
   c->demag_ready = true;
@@ -539,8 +561,9 @@ template <typename T> static FastBufs<T> fast_bufs_of(mm_ctx* c) {
   b.posy = reinterpret_cast<const uint16_t*>(c->pers + c->off_posy);
   b.T2x = reinterpret_cast<const Cx<T>*>(c->pers + c->off_t2x);
   b.T2y = reinterpret_cast<const Cx<T>*>(c->pers + c->off_t2y);
-  b.two_x = fast_two_stage(c->dnx, c->es);
-  b.two_y = fast_two_stage(c->dny, c->es);
+  b.T2z = reinterpret_cast<const Cx<T>*>(c->pers + c->off_t2z);
+  b.two_x = fast_two_stage(c->dnx);
+  b.two_y = fast_two_stage(c->dny);
   b.table = reinterpret_cast<const T*>(c->pers + c->off_table);
   b.A1 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a1);
   b.A2 = reinterpret_cast<Cx<T>*>(c->scr + c->off_a2);
@@ -590,12 +613,12 @@ template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H
     T* mE = reinterpret_cast<T*>(c->scr + c->off_emb_m);
     T* HE = reinterpret_cast<T*>(c->scr + c->off_emb_h);
     c->prof.mark(0, c->stream);
-    cudaError_t e = embed_copy_launch<T>(static_cast<const T*>(m), mE, c->nx, c->ny, c->nz, c->dny, c->dnz, 1, c->stream);
+    cudaError_t e = embed_copy_launch<T>(static_cast<const T*>(m), mE, c->nx, c->ny, c->nz, c->dnx, c->dny, c->dnz, 1, c->stream);
     if (e == cudaSuccess)
       e = demag_fast_launch<T>(c->fgeom, fast_bufs_of<T>(c), mE, HE, (T)(-c->Ms), c->stream, &c->launches, &c->prof);
     c->prof.mark(4, c->stream);
     if (e == cudaSuccess)
-      e = embed_copy_launch<T>(HE, static_cast<T*>(H), c->nx, c->ny, c->nz, c->dny, c->dnz, 0, c->stream);
+      e = embed_copy_launch<T>(HE, static_cast<T*>(H), c->nx, c->ny, c->nz, c->dnx, c->dny, c->dnz, 0, c->stream);
     c->prof.mark(-1, c->stream);
     c->launches += 2;
     return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag (embedded fast path) launch", e);

@@ -284,7 +284,8 @@ __global__ void __launch_bounds__(256) pw_cell_kernel(PwParams<T> p, const T* __
 }
 
 // Per-cell Ms and A (eq. 2 as div(A grad M); reading Q31): thread = one cell.
-//   exchange  2/(mu0 Ms_i) sum A_ij (m_j - m_i)/d^2, A_ij = 2 A_i A_j/(A_i + A_j), missing neighbour: no term
+//   exchange  2/(mu0 Ms_i) sum A_ij (m_j - m_i)/d^2, A_ij = 2 A_i A_j/(A_i + A_j); a neighbour outside the
+//             mesh or in vacuum (Ms_j = 0): no term
 //   DMI, anisotropy with Ms_i; for DMI a neighbour outside the mesh or with Ms_j = 0 is the cell itself
 //   Ms_i = 0: vacuum -- those terms vanish, dm/dt = 0, a zero vector is not renormalised
 template <typename T, int MODE>
@@ -316,7 +317,7 @@ __global__ void __launch_bounds__(256) pw_inhom_kernel(PwParams<T> p, const T* _
         const size_t cj = inside ? (sg < 0 ? g - off[d] : g + off[d]) : g;
         const T Msj = p.ms_cells ? p.ms_cells[cj] : p.ms_ref, Aj = p.a_cells ? p.a_cells[cj] : p.a_ref;
         const T mj[3] = {m[3 * cj], m[3 * cj + 1], m[3 * cj + 2]};
-        if (want_ex && inside && Ai + Aj > (T)0) {
+        if (want_ex && inside && Msj > (T)0 && Ai + Aj > (T)0) {   // a vacuum neighbour is no exchange partner
           const T w = p.exq[d] * ((T)2 * Ai * Aj / (Ai + Aj));
 #pragma unroll
           for (int c = 0; c < 3; ++c) lap[c] += w * (mj[c] - mc[c]);
@@ -450,24 +451,31 @@ cudaError_t pointwise_launch(int mode, const PwParams<T>& p, const T* m, const T
   return cudaGetLastError();
 }
 
+// embed != 0: one CTA per (x, y) row of the EMBEDDED array; cells outside the mesh are written as zero on
+// every call, so the scratch array needs no state between calls.  embed == 0: one CTA per mesh row.
 template <typename T>
-__global__ void __launch_bounds__(128) embed_copy_kernel(const T* __restrict__ src, T* __restrict__ dst, int ny, int nz,
-                                                         int eny, int enz, int embed) {
-  const int x = blockIdx.x / ny, y = blockIdx.x - x * ny;
+__global__ void __launch_bounds__(128) embed_copy_kernel(const T* __restrict__ src, T* __restrict__ dst, int nx, int ny,
+                                                         int nz, int eny, int enz, int embed) {
+  const int rows = embed ? eny : ny;
+  const int x = blockIdx.x / rows, y = blockIdx.x - x * rows;
   const size_t small = ((size_t)x * ny + y) * nz * 3, big = ((size_t)x * eny + y) * enz * 3;
-  const T* s = src + (embed ? small : big);
-  T* d = dst + (embed ? big : small);
-  for (int q = threadIdx.x; q < 3 * nz; q += blockDim.x) d[q] = s[q];
+  if (embed) {
+    const bool in = x < nx && y < ny;
+    for (int q = threadIdx.x; q < 3 * enz; q += blockDim.x) dst[big + q] = (in && q < 3 * nz) ? src[small + q] : (T)0;
+  } else {
+    for (int q = threadIdx.x; q < 3 * nz; q += blockDim.x) dst[small + q] = src[big + q];
+  }
 }
 
 template <typename T>
-cudaError_t embed_copy_launch(const T* src, T* dst, int nx, int ny, int nz, int eny, int enz, int embed,
+cudaError_t embed_copy_launch(const T* src, T* dst, int nx, int ny, int nz, int enx, int eny, int enz, int embed,
                               cudaStream_t st) {
-  embed_copy_kernel<T><<<(unsigned)(nx * ny), 128, 0, st>>>(src, dst, ny, nz, eny, enz, embed);
+  const unsigned grid = embed ? (unsigned)(enx * eny) : (unsigned)(nx * ny);
+  embed_copy_kernel<T><<<grid, 128, 0, st>>>(src, dst, nx, ny, nz, eny, enz, embed);
   return cudaGetLastError();
 }
-template cudaError_t embed_copy_launch<float>(const float*, float*, int, int, int, int, int, int, cudaStream_t);
-template cudaError_t embed_copy_launch<double>(const double*, double*, int, int, int, int, int, int, cudaStream_t);
+template cudaError_t embed_copy_launch<float>(const float*, float*, int, int, int, int, int, int, int, cudaStream_t);
+template cudaError_t embed_copy_launch<double>(const double*, double*, int, int, int, int, int, int, int, cudaStream_t);
 
 template cudaError_t pointwise_launch<float>(int, const PwParams<float>&, const float*,
                                              const float*, float*, float*, float*, cudaStream_t,

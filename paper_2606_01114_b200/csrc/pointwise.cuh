@@ -45,10 +45,10 @@ template <typename T>
 cudaError_t scale_by_ms_launch(const T* m, const T* ms_cells, T* out, size_t ncell, cudaStream_t st);
 
 // Copies between the mesh [nx][ny][nz][3] and its embedding in the corner of [..][eny][enz][3]
-// (mm_api.cu "Embedding").  embed != 0: mesh -> embedded array (padding cells untouched);
-// embed == 0: embedded array -> mesh.
+// (mm_api.cu "Embedding") of enx x eny x enz cells.  embed != 0: mesh -> embedded array, the cells
+// outside the mesh written as zero; embed == 0: embedded array -> mesh.
 template <typename T>
-cudaError_t embed_copy_launch(const T* src, T* dst, int nx, int ny, int nz, int eny, int enz, int embed,
+cudaError_t embed_copy_launch(const T* src, T* dst, int nx, int ny, int nz, int enx, int eny, int enz, int embed,
                               cudaStream_t st);
 
 }  // namespace mm

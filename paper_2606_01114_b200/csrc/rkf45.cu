@@ -55,7 +55,10 @@ __global__ void __launch_bounds__(256) rkf_final_kernel(RkfState* __restrict__ s
       e += d.c[j] * k;
     }
     cand[q] = m0[q] + dt * s5;
-    emax = fmax(emax, fabs(dt * e));
+    // a non-finite estimate (blown-up state) must not vanish in fmax: it counts as +inf, which the
+    // controller rejects (err <= tol fails) and mm_rkf45_state reports
+    const T ae = fabs(dt * e);
+    emax = fmax(emax, ae == ae ? ae : (T)INFINITY);
   }
   // maximum is order-independent: the atomic keeps the result deterministic
 #pragma unroll

@@ -52,32 +52,57 @@ def test_create_validates_arguments(lib):
 
 def test_workspace_sizes_match_design(lib):
     """Config 4 fp32.  Generic passes: table 6*129*1024*1024*4 B, spectra 3*129*(512+1024)*512*8 B.
-    Fast path (selected automatically): octant table 6*513*513*130*4 B (kz pitch nz+2: 16-byte rows for bulk copies), A1 513*512*384*8 B,
-    A2 = kchunk (or 513) planes of 1024*384*8 B.  Field-sized scratch arrays: H_demag, two stage states,
+    Fast path (selected automatically): octant table 6*513*513*130*4 B (kz pitch nz+2: 16-byte rows for bulk
+    copies), A1 513*512*384*8 B, A2 513*1024*384*8 B.  Field-sized scratch arrays: H_demag, two stage states,
     RK4 accumulator, two host-call staging buffers, six RKF45 k arrays, M = Ms_i m for per-cell Ms."""
     fields = 13 * 512 * 512 * 128 * 3 * 4
     p, s = C.c_size_t(), C.c_size_t()
-    fast, kc = C.c_int(), C.c_int()
-    for path, kchunk, table, spectra in (
-            (1, 0, 6 * 129 * 1024 * 1024 * 4, 3 * 129 * (512 + 1024) * 512 * 8),
-            (0, 0, 6 * 513 * 513 * 130 * 4, 513 * 512 * 384 * 8 + 513 * 1024 * 384 * 8),
-            (2, 16, 6 * 513 * 513 * 130 * 4, 513 * 512 * 384 * 8 + 16 * 1024 * 384 * 8)):
+    path = C.c_int()
+    for want, table, spectra in (
+            (1, 6 * 129 * 1024 * 1024 * 4, 3 * 129 * (512 + 1024) * 512 * 8),
+            (0, 6 * 513 * 513 * 130 * 4, 513 * 512 * 384 * 8 + 513 * 1024 * 384 * 8),
+            (2, 6 * 513 * 513 * 130 * 4, 513 * 512 * 384 * 8 + 513 * 1024 * 384 * 8)):
         h = C.c_void_p()
         assert lib.mm_ctx_create(512, 512, 128, 4e-9, 4e-9, 4e-9, 0, C.byref(h)) == 0
-        assert lib.mm_ctx_set_path(h, path, kchunk) == 0
+        assert lib.mm_ctx_set_path(h, want) == 0
         lib.mm_ctx_workspace_bytes(h, C.byref(p), C.byref(s))
         assert table <= p.value < table + (1 << 20)
         assert spectra + fields <= s.value < spectra + fields + (1 << 20)
-        assert lib.mm_ctx_path(h, C.byref(fast), C.byref(kc)) == 0
-        assert fast.value == (0 if path == 1 else 1) and kc.value == kchunk
+        assert lib.mm_ctx_path(h, C.byref(path)) == 0
+        assert path.value == (0 if want == 1 else 1)
         lib.mm_ctx_destroy(h)
     h = C.c_void_p()
     assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 0, C.byref(h)) == 0
-    assert lib.mm_ctx_set_path(h, 2, 0) == 2          # fast kernels do not cover thin films
-    assert lib.mm_ctx_set_path(h, 3, 0) == 0          # the mixed-radix x-first kernels do
-    assert lib.mm_ctx_path(h, C.byref(fast), C.byref(kc)) == 0 and fast.value == 2
-    assert lib.mm_ctx_set_path(h, 4, 0) == 1
+    assert lib.mm_ctx_set_path(h, 2) == 2             # fast kernels do not cover thin films
+    assert lib.mm_ctx_set_path(h, 3) == 0             # the mixed-radix x-first kernels do
+    assert lib.mm_ctx_path(h, C.byref(path)) == 0 and path.value == 2
+    assert lib.mm_ctx_set_path(h, 4) == 1
     lib.mm_ctx_destroy(h)
     assert lib.mm_ctx_create(100, 25, 1, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 0
-    assert lib.mm_ctx_set_path(h, 3, 0) == 2          # one-cell axis: generic passes only
+    assert lib.mm_ctx_set_path(h, 3) == 2             # one-cell axis: generic passes only
     lib.mm_ctx_destroy(h)
+
+
+def test_kernel_names_follow_the_selected_path(lib):
+    lib.mm_ctx_kernel_name.restype = C.c_char_p
+    lib.mm_ctx_kernel_name.argtypes = [C.c_void_p, C.c_int]
+    h = C.c_void_p()
+    assert lib.mm_ctx_create(512, 512, 128, 4e-9, 4e-9, 4e-9, 0, C.byref(h)) == 0
+    names = [lib.mm_ctx_kernel_name(h, k).decode() for k in range(8)]
+    assert names == ["xf2_kernel", "yf2_kernel", "zp_fast_kernel", "yi2_kernel", "xi2_kernel", "pw_vec_kernel", "", ""]
+    lib.mm_ctx_destroy(h)
+    assert lib.mm_ctx_create(1024, 64, 256, 4e-9, 4e-9, 4e-9, 1, C.byref(h)) == 0
+    names = [lib.mm_ctx_kernel_name(h, k).decode() for k in range(5)]
+    assert names == ["xf_fast_kernel", "yf2_kernel", "zw_fast_kernel", "yi2_kernel", "xi_fast_kernel"]
+    lib.mm_ctx_destroy(h)
+    assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 0
+    assert lib.mm_ctx_kernel_name(h, 2) == b"xp_kernel" and lib.mm_ctx_kernel_name(h, 5) == b"pw_vec_kernel"
+    lib.mm_ctx_destroy(h)
+
+
+def test_oversized_axis_is_rejected_before_planning(lib):
+    """A length whose radix plan would overflow the stage array is refused by the range check, not by
+    writing past the plan (n = 2^27 needs nine radix-8 stages)."""
+    h = C.c_void_p()
+    assert lib.mm_ctx_create(1 << 27, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 2
+    assert lib.mm_ctx_create(16, 16, 1 << 27, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 2

@@ -1,6 +1,6 @@
-"""The x-first fast demag kernels (demag_fast.cu, K1..K5) against the oracle and against the
-generic z-first passes, through the C ABI: several tiles per pass, every supported radix plan,
-chunked and unchunked plane groups (with a ragged last chunk)."""
+"""The x-first fast demag kernels (demag_fast.cu, demag_fast2.cu; K1..K5) against the oracle and
+against the generic z-first passes, through the C ABI: several tiles per pass, every supported
+radix plan."""
 import numpy as np
 import pytest
 
@@ -25,21 +25,17 @@ def test_fast_demag_vs_oracle_fft(oracle, n, dt):
     P = make_problem(oracle, cfg, terms=1)
     ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
     md = to_dev(m)
-    results = []
-    for kchunk in (0, 7):
-        ctx = make_ctx(cfg, dt, terms=1, path=2, kchunk=kchunk)
-        assert ctx.path == (True, kchunk)
-        got = ctx.demag_field(md).cpu().numpy()
-        l2, mx = w.field_errors(got, ref)
-        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (kchunk, l2, mx)
-        assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())      # deterministic
-        results.append(got)
-        ctx.close()
-    assert np.array_equal(results[0], results[1])                           # chunking changes nothing
+    ctx = make_ctx(cfg, dt, terms=1, path=2)
+    assert ctx.path_name == "fast"
+    got = ctx.demag_field(md).cpu().numpy()
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+    assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())      # deterministic
+    ctx.close()
     # the generic passes agree with the fast kernels to rounding
     ctx = make_ctx(cfg, dt, terms=1, path=1)
-    assert ctx.path[0] is False
-    l2, mx = w.field_errors(ctx.demag_field(md).cpu().numpy(), results[0])
+    assert ctx.path_name == "generic"
+    l2, mx = w.field_errors(ctx.demag_field(md).cpu().numpy(), got)
     assert l2 <= TOL[dt], (l2, mx)
     ctx.close()
 
@@ -72,23 +68,19 @@ def test_fast_vs_direct_sum_sampled(oracle):
 @pytest.mark.parametrize("n", [(64, 64, 256), (128, 64, 256)])
 def test_fast_wide_pencil_nz256(oracle, n, dt):
     """nz = 256 (Pz = 512): the one-pencil-per-warp z kernel with the split second stage, fp32 and fp64;
-    several planes and mirror pairs per warp, ragged last chunk."""
+    several planes and mirror pairs per warp."""
     cfg = cfg_for(n)
     m, m64 = round_input(w.random_unit_vectors(606, n), dt)
     P = make_problem(oracle, cfg, terms=1)
     ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
     md = to_dev(m)
-    results = []
-    for kchunk in (0, 5):
-        ctx = make_ctx(cfg, dt, terms=1, path=2, kchunk=kchunk)
-        assert ctx.path == (True, kchunk)
-        got = ctx.demag_field(md).cpu().numpy()
-        l2, mx = w.field_errors(got, ref)
-        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (kchunk, l2, mx)
-        assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
-        results.append(got)
-        ctx.close()
-    assert np.array_equal(results[0], results[1])
+    ctx = make_ctx(cfg, dt, terms=1, path=2)
+    assert ctx.path_name == "fast"
+    got = ctx.demag_field(md).cpu().numpy()
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+    assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
+    ctx.close()
 
 
 def test_fast_path_rejects_meshes_it_does_not_cover():
@@ -98,5 +90,5 @@ def test_fast_path_rejects_meshes_it_does_not_cover():
         make_ctx(cfg_for((64, 64, 32)), "f64", terms=1, path=2)
     assert ei.value.status == 2
     ctx = make_ctx(cfg_for((64, 64, 32)), "f64", terms=1, path=0)
-    assert ctx.path[0] is False and ctx.path_name in ("generic", "embedded")
+    assert ctx.path_name in ("generic", "embedded")
     ctx.close()

@@ -101,16 +101,23 @@ def test_config3_dense_heff_and_rhs(oracle):
     ctx.close()
 
 
-@pytest.mark.parametrize("n", [(64, 64, 64), (128, 128, 128), (256, 256, 256), (1024, 1024, 64)])
-def test_sweep_meshes_sparse(oracle, n):
-    """Config 5 sweep sizes (incl. the 1024-point axes): sparse-source parity, fp32."""
+@pytest.mark.parametrize("dt", ["f32", "f64"])
+@pytest.mark.parametrize("n", w.SWEEP_MESHES)
+def test_sweep_meshes_sparse(oracle, n, dt):
+    """Config 5: every sweep size (64^3 ... 1024 x 1024 x 128, incl. the 1024-point axes), fp32 and
+    fp64: sparse-source parity against the oracle's literal Newell definition."""
     cfg = w.get_config(5).with_mesh(n)
     m64, ids = w.sparse_sources(cfg.seed, cfg.n, 4)
-    m, mref = round_input(m64, "f32")
+    m, mref = round_input(m64, dt)
     cells = np.unique(np.concatenate([w.sample_cells(cfg.seed, cfg.n, 60), ids]))
     ref = sparse_reference(oracle, cfg, ids, mref.reshape(-1, 3)[ids], cells)
-    ctx = make_ctx(cfg, "f32", terms=1)
-    got = ctx.demag_field(to_dev(m)).cpu().numpy().reshape(-1, 3)[cells]
+    ctx = make_ctx(cfg, dt, terms=1)
+    assert ctx.path_name == "fast"
+    md = to_dev(m)
+    del m, mref, m64
+    got = ctx.demag_field(md).reshape(-1, 3)[to_dev(cells)].cpu().numpy()
     l2, mx = w.field_errors(got, ref)
-    assert l2 <= TOL["f32"] and mx <= 10 * TOL["f32"], (l2, mx)
+    assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
     ctx.close()
+    del ctx, md
+    torch.cuda.empty_cache()

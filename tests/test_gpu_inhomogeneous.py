@@ -111,3 +111,27 @@ def test_cells_can_be_cleared_again(oracle):
     ref = make_problem(oracle, cfg).heff(m)
     l2, mx = w.field_errors(ctx.heff(to_dev(m)).cpu().numpy(), ref)
     assert l2 <= TOL["f64"]
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+def test_uniform_A_vacuum_neighbour_is_no_exchange_partner(oracle, dt):
+    """Ms_cells with zeros, A_cells = NULL (uniform A), arbitrary non-zero vectors stored in the vacuum cells:
+    the exchange field of the magnet does not see them (reading Q31: vacuum interface = mesh boundary)."""
+    n, d = (16, 12, 4), (3e-9, 3e-9, 2e-9)
+    cfg = cfg_for(n, d, terms=2)
+    Ms = np.full(n, 8e5)
+    Ms[8:] = 0.0
+    m, m64 = round_input(w.random_unit_vectors(909, n), dt)          # vacuum cells hold unit vectors too
+    Msr = Ms.astype(np_dtype(dt))
+    P = oracle.Problem(n=n, d=d, Ms=cfg.Ms, Aex=cfg.Aex, terms=2, Ms_cells=Msr.astype(np.float64))
+    ctx = make_ctx(cfg, dt)
+    ctx.set_material_cells(to_dev(Msr), None)
+    for got in (ctx.exchange_field(to_dev(m)), ctx.heff(to_dev(m))):
+        got = got.cpu().numpy()
+        l2, mx = w.field_errors(got, P.heff(m64))
+        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+        ref_magnet = oracle.exchange(d, cfg.Ms, cfg.Aex, m64[:8])    # the magnet alone, Neumann at x = 7
+        l2, mx = w.field_errors(got[:8], ref_magnet)
+        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+        assert np.all(got[8:] == 0.0)
+    ctx.close()

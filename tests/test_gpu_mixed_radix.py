@@ -1,8 +1,9 @@
 """Meshes whose sides are not powers of two: the paper's own workloads are
 100 x 25 x 1, N = 100, 350, 400 cubes and 512 x 512 x 90
-(PAPER.md:250).  The CUDA path pads to exactly 2n with radix 2/3/4/5/7/8 stages; references
-are the direct sum (O3), the oracle FFT path at its own power-of-two period (reading Q27) and,
-at full size, sparse sources and the trace rule."""
+(PAPER.md:250).  The CUDA path pads to exactly 2n; references are the direct sum (O3), the oracle
+FFT path at its own power-of-two period (reading Q27) and, at full size, sparse sources and the
+trace rule.  The cubes and the multilayer run the two-register-stage x-first kernels
+(demag_fast2.cu, demag_ztile.cu), everything else the generic run-time radix stages."""
 import numpy as np
 import pytest
 import torch
@@ -159,8 +160,14 @@ def test_mixed_radix_xfirst_kernels_explicitly(oracle, n, dt):
 
 def test_mixed_radix_selection():
     from paper_2606_01114_b200 import MMError
-    assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0).path_name == "generic"
+    # the paper's own meshes run the x-first register-stage kernels (two-stage plans 700 = 28 x 25, 800 = 32 x 25,
+    # 200 = 20 x 10, 180 = 20 x 9)
+    for n in ((350, 350, 350), (400, 400, 400), (100, 100, 100), (512, 512, 90), (350, 64, 90), (128, 400, 100)):
+        assert make_ctx(cfg_for(n, (4e-9,) * 3), "f64", terms=0).path_name == "fast", n
     assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0, path=3).path_name == "mixed"
+    assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0, path=1).path_name == "generic"
+    assert make_ctx(cfg_for((350, 350, 175), (4e-9,) * 3), "f64", terms=0).path_name == "embedded"  # in 350 x 350 x 256
+    assert make_ctx(cfg_for((350, 350, 20), (4e-9,) * 3), "f64", terms=0).path_name == "generic"    # 64 layers: 3.2 x the cells
     assert make_ctx(cfg_for((512, 512, 128), (4e-9,) * 3), "f32", terms=0).path_name == "fast"
     assert make_ctx(cfg_for((100, 25, 1), (5e-9, 5e-9, 3e-9)), "f64", terms=0).path_name == "generic"
     assert make_ctx(cfg_for((9, 15, 5), (1e-9,) * 3), "f64", terms=0).path_name == "generic"   # ny 3 nz odd
@@ -169,11 +176,12 @@ def test_mixed_radix_selection():
 
 
 @pytest.mark.parametrize("dt", ["f64", "f32"])
-@pytest.mark.parametrize("n", [(60, 50, 40), (40, 64, 100), (100, 100, 100)])
-def test_embedding_in_the_enclosing_power_of_two_mesh(oracle, n, dt):
-    """Automatic selection places these meshes in the corner of 64^3 / 64 x 64 x 128 / 128^3 and runs the
-    power-of-two kernels there (cells outside carry no magnetisation): dense parity vs the oracle FFT
-    path, agreement with the generic passes, H_eff + LLG through the cropped field, determinism."""
+@pytest.mark.parametrize("n", [(60, 50, 40), (40, 64, 96), (96, 100, 80)])
+def test_embedding_in_the_enclosing_mesh(oracle, n, dt):
+    """Automatic selection places these meshes in the corner of 64^3 / 64 x 64 x 100 / 100 x 100 x 90, the
+    smallest meshes the x-first kernels cover, and runs them there (cells outside carry no magnetisation):
+    dense parity vs the oracle FFT path, agreement with the generic passes, H_eff + LLG through the cropped
+    field, determinism."""
     cfg = cfg_for(n, (4e-9, 3e-9, 2e-9), terms=1 | 2 | 8, Hext=(1e4, 2e4, -3e4))
     m, m64 = round_input(w.random_unit_vectors(414, n), dt)
     P = make_problem(oracle, cfg)
@@ -184,6 +192,9 @@ def test_embedding_in_the_enclosing_power_of_two_mesh(oracle, n, dt):
     l2, mx = w.field_errors(got, oracle.demag_fft(P.Nhat, cfg.Ms, m64))
     assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
     assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
+    # the scratch workspace holds no state between calls (mm_b200.h): garbage in it changes nothing
+    ctx._ws[1].fill_(0x7F)
+    assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
     l2, mx = w.field_errors(ctx.llg_rhs(md).cpu().numpy(), P.llg_rhs(m64))
     assert l2 <= TOL[dt], (l2, mx)
     gen = make_ctx(cfg, dt, path=1)
@@ -193,3 +204,54 @@ def test_embedding_in_the_enclosing_power_of_two_mesh(oracle, n, dt):
     from paper_2606_01114_b200 import MMError
     with pytest.raises(MMError):
         ctx.nhat_export()
+
+
+# every mixed-radix two-stage plan along each axis it serves, with dense input and several tiles per pass
+PLAN_MESHES = [(100, 100, 100), (350, 64, 64), (64, 350, 64), (64, 64, 350), (400, 64, 90), (64, 400, 100),
+               (64, 64, 400)]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("n", PLAN_MESHES)
+def test_register_stage_plans_dense_vs_oracle_fft(oracle, n):
+    """700 = 28 x 25, 800 = 32 x 25, 200 = 20 x 10 along x, y and z and 180 = 20 x 9 along z: dense seeded input,
+    fp32 and fp64, element by element against the oracle FFT path (its own power-of-two period, reading Q27);
+    ragged last tiles (3 nz and ny 3 nz / 2 are not multiples of a tile row); agreement with the generic passes."""
+    cfg = cfg_for(n, (4e-9, 3e-9, 2e-9))
+    m32 = w.random_unit_vectors(515, n).astype(np.float32)
+    m64 = m32.astype(np.float64)                      # one input for both dtypes
+    P = make_problem(oracle, cfg, terms=1)
+    ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
+    for dt in ("f32", "f64"):
+        md = to_dev(m64.astype(np.float32 if dt == "f32" else np.float64))
+        ctx = make_ctx(cfg, dt, terms=1)
+        assert ctx.path_name == "fast"
+        got = ctx.demag_field(md).cpu().numpy()
+        l2, mx = w.field_errors(got, ref)
+        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (n, dt, l2, mx)
+        assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
+        ctx.close()
+        if n[0] * n[1] * n[2] <= 1 << 21:
+            gen = make_ctx(cfg, dt, terms=1, path=1)
+            l2, mx = w.field_errors(gen.demag_field(md).cpu().numpy(), got)
+            assert l2 <= TOL[dt], (n, dt, l2, mx)
+            gen.close()
+
+
+@pytest.mark.parametrize("dt", ["f64", "f32"])
+def test_register_stage_plans_nhat_and_direct_sum(oracle, dt):
+    """100 x 100 x 90 (plans 20 x 10, 20 x 10, 20 x 9): the exported N-hat octant against numpy's FFT of the
+    mirrored oracle table, and the field against sampled direct sums O3 (no FFT on the reference side)."""
+    n, d = (100, 100, 90), (5e-9, 4e-9, 3e-9)
+    cfg = cfg_for(n, d)
+    ctx = make_ctx(cfg, dt, terms=1)
+    assert ctx.path_name == "fast"
+    nh = ctx.nhat_export().cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(nh - mirrored_nhat(oracle, n, d))) < (5e-14 if dt == "f64" else 2e-7)
+    m, m64 = round_input(w.random_unit_vectors(616, n), dt)
+    cells = w.sample_cells(17, n, 50)
+    ref = oracle.demag_direct_sampled(oracle.newell_octant(n, d), cfg.Ms, m64, cells)
+    got = ctx.demag_field(to_dev(m)).cpu().numpy().reshape(-1, 3)[cells]
+    l2, mx = w.field_errors(got, ref)
+    assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (l2, mx)
+    ctx.close()

@@ -124,3 +124,44 @@ def test_rkf45_attempt_is_graph_capturable(oracle):
         ctx.close()
     assert outs[0][1] == outs[1][1] and outs[0][2] == outs[1][2]
     assert np.array_equal(outs[0][0], outs[1][0])
+
+
+def test_controller_state_survives_a_later_demag_init(oracle):
+    """mm_rkf45_init and mm_minimize_init BEFORE the first mm_demag_init (the header fixes no order): the
+    table upload of mm_demag_init must not clear the device-resident controller records."""
+    from paper_2606_01114_b200 import Context
+    cfg = w.get_config(1)
+    ctx = Context(cfg.n, cfg.d, dtype=torch.float64)
+    ctx.set_material(cfg.Ms, cfg.Aex, cfg.Ku, cfg.axis, cfg.alpha, cfg.gamma)
+    ctx.set_terms(cfg.terms)
+    ctx.rkf45_init(t0=0.0, dt0=2e-13, tol=1e-6, dt_min=0.0, dt_max=1e-12)
+    ctx.minimize_init(tau0=1e-7, tau_min=1e-10, tau_max=1e-4, tol=1e-9)
+    ctx.demag_init()
+    st = ctx.rkf45_state()
+    assert st["dt_next"] == 2e-13 and st["t"] == 0.0
+    m, m64 = round_input(cfg.initial_m(), "f64")
+    md = to_dev(m)
+    ctx.rkf45_step(md)
+    ref, err, acc, dt_next = make_problem(oracle, cfg).rkf45_step(m64, 2e-13, 1e-6, 0.0, 1e-12)
+    st = ctx.rkf45_state()
+    assert st["dt_last"] == 2e-13 and st["accepted"] == acc and abs(st["err"] - err) <= 1e-7 * err
+    assert w.traj_error(md.cpu().numpy(), ref) <= TRAJ_TOL["f64"]
+    md2 = to_dev(m)
+    ctx.minimize_step(md2)
+    n_it, tau, dm, conv = ctx.minimize_state()
+    assert n_it == 1 and tau == 1e-7 and dm > 0
+    ctx.close()
+
+
+def test_rkf45_non_finite_state_is_rejected_not_accepted():
+    """A blown-up state (NaN in m) must not read as err = 0 and be accepted with dt * 5."""
+    cfg = w.get_config(1)
+    ctx = make_ctx(cfg, "f64")
+    m = cfg.initial_m()
+    m[3, 4, 1, :] = np.nan
+    md = to_dev(m)
+    ctx.rkf45_init(t0=0.0, dt0=1e-13, tol=1e-6)
+    ctx.rkf45_step(md)
+    st = ctx.rkf45_state()
+    assert not st["accepted"] and st["err"] == np.inf and st["dt_next"] == pytest.approx(0.2e-13)
+    ctx.close()

@@ -16,25 +16,26 @@ import os, sys, json
 sys.path.insert(0, %r)
 import numpy as np, torch, torch.distributed as dist
 import workloads as w
+import bench                                                       # the functions under test are bench.py's own
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
 cfg = w.get_config(1)
-m = w.random_unit_vectors(cfg.seed + 1000 * rank, cfg.n)          # bench.py's per-rank seed rule
+m = w.random_unit_vectors(bench.rank_seed(cfg, rank), cfg.n)       # per-rank replica input
 ms_local = 3.0 + 2.0 * rank                                        # pretend device times
-t = torch.tensor([ms_local], dtype=torch.float64)
-dist.all_reduce(t, op=dist.ReduceOp.MAX)
+ms = bench.max_over_ranks(ms_local, dist, device="cpu")
 chk = torch.tensor([float(m.sum())], dtype=torch.float64)
 gathered = [torch.zeros(1, dtype=torch.float64) for _ in range(world)]
 dist.all_gather(gathered, chk)
 dist.barrier()
 if rank == 0:
-    value = world * cfg.ncell / (t.item() / 1e3)
-    print(json.dumps({"ms": t.item(), "value": value, "sums": [g.item() for g in gathered]}))
+    print(json.dumps({"ms": ms, "value": bench.job_value(world, cfg.ncell, ms),
+                      "sums": [g.item() for g in gathered]}))
 dist.destroy_process_group()
 """ % ROOT
 
 
 def test_replica_aggregation_gloo_world2(tmp_path):
+    """bench.py's own rank_seed / max_over_ranks / job_value under a world_size-2 gloo group."""
     script = tmp_path / "worker.py"
     script.write_text(WORKER)
     env = dict(os.environ, MASTER_ADDR="127.0.0.1")
@@ -49,6 +50,16 @@ def test_replica_aggregation_gloo_world2(tmp_path):
     assert out["sums"][0] != out["sums"][1]                  # independent replicas
 
 
+def test_rank_helpers_single_process():
+    sys.path.insert(0, ROOT)
+    import bench
+    import workloads as w
+    cfg = w.get_config(4)
+    assert bench.rank_seed(cfg, 0) == cfg.seed and bench.rank_seed(cfg, 3) == cfg.seed + 3000
+    assert bench.max_over_ranks(2.5) == 2.5                  # no process group: the local time
+    assert bench.job_value(8, 1000, 2.0) == 8 * 1000 / 2e-3
+
+
 def test_byte_model_matches_design():
     sys.path.insert(0, ROOT)
     import bench
@@ -56,9 +67,9 @@ def test_byte_model_matches_design():
     n = 512 * 512 * 128
     # 93*s B/cell up to the (nz+1)/nz and (n+1)^3 corrections (< 1.5 %)
     assert 93 * 4 * n <= total <= 1.015 * 93 * 4 * n
-    assert k["S6_pointwise"] == 9 * n * 4
+    assert k["S6"] == 9 * n * 4
     k1, t1 = bench.byte_model((128, 32, 1), 8)
-    assert k1["S1_zf"] == 3 * 4096 * 8 + 3 * 4096 * 16
+    assert k1["S1"] == 3 * 4096 * 8 + 3 * 4096 * 16
 
 
 def test_reference_arm_other_ranks_do_no_work():
