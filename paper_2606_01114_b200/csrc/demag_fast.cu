@@ -498,12 +498,16 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T sy, Cx<T>* X
 // NPW/2 mirror pairs (ky, Py - ky) of one plane, which share their Nhat rows.  Pencils and
 // table rows arrive by bulk asynchronous copies one task ahead; the pencil's own buffer is
 // the exchange buffer of its transforms once its samples sit in registers.
-template <typename T, int G, int WARPS, int MINB>
+// MASK: the mesh has nzd < 8 G layers (any period Pz >= 2 nzd - 1 gives the same linear convolution, reading
+// Q27): pencils in HBM hold 3 nzd values, the samples z >= nzd read as zero and only 3 nzd values go back.
+template <typename T, int G, int WARPS, int MINB, bool MASK>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
-               const uint16_t* __restrict__ posy, int ny, int kx0, int ntask) {
+               const uint16_t* __restrict__ posy, int ny, int kx0, int ntask, int nzd) {
   using C = ZpCfg<T, G>;
   constexpr int Q = C::Q, NPW = C::NPW;
+  const int qd = MASK ? 3 * nzd : Q;                                    // values of a pencil in HBM
+  const uint32_t pbytes = MASK ? (uint32_t)(qd * sizeof(Cx<T>)) : (uint32_t)C::pencil_bytes;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 3 * warp;  // stage 0, stage 1, table
@@ -536,12 +540,12 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     const int pair = task * (NPW / 2) + (p >> 1);
     const int plane = pair / ny, i = pair - plane * ny;
     const int ky = (p & 1) ? (i == 0 ? ny : Py - i) : i;
-    return A2 + ((size_t)plane * Py + posy[ky]) * Q;
+    return A2 + ((size_t)plane * Py + posy[ky]) * qd;
   };
   auto issue = [&](int task, int stage) {
-    mbar_expect_tx(bars + stage, NPW * C::pencil_bytes);
+    mbar_expect_tx(bars + stage, NPW * pbytes);
     for (int p = 0; p < NPW; ++p)
-      bulk_load(pbase + (stage * NPW + p) * Q, pencil_ptr(task, p), C::pencil_bytes, bars + stage);
+      bulk_load(pbase + (stage * NPW + p) * Q, pencil_ptr(task, p), pbytes, bars + stage);
   };
   // table rows of a task: ky = i for mirror pair i; the pair i = 0 (always the first of its
   // task) is (ky = 0, ky = ny) and needs the row ky = ny as well, in the extra slot
@@ -576,7 +580,8 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
 #pragma unroll
       for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) a[c][j] = pen[(t + G * j) * 3 + c];
+        for (int j = 0; j < 8; ++j)
+          a[c][j] = (!MASK || t + G * j < nzd) ? pen[(t + G * j) * 3 + c] : mk<T>((T)0, (T)0);
       __syncwarp();  // every sample is in registers: the pencil buffer becomes the exchange buffer
 #pragma unroll
       for (int c = 0; c < 3; ++c) zp_forward<T, G>(a[c], pen, tw, t, X[c]);
@@ -609,7 +614,7 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     __syncwarp();
     if (lane == 0) {
       for (int p = 0; p < NPW; ++p)
-        bulk_store(pencil_ptr(task, p), pbase + (stage * NPW + p) * Q, C::pencil_bytes);
+        bulk_store(pencil_ptr(task, p), pbase + (stage * NPW + p) * Q, pbytes);
       bulk_commit();
     }
   }
@@ -750,12 +755,14 @@ __device__ __forceinline__ void zw_multiply(const T* trow, int t, T sy, Cx<T>* X
 
 // A2 points at the first plane of the launch (kx = kx0).  A warp walks mirror pairs
 // pair = plane ny + i -> pencils ky = i and ky = (i == 0 ? ny : Py - i), one pencil per step.
-template <typename T>
+template <typename T, bool MASK>
 __global__ void __launch_bounds__(ZwCfg<T>::WARPS * 32, 1)
 zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
-               const uint16_t* __restrict__ posy, int ny, int kx0, int npair) {
+               const uint16_t* __restrict__ posy, int ny, int kx0, int npair, int nzd) {
   using C = ZwCfg<T>;
   constexpr int Q = C::Q;
+  const int qd = MASK ? 3 * nzd : Q;                                    // values of a pencil in HBM (see zp_fast_kernel)
+  const uint32_t pbytes = MASK ? (uint32_t)(qd * sizeof(Cx<T>)) : (uint32_t)C::pencil_bytes;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, t = threadIdx.x & 31;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 3 * warp;  // pencil buffer 0, 1, table
@@ -789,7 +796,7 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     const int pair = gw + (step >> 1) * stride;
     const int plane = pair / ny, i = pair - plane * ny;
     const int ky = (step & 1) ? (i == 0 ? ny : Py - i) : i;
-    return A2 + ((size_t)plane * Py + posy[ky]) * Q;
+    return A2 + ((size_t)plane * Py + posy[ky]) * qd;
   };
   // Nhat row of a step; -1 if it is the row already staged (second pencil of a pair i != 0)
   auto table_row = [&](int step) -> long long {
@@ -799,8 +806,8 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     return ((long long)(kx0 + plane) * (ny + 1) + ((step & 1) ? ny : i));
   };
   if (t == 0 && nsteps > 0) {
-    mbar_expect_tx(bars + 0, C::pencil_bytes);
-    bulk_load(pbase, pencil_ptr(0), C::pencil_bytes, bars + 0);
+    mbar_expect_tx(bars + 0, pbytes);
+    bulk_load(pbase, pencil_ptr(0), pbytes, bars + 0);
     mbar_expect_tx(bars + 2, C::table_bytes);
     bulk_load(trow, tab + (size_t)table_row(0) * 6 * C::OZP, C::table_bytes, bars + 2);
   }
@@ -811,8 +818,8 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     if (t == 0) {
       bulk_wait_read0();  // the previous step's store has finished reading the other buffer
       if (step + 1 < nsteps) {
-        mbar_expect_tx(bars + (buf ^ 1), C::pencil_bytes);
-        bulk_load(pbase + (buf ^ 1) * Q, pencil_ptr(step + 1), C::pencil_bytes, bars + (buf ^ 1));
+        mbar_expect_tx(bars + (buf ^ 1), pbytes);
+        bulk_load(pbase + (buf ^ 1) * Q, pencil_ptr(step + 1), pbytes, bars + (buf ^ 1));
       }
     }
     __syncwarp();
@@ -824,7 +831,8 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
 #pragma unroll
       for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) a[c][j] = pen[(t + 32 * j) * 3 + c];
+        for (int j = 0; j < 8; ++j)
+          a[c][j] = (!MASK || t + 32 * j < nzd) ? pen[(t + 32 * j) * 3 + c] : mk<T>((T)0, (T)0);
       __syncwarp();  // every sample is in registers: the pencil buffer becomes the exchange buffer
 #pragma unroll
       for (int c = 0; c < 3; ++c) zw_forward<T>(a[c], pen, tw, t, X[c]);
@@ -857,7 +865,7 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     fence_async_smem();
     __syncwarp();
     if (t == 0) {
-      bulk_store(pencil_ptr(step), pen, C::pencil_bytes);
+      bulk_store(pencil_ptr(step), pen, pbytes);
       bulk_commit();
     }
   }
@@ -866,12 +874,19 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
 
 // ---------------------------------------------------------------- host side
 
-// x, y: a two-stage plan (plan2.cuh) or the three-stage L = 1024 kernels; z: the warp-per-pencil kernels
-// (64, 128, 256) or the tile pass of demag_ztile.cu.  K1 / K5 move the real arrays as complex pairs.
-bool fast_supported(int nx, int ny, int nz) {
+// z: the warp-per-pencil kernels hold nzt = 64, 128 or 256 layers and take any 16 <= nz <= nzt (at most four
+// times the layers: K3 is a third of the work) whose pencils are multiples of 16 bytes (bulk copies); above
+// 256 layers the tile pass of demag_ztile.cu with a plan of its own.
+int fast_z_transform(int nz, size_t real_bytes) {
+  if (nz >= 16 && nz <= 256 && ((size_t)3 * nz * 2 * real_bytes) % 16 == 0) return nz <= 64 ? 64 : (nz <= 128 ? 128 : 256);
+  return ztile_supported(nz) ? nz : 0;
+}
+// x, y: a two-stage plan (plan2.cuh) or the three-stage L = 1024 kernels.  K1 / K5 move the real arrays as
+// complex pairs; the nzt = 64 kernel walks two mirror pairs of ky per task.
+bool fast_supported(int nx, int ny, int nz, size_t real_bytes) {
   auto okxy = [](int n) { return fast_two_stage(n) || n == 1024; };
-  return okxy(nx) && okxy(ny) && (nz == 64 || nz == 128 || nz == 256 || ztile_supported(nz)) &&
-         ((size_t)ny * 3 * nz) % 2 == 0;
+  const int nzt = fast_z_transform(nz, real_bytes);
+  return okxy(nx) && okxy(ny) && nzt != 0 && ((size_t)ny * 3 * nz) % 2 == 0 && !(nzt == 64 && ny % 2);
 }
 
 template <typename K> static cudaError_t opt_in_smem(K kernel, int bytes) {
@@ -935,25 +950,36 @@ template <typename T, int G>
 static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
   using C = ZpCfg<T, G>;
   constexpr int WARPS = C::WARPS, MINB = C::MINB;
-  cudaError_t e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB>, C::smem_bytes);
-  if (e != cudaSuccess) return e;
   const int ntask = (int)((size_t)nk * g.ny * 2 / C::NPW);
   int grid = sm_count() * MINB;
   if (grid * WARPS > ntask) grid = (ntask + WARPS - 1) / WARPS;
-  zp_fast_kernel<T, G, WARPS, MINB><<<grid, WARPS * 32, C::smem_bytes, st>>>(
-      b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask);
+  cudaError_t e;
+  if (g.nz == C::nz) {
+    if ((e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB, false>, C::smem_bytes)) != cudaSuccess) return e;
+    zp_fast_kernel<T, G, WARPS, MINB, false><<<grid, WARPS * 32, C::smem_bytes, st>>>(
+        b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz);
+  } else {   // fewer layers than the transform holds: masked reads, shorter copies
+    if ((e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB, true>, C::smem_bytes)) != cudaSuccess) return e;
+    zp_fast_kernel<T, G, WARPS, MINB, true><<<grid, WARPS * 32, C::smem_bytes, st>>>(
+        b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz);
+  }
   return cudaSuccess;
 }
 
 template <typename T>
 static cudaError_t launch_zw(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
   using C = ZwCfg<T>;
-  cudaError_t e = opt_in_smem(zw_fast_kernel<T>, C::smem_bytes);
-  if (e != cudaSuccess) return e;
   const int npair = nk * g.ny;
   int grid = sm_count();
   if (grid * C::WARPS > npair) grid = (npair + C::WARPS - 1) / C::WARPS;
-  zw_fast_kernel<T><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair);
+  cudaError_t e;
+  if (g.nz == C::nz) {
+    if ((e = opt_in_smem(zw_fast_kernel<T, false>, C::smem_bytes)) != cudaSuccess) return e;
+    zw_fast_kernel<T, false><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair, g.nz);
+  } else {
+    if ((e = opt_in_smem(zw_fast_kernel<T, true>, C::smem_bytes)) != cudaSuccess) return e;
+    zw_fast_kernel<T, true><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair, g.nz);
+  }
   return cudaSuccess;
 }
 
@@ -969,9 +995,9 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   e = b.two_y ? strided2_launch<T>(1, g, b, m, H, scale, st) : launch_yf<T, 1024>(g, b, 0, nplanes, st);
   if (e != cudaSuccess) return e;
   prof->mark(2, st);
-  if (g.nz == 256) e = launch_zw<T>(g, b, 0, nplanes, st);
-  else if (g.nz == 128) e = launch_zp<T, 16>(g, b, 0, nplanes, st);
-  else if (g.nz == 64) e = launch_zp<T, 8>(g, b, 0, nplanes, st);
+  if (g.nzt == 256) e = launch_zw<T>(g, b, 0, nplanes, st);
+  else if (g.nzt == 128) e = launch_zp<T, 16>(g, b, 0, nplanes, st);
+  else if (g.nzt == 64) e = launch_zp<T, 8>(g, b, 0, nplanes, st);
   else e = ztile_launch<T>(g, b, st);
   if (e != cudaSuccess) return e;
   prof->mark(3, st);

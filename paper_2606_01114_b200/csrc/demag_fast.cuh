@@ -12,12 +12,17 @@ namespace mm {
 
 struct FastGeom {
   int nx, ny, nz;
-  int Px, Py, Pz;  // 2 n_d
+  int nzt;         // the z transform runs at period Pz = 2 nzt, nzt >= nz (fast_z_transform)
+  int Px, Py, Pz;  // 2 nx, 2 ny, 2 nzt
   int Q;           // complex columns per (kx, y) row: 3 nz
 };
 
 // true if the fast kernels cover this mesh (otherwise the generic path of demag_passes.cu runs)
-bool fast_supported(int nx, int ny, int nz);
+bool fast_supported(int nx, int ny, int nz, size_t real_bytes);
+// nzt of the K3 kernel that serves nz (0: none): 64, 128, 256 for the warp-per-pencil kernels of demag_fast.cu,
+// which take any nz up to their capacity with the missing layers read as zero (the period 2 nzt >= 2 nz - 1
+// gives the same linear convolution, reading Q27), or nz itself for the tile pass of demag_ztile.cu.
+int fast_z_transform(int nz, size_t real_bytes);
 
 template <typename T> struct FastBufs {
   const Cx<T>* Wx;        // Wx[q] = exp(-2 pi i q / Px), q < Px

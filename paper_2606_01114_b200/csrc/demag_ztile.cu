@@ -57,9 +57,9 @@ template <typename T, int NZ> struct ZTile {
   static constexpr int SLOT = sizeof(T) == 4 ? 6 * OZS + ((4 - 6 * OZS % 32) + 32) % 32 : 6 * OZS;
   static constexpr int smem_bytes = tile_bytes + NPAIR * SLOT * (int)sizeof(T) + 16;
   // resident CTAs the kernel is compiled for: what shared memory admits and what the register file admits at
-  // the ~80 (fp32) / ~168 (fp64) registers the stages need without spilling
+  // ~80 (fp32) / ~144 (fp64) registers per thread (fp64, K1 = 32: a few hundred bytes of spills beat one CTA per SM)
   static constexpr int by_smem = (220 * 1024) / (smem_bytes + 1024);
-  static constexpr int by_regs = 65536 / ((sizeof(T) == 4 ? 80 : 168) * NT);
+  static constexpr int by_regs = 65536 / ((sizeof(T) == 4 ? 72 : 144) * NT);
   static constexpr int min_blocks = by_smem < by_regs ? (by_smem < 1 ? 1 : by_smem) : (by_regs < 1 ? 1 : by_regs);
   static_assert(K1 * K2 == Pz && K1 % 2 == 0 && NT <= 512 && NZ % 2 == 0, "plan");
   static_assert(pencil_bytes % 16 == 0 && tile_bytes % 16 == 0, "bulk copies move 16-byte multiples");

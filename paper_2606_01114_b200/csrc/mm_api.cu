@@ -48,6 +48,7 @@ struct mm_ctx {
   bool mixed = false;    // the mixed-radix x-first kernels of demag_mixed.cu are selected
   bool embed = false;    // the demag passes run on the enclosing power-of-two mesh dnx x dny x dnz
   int dnx = 0, dny = 0, dnz = 0;   // mesh of the demag passes (= nx, ny, nz unless embedded)
+  int nzt = 0;                      // x-first path: the z transform has period 2 nzt >= 2 dnz (demag_fast.cuh)
   bool xfirst() const { return fast || mixed; }   // x-first spectra and the octant table
   int path_pref = 0;     // 0 auto, 1 generic (demag_passes.cu), 2 fast required
   int want_bz = 0, want_by = 0, want_bk = 0;
@@ -100,10 +101,14 @@ static bool smooth7(int n) { return n >= 1 && make_plan(n).nstages >= 0; }
 // the paper's meshes (profiles/r01_v4_paper_meshes.md): about 4.6 in fp32, 3.1 in fp64.
 static bool embed_mesh(const mm_ctx* c, int* ex, int* ey, int* ez) {
   // smallest length the x-first kernels cover that holds n (0: none)
-  static const int kxy[] = {64, 100, 128, 256, 350, 400, 512, 1024}, kz[] = {64, 90, 100, 128, 256, 350, 400};
+  static const int kxy[] = {64, 100, 128, 256, 350, 400, 512, 1024};
   auto up = [](int n, const int* list, int count) { for (int i = 0; i < count; ++i) if (list[i] >= n) return list[i]; return 0; };
-  const int x = up(c->nx, kxy, 8), y = up(c->ny, kxy, 8), z = up(c->nz, kz, 7);
-  if (!x || !y || !z || !fast_supported(x, y, z)) return false;
+  const int x = up(c->nx, kxy, 8), y = up(c->ny, kxy, 8);
+  int z = 0;
+  const int zc[] = {c->nz, c->nz + 1, 16, 350, 400};
+  for (int v : zc)
+    if (!z && v >= c->nz && fast_z_transform(v, c->es)) z = v;
+  if (!x || !y || !z || !fast_supported(x, y, z, c->es)) return false;
   const double r = (double)x * y * z / ((double)c->nx * c->ny * c->nz);
   // fp64 with nz' = 256 runs the wide-pencil K3 at 0.34 of the roofline: a smaller margin
   if (r > (c->es == 4 ? 3.0 : (z == 256 ? 1.7 : 2.2))) return false;
@@ -114,9 +119,13 @@ static bool embed_mesh(const mm_ctx* c, int* ex, int* ey, int* ez) {
 static void plan_layout(mm_ctx* c) {
   DemagGeom& g = c->geom;
   c->dnx = c->nx; c->dny = c->ny; c->dnz = c->nz;
-  c->embed = c->path_pref == 0 && !fast_supported(c->nx, c->ny, c->nz) && embed_mesh(c, &c->dnx, &c->dny, &c->dnz);
+  c->embed = c->path_pref == 0 && !fast_supported(c->nx, c->ny, c->nz, c->es) && embed_mesh(c, &c->dnx, &c->dny, &c->dnz);
   g.nx = c->dnx; g.ny = c->dny; g.nz = c->dnz;
-  g.Px = padded(c->dnx); g.Py = padded(c->dny); g.Pz = padded(c->dnz);
+  c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->dnx, c->dny, c->dnz, c->es);
+  // x-first kernels: the z transform may be longer than 2 nz (any period >= 2 nz - 1 yields the same linear
+  // convolution, reading Q27); the table and the z twiddles follow the transform
+  c->nzt = c->fast ? fast_z_transform(c->dnz, c->es) : c->dnz;
+  g.Px = padded(c->dnx); g.Py = padded(c->dny); g.Pz = padded(c->nzt);
   g.Kz = g.Pz == 1 ? 1 : g.Pz / 2 + 1;
   g.px = make_plan(c->dnx); g.py = make_plan(c->dny); g.pz = make_plan(c->dnz);
   const size_t cs = 2 * c->es;
@@ -133,15 +142,14 @@ static void plan_layout(mm_ctx* c) {
   ig.Px = g.Px; ig.Py = g.Py; ig.Pz = g.Pz; ig.Kz = g.Kz;
   ig.ox = c->dnx == 1 ? 1 : c->dnx + 1;
   ig.oy = c->dny == 1 ? 1 : c->dny + 1;
-  ig.oz = c->dnz == 1 ? 1 : c->dnz + 1;
+  ig.oz = c->nzt == 1 ? 1 : c->nzt + 1;
   ig.ozp = (ig.oz + 1) / 2 * 2;
   ig.Bk = g.Bk;
-  c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->dnx, c->dny, c->dnz);
   // measured (profiles/r01_v4_paper_meshes.md): the mixed-radix x-first kernels only tie with the generic
   // z-first passes, so they are opt-in (path 3) until their stages move into registers
   c->mixed = c->path_pref == 3 && mixed_supported(c->dnx, c->dny, c->dnz, c->es);
   FastGeom& fg = c->fgeom;
-  fg.nx = c->dnx; fg.ny = c->dny; fg.nz = c->dnz;
+  fg.nx = c->dnx; fg.ny = c->dny; fg.nz = c->dnz; fg.nzt = c->nzt;
   fg.Px = g.Px; fg.Py = g.Py; fg.Pz = g.Pz;
   fg.Q = 3 * c->dnz;
   // persistent
@@ -260,7 +268,7 @@ mm_status mm_ctx_set_path(mm_ctx* ctx, int path) {
   if (path == 3 && !mixed_supported(ctx->nx, ctx->ny, ctx->nz, ctx->es))
     return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_path: the mixed-radix x-first kernels do not cover %dx%dx%d",
                 ctx->nx, ctx->ny, ctx->nz);
-  if (path == 2 && !fast_supported(ctx->nx, ctx->ny, ctx->nz))
+  if (path == 2 && !fast_supported(ctx->nx, ctx->ny, ctx->nz, ctx->es))
     return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_path: the fast kernels do not cover %dx%dx%d",
                 ctx->nx, ctx->ny, ctx->nz);
   ctx->path_pref = path;
@@ -380,7 +388,7 @@ const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
     switch (kind) {
       case 0: return two_x ? "xf2_kernel" : "xf_fast_kernel";
       case 1: return two_y ? "yf2_kernel" : "yf_fast_kernel";
-      case 2: return ctx->dnz == 256 ? "zw_fast_kernel" : (ztile_supported(ctx->dnz) ? "zt_kernel" : "zp_fast_kernel");
+      case 2: return ctx->nzt == 256 ? "zw_fast_kernel" : (ctx->nzt > 256 ? "zt_kernel" : "zp_fast_kernel");
       case 3: return two_y ? "yi2_kernel" : "yi_fast_kernel";
       default: return two_x ? "xi2_kernel" : "xi_fast_kernel";
     }
@@ -463,7 +471,7 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   const bool two_x = c->fast && fast_two_stage(c->dnx), two_y = c->fast && fast_two_stage(c->dny);
   if (two_x) fill_twiddles2<T>(host, c->off_t2x - small_off, c->dnx);
   if (two_y) fill_twiddles2<T>(host, c->off_t2y - small_off, c->dny);
-  if (c->fast && ztile_supported(c->dnz)) fill_twiddles2<T>(host, c->off_t2z - small_off, c->dnz);
+  if (c->fast && ztile_supported(c->nzt)) fill_twiddles2<T>(host, c->off_t2z - small_off, c->nzt);
   auto u16 = [&](size_t off) { return reinterpret_cast<uint16_t*>(host.data() + (off - small_off)); };
   for (int k = 0; k < g.Pz; ++k) {
     const int p = pos_of_freq(g.pz, k);
@@ -683,6 +691,9 @@ mm_status mm_demag_nhat_export(mm_ctx* ctx, void* out) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (!ctx->demag_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_demag_nhat_export: mm_demag_init not called");
   if (!out || ((uintptr_t)out & 15)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_demag_nhat_export: bad pointer");
+  if (ctx->fast && ctx->nzt != ctx->dnz)
+    return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_demag_nhat_export: this context transforms z with period %d, not 2 nz; "
+                "select the generic passes (mm_ctx_set_path 1) to export the table at period 2 n", 2 * ctx->nzt);
   if (ctx->embed)
     return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_demag_nhat_export: this context holds the table of the enclosing "
                 "%dx%dx%d mesh; select the generic passes (mm_ctx_set_path 1) to export the mesh's own table",

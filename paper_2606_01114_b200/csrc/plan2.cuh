@@ -15,18 +15,14 @@ template <> struct Plan2<100> { static constexpr int K1 = 20, K2 = 10; };
 template <> struct Plan2<350> { static constexpr int K1 = 28, K2 = 25; };
 template <> struct Plan2<400> { static constexpr int K1 = 32, K2 = 25; };
 
-// z only (demag_ztile.cu): 180 = 20 x 9 for the 512 x 512 x 90 multilayer
-template <> struct Plan2<90> { static constexpr int K1 = 20, K2 = 9; };
-
 #define MM_PLAN2_LENGTHS(X) X(64) X(128) X(256) X(512) X(100) X(350) X(400)   // strided passes (x, y)
-#define MM_ZTILE_LENGTHS(X) X(90) X(100) X(350) X(400)                        // tile pass (z)
+#define MM_ZTILE_LENGTHS(X) X(350) X(400)                                     // tile pass (z), nz > 256
 
 // run-time view of the table above; false if L has no plan
 inline bool plan2_of(int L, int* K1, int* K2) {
   switch (L) {
 #define MM_PLAN2_ROW(LL) case LL: *K1 = Plan2<LL>::K1; *K2 = Plan2<LL>::K2; return true;
     MM_PLAN2_LENGTHS(MM_PLAN2_ROW)
-    case 90: *K1 = Plan2<90>::K1; *K2 = Plan2<90>::K2; return true;
 #undef MM_PLAN2_ROW
     default: return false;
   }

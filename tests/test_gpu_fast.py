@@ -84,11 +84,35 @@ def test_fast_wide_pencil_nz256(oracle, n, dt):
 
 
 def test_fast_path_rejects_meshes_it_does_not_cover():
-    """nz = 32 is served by the generic passes; requiring the power-of-two kernels fails loudly."""
+    """Fewer than 16 layers are served by the generic passes; requiring the x-first kernels fails loudly."""
     from paper_2606_01114_b200 import MMError
     with pytest.raises(MMError) as ei:
-        make_ctx(cfg_for((64, 64, 32)), "f64", terms=1, path=2)
+        make_ctx(cfg_for((64, 64, 8)), "f64", terms=1, path=2)
     assert ei.value.status == 2
-    ctx = make_ctx(cfg_for((64, 64, 32)), "f64", terms=1, path=0)
+    ctx = make_ctx(cfg_for((64, 64, 8)), "f64", terms=1, path=0)
     assert ctx.path_name in ("generic", "embedded")
     ctx.close()
+
+
+# nz below the capacity of the warp-per-pencil z kernels (64, 128, 256 layers): the missing layers are read as
+# zero and the transform runs at period 2 nzt >= 2 nz - 1, the same linear convolution (reading Q27)
+MASKED = [(64, 64, 16), (64, 64, 50), (64, 128, 90), (128, 64, 100), (64, 64, 140), (64, 64, 200), (64, 64, 35)]
+
+
+@pytest.mark.parametrize("n", MASKED)
+def test_fast_fewer_layers_than_the_z_transform(oracle, n):
+    cfg = cfg_for(n)
+    m32 = w.random_unit_vectors(717, n).astype(np.float32)
+    m64 = m32.astype(np.float64)
+    P = make_problem(oracle, cfg, terms=1)
+    ref = oracle.demag_fft(P.Nhat, cfg.Ms, m64)
+    for dt in ("f32", "f64"):
+        ctx = make_ctx(cfg, dt, terms=1)
+        # an odd nz in fp32 gives pencils that are no multiple of 16 bytes: embedded in nz + 1 layers
+        assert ctx.path_name == ("embedded" if (dt == "f32" and n[2] % 2) else "fast"), (n, dt)
+        md = to_dev(m64.astype(np.float32 if dt == "f32" else np.float64))
+        got = ctx.demag_field(md).cpu().numpy()
+        l2, mx = w.field_errors(got, ref)
+        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (n, dt, l2, mx)
+        assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
+        ctx.close()

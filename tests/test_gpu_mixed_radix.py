@@ -161,13 +161,15 @@ def test_mixed_radix_xfirst_kernels_explicitly(oracle, n, dt):
 def test_mixed_radix_selection():
     from paper_2606_01114_b200 import MMError
     # the paper's own meshes run the x-first register-stage kernels (two-stage plans 700 = 28 x 25, 800 = 32 x 25,
-    # 200 = 20 x 10, 180 = 20 x 9)
+    # 200 = 20 x 10; z below 256 layers at period 128, 256 or 512)
     for n in ((350, 350, 350), (400, 400, 400), (100, 100, 100), (512, 512, 90), (350, 64, 90), (128, 400, 100)):
         assert make_ctx(cfg_for(n, (4e-9,) * 3), "f64", terms=0).path_name == "fast", n
     assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0, path=3).path_name == "mixed"
     assert make_ctx(cfg_for((350, 350, 350), (4e-9,) * 3), "f64", terms=0, path=1).path_name == "generic"
-    assert make_ctx(cfg_for((350, 350, 175), (4e-9,) * 3), "f64", terms=0).path_name == "embedded"  # in 350 x 350 x 256
-    assert make_ctx(cfg_for((350, 350, 20), (4e-9,) * 3), "f64", terms=0).path_name == "generic"    # 64 layers: 3.2 x the cells
+    assert make_ctx(cfg_for((350, 350, 175), (4e-9,) * 3), "f64", terms=0).path_name == "fast"      # z at period 512
+    assert make_ctx(cfg_for((350, 350, 300), (4e-9,) * 3), "f64", terms=0).path_name == "embedded"  # in 350^3
+    assert make_ctx(cfg_for((350, 350, 8), (4e-9,) * 3), "f64", terms=0).path_name == "embedded"    # in 16 layers
+    assert make_ctx(cfg_for((350, 350, 4), (4e-9,) * 3), "f64", terms=0).path_name == "generic"     # too thin
     assert make_ctx(cfg_for((512, 512, 128), (4e-9,) * 3), "f32", terms=0).path_name == "fast"
     assert make_ctx(cfg_for((100, 25, 1), (5e-9, 5e-9, 3e-9)), "f64", terms=0).path_name == "generic"
     assert make_ctx(cfg_for((9, 15, 5), (1e-9,) * 3), "f64", terms=0).path_name == "generic"   # ny 3 nz odd
@@ -240,14 +242,22 @@ def test_register_stage_plans_dense_vs_oracle_fft(oracle, n):
 
 @pytest.mark.parametrize("dt", ["f64", "f32"])
 def test_register_stage_plans_nhat_and_direct_sum(oracle, dt):
-    """100 x 100 x 90 (plans 20 x 10, 20 x 10, 20 x 9): the exported N-hat octant against numpy's FFT of the
-    mirrored oracle table, and the field against sampled direct sums O3 (no FFT on the reference side)."""
-    n, d = (100, 100, 90), (5e-9, 4e-9, 3e-9)
+    """100 x 100 x 64 (plans 20 x 10 along x and y): the exported N-hat octant against numpy's FFT of the
+    mirrored oracle table; 100 x 100 x 90 (z at period 256): the field against sampled direct sums O3 (no FFT
+    on the reference side); its table is not exported at period 2 n."""
+    from paper_2606_01114_b200 import MMError
+    n0, d = (100, 100, 64), (5e-9, 4e-9, 3e-9)
+    ctx = make_ctx(cfg_for(n0, d), dt, terms=1)
+    assert ctx.path_name == "fast"
+    nh = ctx.nhat_export().cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(nh - mirrored_nhat(oracle, n0, d))) < (5e-14 if dt == "f64" else 2e-7)
+    ctx.close()
+    n = (100, 100, 90)
     cfg = cfg_for(n, d)
     ctx = make_ctx(cfg, dt, terms=1)
     assert ctx.path_name == "fast"
-    nh = ctx.nhat_export().cpu().numpy().astype(np.float64)
-    assert np.max(np.abs(nh - mirrored_nhat(oracle, n, d))) < (5e-14 if dt == "f64" else 2e-7)
+    with pytest.raises(MMError):
+        ctx.nhat_export()
     m, m64 = round_input(w.random_unit_vectors(616, n), dt)
     cells = w.sample_cells(17, n, 50)
     ref = oracle.demag_direct_sampled(oracle.newell_octant(n, d), cfg.Ms, m64, cells)
