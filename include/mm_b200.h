@@ -132,6 +132,13 @@ mm_status mm_llg_rhs(mm_ctx *ctx, const void *m, void *dmdt);
 /* One classic RK4 step of size dt [s] followed by m <- m/|m|; m updated in place
  * (fixed-step stand-in for the paper's RKF45; reading Q14). */
 mm_status mm_rk_step(mm_ctx *ctx, void *m_inout, double dt);
+/* n_steps RK4 steps of size dt, as mm_rk_step n_steps times (bit-identical results), enqueued as replays of
+ * a CUDA graph of up to 128 steps that the library captures on first use and keeps until m_inout, dt or
+ * any setting of the context changes: small meshes are bound by launch latency (the paper's own diagnosis,
+ * "CPU dispatch latency", CUDA graphs named as the cure), and a replayed graph removes the
+ * per-kernel launch cost.  Asynchronous on the context's stream like mm_rk_step; must not itself be called
+ * while that stream is being captured (use mm_rk_step inside a capture of your own). */
+mm_status mm_rk_steps(mm_ctx *ctx, void *m_inout, double dt, int n_steps);
 
 /* Adaptive Runge-Kutta-Fehlberg 4(5) stepping (the integrator the paper supports;
  * the maximum error is reduced before the next step size is computed).  The controller state

@@ -64,6 +64,7 @@ def load_library():
         "mm_dmi_field": [vp, vp, vp],
         "mm_llg_rhs": [vp, vp, vp],
         "mm_rk_step": [vp, vp, dbl],
+        "mm_rk_steps": [vp, vp, dbl, i32],
         "mm_rkf45_init": [vp, dbl, dbl, dbl, dbl, dbl],
         "mm_rkf45_step": [vp, vp],
         "mm_rkf45_state": [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl),
@@ -255,6 +256,12 @@ class Context:
     def rk_step(self, m, dt):
         self._check(m)
         self._call("mm_rk_step", m.data_ptr(), float(dt))
+        return m
+
+    def rk_steps(self, m, dt, n):
+        """n RK4 steps as replays of a CUDA graph the library captures and caches (mm_rk_steps)."""
+        self._check(m)
+        self._call("mm_rk_steps", m.data_ptr(), float(dt), int(n))
         return m
 
     def rkf45_init(self, t0=0.0, dt0=1e-13, tol=1e-6, dt_min=0.0, dt_max=1.0):

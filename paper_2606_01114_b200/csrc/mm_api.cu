@@ -65,6 +65,14 @@ struct mm_ctx {
   bool rk_ready = false;
   bool bb_ready = false;
   unsigned long long launches = 0;
+  // mm_rk_steps: a captured chunk of RK4 steps, valid for (m, dt, chunk length, settings epoch)
+  unsigned long long epoch = 0;          // bumped by every call that changes what a step computes
+  cudaGraphExec_t rk_graph = nullptr;
+  cudaStream_t rk_capture_stream = nullptr;
+  void* rk_graph_m = nullptr;
+  double rk_graph_dt = 0;
+  int rk_graph_steps = 0;
+  unsigned long long rk_graph_epoch = 0, rk_graph_launches = 0;
   Prof prof;
   double prof_ms[Prof::kKinds] = {0};
   unsigned long long prof_cnt[Prof::kKinds] = {0};
@@ -227,6 +235,10 @@ mm_status mm_ctx_create(int nx, int ny, int nz, double dx, double dy, double dz,
 }
 
 mm_status mm_ctx_destroy(mm_ctx* ctx) {
+  if (ctx) {
+    if (ctx->rk_graph) cudaGraphExecDestroy(ctx->rk_graph);
+    if (ctx->rk_capture_stream) cudaStreamDestroy(ctx->rk_capture_stream);
+  }
   delete ctx;
   return MM_OK;
 }
@@ -234,6 +246,7 @@ mm_status mm_ctx_destroy(mm_ctx* ctx) {
 mm_status mm_ctx_set_stream(mm_ctx* ctx, void* cuda_stream) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -304,6 +317,7 @@ mm_status mm_ctx_set_workspace(mm_ctx* ctx, void* persistent, size_t pbytes, voi
   ctx->demag_ready = false;
   ctx->rk_ready = false;
   ctx->bb_ready = false;
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -323,12 +337,14 @@ mm_status mm_set_material(mm_ctx* ctx, double Ms, double Aex, double Ku, const d
   for (int i = 0; i < 3; ++i) ctx->axis[i] = u[i];
   ctx->alpha = alpha; ctx->gamma = gamma;
   ctx->have_material = true;
+  ++ctx->epoch;
   return MM_OK;
 }
 
 mm_status mm_set_zeeman(mm_ctx* ctx, const double Hext[3]) {
   if (!ctx || !Hext) return MM_ERR_INVALID_ARG;
   for (int i = 0; i < 3; ++i) ctx->Hext[i] = Hext[i];
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -339,6 +355,7 @@ mm_status mm_set_dmi(mm_ctx* ctx, double D, const double e[9]) {
   if (!std::isfinite(D)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_dmi: D must be finite");
   ctx->Ddmi = D;
   for (int i = 0; i < 9; ++i) ctx->edmi[i] = e[i];
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -350,6 +367,7 @@ mm_status mm_set_stt(mm_ctx* ctx, const double p[3], double a_damp, double a_fie
   for (int i = 0; i < 3; ++i) ctx->stt_p[i] = p[i] / n;
   ctx->stt_damp = a_damp;
   ctx->stt_field = a_field;
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -359,6 +377,7 @@ mm_status mm_set_material_cells(mm_ctx* ctx, const void* Ms_cells, const void* A
     return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_material_cells: device pointers must be 16-byte aligned");
   ctx->ms_cells = Ms_cells;
   ctx->a_cells = A_cells;
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -366,6 +385,7 @@ mm_status mm_set_terms(mm_ctx* ctx, unsigned term_mask) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (term_mask & ~63u) return fail(ctx, MM_ERR_INVALID_ARG, "mm_set_terms: unknown term bits 0x%x", term_mask);
   ctx->terms = term_mask;
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -402,6 +422,7 @@ const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
 mm_status mm_ctx_set_profiling(mm_ctx* ctx, int enable) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   ctx->prof.on = enable != 0;
+  ++ctx->epoch;
   return MM_OK;
 }
 
@@ -764,6 +785,68 @@ mm_status mm_rk_step(mm_ctx* ctx, void* m_inout, double dt) {
   if (!(dt > 0)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_rk_step: dt must be positive");
   if ((s = need_ready(ctx, "mm_rk_step", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
   return ctx->dtype == MM_F32 ? rk_t<float>(ctx, m_inout, dt) : rk_t<double>(ctx, m_inout, dt);
+}
+
+// Captures `steps` RK4 steps on m into an executable graph (on a stream of the library's own: the legacy
+// default stream cannot be captured).
+static mm_status rk_capture(mm_ctx* ctx, void* m, double dt, int steps) {
+  if (ctx->rk_graph) { cudaGraphExecDestroy(ctx->rk_graph); ctx->rk_graph = nullptr; }
+  cudaError_t e = cudaSuccess;
+  if (!ctx->rk_capture_stream) e = cudaStreamCreateWithFlags(&ctx->rk_capture_stream, cudaStreamNonBlocking);
+  if (e != cudaSuccess) return cuda_fail(ctx, "mm_rk_steps: stream", e);
+  cudaStream_t user = ctx->stream;
+  const unsigned long long l0 = ctx->launches;
+  ctx->stream = ctx->rk_capture_stream;
+  e = cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal);
+  mm_status s = e == cudaSuccess ? MM_OK : cuda_fail(ctx, "mm_rk_steps: begin capture", e);
+  for (int i = 0; i < steps && s == MM_OK; ++i)
+    s = ctx->dtype == MM_F32 ? rk_t<float>(ctx, m, dt) : rk_t<double>(ctx, m, dt);
+  cudaGraph_t graph = nullptr;
+  if (e == cudaSuccess) {
+    const cudaError_t e2 = cudaStreamEndCapture(ctx->stream, &graph);
+    if (s == MM_OK && e2 != cudaSuccess) s = cuda_fail(ctx, "mm_rk_steps: end capture", e2);
+  }
+  ctx->stream = user;
+  ctx->rk_graph_launches = ctx->launches - l0;   // kernels one replay enqueues
+  ctx->launches = l0;
+  if (s == MM_OK) {
+    e = cudaGraphInstantiate(&ctx->rk_graph, graph, 0);
+    if (e != cudaSuccess) s = cuda_fail(ctx, "mm_rk_steps: instantiate", e);
+  }
+  if (graph) cudaGraphDestroy(graph);
+  if (s != MM_OK) { ctx->rk_graph = nullptr; return s; }
+  ctx->rk_graph_m = m; ctx->rk_graph_dt = dt; ctx->rk_graph_steps = steps; ctx->rk_graph_epoch = ctx->epoch;
+  return MM_OK;
+}
+
+mm_status mm_rk_steps(mm_ctx* ctx, void* m_inout, double dt, int n_steps) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_rk_steps", m_inout, m_inout)) != MM_OK) return s;
+  if (!(dt > 0) || n_steps < 0) return fail(ctx, MM_ERR_INVALID_ARG, "mm_rk_steps: need dt > 0 and n_steps >= 0");
+  if ((s = need_ready(ctx, "mm_rk_steps", ctx->terms & MM_TERM_DEMAG)) != MM_OK) return s;
+  constexpr int kChunk = 128;
+  int left = n_steps;
+  if (ctx->prof.on) {   // per-kernel events cannot be recorded from a graph: plain launches
+    for (; left > 0 && s == MM_OK; --left) s = mm_rk_step(ctx, m_inout, dt);
+    return s;
+  }
+  while (left > 0) {
+    const int chunk = left < kChunk ? left : kChunk;
+    const bool have = ctx->rk_graph && ctx->rk_graph_m == m_inout && ctx->rk_graph_dt == dt &&
+                      ctx->rk_graph_steps == chunk && ctx->rk_graph_epoch == ctx->epoch;
+    // a short tail that would evict a cached full chunk runs as plain steps instead
+    if (!have && chunk < kChunk && ctx->rk_graph && ctx->rk_graph_steps == kChunk && chunk < 16) {
+      for (; left > 0 && s == MM_OK; --left) s = mm_rk_step(ctx, m_inout, dt);
+      return s;
+    }
+    if (!have && (s = rk_capture(ctx, m_inout, dt, chunk)) != MM_OK) return s;
+    const cudaError_t e = cudaGraphLaunch(ctx->rk_graph, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "mm_rk_steps: graph launch", e);
+    ctx->launches += ctx->rk_graph_launches;
+    left -= chunk;
+  }
+  return MM_OK;
 }
 
 }  // extern "C"
