@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmm_b200.so")
-SOURCES = ["mm_api.cu", "demag_passes.cu", "demag_fast.cu", "demag_fast2.cu", "demag_ztile.cu", "demag_mixed.cu", "demag_init.cu", "pointwise.cu", "rkf45.cu", "bb.cu"]
+SOURCES = ["mm_api.cu", "demag_passes.cu", "demag_fast.cu", "demag_fast2.cu", "demag_ztile.cu", "demag_tma.cu", "demag_mixed.cu", "demag_init.cu", "pointwise.cu", "rkf45.cu", "bb.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

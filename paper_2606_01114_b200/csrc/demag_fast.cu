@@ -992,7 +992,9 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   e = b.two_x ? strided2_launch<T>(0, g, b, m, H, scale, st) : launch_xf<T, 1024>(g, b, m, st);
   if (e != cudaSuccess) return e;
   prof->mark(1, st);
-  e = b.two_y ? strided2_launch<T>(1, g, b, m, H, scale, st) : launch_yf<T, 1024>(g, b, 0, nplanes, st);
+  e = b.two_y ? strided_tma_launch<T>(1, g, b, st) : cudaErrorNotSupported;
+  if (e == cudaErrorNotSupported)
+    e = b.two_y ? strided2_launch<T>(1, g, b, m, H, scale, st) : launch_yf<T, 1024>(g, b, 0, nplanes, st);
   if (e != cudaSuccess) return e;
   prof->mark(2, st);
   if (g.nzt == 256) e = launch_zw<T>(g, b, 0, nplanes, st);
@@ -1001,7 +1003,9 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   else e = ztile_launch<T>(g, b, st);
   if (e != cudaSuccess) return e;
   prof->mark(3, st);
-  e = b.two_y ? strided2_launch<T>(3, g, b, m, H, scale, st) : launch_yi<T, 1024>(g, b, 0, nplanes, st);
+  e = b.two_y ? strided_tma_launch<T>(3, g, b, st) : cudaErrorNotSupported;
+  if (e == cudaErrorNotSupported)
+    e = b.two_y ? strided2_launch<T>(3, g, b, m, H, scale, st) : launch_yi<T, 1024>(g, b, 0, nplanes, st);
   if (e != cudaSuccess) return e;
   prof->mark(4, st);
   e = b.two_x ? strided2_launch<T>(4, g, b, m, H, scale, st) : launch_xi<T, 1024>(g, b, H, scale, st);

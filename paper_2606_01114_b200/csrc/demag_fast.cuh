@@ -53,6 +53,12 @@ cudaError_t strided2_launch(int which, const FastGeom& g, const FastBufs<T>& b, 
 bool fast_two_stage(int L);                      // the two-stage kernels cover length L (both precisions)
 void fast2_plan(int L, int* K1, int* K2);        // P = 2L = K1 K2 (plan2.cuh; 0, 0 if L has no plan)
 
+// K2 / K4 with their tiles moved by 2D TMA boxes (demag_tma.cu); which: 1 = K2, 3 = K4.  Returns
+// cudaErrorNotSupported when the driver entry point, the plan or the alignment is missing or MM_B200_TMA=0 is
+// set: the caller then runs the LDG / STG kernels of demag_fast2.cu.
+template <typename T>
+cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st);
+
 // Host helpers for the tables above (plan order of the fast kernels).
 int fast_pos_logical(int L, int k);   // row of frequency k < 2L in the [even half | odd half] layout
 int fast_swizzle(int L, int row);     // shared-memory row of logical row
