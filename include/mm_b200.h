@@ -224,6 +224,18 @@ mm_status mm_ctx_set_tiles(mm_ctx *ctx, int bz, int by, int bk);
 mm_status mm_ctx_set_path(mm_ctx *ctx, int path);
 mm_status mm_ctx_path(const mm_ctx *ctx, int *path);
 
+/* Slab decomposition of the demag convolution over `ranks` ranks (1 .. 8; 0 = off), the paper's own scheme
+ * (PAPER.md:30 "sharded into contiguous slabs along the x-axis", :47 "all-to-all transpose", :227), emulated on
+ * ONE device: rank r owns the x planes [r nx/R, (r+1) nx/R) of m and H and the rows ky in [r rpr, (r+1) rpr),
+ * rpr = ceil((ny + 1) / R), of the half spectrum and of the Fourier-space tensor (the paper's y-sharded kernel).
+ * The passes run y (r2c) -> x -> z . Nhat . z^-1 -> x^-1 -> y^-1 (c2r); the forward y pass of a rank stores every
+ * spectrum row straight into the buffer of its owner and the inverse y pass gathers them the same way, through
+ * a per-rank pointer table: on several GPUs those are peer pointers and the two all-to-all transposes are these
+ * stores and loads.  Needs a mesh the x-first kernels cover with two-stage plans along
+ * x and y; call before mm_ctx_workspace_bytes / mm_ctx_set_workspace.  The result equals the unsharded path's
+ * to rounding (different transform order). */
+mm_status mm_ctx_set_slabs(mm_ctx *ctx, int ranks);
+
 /* Last error text of this context (or of the last failed mm_ctx_create if ctx is NULL).
  * Not thread-safe. */
 const char *mm_last_error(const mm_ctx *ctx);

@@ -80,6 +80,7 @@ def load_library():
         "mm_ctx_launch_count": [vp, C.POINTER(C.c_ulonglong)],
         "mm_ctx_set_tiles": [vp, i32, i32, i32],
         "mm_ctx_set_path": [vp, i32],
+        "mm_ctx_set_slabs": [vp, i32],
         "mm_ctx_path": [vp, C.POINTER(i32)],
         "mm_ctx_set_profiling": [vp, i32],
         "mm_ctx_kernel_times": [vp, i32, C.POINTER(dbl), C.POINTER(C.c_ulonglong)],
@@ -108,7 +109,7 @@ class Context:
     """One mesh on one GPU (mm_ctx).  Mirrors Mesh(n, dx) + State.material + the field-term
     list of the paper's scripts."""
 
-    def __init__(self, n, d, dtype=torch.float32, device="cuda:0", tiles=None, allocate=True, path=0):
+    def __init__(self, n, d, dtype=torch.float32, device="cuda:0", tiles=None, allocate=True, path=0, slabs=0):
         self.lib = load_library()
         self.n = tuple(int(v) for v in n)
         self.d = tuple(float(v) for v in d)
@@ -122,6 +123,8 @@ class Context:
             self._call("mm_ctx_set_tiles", *[int(t) for t in tiles])
         if path:
             self._call("mm_ctx_set_path", int(path))
+        if slabs:
+            self._call("mm_ctx_set_slabs", int(slabs))
         self._ws = None
         if allocate:
             self.allocate()

@@ -467,10 +467,11 @@ __device__ __forceinline__ void zp_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw,
 }
 
 // Hhat = Nhat mhat at the 16 frequencies of this lane.  trow: the (kx, ky) table row in shared
-// memory, [6][OZP]; sy = -1 on the mirrored ky half (N_xy, N_yz are odd in ky), the kz mirror
-// (N_xz, N_yz odd in kz) is resolved per frequency.
+// memory, [6][OZP]; s3, s4, s5: signs of N_xy, N_xz, N_yz on the mirrored half of the row axis (ky rows:
+// N_xy, N_yz are odd in ky, so (s, 1, s); kx rows of the slab layout: N_xy, N_xz odd in kx, (s, s, 1)); the kz
+// mirror (N_xz, N_yz odd in kz) is resolved per frequency.
 template <typename T, int G>
-__device__ __forceinline__ void zp_multiply(const T* trow, int t, T sy, Cx<T>* X0, Cx<T>* X1,
+__device__ __forceinline__ void zp_multiply(const T* trow, int t, T s3, T s4, T s5, Cx<T>* X0, Cx<T>* X1,
                                             Cx<T>* X2) {
   using C = ZpCfg<T, G>;
 #pragma unroll
@@ -484,8 +485,8 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T sy, Cx<T>* X
     else mir = kz > C::nz;
     const int idx = mir ? C::Pz - kz : kz;
     const T nxx = trow[idx], nyy = trow[C::OZP + idx], nzz = trow[2 * C::OZP + idx],
-            nxy = sy * trow[3 * C::OZP + idx];
-    T nxz = trow[4 * C::OZP + idx], nyz = sy * trow[5 * C::OZP + idx];
+            nxy = s3 * trow[3 * C::OZP + idx];
+    T nxz = s4 * trow[4 * C::OZP + idx], nyz = s5 * trow[5 * C::OZP + idx];
     if (mir) { nxz = -nxz; nyz = -nyz; }
     const Cx<T> a = X0[f], b = X1[f], c = X2[f];
     X0[f] = mk<T>(nxx * a.x + nxy * b.x + nxz * c.x, nxx * a.y + nxy * b.y + nxz * c.y);
@@ -498,12 +499,13 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T sy, Cx<T>* X
 // NPW/2 mirror pairs (ky, Py - ky) of one plane, which share their Nhat rows.  Pencils and
 // table rows arrive by bulk asynchronous copies one task ahead; the pencil's own buffer is
 // the exchange buffer of its transforms once its samples sit in registers.
+// xm != 0 (MASK variant only): the rows of a plane are kx, not ky (slab layout, demag_slab.cuh).
 // MASK: the mesh has nzd < 8 G layers (any period Pz >= 2 nzd - 1 gives the same linear convolution, reading
 // Q27): pencils in HBM hold 3 nzd values, the samples z >= nzd read as zero and only 3 nzd values go back.
 template <typename T, int G, int WARPS, int MINB, bool MASK>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
-               const uint16_t* __restrict__ posy, int ny, int kx0, int ntask, int nzd) {
+               const uint16_t* __restrict__ posy, int ny, int kx0, int ntask, int nzd, int xm) {
   using C = ZpCfg<T, G>;
   constexpr int Q = C::Q, NPW = C::NPW;
   const int qd = MASK ? 3 * nzd : Q;                                    // values of a pencil in HBM
@@ -593,9 +595,10 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
       // the odd pencil of pair i is ky = Py - i (row i, odd components negated), of pair 0 ky = ny
       const bool nyq = (pw & 1) && i == 0;
       const T sy = ((pw & 1) && i != 0) ? (T)-1 : (T)1;
+      const T s4 = (MASK && xm) ? sy : (T)1, s5 = (MASK && xm) ? (T)1 : sy;
       mbar_wait(bars + 2, it & 1);
       const T* trow = tbase + (nyq ? NPW / 2 : (pw >> 1)) * 6 * C::OZP;
-      zp_multiply<T, G>(trow, t, sy, X[0], X[1], X[2]);
+      zp_multiply<T, G>(trow, t, sy, s4, s5, X[0], X[1], X[2]);
       __syncwarp();
       if (lane == 0 && more) issue_table(task + stride);
     }
@@ -732,7 +735,7 @@ __device__ __forceinline__ void zw_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw,
 }
 
 template <typename T>
-__device__ __forceinline__ void zw_multiply(const T* trow, int t, T sy, Cx<T>* X0, Cx<T>* X1, Cx<T>* X2) {
+__device__ __forceinline__ void zw_multiply(const T* trow, int t, T s3, T s4, T s5, Cx<T>* X0, Cx<T>* X1, Cx<T>* X2) {
   using C = ZwCfg<T>;
 #pragma unroll
   for (int u = 0; u < 16; ++u) {
@@ -743,8 +746,8 @@ __device__ __forceinline__ void zw_multiply(const T* trow, int t, T sy, Cx<T>* X
     else mir = t > 0;
     const int idx = mir ? C::Pz - kz : kz;
     const T nxx = trow[idx], nyy = trow[C::OZP + idx], nzz = trow[2 * C::OZP + idx],
-            nxy = sy * trow[3 * C::OZP + idx];
-    T nxz = trow[4 * C::OZP + idx], nyz = sy * trow[5 * C::OZP + idx];
+            nxy = s3 * trow[3 * C::OZP + idx];
+    T nxz = s4 * trow[4 * C::OZP + idx], nyz = s5 * trow[5 * C::OZP + idx];
     if (mir) { nxz = -nxz; nyz = -nyz; }
     const Cx<T> a = X0[u], b = X1[u], c = X2[u];
     X0[u] = mk<T>(nxx * a.x + nxy * b.x + nxz * c.x, nxx * a.y + nxy * b.y + nxz * c.y);
@@ -758,7 +761,7 @@ __device__ __forceinline__ void zw_multiply(const T* trow, int t, T sy, Cx<T>* X
 template <typename T, bool MASK>
 __global__ void __launch_bounds__(ZwCfg<T>::WARPS * 32, 1)
 zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
-               const uint16_t* __restrict__ posy, int ny, int kx0, int npair, int nzd) {
+               const uint16_t* __restrict__ posy, int ny, int kx0, int npair, int nzd, int xm) {
   using C = ZwCfg<T>;
   constexpr int Q = C::Q;
   const int qd = MASK ? 3 * nzd : Q;                                    // values of a pencil in HBM (see zp_fast_kernel)
@@ -841,8 +844,9 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
       const int pair = gw + (step >> 1) * stride;
       const int i = pair % ny;
       const T sy = ((step & 1) && i != 0) ? (T)-1 : (T)1;
+      const T s4 = (MASK && xm) ? sy : (T)1, s5 = (MASK && xm) ? (T)1 : sy;
       if (table_row(step) >= 0) { mbar_wait(bars + 2, tphase); tphase ^= 1; }
-      zw_multiply<T>(trow, t, sy, X[0], X[1], X[2]);
+      zw_multiply<T>(trow, t, sy, s4, s5, X[0], X[1], X[2]);
       __syncwarp();
       if (t == 0 && step + 1 < nsteps) {
         const long long row = table_row(step + 1);
@@ -947,41 +951,52 @@ static cudaError_t launch_yi(const FastGeom& g, const FastBufs<T>& b, int k0, in
   return cudaSuccess;
 }
 template <typename T, int G>
-static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
+static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, int xm, cudaStream_t st) {
   using C = ZpCfg<T, G>;
   constexpr int WARPS = C::WARPS, MINB = C::MINB;
   const int ntask = (int)((size_t)nk * g.ny * 2 / C::NPW);
   int grid = sm_count() * MINB;
   if (grid * WARPS > ntask) grid = (ntask + WARPS - 1) / WARPS;
   cudaError_t e;
-  if (g.nz == C::nz) {
+  if (g.nz == C::nz && !xm) {
     if ((e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB, false>, C::smem_bytes)) != cudaSuccess) return e;
     zp_fast_kernel<T, G, WARPS, MINB, false><<<grid, WARPS * 32, C::smem_bytes, st>>>(
-        b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz);
+        b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz, 0);
   } else {   // fewer layers than the transform holds: masked reads, shorter copies
     if ((e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB, true>, C::smem_bytes)) != cudaSuccess) return e;
     zp_fast_kernel<T, G, WARPS, MINB, true><<<grid, WARPS * 32, C::smem_bytes, st>>>(
-        b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz);
+        b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz, xm);
   }
   return cudaSuccess;
 }
 
 template <typename T>
-static cudaError_t launch_zw(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, cudaStream_t st) {
+static cudaError_t launch_zw(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, int xm, cudaStream_t st) {
   using C = ZwCfg<T>;
   const int npair = nk * g.ny;
   int grid = sm_count();
   if (grid * C::WARPS > npair) grid = (npair + C::WARPS - 1) / C::WARPS;
   cudaError_t e;
-  if (g.nz == C::nz) {
+  if (g.nz == C::nz && !xm) {
     if ((e = opt_in_smem(zw_fast_kernel<T, false>, C::smem_bytes)) != cudaSuccess) return e;
-    zw_fast_kernel<T, false><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair, g.nz);
+    zw_fast_kernel<T, false><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair, g.nz, 0);
   } else {
     if ((e = opt_in_smem(zw_fast_kernel<T, true>, C::smem_bytes)) != cudaSuccess) return e;
-    zw_fast_kernel<T, true><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair, g.nz);
+    zw_fast_kernel<T, true><<<grid, C::WARPS * 32, C::smem_bytes, st>>>(b.A2, b.table, b.Wz, b.posy, g.ny, k0, npair, g.nz, xm);
   }
   return cudaSuccess;
 }
+
+// K3 on nk planes of b.A2 starting at table plane k0; xm: the rows of a plane are kx (slab layout)
+template <typename T>
+cudaError_t k3_launch(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, int xm, cudaStream_t st) {
+  if (g.nzt == 256) return launch_zw<T>(g, b, k0, nk, xm, st);
+  if (g.nzt == 128) return launch_zp<T, 16>(g, b, k0, nk, xm, st);
+  if (g.nzt == 64) return launch_zp<T, 8>(g, b, k0, nk, xm, st);
+  return ztile_launch<T>(g, b, k0, nk, xm, st);
+}
+template cudaError_t k3_launch<float>(const FastGeom&, const FastBufs<float>&, int, int, int, cudaStream_t);
+template cudaError_t k3_launch<double>(const FastGeom&, const FastBufs<double>&, int, int, int, cudaStream_t);
 
 template <typename T>
 cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
@@ -997,10 +1012,7 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
     e = b.two_y ? strided2_launch<T>(1, g, b, m, H, scale, st) : launch_yf<T, 1024>(g, b, 0, nplanes, st);
   if (e != cudaSuccess) return e;
   prof->mark(2, st);
-  if (g.nzt == 256) e = launch_zw<T>(g, b, 0, nplanes, st);
-  else if (g.nzt == 128) e = launch_zp<T, 16>(g, b, 0, nplanes, st);
-  else if (g.nzt == 64) e = launch_zp<T, 8>(g, b, 0, nplanes, st);
-  else e = ztile_launch<T>(g, b, st);
+  e = k3_launch<T>(g, b, 0, nplanes, 0, st);
   if (e != cudaSuccess) return e;
   prof->mark(3, st);
   e = b.two_y ? strided_tma_launch<T>(3, g, b, st) : cudaErrorNotSupported;

@@ -45,6 +45,28 @@ template <typename T>
 cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
                               cudaStream_t st, unsigned long long* launches, Prof* prof);
 
+// Slab layout ("sharded into contiguous slabs along the x-axis", "all-to-all
+// transpose"): R ranks, rank r owns the x planes [r nx/R, (r+1) nx/R) of m and H and the rows ky in [r rpr, (r+1) rpr)
+// of the half spectrum, rpr = ceil((ny + 1) / R), held as S_r[ky - r rpr][x < nx][Q].  The y pass of a rank
+// writes every spectrum row straight into the buffer of the rank that owns it, p[ky / rpr] (the transpose is the
+// store; between GPUs these are peer pointers over NVLink), the inverse y pass gathers them the same way.
+template <typename T> struct SlabView {
+  Cx<T>* p[8];   // S_r of every rank
+  int rpr;       // ky rows per rank
+  int nx;        // x planes of the whole mesh
+  int x0;        // first x plane of the launching rank
+};
+// which: 0 = forward y (r2c, pruned) of the x planes [sv.x0, sv.x0 + nxl) of m into the S buffers,
+// 4 = inverse y (c2r, truncated) from the S buffers into the same planes of H.  Wt: two-stage table of length ny.
+template <typename T>
+cudaError_t slab_y_launch(int which, int ny, int nxl, int Q, const Cx<T>* Wt, const SlabView<T>& sv, const T* m, T* H,
+                          T scale, cudaStream_t st);
+
+// K3 (S3) on nk planes of b.A2 (g.ny mirror pairs of rows each) whose table planes start at k0; xm != 0: the
+// rows of a plane are kx instead of ky (slab layout of demag_slab.cu).
+template <typename T>
+cudaError_t k3_launch(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, int xm, cudaStream_t st);
+
 // Two-stage strided passes (demag_fast2.cu).  which: 0 = K1 (x forward), 1 = K2 (y forward),
 // 3 = K4 (y inverse), 4 = K5 (x inverse).
 template <typename T>
@@ -58,6 +80,7 @@ void fast2_plan(int L, int* K1, int* K2);        // P = 2L = K1 K2 (plan2.cuh; 0
 // set: the caller then runs the LDG / STG kernels of demag_fast2.cu.
 template <typename T>
 cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st);
+bool strided_tma_usable(int L, int Q, size_t real_bytes);   // the box kernels will run for this length / row / precision
 
 // Host helpers for the tables above (plan order of the fast kernels).
 int fast_pos_logical(int L, int k);   // row of frequency k < 2L in the [even half | odd half] layout

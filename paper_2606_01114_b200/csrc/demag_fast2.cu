@@ -119,14 +119,18 @@ template <typename T> __device__ __forceinline__ Cx<T> shfl_xor_cx(Cx<T> v, int 
 // thread's t[K2 - 1 - j] (k1' = K1 - k1), the thread's own t[K2 - 1 - j] for the self-paired k1 = K1/2
 // and its own t[(K2 - j) % K2] for k1 = 0.  Every lane of a warp takes part in the shuffles (threads
 // past the last slot with dummy values).
-template <typename T, int L>
+// SLAB (demag_slab.cuh): the transform axis is y of the x plane sv.x0 + blockIdx.y (npairs = pairs of one
+// (x, y) row), and spectrum row ky goes to the rank that owns it: sv.p[ky / rpr] + ((ky % rpr) nx + x) rowc.
+template <typename T, int L, bool SLAB>
 __global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
-xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ Wt, size_t npairs) {
+xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ Wt, size_t npairs,
+           SlabView<T> sv) {
   MM_T2_PROLOGUE
   const size_t pairq = (size_t)blockIdx.x * B + lane;
   const bool ok = pairq < npairs;
   const size_t pair = ok ? pairq : 0;
-  const Cx<T>* in = mp + pair;
+  const int xg = SLAB ? sv.x0 + (int)blockIdx.y : 0;
+  const Cx<T>* in = mp + (SLAB ? (size_t)xg * L * npairs : (size_t)0) + pair;
   if (slot < K2) {
     Cx<T> v[A];
 #pragma unroll
@@ -140,14 +144,17 @@ xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __
     const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
     Cx<T> t[K2];
     fwdB<T, L>(sm, lane, k1, t);
-    Cx<T>* out = A1 + 2 * pair;
     const size_t rowc = 2 * npairs;
+    auto row = [&](int k) -> Cx<T>* {
+      if constexpr (SLAB) return sv.p[k / sv.rpr] + ((size_t)(k % sv.rpr) * sv.nx + xg) * rowc + 2 * pair;
+      else return A1 + (size_t)k * rowc + 2 * pair;
+    };
 #pragma unroll
     for (int j = 0; j < JN; ++j) {
       if (K2 % 2 == 0 && j == K2 / 2) {   // even K2: the last j holds only k = L (k1 = 0), its own mirror
         if (live && ok && k1 == 0) {
           const Cx<T> z = t[j % K2];
-          Vec2<T>::st(out + (size_t)L * rowc, mk<T>(2 * z.x, (T)0), mk<T>(2 * z.y, (T)0));
+          Vec2<T>::st(row(L), mk<T>(2 * z.x, (T)0), mk<T>(2 * z.y, (T)0));
         }
         continue;
       }
@@ -156,7 +163,7 @@ xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __
       if (live && ok && TL::has_row(j, pair0, odd)) {
         const Cx<T> z = t[j % K2], zm = cconj(pair0 ? own : r);
         const Cx<T> s = cadd(z, zm), d = csub(z, zm);
-        Vec2<T>::st(out + (size_t)(k1 + K1 * j) * rowc, s, mk<T>(d.y, -d.x));
+        Vec2<T>::st(row(k1 + K1 * j), s, mk<T>(d.y, -d.x));
       }
     }
   }
@@ -168,27 +175,31 @@ xf2_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __
 // its rows k = k1 + K1 j <= L, keeps Z[k] in t[j] and hands S = conj A + i conj B = Z[P - k] to the
 // thread that owns P - k: the partner's (or, for k1 = K1/2, its own) slot K2 - 1 - j, for k1 = 0 its own
 // slot (K2 - j) % K2.  The self-mirrored rows k = 0 and k = L keep Z[k].
-template <typename T, int L>
+template <typename T, int L, bool SLAB>
 __global__ void __launch_bounds__(Tile2<T, L>::NT, Tile2<T, L>::min_blocks)
 xi2_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>* __restrict__ Wt, size_t npairs,
-           T scale) {
+           T scale, SlabView<T> sv) {
   MM_T2_PROLOGUE
   const size_t pairq = (size_t)blockIdx.x * B + lane;
   const bool ok = pairq < npairs;
   const size_t pair = ok ? pairq : 0;
+  const int xg = SLAB ? sv.x0 + (int)blockIdx.y : 0;
   if (slot < TL::slotsB) {   // whole warps: every lane takes part in the shuffles
     const bool live = TL::slotsB == K1 || slot < K1;
     const int k1 = slot_k1<K1>(live ? slot : 0);
     const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
-    const Cx<T>* in = A1 + 2 * pair;
     const size_t rowc = 2 * npairs;
+    auto row = [&](int k) -> const Cx<T>* {
+      if constexpr (SLAB) return sv.p[k / sv.rpr] + ((size_t)(k % sv.rpr) * sv.nx + xg) * rowc + 2 * pair;
+      else return A1 + (size_t)k * rowc + 2 * pair;
+    };
     Cx<T> t[K2];
     Cx<T> a[JN], b[JN];
 #pragma unroll
     for (int j = 0; j < JN; ++j) {
       const bool last_even = K2 % 2 == 0 && j == K2 / 2;   // only k = L of k1 = 0
       if (live && (last_even ? k1 == 0 : TL::has_row(j, pair0, odd)))
-        Vec2<T>::ld(in + (size_t)(k1 + K1 * j) * rowc, a[j], b[j]);
+        Vec2<T>::ld(row(k1 + K1 * j), a[j], b[j]);
       else a[j] = b[j] = mk<T>((T)0, (T)0);
     }
 #pragma unroll
@@ -214,7 +225,7 @@ xi2_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>* __
   if (slot < K2 && ok) {
     Cx<T> v[A];
     invA<T, L>(sm, Wt, lane, slot, v);
-    Cx<T>* out = Hp + pair;
+    Cx<T>* out = Hp + (SLAB ? (size_t)xg * L * npairs : (size_t)0) + pair;
 #pragma unroll
     for (int s = 0; s < A; ++s)
       out[(size_t)(slot + K2 * s) * npairs] = mk<T>(scale * v[s].x, scale * v[s].y);
@@ -238,8 +249,9 @@ static cudaError_t launch2(int which, const FastGeom& g, const FastBufs<T>& b, c
   cudaError_t e;
   switch (which) {
     case 0:
-      if ((e = opt_in(xf2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
-      xf2_kernel<T, L><<<gx, TL::NT, TL::smem_bytes, st>>>(reinterpret_cast<const Cx<T>*>(m), b.A1, b.T2x, npairs);
+      if ((e = opt_in(xf2_kernel<T, L, false>, TL::smem_bytes)) != cudaSuccess) return e;
+      xf2_kernel<T, L, false><<<gx, TL::NT, TL::smem_bytes, st>>>(reinterpret_cast<const Cx<T>*>(m), b.A1, b.T2x, npairs,
+                                                                 SlabView<T>{});
       break;
     case 1:
       if ((e = opt_in(yf2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
@@ -250,9 +262,9 @@ static cudaError_t launch2(int which, const FastGeom& g, const FastBufs<T>& b, c
       yi2_kernel<T, L><<<dim3(gq, nk), TL::NT, TL::smem_bytes, st>>>(b.A2, b.A1, b.T2y, g.Q);
       break;
     default:
-      if ((e = opt_in(xi2_kernel<T, L>, TL::smem_bytes)) != cudaSuccess) return e;
-      xi2_kernel<T, L><<<gx, TL::NT, TL::smem_bytes, st>>>(b.A1, reinterpret_cast<Cx<T>*>(H), b.T2x, npairs,
-                                                           (T)0.5 * scale);
+      if ((e = opt_in(xi2_kernel<T, L, false>, TL::smem_bytes)) != cudaSuccess) return e;
+      xi2_kernel<T, L, false><<<gx, TL::NT, TL::smem_bytes, st>>>(b.A1, reinterpret_cast<Cx<T>*>(H), b.T2x, npairs,
+                                                                 (T)0.5 * scale, SlabView<T>{});
       break;
   }
   return cudaSuccess;
@@ -274,6 +286,40 @@ template cudaError_t strided2_launch<float>(int, const FastGeom&, const FastBufs
                                             float*, float, cudaStream_t);
 template cudaError_t strided2_launch<double>(int, const FastGeom&, const FastBufs<double>&, const double*,
                                              double*, double, cudaStream_t);
+
+// ---- slab layout (demag_slab.cuh): y is the first transformed axis, x planes [sv.x0, sv.x0 + nxl) of one rank
+template <typename T, int L>
+static cudaError_t launch_slab(int which, int nxl, int Q, const Cx<T>* Wt, const SlabView<T>& sv, const T* m, T* H,
+                               T scale, cudaStream_t st) {
+  using TL = Tile2<T, L>;
+  const size_t npairs = (size_t)Q / 2;
+  const dim3 grid((unsigned)((npairs + TL::B - 1) / TL::B), nxl);
+  cudaError_t e;
+  if (which == 0) {
+    if ((e = opt_in(xf2_kernel<T, L, true>, TL::smem_bytes)) != cudaSuccess) return e;
+    xf2_kernel<T, L, true><<<grid, TL::NT, TL::smem_bytes, st>>>(reinterpret_cast<const Cx<T>*>(m), nullptr, Wt, npairs, sv);
+  } else {
+    if ((e = opt_in(xi2_kernel<T, L, true>, TL::smem_bytes)) != cudaSuccess) return e;
+    xi2_kernel<T, L, true><<<grid, TL::NT, TL::smem_bytes, st>>>(nullptr, reinterpret_cast<Cx<T>*>(H), Wt, npairs,
+                                                                 (T)0.5 * scale, sv);
+  }
+  return cudaSuccess;
+}
+
+template <typename T>
+cudaError_t slab_y_launch(int which, int ny, int nxl, int Q, const Cx<T>* Wt, const SlabView<T>& sv, const T* m, T* H,
+                          T scale, cudaStream_t st) {
+  switch (ny) {
+#define MM_PLAN2_CASE(LL) case LL: return launch_slab<T, LL>(which, nxl, Q, Wt, sv, m, H, scale, st);
+    MM_PLAN2_LENGTHS(MM_PLAN2_CASE)
+#undef MM_PLAN2_CASE
+    default: return cudaErrorInvalidValue;
+  }
+}
+template cudaError_t slab_y_launch<float>(int, int, int, int, const float2*, const SlabView<float>&, const float*, float*,
+                                          float, cudaStream_t);
+template cudaError_t slab_y_launch<double>(int, int, int, int, const double2*, const SlabView<double>&, const double*,
+                                           double*, double, cudaStream_t);
 
 void fast2_plan(int L, int* K1, int* K2) {
   if (!plan2_of(L, K1, K2)) { *K1 = 0; *K2 = 0; }

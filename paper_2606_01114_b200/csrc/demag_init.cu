@@ -178,14 +178,16 @@ __global__ void unpack_table_kernel(int comp, InitGeom g, const T* __restrict__ 
 // the pitch ozp keeps every (kx, ky) row a multiple of 16 bytes for bulk copies), with the
 // (-i)^2 of the two odd axes and the normalisation folded in; the mirror signs are applied
 // by the z pass.
+// transpose != 0 (slab layout, demag_fast.cuh SlabView): rows ordered T[ky][kx] instead of T[kx][ky].
 template <typename T>
 __global__ void pack_fast_kernel(int comp, InitGeom g, const double* __restrict__ oct,
-                                 T* __restrict__ table, double scale) {
+                                 T* __restrict__ table, double scale, int transpose) {
   const size_t total = (size_t)g.ox * g.oy * g.oz;
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= total) return;
   const int kz = (int)(e % g.oz);
-  const size_t xy = e / g.oz;
+  size_t xy = e / g.oz;
+  if (transpose) xy = (xy % g.oy) * g.ox + xy / g.oy;
   const double v = comp >= 3 ? -oct[e] : oct[e];
   table[(xy * 6 + comp) * g.ozp + kz] = (T)(v * scale);
   if (kz == g.oz - 1)
@@ -242,7 +244,7 @@ cudaError_t demag_init_launch(const InitGeom& g, double dx, double dy, double dz
     parity_transform_kernel<<<blocks_for(nO, 256), 256, 0, st>>>(
         ping, pong, (size_t)g.ox * g.oy, g.nz, g.oz, 1, g.Pz, odd[comp][2], c, s);
     if (fast)
-      pack_fast_kernel<T><<<blocks_for(nO, 256), 256, 0, st>>>(comp, g, pong, table, scale);
+      pack_fast_kernel<T><<<blocks_for(nO, 256), 256, 0, st>>>(comp, g, pong, table, scale, fast == 2);
     else
       pack_table_kernel<T><<<blocks_for((size_t)g.Kz * g.Py * g.Px, 256), 256, 0, st>>>(
           comp, g, pong, fx, fy, table, scale);

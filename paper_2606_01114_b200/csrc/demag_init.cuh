@@ -16,7 +16,8 @@ struct InitGeom {
 size_t demag_init_scratch_bytes(const InitGeom& g);
 
 // fx[pos] / fy[pos]: frequency held at position pos of the digit-reversed x / y transform.
-// fast != 0: pack the natural-order octant T[kx][ky][6][ozp] for demag_fast.cu instead.
+// fast == 1: pack the natural-order octant T[kx][ky][6][ozp] for demag_fast.cu instead; fast == 2: T[ky][kx][6][ozp]
+// (slab layout).
 template <typename T>
 cudaError_t demag_init_launch(const InitGeom& g, double dx, double dy, double dz, void* scratch,
                               const uint16_t* fx, const uint16_t* fy, T* table, int fast,

@@ -290,6 +290,11 @@ bool tma_enabled() {
   return on == 1;
 }
 
+// true when strided_tma_launch will run the box kernels for this transform length, row length and precision
+bool strided_tma_usable(int L, int Q, size_t real_bytes) {
+  return tma_enabled() && encode_fn() && fast_two_stage(L) && ((size_t)Q * 2 * real_bytes) % 32 == 0;
+}
+
 // which: 1 = K2 (forward y), 3 = K4 (inverse y).  cudaErrorNotSupported: the caller runs the LDG / STG kernel.
 template <typename T>
 cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st) {

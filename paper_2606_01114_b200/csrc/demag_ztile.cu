@@ -98,12 +98,13 @@ template <typename T> __device__ __forceinline__ Cx<T> shfl_cx(Cx<T> v, int src)
   return r;
 }
 
-// grid (ceil(ny / NPAIR), nx + 1).  Wt[bf K1 + k1] = exp(-2 pi i bf k1 / Pz).  tab: Nhat octant rows
+// grid (ceil(ny / NPAIR), planes); the table plane of blockIdx.y is k0 + blockIdx.y; xm: the rows of a plane
+// are kx, not ky (slab layout: N_xy, N_xz instead of N_xy, N_yz change sign on the mirrored half).  Wt[bf K1 + k1] = exp(-2 pi i bf k1 / Pz).  tab: Nhat octant rows
 // [kx][ky <= ny][6][OZP].  posy: row of y frequency ky in a plane of A2.
 template <typename T, int NZ>
 __global__ void __launch_bounds__(ZTile<T, NZ>::NT, ZTile<T, NZ>::min_blocks)
 zt_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wt,
-          const uint16_t* __restrict__ posy, int ny) {
+          const uint16_t* __restrict__ posy, int ny, int k0, int xm) {
   using Z = ZTile<T, NZ>;
   constexpr int K1 = Z::K1, K2 = Z::K2, A = Z::A, Pz = Z::Pz, Q = Z::Q, NP = Z::NP, C = Z::C, PITCH = Z::PITCH,
                 NPAIR = Z::NPAIR, OZP = Z::OZP, OZS = Z::OZS, SLOT = Z::SLOT;
@@ -129,7 +130,7 @@ zt_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __rest
   // the table rows of the pairs, element by element into the padded layout (asynchronous copies, waited for
   // before stage B)
   {
-    const T* rows = tab + ((size_t)plane * (ny + 1) + i0) * 6 * OZP;
+    const T* rows = tab + ((size_t)(k0 + plane) * (ny + 1) + i0) * 6 * OZP;
     for (int e = tid; e < npair * 6 * OZP; e += Z::NT) {
       const int pp = e / (6 * OZP), r = e - pp * 6 * OZP, cc = r / OZP;
       cp_async_elem<T>(tabs + pp * SLOT + cc * OZS + (r - cc * OZP), rows + e);
@@ -185,9 +186,10 @@ zt_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __rest
     // pencil of pair 0 is ky = ny, whose own row is read from global memory (one pencil per plane)
     const bool nyq = odd && i == 0;
     const T* ts = tabs + pair * SLOT;
-    const T* tg = tab + ((size_t)plane * (ny + 1) + ny) * 6 * OZP;
+    const T* tg = tab + ((size_t)(k0 + plane) * (ny + 1) + ny) * 6 * OZP;
     const T sy = (odd && i != 0) ? (T)-1 : (T)1;
-    const T fya = (ca == 3 || ca == 5) ? sy : (T)1, fyb = (cb == 3 || cb == 5) ? sy : (T)1;
+    const int co = xm ? 4 : 5;   // with xy, the component that is odd along the row axis
+    const T fya = (ca == 3 || ca == co) ? sy : (T)1, fyb = (cb == 3 || cb == co) ? sy : (T)1;
     const bool za = ca == 4 || ca == 5, zb = cb == 4 || cb == 5;     // odd in kz
 #pragma unroll
     for (int k2 = 0; k2 < K2; ++k2) {
@@ -249,27 +251,28 @@ bool ztile_supported(int nz) {
 }
 
 template <typename T, int NZ>
-static cudaError_t launch_zt(const FastGeom& g, const FastBufs<T>& b, cudaStream_t st) {
+static cudaError_t launch_zt(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, int xm, cudaStream_t st) {
   using Z = ZTile<T, NZ>;
   if (Z::smem_bytes > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(zt_kernel<T, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, Z::smem_bytes);
     if (e != cudaSuccess) return e;
   }
-  zt_kernel<T, NZ><<<dim3((g.ny + Z::NPAIR - 1) / Z::NPAIR, g.nx + 1), Z::NT, Z::smem_bytes, st>>>(
-      b.A2, b.table, b.T2z, b.posy, g.ny);
+  zt_kernel<T, NZ><<<dim3((g.ny + Z::NPAIR - 1) / Z::NPAIR, nk), Z::NT, Z::smem_bytes, st>>>(
+      b.A2, b.table, b.T2z, b.posy, g.ny, k0, xm);
   return cudaSuccess;
 }
 
-template <typename T> cudaError_t ztile_launch(const FastGeom& g, const FastBufs<T>& b, cudaStream_t st) {
+template <typename T>
+cudaError_t ztile_launch(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, int xm, cudaStream_t st) {
   switch (g.nz) {
-#define MM_ZT_CASE(LL) case LL: return launch_zt<T, LL>(g, b, st);
+#define MM_ZT_CASE(LL) case LL: return launch_zt<T, LL>(g, b, k0, nk, xm, st);
     MM_ZTILE_LENGTHS(MM_ZT_CASE)
 #undef MM_ZT_CASE
     default: return cudaErrorInvalidValue;
   }
 }
 
-template cudaError_t ztile_launch<float>(const FastGeom&, const FastBufs<float>&, cudaStream_t);
-template cudaError_t ztile_launch<double>(const FastGeom&, const FastBufs<double>&, cudaStream_t);
+template cudaError_t ztile_launch<float>(const FastGeom&, const FastBufs<float>&, int, int, int, cudaStream_t);
+template cudaError_t ztile_launch<double>(const FastGeom&, const FastBufs<double>&, int, int, int, cudaStream_t);
 
 }  // namespace mm

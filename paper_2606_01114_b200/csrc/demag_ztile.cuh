@@ -8,7 +8,9 @@ namespace mm {
 
 bool ztile_supported(int nz);
 
-// In place on b.A2 (all nx + 1 planes); b.T2z is the plan's stage twiddle table.
-template <typename T> cudaError_t ztile_launch(const FastGeom& g, const FastBufs<T>& b, cudaStream_t st);
+// In place on nk planes of b.A2 whose table planes start at k0; b.T2z is the plan's stage twiddle table;
+// xm: the rows of a plane are kx (slab layout).
+template <typename T>
+cudaError_t ztile_launch(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, int xm, cudaStream_t st);
 
 }  // namespace mm

@@ -49,6 +49,8 @@ struct mm_ctx {
   bool embed = false;    // the demag passes run on the enclosing power-of-two mesh dnx x dny x dnz
   int dnx = 0, dny = 0, dnz = 0;   // mesh of the demag passes (= nx, ny, nz unless embedded)
   int nzt = 0;                      // x-first path: the z transform has period 2 nzt >= 2 dnz (demag_fast.cuh)
+  int slabs = 0;                    // > 0: slab decomposition over this many (emulated) ranks, demag_fast.cuh SlabView
+  int slab_rpr() const { return (dny + 1 + slabs - 1) / slabs; }   // ky rows per rank
   bool xfirst() const { return fast || mixed; }   // x-first spectra and the octant table
   int path_pref = 0;     // 0 auto, 1 generic (demag_passes.cu), 2 fast required
   int want_bz = 0, want_by = 0, want_bk = 0;
@@ -184,7 +186,11 @@ static void plan_layout(mm_ctx* c) {
   // scratch
   const size_t n3 = (size_t)c->nx * c->ny * c->nz * 3 * c->es;
   o = 0;
-  if (c->xfirst()) {
+  if (c->fast && c->slabs) {   // S_r[rpr][nx][Q] and A2_r[rpr][Px][Q] of every rank, back to back
+    const size_t rows = (size_t)c->slabs * c->slab_rpr();
+    c->off_a1 = o; o += align256(rows * g.nx * fg.Q * cs);
+    c->off_a2 = o; o += align256(rows * g.Px * fg.Q * cs);
+  } else if (c->xfirst()) {
     const size_t planes2 = c->dnx + 1;
     c->off_a1 = o; o += align256((size_t)(c->dnx + 1) * g.ny * fg.Q * cs);
     c->off_a2 = o; o += align256(planes2 * g.Py * fg.Q * cs);
@@ -292,6 +298,18 @@ mm_status mm_ctx_set_path(mm_ctx* ctx, int path) {
 mm_status mm_ctx_path(const mm_ctx* ctx, int* path) {
   if (!ctx || !path) return MM_ERR_INVALID_ARG;
   *path = ctx->fast ? (ctx->embed ? 3 : 1) : (ctx->mixed ? 2 : 0);
+  return MM_OK;
+}
+
+mm_status mm_ctx_set_slabs(mm_ctx* ctx, int ranks) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (ctx->pers) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_slabs: call before mm_ctx_set_workspace");
+  if (ranks < 0 || ranks > 8) return fail(ctx, MM_ERR_INVALID_ARG, "mm_ctx_set_slabs: ranks must be 0 .. 8");
+  if (ranks && !(ctx->fast && !ctx->embed && fast_two_stage(ctx->nx) && fast_two_stage(ctx->ny) && ranks <= ctx->nx))
+    return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_ctx_set_slabs: the slab layout needs a mesh the x-first kernels cover "
+                "with two-stage plans along x and y (%dx%dx%d does not qualify)", ctx->nx, ctx->ny, ctx->nz);
+  ctx->slabs = ranks;
+  plan_layout(ctx);
   return MM_OK;
 }
 
@@ -407,9 +425,9 @@ const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
     const bool two_x = fast_two_stage(ctx->dnx), two_y = fast_two_stage(ctx->dny);
     switch (kind) {
       case 0: return two_x ? "xf2_kernel" : "xf_fast_kernel";
-      case 1: return two_y ? "yf2_kernel" : "yf_fast_kernel";
+      case 1: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yf2_tma_kernel" : "yf2_kernel") : "yf_fast_kernel";
       case 2: return ctx->nzt == 256 ? "zw_fast_kernel" : (ctx->nzt > 256 ? "zt_kernel" : "zp_fast_kernel");
-      case 3: return two_y ? "yi2_kernel" : "yi_fast_kernel";
+      case 3: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yi2_tma_kernel" : "yi2_kernel") : "yi_fast_kernel";
       default: return two_x ? "xi2_kernel" : "xi_fast_kernel";
     }
   }
@@ -501,7 +519,7 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   }
   for (int k = 0; k < g.Px; ++k) {
     const int p = pos_of_freq(g.px, k);
-    u16(c->off_posx)[k] = (uint16_t)(c->fast ? fast_swizzle(c->dnx, fast_pos_logical(c->dnx, k)) : p);
+    u16(c->off_posx)[k] = (uint16_t)(c->fast ? (two_x ? k : fast_swizzle(c->dnx, fast_pos_logical(c->dnx, k))) : p);
     u16(c->off_fx)[p] = (uint16_t)k;
   }
   for (int k = 0; k < g.Py; ++k) {
@@ -515,8 +533,8 @@ template <typename T> static mm_status demag_init_t(mm_ctx* c) {
   e = demag_init_launch<T>(c->igeom, c->dx, c->dy, c->dz, c->scr,
                            reinterpret_cast<const uint16_t*>(c->pers + c->off_fx),
                            reinterpret_cast<const uint16_t*>(c->pers + c->off_fy),
-                           reinterpret_cast<T*>(c->pers + c->off_table), c->xfirst() ? 1 : 0, c->stream,
-                           &c->launches);
+                           reinterpret_cast<T*>(c->pers + c->off_table), c->xfirst() ? ((c->fast && c->slabs) ? 2 : 1) : 0,
+                           c->stream, &c->launches);
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: launch", e);
   e = cudaStreamSynchronize(c->stream);  // also keeps `host` alive until the copy is done
   if (e != cudaSuccess) return cuda_fail(c, "mm_demag_init: execution", e);
@@ -615,6 +633,55 @@ template <typename T> static MixedBufs<T> mixed_bufs_of(mm_ctx* c) {
 
 template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H);
 
+// Slab decomposition emulated on one device (mm_ctx_set_slabs): per rank the y pass of its x
+// planes (stores go to the owners of the spectrum rows: the first transpose), then per rank x forward, z . Nhat .
+// z^-1 and x inverse on its own ky rows, then per rank the inverse y pass of its x planes (loads come from the
+// owners: the second transpose).  On R GPUs every "for r" body is what rank r enqueues, with peer pointers in sv.p.
+template <typename T> static mm_status demag_slab_t(mm_ctx* c, const T* m, T* H) {
+  const FastGeom& g = c->fgeom;
+  const FastBufs<T> b = fast_bufs_of<T>(c);
+  const int R = c->slabs, rpr = c->slab_rpr(), rows_all = g.ny + 1;
+  const size_t s_stride = (size_t)rpr * g.nx * g.Q, a2_stride = (size_t)rpr * g.Px * g.Q;
+  SlabView<T> sv{};
+  for (int r = 0; r < R; ++r) sv.p[r] = b.A1 + r * s_stride;
+  sv.rpr = rpr; sv.nx = g.nx;
+  cudaError_t e = cudaSuccess;
+  auto x_first = [&](int r) { return (int)((long long)r * g.nx / R); };
+  for (int r = 0; r < R && e == cudaSuccess; ++r) {
+    sv.x0 = x_first(r);
+    c->prof.mark(0, c->stream);
+    e = slab_y_launch<T>(0, g.ny, x_first(r + 1) - sv.x0, g.Q, b.T2y, sv, m, H, (T)(-c->Ms), c->stream);
+    ++c->launches;
+  }
+  for (int r = 0; r < R && e == cudaSuccess; ++r) {
+    const int rows = rows_all - r * rpr < rpr ? rows_all - r * rpr : rpr;   // ky rows this rank owns
+    if (rows <= 0) break;
+    FastGeom gx = g;            // the x transform of rank r: `rows` planes of [nx][Q], transform length nx
+    gx.nx = rows - 1; gx.ny = g.nx; gx.Py = g.Px;
+    FastBufs<T> bx = b;
+    bx.A1 = b.A1 + r * s_stride; bx.A2 = b.A2 + r * a2_stride; bx.T2y = b.T2x; bx.posy = b.posx;
+    c->prof.mark(1, c->stream);
+    e = strided_tma_launch<T>(1, gx, bx, c->stream);
+    if (e == cudaErrorNotSupported) e = strided2_launch<T>(1, gx, bx, m, H, (T)0, c->stream);
+    if (e != cudaSuccess) break;
+    c->prof.mark(2, c->stream);
+    if ((e = k3_launch<T>(gx, bx, r * rpr, rows, 1, c->stream)) != cudaSuccess) break;
+    c->prof.mark(3, c->stream);
+    e = strided_tma_launch<T>(3, gx, bx, c->stream);
+    if (e == cudaErrorNotSupported) e = strided2_launch<T>(3, gx, bx, m, H, (T)0, c->stream);
+    c->launches += 3;
+  }
+  for (int r = 0; r < R && e == cudaSuccess; ++r) {
+    sv.x0 = x_first(r);
+    c->prof.mark(4, c->stream);
+    e = slab_y_launch<T>(4, g.ny, x_first(r + 1) - sv.x0, g.Q, b.T2y, sv, m, H, (T)(-c->Ms), c->stream);
+    ++c->launches;
+  }
+  c->prof.mark(-1, c->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag (slab layout) launch", e);
+}
+
 // per-cell Ms: the passes transform M = Ms_i m and the final scale is -1 (eq. 4 with M = Ms m)
 template <typename T> static mm_status demag_cells_t(mm_ctx* c, const void* m, void* H) {
   T* M = reinterpret_cast<T*>(c->scr + c->off_mscaled);
@@ -652,6 +719,7 @@ template <typename T> static mm_status demag_t(mm_ctx* c, const void* m, void* H
     c->launches += 2;
     return e == cudaSuccess ? MM_OK : cuda_fail(c, "demag (embedded fast path) launch", e);
   }
+  if (c->fast && c->slabs) return demag_slab_t<T>(c, static_cast<const T*>(m), static_cast<T*>(H));
   if (c->fast) {
     cudaError_t e = demag_fast_launch<T>(c->fgeom, fast_bufs_of<T>(c), static_cast<const T*>(m),
                                          static_cast<T*>(H), (T)(-c->Ms), c->stream, &c->launches,
@@ -712,6 +780,8 @@ mm_status mm_demag_nhat_export(mm_ctx* ctx, void* out) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (!ctx->demag_ready) return fail(ctx, MM_ERR_NOT_INITIALISED, "mm_demag_nhat_export: mm_demag_init not called");
   if (!out || ((uintptr_t)out & 15)) return fail(ctx, MM_ERR_INVALID_ARG, "mm_demag_nhat_export: bad pointer");
+  if (ctx->fast && ctx->slabs)
+    return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_demag_nhat_export: not available in the slab layout");
   if (ctx->fast && ctx->nzt != ctx->dnz)
     return fail(ctx, MM_ERR_UNSUPPORTED_SIZE, "mm_demag_nhat_export: this context transforms z with period %d, not 2 nz; "
                 "select the generic passes (mm_ctx_set_path 1) to export the table at period 2 n", 2 * ctx->nzt);

@@ -16,9 +16,9 @@ def torch_dtype(dt):
     return torch.float32 if dt == "f32" else torch.float64
 
 
-def make_ctx(cfg, dt, terms=None, tiles=None, path=0):
+def make_ctx(cfg, dt, terms=None, tiles=None, path=0, slabs=0):
     from paper_2606_01114_b200 import Context
-    ctx = Context(cfg.n, cfg.d, dtype=torch_dtype(dt), tiles=tiles, path=path)
+    ctx = Context(cfg.n, cfg.d, dtype=torch_dtype(dt), tiles=tiles, path=path, slabs=slabs)
     ctx.set_material(cfg.Ms, cfg.Aex, cfg.Ku, cfg.axis, cfg.alpha, cfg.gamma)
     ctx.set_zeeman(cfg.Hext)
     t = cfg.terms if terms is None else terms

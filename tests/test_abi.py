@@ -89,11 +89,13 @@ def test_kernel_names_follow_the_selected_path(lib):
     h = C.c_void_p()
     assert lib.mm_ctx_create(512, 512, 128, 4e-9, 4e-9, 4e-9, 0, C.byref(h)) == 0
     names = [lib.mm_ctx_kernel_name(h, k).decode() for k in range(8)]
-    assert names == ["xf2_kernel", "yf2_kernel", "zp_fast_kernel", "yi2_kernel", "xi2_kernel", "pw_vec_kernel", "", ""]
+    # the y passes run the TMA box kernels where the driver offers cuTensorMapEncodeTiled (not on a CPU-only box)
+    assert names[1] in ("yf2_kernel", "yf2_tma_kernel") and names[3] in ("yi2_kernel", "yi2_tma_kernel")
+    assert names[0::2] == ["xf2_kernel", "zp_fast_kernel", "xi2_kernel", ""] and names[5] == "pw_vec_kernel" and names[7] == ""
     lib.mm_ctx_destroy(h)
     assert lib.mm_ctx_create(1024, 64, 256, 4e-9, 4e-9, 4e-9, 1, C.byref(h)) == 0
     names = [lib.mm_ctx_kernel_name(h, k).decode() for k in range(5)]
-    assert names == ["xf_fast_kernel", "yf2_kernel", "zw_fast_kernel", "yi2_kernel", "xi_fast_kernel"]
+    assert names[0::2] == ["xf_fast_kernel", "zw_fast_kernel", "xi_fast_kernel"] and names[1].startswith("yf2_")
     lib.mm_ctx_destroy(h)
     assert lib.mm_ctx_create(16, 16, 2, 5e-9, 5e-9, 3e-9, 1, C.byref(h)) == 0
     assert lib.mm_ctx_kernel_name(h, 2) == b"xp_kernel" and lib.mm_ctx_kernel_name(h, 5) == b"pw_vec_kernel"
