@@ -1004,7 +1004,9 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   cudaError_t e = cudaSuccess;
   const int nplanes = g.nx + 1;
   prof->mark(0, st);
-  e = b.two_x ? strided2_launch<T>(0, g, b, m, H, scale, st) : launch_xf<T, 1024>(g, b, m, st);
+  e = b.two_x ? strided_tma_x_launch<T>(0, g, b, m, H, scale, st) : cudaErrorNotSupported;
+  if (e == cudaErrorNotSupported)
+    e = b.two_x ? strided2_launch<T>(0, g, b, m, H, scale, st) : launch_xf<T, 1024>(g, b, m, st);
   if (e != cudaSuccess) return e;
   prof->mark(1, st);
   e = b.two_y ? strided_tma_launch<T>(1, g, b, st) : cudaErrorNotSupported;
@@ -1020,7 +1022,9 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
     e = b.two_y ? strided2_launch<T>(3, g, b, m, H, scale, st) : launch_yi<T, 1024>(g, b, 0, nplanes, st);
   if (e != cudaSuccess) return e;
   prof->mark(4, st);
-  e = b.two_x ? strided2_launch<T>(4, g, b, m, H, scale, st) : launch_xi<T, 1024>(g, b, H, scale, st);
+  e = b.two_x ? strided_tma_x_launch<T>(4, g, b, m, H, scale, st) : cudaErrorNotSupported;
+  if (e == cudaErrorNotSupported)
+    e = b.two_x ? strided2_launch<T>(4, g, b, m, H, scale, st) : launch_xi<T, 1024>(g, b, H, scale, st);
   if (e != cudaSuccess) return e;
   *launches += 5;
   prof->mark(-1, st);

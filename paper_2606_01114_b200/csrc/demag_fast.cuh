@@ -81,6 +81,11 @@ void fast2_plan(int L, int* K1, int* K2);        // P = 2L = K1 K2 (plan2.cuh; 0
 template <typename T>
 cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st);
 bool strided_tma_usable(int L, int Q, size_t real_bytes);   // the box kernels will run for this length / row / precision
+// K1 / K5 the same way; which: 0 = K1, 4 = K5 (m, H, scale as for strided2_launch).
+template <typename T>
+cudaError_t strided_tma_x_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
+                                 cudaStream_t st);
+bool strided_tma_x_usable(int L, int ny, int Q, size_t real_bytes);
 
 // Host helpers for the tables above (plan order of the fast kernels).
 int fast_pos_logical(int L, int k);   // row of frequency k < 2L in the [even half | odd half] layout

@@ -1,16 +1,21 @@
-// K2 and K4, the y passes of the x-first demag path (S2 / S4, "zero-padding and ... FFT ... in
-// the y- and z-directions", "the output is then truncated"), with their tiles moved by the TMA engine: 2D
-// cp.async.bulk.tensor boxes of {64 bytes x up to 256 rows} instead of LDG / STG from every lane
-// (BASELINE.json north_star: "TMA or cp.async staging of pencil tiles for the strided y/z passes").
+// K1, K2, K4, K5, the strided passes of the x-first demag path (S1, S2, S4, S5; "zero-padding and ...
+// FFT ... in the y- and z-directions", "the output is then truncated"), with their tiles moved by the TMA
+// engine: 2D cp.async.bulk.tensor boxes of {64 or 128 bytes x up to 256 rows} instead of LDG / STG from every
+// lane (BASELINE.json north_star: "TMA or cp.async staging of pencil tiles for the strided y/z passes").
 // Same plans and stage arithmetic as demag_fast2.cu (strided2.cuh), bit-identical results.  A persistent CTA
-// walks tiles (column block of 64 bytes, kx plane); the box loads of the next tile are issued as soon as the
-// input buffer has been read, so they overlap the arithmetic and the stores of the current one.
+// walks tiles (column block of 64 bytes; K2 / K4: of one kx plane); the box loads of the next tile are issued as
+// soon as the input buffer has been read, so they overlap the arithmetic and the stores of the current one.
 //   K2: input tile [L rows] -> stage A -> exchange tile -> stage B -> the same buffer in natural row order
 //       -> box stores.
 //   K4: input tile [2L rows] -> stage B' reads its rows k1 + K1 k2, the tile itself becomes the exchange
 //       tile (value bf of thread k1 at row (k1 ^ (bf & 1)) + K1 bf: the four bf of a warp then read rows of
 //       both parities, i.e. both 64-byte halves of the banks) -> stage A' -> output tile [L rows] -> box stores.
+//   K1: input tile of m [L rows x 64 B] -> stage A -> exchange tile -> stage B + Hermitian separation by warp
+//       shuffles -> the same buffer as [L + 1 rows x 128 B] (A[k], B[k] side by side) -> box stores.
+//   K5: the mirror image: input tile [L + 1 rows x 128 B] becomes the exchange tile -> output tile of H.
 // Columns beyond the end of a row are zero-filled on load and clipped on store by the tensor map.
+// Every place where threads have READ a buffer that the next box load will overwrite carries a
+// fence.proxy.async before the barrier (see xf2_tma_kernel).
 // Measured against the LDG / STG kernels in profiles/r02_tma_strided.md; MM_B200_TMA=0 selects the latter.
 #define MM_NO_PACKED_F32
 #include <cuda.h>
@@ -98,6 +103,7 @@ yf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
     }
     // the previous tile's stores must have read the exchange / output buffer before it is overwritten
     if (threadIdx.x == 0) bulk_wait_read0();
+    fence_async_smem();   // the reads above are performed before the next box loads (async proxy) may overwrite the tile
     __syncthreads();   // every thread holds its inputs: the input buffer is free, and so is the output buffer
     if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
     if (slot < K2) fwdA<T, L>(ex, Wt, lane, slot, v);
@@ -188,6 +194,7 @@ yi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
     }
     // the previous tile's stores must have read the output buffer before it is overwritten
     if (threadIdx.x == 0) bulk_wait_read0();
+    fence_async_smem();   // reads of the exchange tile performed before the async proxy overwrites it
     __syncthreads();   // the exchange tile has been read: the loads of the next tile may land in it
     if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
     if (slot < K2) {
@@ -199,6 +206,194 @@ yi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
     if (threadIdx.x == 0) {
 #pragma unroll
       for (int q = 0; q < L / R; ++q) tma_store_2d(&mapOut, cb * TT::EW, plane * L + q * R, outb + q * R * B);
+      bulk_commit();
+    }
+  }
+  if (threadIdx.x == 0) bulk_wait0();
+}
+
+// ---------------------------------------------------------------- K1: forward x, r2c
+// Same arithmetic as xf2_kernel (demag_fast2.cu: two real columns ride as one complex column and are separated by
+// Hermitian symmetry with warp shuffles).  mapIn: m as [nx rows][ny Q reals], box {EW, R}; mapOut: A1 as
+// [(nx + 1) rows][2 ny Q reals], box {2 EW, R}; mapRow: the same array with a box of one row, for the row k = L.
+// The exchange tile becomes the output tile [L + 1 rows][2 B complex] once stage B has read it.
+template <typename T, int L> struct TmaTileX {
+  using TL = Tile2<T, L>;
+  using TT = TmaTile<T, L>;
+  static constexpr int io_bytes = (L + 1) * 128;                    // the tile of A1: rows k <= L of 128 bytes
+  static constexpr int ex_bytes = (TT::ex_bytes > io_bytes ? TT::ex_bytes : io_bytes + 127) / 128 * 128;
+  static constexpr int smem1 = TT::in2_bytes + ex_bytes + 64;       // K1: input tile of m, exchange / output tile
+  static constexpr int smem5 = ex_bytes + TT::out4_bytes + 64;      // K5: input / exchange tile, output tile of H
+  static constexpr int NT = TL::NT;
+  static constexpr int mb1 = sizeof(T) == 8 ? (NT <= 128 ? 2 : 1) : (smem1 <= 72 * 1024 ? 3 : 2);
+  static constexpr int mb5 = sizeof(T) == 8 ? (NT <= 128 ? 2 : 1) : (smem5 <= 72 * 1024 ? 3 : 2);
+};
+
+template <typename T> __device__ __forceinline__ Cx<T> shfl_xor_cx(Cx<T> v, int m) {
+  Cx<T> r;
+  r.x = __shfl_xor_sync(0xffffffffu, v.x, m);
+  r.y = __shfl_xor_sync(0xffffffffu, v.y, m);
+  return r;
+}
+
+template <typename T, int L>
+__global__ void __launch_bounds__(TmaTileX<T, L>::NT, TmaTileX<T, L>::mb1)
+xf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant__ CUtensorMap mapOut,
+               const __grid_constant__ CUtensorMap mapRow, const Cx<T>* __restrict__ Wt, int ntile) {
+  using TT = TmaTile<T, L>;
+  using TX = TmaTileX<T, L>;
+  using TL = Tile2<T, L>;
+  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B, R = TT::R, JN = TL::JN;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [L][B]
+  Cx<T>* ex = reinterpret_cast<Cx<T>*>(smem_raw + TT::in2_bytes);        // exchange tile, then output [L + 1][2 B]
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TT::in2_bytes + TX::ex_bytes);
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  auto issue = [&](int tile) {
+    mbar_expect_tx(bar, TT::in2_bytes);
+#pragma unroll
+    for (int q = 0; q < L / R; ++q) tma_load_2d(in + q * R * B, &mapIn, tile * TT::EW, q * R, bar);
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if ((int)blockIdx.x < ntile) issue(blockIdx.x);
+  }
+  __syncthreads();
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+    mbar_wait(bar, it & 1);
+    Cx<T> v[A];
+    if (slot < K2) {
+#pragma unroll
+      for (int s = 0; s < A; ++s) v[s] = in[(slot + K2 * s) * B + lane];
+    }
+    if (threadIdx.x == 0) bulk_wait_read0();   // the previous tile's stores have read the output tile
+    // Generic-proxy reads followed by an async-proxy write of the same shared memory need a proxy fence: the
+    // barrier alone does not wait for loads that have been issued but not performed.  Without it the box load
+    // of the next tile was seen to overwrite a row before its LDS executed (about one tile in 1e5, fp64).
+    fence_async_smem();
+    __syncthreads();                           // the input tile is in registers
+    if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
+    if (slot < K2) fwdA<T, L>(ex, Wt, lane, slot, v);
+    __syncthreads();
+    const bool live = slot < K1;
+    const int k1 = slot_k1<K1>(live ? slot : 0);
+    Cx<T> t[K2];
+    if (slot < TL::slotsB) fwdB<T, L>(ex, lane, k1, t);
+    __syncthreads();   // the exchange tile has been read: it becomes the output tile
+    if (slot < TL::slotsB) {   // whole warps: every lane takes part in the shuffles
+      const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
+      Cx<T>* orow = ex + 2 * lane;
+#pragma unroll
+      for (int j = 0; j < JN; ++j) {
+        if (K2 % 2 == 0 && j == K2 / 2) {   // even K2: the last j holds only k = L (k1 = 0), its own mirror
+          if (live && k1 == 0) {
+            const Cx<T> z = t[j % K2];
+            Vec2<T>::st(orow + (size_t)L * 2 * B, mk<T>(2 * z.x, (T)0), mk<T>(2 * z.y, (T)0));
+          }
+          continue;
+        }
+        const Cx<T> r = shfl_xor_cx<T>(t[(2 * K2 - 1 - j) % K2], B);
+        const Cx<T> own = odd ? t[(2 * K2 - 1 - j) % K2] : t[(K2 - j) % K2];
+        if (live && TL::has_row(j, pair0, odd)) {
+          const Cx<T> z = t[j % K2], zm = cconj(pair0 ? own : r);
+          const Cx<T> s = cadd(z, zm), d = csub(z, zm);
+          Vec2<T>::st(orow + (size_t)(k1 + K1 * j) * 2 * B, s, mk<T>(d.y, -d.x));
+        }
+      }
+    }
+    fence_async_smem();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+      for (int q = 0; q < L / R; ++q) tma_store_2d(&mapOut, tile * 2 * TT::EW, q * R, ex + q * R * 2 * B);
+      tma_store_2d(&mapRow, tile * 2 * TT::EW, L, ex + L * 2 * B);
+      bulk_commit();
+    }
+  }
+  if (threadIdx.x == 0) bulk_wait0();
+}
+
+// ---------------------------------------------------------------- K5: inverse x, c2r, truncated
+// Same arithmetic as xi2_kernel.  mapIn / mapRow: A1 as for K1; mapOut: H as [nx rows][ny Q reals], box {EW, R}.
+// The input tile [L + 1][2 B] becomes the exchange tile once every stage-B' thread holds its rows.
+template <typename T, int L>
+__global__ void __launch_bounds__(TmaTileX<T, L>::NT, TmaTileX<T, L>::mb5)
+xi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant__ CUtensorMap mapRow,
+               const __grid_constant__ CUtensorMap mapOut, const Cx<T>* __restrict__ Wt, T scale, int ntile) {
+  using TT = TmaTile<T, L>;
+  using TX = TmaTileX<T, L>;
+  using TL = Tile2<T, L>;
+  constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B, R = TT::R, JN = TL::JN;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [L + 1][2 B], then the exchange tile
+  Cx<T>* outb = reinterpret_cast<Cx<T>*>(smem_raw + TX::ex_bytes);       // [L][B]
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TX::ex_bytes + TT::out4_bytes);
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  auto issue = [&](int tile) {
+    mbar_expect_tx(bar, TX::io_bytes);
+#pragma unroll
+    for (int q = 0; q < L / R; ++q) tma_load_2d(in + q * R * 2 * B, &mapIn, tile * 2 * TT::EW, q * R, bar);
+    tma_load_2d(in + L * 2 * B, &mapRow, tile * 2 * TT::EW, L, bar);
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if ((int)blockIdx.x < ntile) issue(blockIdx.x);
+  }
+  __syncthreads();
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+    mbar_wait(bar, it & 1);
+    const bool live = slot < K1;
+    const int k1 = slot_k1<K1>(live ? slot : 0);
+    Cx<T> t[K2];
+    if (slot < TL::slotsB) {   // whole warps: every lane takes part in the shuffles
+      const bool pair0 = (slot >> 1) == 0, odd = slot & 1;
+      const Cx<T>* irow = in + 2 * lane;
+      Cx<T> a[JN], b[JN];
+#pragma unroll
+      for (int j = 0; j < JN; ++j) {
+        const bool last_even = K2 % 2 == 0 && j == K2 / 2;   // only k = L of k1 = 0
+        if (live && (last_even ? k1 == 0 : TL::has_row(j, pair0, odd)))
+          Vec2<T>::ld(irow + (size_t)(k1 + K1 * j) * 2 * B, a[j], b[j]);
+        else a[j] = b[j] = mk<T>((T)0, (T)0);
+      }
+#pragma unroll
+      for (int k2 = 0; k2 < K2; ++k2) t[k2] = mk<T>((T)0, (T)0);
+#pragma unroll
+      for (int j = 0; j < JN; ++j) {
+        if (K2 % 2 == 0 && j == K2 / 2) {   // k = L (k1 = 0): its own mirror
+          if (k1 == 0) t[j % K2] = mk<T>(a[j].x - b[j].y, a[j].y + b[j].x);
+          continue;
+        }
+        const Cx<T> S = mk<T>(a[j].x + b[j].y, b[j].x - a[j].y);
+        const Cx<T> r = shfl_xor_cx<T>(S, B);
+        if (!pair0) { if (TL::has_row(j, false, !odd)) t[(2 * K2 - 1 - j) % K2] = r; }
+        else if (odd) { if (!(K2 % 2 == 1 && j == K2 / 2)) t[(2 * K2 - 1 - j) % K2] = S; }
+        else if (j >= 1) t[(K2 - j) % K2] = S;
+        if (TL::has_row(j, pair0, odd)) t[j % K2] = mk<T>(a[j].x - b[j].y, a[j].y + b[j].x);
+      }
+    }
+    __syncthreads();   // every input row is in registers: the tile becomes the exchange tile
+    if (live) invB<T, L>(in, lane, k1, t);
+    __syncthreads();
+    Cx<T> v[A];
+    if (slot < K2) invA<T, L>(in, Wt, lane, slot, v);
+    if (threadIdx.x == 0) bulk_wait_read0();   // the previous tile's stores have read the output buffer
+    fence_async_smem();                        // reads of the exchange tile performed before the async proxy overwrites it
+    __syncthreads();                           // the exchange tile has been read: the next tile may land in it
+    if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
+    if (slot < K2) {
+#pragma unroll
+      for (int s = 0; s < A; ++s) outb[(slot + K2 * s) * B + lane] = mk<T>(scale * v[s].x, scale * v[s].y);
+    }
+    fence_async_smem();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+      for (int q = 0; q < L / R; ++q) tma_store_2d(&mapOut, tile * TT::EW, q * R, outb + q * R * B);
       bulk_commit();
     }
   }
@@ -225,16 +420,21 @@ EncodeFn encode_fn() {
   return fn;
 }
 
-// [rows][Q complex] viewed as rows of 2 Q reals; box {64 bytes, R rows}
-template <typename T> bool make_map(CUtensorMap* map, void* base, size_t rows, int Q, int R) {
+// [rows][row_reals] reals; box {box_bytes, R rows}
+template <typename T> bool make_map_rows(CUtensorMap* map, const void* base, size_t rows, size_t row_reals, int box_bytes,
+                                         int R) {
   EncodeFn fn = encode_fn();
   if (!fn) return false;
-  const cuuint64_t dims[2] = {(cuuint64_t)2 * Q, (cuuint64_t)rows};
-  const cuuint64_t strides[1] = {(cuuint64_t)Q * 2 * sizeof(T)};
-  const cuuint32_t box[2] = {(cuuint32_t)(64 / sizeof(T)), (cuuint32_t)R}, estr[2] = {1, 1};
-  return fn(map, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims,
-            strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+  const cuuint64_t dims[2] = {(cuuint64_t)row_reals, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)row_reals * sizeof(T)};
+  const cuuint32_t box[2] = {(cuuint32_t)(box_bytes / sizeof(T)), (cuuint32_t)R}, estr[2] = {1, 1};
+  return fn(map, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2,
+            const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
             CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+// [rows][Q complex] viewed as rows of 2 Q reals; box {64 bytes, R rows}
+template <typename T> bool make_map(CUtensorMap* map, void* base, size_t rows, int Q, int R) {
+  return make_map_rows<T>(map, base, rows, (size_t)2 * Q, 64, R);
 }
 
 int sm_count_tma() {
@@ -279,6 +479,39 @@ cudaError_t launch_tma(int which, const FastGeom& g, const FastBufs<T>& b, cudaS
   return cudaSuccess;
 }
 
+// K1 / K5 by boxes: the x axis is the row axis of m, A1 and H as they lie in memory
+template <typename T, int L>
+cudaError_t launch_tma_x(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale, cudaStream_t st) {
+  using TT = TmaTile<T, L>;
+  using TX = TmaTileX<T, L>;
+  using TL = Tile2<T, L>;
+  const size_t row_reals = (size_t)g.ny * g.Q;   // reals of one x row of m / H; a row of A1 holds twice as many
+  if ((row_reals * sizeof(T)) % 32) return cudaErrorNotSupported;   // rows must start on a sector (see launch_tma)
+  alignas(64) CUtensorMap mapF, mapA, mapRow;
+  if (!make_map_rows<T>(&mapF, which == 0 ? (const void*)m : (const void*)H, g.nx, row_reals, 64, TT::R) ||
+      !make_map_rows<T>(&mapA, b.A1, (size_t)g.nx + 1, 2 * row_reals, 128, TT::R) ||
+      !make_map_rows<T>(&mapRow, b.A1, (size_t)g.nx + 1, 2 * row_reals, 128, 1))
+    return cudaErrorNotSupported;
+  const size_t npairs = row_reals / 2;
+  const int ntile = (int)((npairs + TL::B - 1) / TL::B);
+  cudaError_t e;
+  int per_sm = 1;
+  if (which == 0) {
+    if ((e = cudaFuncSetAttribute(xf2_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TX::smem1)) != cudaSuccess) return e;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xf2_tma_kernel<T, L>, TX::NT, TX::smem1) != cudaSuccess || per_sm < 1) per_sm = 1;
+    int grid = per_sm * sm_count_tma();
+    if (grid > ntile) grid = ntile;
+    xf2_tma_kernel<T, L><<<grid, TX::NT, TX::smem1, st>>>(mapF, mapA, mapRow, b.T2x, ntile);
+  } else {
+    if ((e = cudaFuncSetAttribute(xi2_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TX::smem5)) != cudaSuccess) return e;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xi2_tma_kernel<T, L>, TX::NT, TX::smem5) != cudaSuccess || per_sm < 1) per_sm = 1;
+    int grid = per_sm * sm_count_tma();
+    if (grid > ntile) grid = ntile;
+    xi2_tma_kernel<T, L><<<grid, TX::NT, TX::smem5, st>>>(mapA, mapRow, mapF, b.T2x, (T)0.5 * scale, ntile);
+  }
+  return cudaSuccess;
+}
+
 }  // namespace
 
 bool tma_enabled() {
@@ -309,5 +542,27 @@ cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& 
 
 template cudaError_t strided_tma_launch<float>(int, const FastGeom&, const FastBufs<float>&, cudaStream_t);
 template cudaError_t strided_tma_launch<double>(int, const FastGeom&, const FastBufs<double>&, cudaStream_t);
+
+bool strided_tma_x_usable(int L, int ny, int Q, size_t real_bytes) {
+  return tma_enabled() && encode_fn() && fast_two_stage(L) && ((size_t)ny * Q * real_bytes) % 32 == 0;
+}
+
+// which: 0 = K1 (forward x, r2c), 4 = K5 (inverse x, c2r).  cudaErrorNotSupported: the caller runs the LDG / STG kernel.
+template <typename T>
+cudaError_t strided_tma_x_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
+                                 cudaStream_t st) {
+  if (!tma_enabled() || !encode_fn()) return cudaErrorNotSupported;
+  switch (g.nx) {
+#define MM_TMA_CASE(LL) case LL: return launch_tma_x<T, LL>(which, g, b, m, H, scale, st);
+    MM_PLAN2_LENGTHS(MM_TMA_CASE)
+#undef MM_TMA_CASE
+    default: return cudaErrorNotSupported;
+  }
+}
+
+template cudaError_t strided_tma_x_launch<float>(int, const FastGeom&, const FastBufs<float>&, const float*, float*, float,
+                                                 cudaStream_t);
+template cudaError_t strided_tma_x_launch<double>(int, const FastGeom&, const FastBufs<double>&, const double*, double*,
+                                                  double, cudaStream_t);
 
 }  // namespace mm

@@ -116,3 +116,75 @@ def test_fast_fewer_layers_than_the_z_transform(oracle, n):
         assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (n, dt, l2, mx)
         assert np.array_equal(got, ctx.demag_field(md).cpu().numpy())
         ctx.close()
+
+
+_LDG_WORKER = r"""
+import sys
+import numpy as np
+import torch
+sys.path.insert(0, sys.argv[1]); sys.path.insert(0, sys.argv[1] + "/tests")
+import workloads as w
+from gpu_util import make_ctx, round_input, to_dev
+from test_gpu_fast import cfg_for
+out = {}
+for spec in sys.argv[3:]:
+    nx, ny, nz, dt = spec.split(",")
+    n = (int(nx), int(ny), int(nz))
+    ctx = make_ctx(cfg_for(n), dt, terms=1, path=2)
+    m, _ = round_input(w.random_unit_vectors(717, n), dt)
+    out[spec] = ctx.demag_field(to_dev(m)).cpu().numpy()
+    names = [ctx.kernel_name(k) for k in range(5)]
+    assert not any("tma" in s for s in names), names
+    ctx.close()
+np.savez(sys.argv[2], **out)
+"""
+
+
+def test_tma_box_kernels_bit_identical_to_ldg_kernels(tmp_path):
+    """K1, K2, K4, K5 with their tiles moved by 2D TMA boxes (demag_tma.cu) run the stage arithmetic of the
+    LDG / STG kernels (demag_fast2.cu) in the same order: the fields must agree bit for bit.  The LDG / STG
+    kernels run in a child process with MM_B200_TMA=0 (the switch is read once per process)."""
+    import os
+    import subprocess
+    import sys
+    specs = ["64,128,16,f32", "128,64,32,f64", "100,64,24,f32", "256,100,40,f64", "64,350,16,f64", "400,64,32,f32",
+             "512,128,16,f32", "64,64,18,f32"]
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    npz = str(tmp_path / "ldg.npz")
+    env = dict(os.environ, MM_B200_TMA="0")
+    r = subprocess.run([sys.executable, "-c", _LDG_WORKER, root, npz, *specs], env=env, capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr[-2000:]
+    ref = np.load(npz)
+    n_tma = 0
+    for spec in specs:
+        nx, ny, nz, dt = spec.split(",")
+        n = (int(nx), int(ny), int(nz))
+        ctx = make_ctx(cfg_for(n), dt, terms=1, path=2)
+        n_tma += sum("tma" in ctx.kernel_name(k) for k in range(5))
+        m, _ = round_input(w.random_unit_vectors(717, n), dt)
+        got = ctx.demag_field(to_dev(m)).cpu().numpy()
+        assert np.array_equal(got, ref[spec]), spec
+        ctx.close()
+    assert n_tma >= 4 * (len(specs) - 1)   # 64x64x18 fp32 has rows that are not sector aligned: LDG / STG there
+
+
+@pytest.mark.parametrize("spec", ["128,64,64,f64", "64,128,64,f64", "256,128,32,f32"])
+def test_persistent_box_kernels_are_race_free_over_many_calls(spec):
+    """The persistent TMA kernels prefetch the next tile into a buffer the threads have just read.  Without a
+    proxy fence before the barrier the box load was seen to overwrite a row ahead of its read about once in
+    1e5 tiles (fp64, several CTAs per SM): 600 calls of a mesh whose CTAs walk several tiles must give one
+    result."""
+    import torch
+    nx, ny, nz, dt = spec.split(",")
+    n = (int(nx), int(ny), int(nz))
+    ctx = make_ctx(cfg_for(n), dt, terms=1, path=2)
+    m, _ = round_input(w.random_unit_vectors(717, n), dt)
+    md = to_dev(m)
+    ref = ctx.demag_field(md).clone()
+    out = torch.empty_like(md)
+    bad = 0
+    for _ in range(600):
+        ctx.demag_field(md, out)
+        bad += int(not torch.equal(out, ref))
+    ctx.close()
+    assert bad == 0
