@@ -543,8 +543,13 @@ cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& 
 template cudaError_t strided_tma_launch<float>(int, const FastGeom&, const FastBufs<float>&, cudaStream_t);
 template cudaError_t strided_tma_launch<double>(int, const FastGeom&, const FastBufs<double>&, cudaStream_t);
 
+// The x passes by boxes win or tie for the powers of two and L = 100 and lose for L = 350, 400 (350^3 fp64: K1
+// 0.81 -> 0.90 ms, K5 0.70 -> 0.89 ms; the (L + 1) x 128-byte tile leaves one 224-thread CTA per SM there;
+// profiles/r02_tma_strided.md): those lengths keep the LDG / STG kernels.
+constexpr bool tma_x_wins(int L) { return L != 350 && L != 400; }
+
 bool strided_tma_x_usable(int L, int ny, int Q, size_t real_bytes) {
-  return tma_enabled() && encode_fn() && fast_two_stage(L) && ((size_t)ny * Q * real_bytes) % 32 == 0;
+  return tma_enabled() && encode_fn() && fast_two_stage(L) && tma_x_wins(L) && ((size_t)ny * Q * real_bytes) % 32 == 0;
 }
 
 // which: 0 = K1 (forward x, r2c), 4 = K5 (inverse x, c2r).  cudaErrorNotSupported: the caller runs the LDG / STG kernel.
@@ -553,7 +558,7 @@ cudaError_t strided_tma_x_launch(int which, const FastGeom& g, const FastBufs<T>
                                  cudaStream_t st) {
   if (!tma_enabled() || !encode_fn()) return cudaErrorNotSupported;
   switch (g.nx) {
-#define MM_TMA_CASE(LL) case LL: return launch_tma_x<T, LL>(which, g, b, m, H, scale, st);
+#define MM_TMA_CASE(LL) case LL: if constexpr (tma_x_wins(LL)) return launch_tma_x<T, LL>(which, g, b, m, H, scale, st); else return cudaErrorNotSupported;
     MM_PLAN2_LENGTHS(MM_TMA_CASE)
 #undef MM_TMA_CASE
     default: return cudaErrorNotSupported;

@@ -165,7 +165,8 @@ def test_tma_box_kernels_bit_identical_to_ldg_kernels(tmp_path):
         got = ctx.demag_field(to_dev(m)).cpu().numpy()
         assert np.array_equal(got, ref[spec]), spec
         ctx.close()
-    assert n_tma >= 4 * (len(specs) - 1)   # 64x64x18 fp32 has rows that are not sector aligned: LDG / STG there
+    # 64x64x18 fp32 has rows that are not sector aligned (LDG / STG there); nx = 400 keeps the LDG / STG x passes
+    assert n_tma >= 4 * (len(specs) - 2) + 2
 
 
 @pytest.mark.parametrize("spec", ["128,64,64,f64", "64,128,64,f64", "256,128,32,f32"])
