@@ -25,6 +25,7 @@
 #include "bulk_copy.cuh"
 #include "demag_fast.cuh"
 #include "strided2.cuh"
+#include "strided3.cuh"
 
 namespace mm {
 
@@ -400,6 +401,90 @@ xi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
   if (threadIdx.x == 0) bulk_wait0();
 }
 
+// ---------------------------------------------------------------- L = 1024: three-stage passes by boxes
+// The tile of the three-stage kernels (demag_fast.cu) is 2L rows x 64 B = 128 KB: one CTA per SM, whose global
+// loads, transform and stores then run one after the other (0.43-0.57 of the roofline, profiles/r01_*).  Here a
+// persistent CTA keeps a separate 64 KB input tile that the box loads of the NEXT tile fill while the current one
+// is transformed, and the result leaves by box stores from the transform tile.  Rows of a tile that the boxes
+// move are in global order (no XOR swizzle): the accesses of the last / first stage, whose four (fp32) or eight
+// (fp64) tasks of a warp touch rows of equal parity, swap the order of each row pair in odd slots instead.
+template <typename T, int L> struct Tma3 {
+  using TL = Tile<T, L>;
+  static constexpr int R = 256;                                   // rows per box
+  static constexpr int EW = 64 / (int)sizeof(T);
+  static constexpr int in_bytes = L * 64, sm_bytes = 2 * L * 64;
+  static constexpr int smem2 = in_bytes + sm_bytes + 64;
+  static constexpr int NT = TL::NT;
+  static_assert(L % R == 0, "box rows");
+};
+
+// K2: forward y.  mapIn: A1 as [(nx + 1) L rows][2 Q reals], mapOut: A2 as [(nx + 1) 2L rows][2 Q reals]; box {EW, R}.
+template <typename T, int L>
+__global__ void __launch_bounds__(Tma3<T, L>::NT, 1)
+yf3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant__ CUtensorMap mapOut,
+               const Cx<T>* __restrict__ W, int colblocks, int ntile) {
+  using TT = Tma3<T, L>;
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, R2 = TL::R2, R3 = TL::R3, q1 = TL::q1, B = TL::B, NS = TL::NS, R = TT::R;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [L][B], global row order
+  Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw + TT::in_bytes);         // [2L][B], swizzled; global order at the end
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TT::in_bytes + TT::sm_bytes);
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B, sp = slot & 1;
+  auto issue = [&](int tile) {
+    const int cb = tile % colblocks, plane = tile / colblocks;
+    mbar_expect_tx(bar, TT::in_bytes);
+#pragma unroll
+    for (int q = 0; q < L / R; ++q) tma_load_2d(in + q * R * B, &mapIn, cb * TT::EW, plane * L + q * R, bar);
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if ((int)blockIdx.x < ntile) issue(blockIdx.x);
+  }
+  __syncthreads();
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+    const int cb = tile % colblocks, plane = tile / colblocks;
+    if (threadIdx.x == 0) bulk_wait_read0();   // the previous tile's stores have read the transform tile
+    mbar_wait(bar, it & 1);
+    __syncthreads();
+#pragma unroll 1
+    for (int bf = slot; bf < q1; bf += NS) {
+      Cx<T> v[R1];
+#pragma unroll
+      for (int s = 0; s < R1; ++s) v[s] = in[(bf + q1 * s) * B + lane];
+      fwd_first<T, L>(sm, W, lane, bf, v);
+    }
+    fence_async_smem();   // the reads of the input tile are performed before the next box loads overwrite it
+    __syncthreads();
+    if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
+    fwd_middle<T, L>(sm, W, lane, slot);
+    __syncthreads();
+#pragma unroll 1
+    for (int i = slot; i < 2 * R1 * R2; i += NS) {   // NS is even: the parity of a thread's tasks is that of its slot
+      Cx<T> v[R3];
+      fwd_last<T, L>(sm, lane, i, v);
+      // rows i R3 + u in global order; odd slots write each row pair in swapped order (both bank halves busy)
+      Cx<T>* o = sm + (size_t)i * R3 * B + lane;
+#pragma unroll
+      for (int u = 0; u < R3; u += 2) {
+        const Cx<T> a = sp ? v[u + 1] : v[u], b = sp ? v[u] : v[u + 1];
+        o[(u + sp) * B] = a;
+        o[(u + 1 - sp) * B] = b;
+      }
+    }
+    fence_async_smem();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+      for (int q = 0; q < 2 * L / R; ++q) tma_store_2d(&mapOut, cb * TT::EW, plane * 2 * L + q * R, sm + q * R * B);
+      bulk_commit();
+    }
+  }
+  if (threadIdx.x == 0) bulk_wait0();
+}
+
 // ---------------------------------------------------------------- host side
 
 typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -479,6 +564,29 @@ cudaError_t launch_tma(int which, const FastGeom& g, const FastBufs<T>& b, cudaS
   return cudaSuccess;
 }
 
+// L = 1024 (three-stage plan): which = 1 (K2).  Persistent, one CTA per SM.
+template <typename T>
+cudaError_t launch_tma3(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st) {
+  constexpr int L = 1024;
+  using TT = Tma3<T, L>;
+  using TL = Tile<T, L>;
+  if (((size_t)g.Q * 2 * sizeof(T)) % 32) return cudaErrorNotSupported;
+  alignas(64) CUtensorMap mapA1, mapA2;
+  if (!make_map<T>(&mapA1, b.A1, (size_t)(g.nx + 1) * g.ny, g.Q, TT::R) ||
+      !make_map<T>(&mapA2, b.A2, (size_t)(g.nx + 1) * g.Py, g.Q, TT::R))
+    return cudaErrorNotSupported;
+  const int colblocks = (g.Q + TL::B - 1) / TL::B, ntile = colblocks * (g.nx + 1);
+  int grid = sm_count_tma();
+  if (grid > ntile) grid = ntile;
+  cudaError_t e;
+  if (which == 1) {
+    if ((e = cudaFuncSetAttribute(yf3_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem2)) != cudaSuccess) return e;
+    yf3_tma_kernel<T, L><<<grid, TT::NT, TT::smem2, st>>>(mapA1, mapA2, b.Wy, colblocks, ntile);
+    return cudaSuccess;
+  }
+  return cudaErrorNotSupported;
+}
+
 // K1 / K5 by boxes: the x axis is the row axis of m, A1 and H as they lie in memory
 template <typename T, int L>
 cudaError_t launch_tma_x(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale, cudaStream_t st) {
@@ -525,13 +633,14 @@ bool tma_enabled() {
 
 // true when strided_tma_launch will run the box kernels for this transform length, row length and precision
 bool strided_tma_usable(int L, int Q, size_t real_bytes) {
-  return tma_enabled() && encode_fn() && fast_two_stage(L) && ((size_t)Q * 2 * real_bytes) % 32 == 0;
+  return tma_enabled() && encode_fn() && (fast_two_stage(L) || L == 1024) && ((size_t)Q * 2 * real_bytes) % 32 == 0;
 }
 
 // which: 1 = K2 (forward y), 3 = K4 (inverse y).  cudaErrorNotSupported: the caller runs the LDG / STG kernel.
 template <typename T>
 cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st) {
   if (!tma_enabled() || !encode_fn()) return cudaErrorNotSupported;
+  if (g.ny == 1024) return launch_tma3<T>(which, g, b, st);
   switch (g.ny) {
 #define MM_TMA_CASE(LL) case LL: return launch_tma<T, LL>(which, g, b, st);
     MM_PLAN2_LENGTHS(MM_TMA_CASE)
