@@ -51,6 +51,14 @@ constexpr int box_rows(int L) {
   return r;
 }
 
+// the root table of the plan, Wt[bf K1 + k1], into shared memory with row pitch TWP (every thread of the CTA; the
+// first __syncthreads of the kernel publishes it): a persistent CTA reads it for every tile, and an LDS is not
+// behind the global-load path that `long_scoreboard` showed on top in these kernels (profiles/r02_tma_strided.md)
+template <typename T, int L> __device__ __forceinline__ void stage_roots(Cx<T>* tws, const Cx<T>* __restrict__ Wt) {
+  using TL = Tile2<T, L>;
+  for (int i = threadIdx.x; i < TL::K1 * TL::K2; i += blockDim.x) tws[(i / TL::K1) * TL::TWP + i % TL::K1] = __ldg(Wt + i);
+}
+
 template <typename T, int L> struct TmaTile {
   using TL = Tile2<T, L>;
   static constexpr int R = box_rows(L);
@@ -58,9 +66,12 @@ template <typename T, int L> struct TmaTile {
   static constexpr int EW = 64 / (int)sizeof(T);                    // elements of the map's type per 64-byte row
   static constexpr int in2_bytes = L * 64;                          // K2 input tile
   static constexpr int ex_bytes = TL::K1 * TL::K2P * 64;            // exchange tile (>= 2L rows)
-  static constexpr int smem2 = in2_bytes + ex_bytes + 64;
+  // the root table rides in shared memory where two CTAs still fit with it (not fp64 at L >= 350)
+  static constexpr bool tws2 = in2_bytes + ex_bytes + 64 + TL::tw_bytes <= 110 * 1024;
+  static constexpr int smem2 = in2_bytes + ex_bytes + 64 + (tws2 ? TL::tw_bytes : 0);
   static constexpr int in4_bytes = 2 * L * 64, out4_bytes = L * 64; // K4: input = exchange tile, output tile
-  static constexpr int smem4 = in4_bytes + out4_bytes + 64;
+  static constexpr bool tws4 = in4_bytes + out4_bytes + 64 + TL::tw_bytes <= 110 * 1024;
+  static constexpr int smem4 = in4_bytes + out4_bytes + 64 + (tws4 ? TL::tw_bytes : 0);
   static constexpr int NT = TL::NT;
   // resident CTAs the kernels are compiled for: fp32 three where the tile leaves room (<= 72 KB), else two
   static constexpr int mb2 = sizeof(T) == 8 ? (NT <= 128 ? 2 : 1) : (smem2 <= 72 * 1024 ? 3 : 2);
@@ -80,7 +91,9 @@ yf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
   Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [L][B]
   Cx<T>* ex = reinterpret_cast<Cx<T>*>(smem_raw + TT::in2_bytes);        // exchange tile, then output [2L][B]
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TT::in2_bytes + TT::ex_bytes);
+  Cx<T>* tws = reinterpret_cast<Cx<T>*>(smem_raw + TT::in2_bytes + TT::ex_bytes + 64);
   const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  if constexpr (TT::tws2) stage_roots<T, L>(tws, Wt);
   auto issue = [&](int tile) {
     const int cb = tile % colblocks, plane = tile / colblocks;
     mbar_expect_tx(bar, TT::in2_bytes);
@@ -107,7 +120,7 @@ yf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
     fence_async_smem();   // the reads above are performed before the next box loads (async proxy) may overwrite the tile
     __syncthreads();   // every thread holds its inputs: the input buffer is free, and so is the output buffer
     if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
-    if (slot < K2) fwdA<T, L>(ex, Wt, lane, slot, v);
+    if (slot < K2) fwdA<T, L, TT::tws2>(ex, TT::tws2 ? tws : Wt, lane, slot, v);
     __syncthreads();
     {
       const int k1 = slot < K1 ? slot_k1<K1>(slot) : 0;
@@ -144,7 +157,9 @@ yi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
   Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [2L][B], then the exchange tile
   Cx<T>* outb = reinterpret_cast<Cx<T>*>(smem_raw + TT::in4_bytes);      // [L][B]
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TT::in4_bytes + TT::out4_bytes);
+  Cx<T>* tws = reinterpret_cast<Cx<T>*>(smem_raw + TT::in4_bytes + TT::out4_bytes + 64);
   const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  if constexpr (TT::tws4) stage_roots<T, L>(tws, Wt);
   auto issue = [&](int tile) {
     const int cb = tile % colblocks, plane = tile / colblocks;
     mbar_expect_tx(bar, TT::in4_bytes);
@@ -179,12 +194,12 @@ yi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
     if (slot < K2) {   // stage A' of bf = slot, truncated to the L wanted samples
       const int bf = slot, sw = bf & 1;
       Cx<T> o[A];
-      const Cx<T>* tw = Wt + bf * K1;
+      const Cx<T>* tw = TT::tws4 ? tws + bf * TL::TWP : Wt + bf * K1;
       const Cx<T>* row = in + (K1 * bf) * B + lane;
 #pragma unroll
       for (int u = 0; u < A; ++u) {
         Cx<T> w0, w1;
-        Vec2<T>::ldg(tw + 2 * u, w0, w1);
+        if constexpr (TT::tws4) Vec2<T>::ld(tw + 2 * u, w0, w1); else Vec2<T>::ldg(tw + 2 * u, w0, w1);
         const Cx<T> a = row[((2 * u) ^ sw) * B], b = row[((2 * u + 1) ^ sw) * B];
         v[u] = u ? cmulc(a, w0) : a;
         o[u] = cmulc(b, w1);
@@ -223,8 +238,10 @@ template <typename T, int L> struct TmaTileX {
   using TT = TmaTile<T, L>;
   static constexpr int io_bytes = (L + 1) * 128;                    // the tile of A1: rows k <= L of 128 bytes
   static constexpr int ex_bytes = (TT::ex_bytes > io_bytes ? TT::ex_bytes : io_bytes + 127) / 128 * 128;
-  static constexpr int smem1 = TT::in2_bytes + ex_bytes + 64;       // K1: input tile of m, exchange / output tile
-  static constexpr int smem5 = ex_bytes + TT::out4_bytes + 64;      // K5: input / exchange tile, output tile of H
+  static constexpr bool tws1 = TT::in2_bytes + ex_bytes + 64 + TL::tw_bytes <= 110 * 1024;   // root table in shared memory
+  static constexpr bool tws5 = ex_bytes + TT::out4_bytes + 64 + TL::tw_bytes <= 110 * 1024;
+  static constexpr int smem1 = TT::in2_bytes + ex_bytes + 64 + (tws1 ? TL::tw_bytes : 0);   // K1: input tile of m, exchange / output tile
+  static constexpr int smem5 = ex_bytes + TT::out4_bytes + 64 + (tws5 ? TL::tw_bytes : 0);  // K5: input / exchange tile, output tile of H
   static constexpr int NT = TL::NT;
   static constexpr int mb1 = sizeof(T) == 8 ? (NT <= 128 ? 2 : 1) : (smem1 <= 72 * 1024 ? 3 : 2);
   static constexpr int mb5 = sizeof(T) == 8 ? (NT <= 128 ? 2 : 1) : (smem5 <= 72 * 1024 ? 3 : 2);
@@ -249,7 +266,9 @@ xf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
   Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [L][B]
   Cx<T>* ex = reinterpret_cast<Cx<T>*>(smem_raw + TT::in2_bytes);        // exchange tile, then output [L + 1][2 B]
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TT::in2_bytes + TX::ex_bytes);
+  Cx<T>* tws = reinterpret_cast<Cx<T>*>(smem_raw + TT::in2_bytes + TX::ex_bytes + 64);
   const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  if constexpr (TX::tws1) stage_roots<T, L>(tws, Wt);
   auto issue = [&](int tile) {
     mbar_expect_tx(bar, TT::in2_bytes);
 #pragma unroll
@@ -276,7 +295,7 @@ xf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
     fence_async_smem();
     __syncthreads();                           // the input tile is in registers
     if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
-    if (slot < K2) fwdA<T, L>(ex, Wt, lane, slot, v);
+    if (slot < K2) fwdA<T, L, TX::tws1>(ex, TX::tws1 ? tws : Wt, lane, slot, v);
     __syncthreads();
     const bool live = slot < K1;
     const int k1 = slot_k1<K1>(live ? slot : 0);
@@ -331,7 +350,9 @@ xi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
   Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [L + 1][2 B], then the exchange tile
   Cx<T>* outb = reinterpret_cast<Cx<T>*>(smem_raw + TX::ex_bytes);       // [L][B]
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TX::ex_bytes + TT::out4_bytes);
+  Cx<T>* tws = reinterpret_cast<Cx<T>*>(smem_raw + TX::ex_bytes + TT::out4_bytes + 64);
   const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  if constexpr (TX::tws5) stage_roots<T, L>(tws, Wt);
   auto issue = [&](int tile) {
     mbar_expect_tx(bar, TX::io_bytes);
 #pragma unroll
@@ -381,7 +402,7 @@ xi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
     if (live) invB<T, L>(in, lane, k1, t);
     __syncthreads();
     Cx<T> v[A];
-    if (slot < K2) invA<T, L>(in, Wt, lane, slot, v);
+    if (slot < K2) invA<T, L, TX::tws5>(in, TX::tws5 ? tws : Wt, lane, slot, v);
     if (threadIdx.x == 0) bulk_wait_read0();   // the previous tile's stores have read the output buffer
     fence_async_smem();                        // reads of the exchange tile performed before the async proxy overwrites it
     __syncthreads();                           // the exchange tile has been read: the next tile may land in it

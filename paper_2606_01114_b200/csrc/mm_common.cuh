@@ -41,13 +41,18 @@ __device__ __forceinline__ float2 csub(float2 a, float2 b) {
   return f2_unpack(r);
 }
 #endif
+// Complex products with the rounding pinned (one rounded product, one fused multiply-add per component): which
+// product the compiler fuses otherwise depends on the surrounding code, and the LDG / STG and the box kernels
+// must agree bit for bit (tests/test_gpu_fast.py).
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
 // a * b
 template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
-  C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+  C r; r.x = fma(a.x, b.x, -mul_rn(a.y, b.y)); r.y = fma(a.x, b.y, mul_rn(a.y, b.x)); return r;
 }
 // a * conj(b)
 template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {
-  C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r;
+  C r; r.x = fma(a.x, b.x, mul_rn(a.y, b.y)); r.y = fma(a.y, b.x, -mul_rn(a.x, b.y)); return r;
 }
 template <typename C> __device__ __forceinline__ C cconj(C a) { a.y = -a.y; return a; }
 

@@ -24,6 +24,8 @@ template <typename T, int L> struct Tile2 {
     return j < K2 / 2 || (j == K2 / 2 && (pair0 || !odd));
   }
   static constexpr int smem_bytes = K1 * K2P * 64;
+  // root table staged in shared memory: [K2][TWP], the rows of a warp's slots 16 bytes apart in the banks
+  static constexpr int TWP = K1 + 2, tw_bytes = (K2 * TWP * (int)sizeof(Cx<T>) + 127) / 128 * 128;
   static constexpr int min_blocks = sizeof(T) == 8 ? 2 : (smem_bytes >= 32 * 1024 ? 3 : 4);
   static_assert(K1 * K2 == 2 * L && K1 % 2 == 0 && NT <= 256, "plan");
 };
@@ -71,7 +73,9 @@ template <> struct Vec2<double> {
 };
 
 // ---- stage A, forward: v[s] = a[bf + K2 s] (s < K1/2) -> shared memory
-template <typename T, int L>
+// TWS: the root table has been staged in shared memory with row pitch K1 + 2 (Tile2::TWP; the persistent box
+// kernels of demag_tma.cu), else it is read from global memory (row pitch K1).
+template <typename T, int L, bool TWS = false>
 __device__ __forceinline__ void fwdA(Cx<T>* sm, const Cx<T>* __restrict__ Wt, int lane, int bf, Cx<T>* v) {
   using TL = Tile2<T, L>;
   constexpr int K1 = TL::K1, K2P = TL::K2P, A = TL::A, B = TL::B;
@@ -79,13 +83,13 @@ __device__ __forceinline__ void fwdA(Cx<T>* sm, const Cx<T>* __restrict__ Wt, in
   rot_fwd<T, K1>(v, o, std::make_integer_sequence<int, A>{});
   Dft<T, A, false>::run(v);   // even outputs k1 = 2u
   Dft<T, A, false>::run(o);   // odd outputs  k1 = 2u + 1
-  const Cx<T>* tw = Wt + bf * K1;
+  const Cx<T>* tw = Wt + bf * (TWS ? TL::TWP : K1);
   Cx<T>* lo = sm + bf * B + lane;          // rows of k1 <  K1/2: (k1 K2P + bf)
   Cx<T>* hi = sm + (bf ^ 1) * B + lane;    // rows of k1 >= K1/2: (k1 K2P + (bf ^ 1))
 #pragma unroll
   for (int u = 0; u < A; ++u) {
     Cx<T> w0, w1;
-    Vec2<T>::ldg(tw + 2 * u, w0, w1);
+    if constexpr (TWS) Vec2<T>::ld(tw + 2 * u, w0, w1); else Vec2<T>::ldg(tw + 2 * u, w0, w1);
     (2 * u >= K1 / 2 ? hi : lo)[(2 * u) * K2P * B] = u ? cmul(v[u], w0) : v[0];
     (2 * u + 1 >= K1 / 2 ? hi : lo)[(2 * u + 1) * K2P * B] = cmul(o[u], w1);
   }
@@ -120,18 +124,18 @@ __device__ __forceinline__ void invB(Cx<T>* sm, int lane, int k1, Cx<T>* t) {
 }
 
 // ---- stage A', inverse with truncation: v[s] = x[bf + K2 s], s < K1/2
-template <typename T, int L>
+template <typename T, int L, bool TWS = false>
 __device__ __forceinline__ void invA(const Cx<T>* sm, const Cx<T>* __restrict__ Wt, int lane, int bf, Cx<T>* v) {
   using TL = Tile2<T, L>;
   constexpr int K1 = TL::K1, K2P = TL::K2P, A = TL::A, B = TL::B;
   Cx<T> o[A];
-  const Cx<T>* tw = Wt + bf * K1;
+  const Cx<T>* tw = Wt + bf * (TWS ? TL::TWP : K1);
   const Cx<T>* lo = sm + bf * B + lane;
   const Cx<T>* hi = sm + (bf ^ 1) * B + lane;
 #pragma unroll
   for (int u = 0; u < A; ++u) {
     Cx<T> w0, w1;
-    Vec2<T>::ldg(tw + 2 * u, w0, w1);
+    if constexpr (TWS) Vec2<T>::ld(tw + 2 * u, w0, w1); else Vec2<T>::ldg(tw + 2 * u, w0, w1);
     const Cx<T> a = (2 * u >= K1 / 2 ? hi : lo)[(2 * u) * K2P * B];
     const Cx<T> b = (2 * u + 1 >= K1 / 2 ? hi : lo)[(2 * u + 1) * K2P * B];
     v[u] = u ? cmulc(a, w0) : a;
