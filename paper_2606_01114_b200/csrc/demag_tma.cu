@@ -59,6 +59,9 @@ template <typename T, int L> __device__ __forceinline__ void stage_roots(Cx<T>* 
   for (int i = threadIdx.x; i < TL::K1 * TL::K2; i += blockDim.x) tws[(i / TL::K1) * TL::TWP + i % TL::K1] = __ldg(Wt + i);
 }
 
+// dynamic shared memory per CTA that still lets two CTAs share an SM (228 KB per SM, 1 KB reserved per CTA)
+constexpr int kTwoCtaSmem = (228 * 1024 - 2 * 1024) / 2;
+
 template <typename T, int L> struct TmaTile {
   using TL = Tile2<T, L>;
   static constexpr int R = box_rows(L);
@@ -66,11 +69,11 @@ template <typename T, int L> struct TmaTile {
   static constexpr int EW = 64 / (int)sizeof(T);                    // elements of the map's type per 64-byte row
   static constexpr int in2_bytes = L * 64;                          // K2 input tile
   static constexpr int ex_bytes = TL::K1 * TL::K2P * 64;            // exchange tile (>= 2L rows)
-  // the root table rides in shared memory where two CTAs still fit with it (not fp64 at L >= 350)
-  static constexpr bool tws2 = in2_bytes + ex_bytes + 64 + TL::tw_bytes <= 110 * 1024;
+  // the root table rides in shared memory where two CTAs still fit with it
+  static constexpr bool tws2 = in2_bytes + ex_bytes + 64 + TL::tw_bytes <= kTwoCtaSmem;
   static constexpr int smem2 = in2_bytes + ex_bytes + 64 + (tws2 ? TL::tw_bytes : 0);
   static constexpr int in4_bytes = 2 * L * 64, out4_bytes = L * 64; // K4: input = exchange tile, output tile
-  static constexpr bool tws4 = in4_bytes + out4_bytes + 64 + TL::tw_bytes <= 110 * 1024;
+  static constexpr bool tws4 = in4_bytes + out4_bytes + 64 + TL::tw_bytes <= kTwoCtaSmem;
   static constexpr int smem4 = in4_bytes + out4_bytes + 64 + (tws4 ? TL::tw_bytes : 0);
   static constexpr int NT = TL::NT;
   // resident CTAs the kernels are compiled for: fp32 three where the tile leaves room (<= 72 KB), else two
@@ -238,8 +241,8 @@ template <typename T, int L> struct TmaTileX {
   using TT = TmaTile<T, L>;
   static constexpr int io_bytes = (L + 1) * 128;                    // the tile of A1: rows k <= L of 128 bytes
   static constexpr int ex_bytes = (TT::ex_bytes > io_bytes ? TT::ex_bytes : io_bytes + 127) / 128 * 128;
-  static constexpr bool tws1 = TT::in2_bytes + ex_bytes + 64 + TL::tw_bytes <= 110 * 1024;   // root table in shared memory
-  static constexpr bool tws5 = ex_bytes + TT::out4_bytes + 64 + TL::tw_bytes <= 110 * 1024;
+  static constexpr bool tws1 = TT::in2_bytes + ex_bytes + 64 + TL::tw_bytes <= kTwoCtaSmem;   // root table in shared memory
+  static constexpr bool tws5 = ex_bytes + TT::out4_bytes + 64 + TL::tw_bytes <= kTwoCtaSmem;
   static constexpr int smem1 = TT::in2_bytes + ex_bytes + 64 + (tws1 ? TL::tw_bytes : 0);   // K1: input tile of m, exchange / output tile
   static constexpr int smem5 = ex_bytes + TT::out4_bytes + 64 + (tws5 ? TL::tw_bytes : 0);  // K5: input / exchange tile, output tile of H
   static constexpr int NT = TL::NT;

@@ -419,7 +419,7 @@ const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
   if (!ctx || kind < 0 || kind > 5) return "";
   if (kind == 5) {
     if (ctx->ms_cells || ctx->a_cells) return "pw_inhom_kernel";
-    return ctx->nz % (ctx->es == 4 ? 4 : 2) == 0 ? "pw_vec_kernel" : "pw_cell_kernel";
+    return ctx->nz % 2 == 0 ? "pw_vec_kernel" : "pw_cell_kernel";
   }
   if (ctx->fast) {
     const bool two_x = fast_two_stage(ctx->dnx), two_y = fast_two_stage(ctx->dny);

@@ -18,18 +18,35 @@ namespace mm {
 template <typename T> struct Cpt { static constexpr int value = sizeof(T) == 4 ? 4 : 2; };
 template <typename T, int NR> struct VN;
 template <int NR> struct VN<float, NR> {
+  // NR = 12 (four cells): three 128-bit accesses; NR = 6 (two cells, nz = 2 mod 4: rows are only 8-byte
+  // aligned): three 64-bit accesses
   static __device__ __forceinline__ void ld(const float* p, float (&v)[NR]) {
-    const float4* q = reinterpret_cast<const float4*>(p);
+    if constexpr (NR % 4 == 0) {
+      const float4* q = reinterpret_cast<const float4*>(p);
 #pragma unroll
-    for (int i = 0; i < NR / 4; ++i) {
-      const float4 t = q[i];
-      v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
+      for (int i = 0; i < NR / 4; ++i) {
+        const float4 t = q[i];
+        v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
+      }
+    } else {
+      const float2* q = reinterpret_cast<const float2*>(p);
+#pragma unroll
+      for (int i = 0; i < NR / 2; ++i) {
+        const float2 t = q[i];
+        v[2 * i] = t.x; v[2 * i + 1] = t.y;
+      }
     }
   }
   static __device__ __forceinline__ void st(float* p, const float (&v)[NR]) {
-    float4* q = reinterpret_cast<float4*>(p);
+    if constexpr (NR % 4 == 0) {
+      float4* q = reinterpret_cast<float4*>(p);
 #pragma unroll
-    for (int i = 0; i < NR / 4; ++i) q[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+      for (int i = 0; i < NR / 4; ++i) q[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+    } else {
+      float2* q = reinterpret_cast<float2*>(p);
+#pragma unroll
+      for (int i = 0; i < NR / 2; ++i) q[i] = make_float2(v[2 * i], v[2 * i + 1]);
+    }
   }
 };
 template <int NR> struct VN<double, NR> {
@@ -130,11 +147,11 @@ __device__ __forceinline__ void cell_update(const PwParams<T>& p, const T* mc, c
 }
 
 // Vector path: nz % CPT == 0.  Thread = CPT consecutive z cells of one (x, y) line.
-template <typename T, int MODE, bool DMI>
+template <typename T, int MODE, bool DMI, int CPT>
 __global__ void __launch_bounds__(256) pw_vec_kernel(PwParams<T> p, const T* __restrict__ m,
                                                      const T* __restrict__ Hd, T* __restrict__ out,
                                                      T* __restrict__ m0, T* __restrict__ acc) {
-  constexpr int CPT = Cpt<T>::value, NR = 3 * CPT;
+  constexpr int NR = 3 * CPT;
   using V = VN<T, NR>;
   const int nzq = p.nz / CPT;
   const size_t total = (size_t)p.nx * p.ny * nzq;
@@ -415,7 +432,10 @@ static void launch_mode_dmi(const PwParams<T>& p, const T* m, const T* Hd, T* ou
                             cudaStream_t st) {
   if (p.nz % Cpt<T>::value == 0) {
     const size_t total = (size_t)p.nx * p.ny * (p.nz / Cpt<T>::value);
-    pw_vec_kernel<T, MODE, DMI><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
+    pw_vec_kernel<T, MODE, DMI, Cpt<T>::value><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
+  } else if (p.nz % 2 == 0) {   // fp32 with nz = 2 mod 4 (the paper's nz = 350, 90): two cells per thread, 64-bit accesses
+    const size_t total = (size_t)p.nx * p.ny * (p.nz / 2);
+    pw_vec_kernel<T, MODE, DMI, 2><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);
   } else {
     const size_t total = (size_t)p.nx * p.ny * p.nz;
     pw_cell_kernel<T, MODE, DMI><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p, m, Hd, out, m0, acc);

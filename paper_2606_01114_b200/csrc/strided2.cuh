@@ -24,8 +24,8 @@ template <typename T, int L> struct Tile2 {
     return j < K2 / 2 || (j == K2 / 2 && (pair0 || !odd));
   }
   static constexpr int smem_bytes = K1 * K2P * 64;
-  // root table staged in shared memory: [K2][TWP], the rows of a warp's slots 16 bytes apart in the banks
-  static constexpr int TWP = K1 + 2, tw_bytes = (K2 * TWP * (int)sizeof(Cx<T>) + 127) / 128 * 128;
+  // root table staged in shared memory: [K2][TWP], TWP = K1 + 16 bytes: the rows of a warp's slots 16 bytes apart in the banks
+  static constexpr int TWP = K1 + 32 / (int)sizeof(Cx<T>) / 2, tw_bytes = (K2 * TWP * (int)sizeof(Cx<T>) + 127) / 128 * 128;
   static constexpr int min_blocks = sizeof(T) == 8 ? 2 : (smem_bytes >= 32 * 1024 ? 3 : 4);
   static_assert(K1 * K2 == 2 * L && K1 % 2 == 0 && NT <= 256, "plan");
 };
