@@ -61,7 +61,10 @@ template <typename T, int L>
 __global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 yf_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>* __restrict__ W, int Q) {
   MM_TILE_PROLOGUE
-  const size_t col = (size_t)blockIdx.x * B + lane;
+  // columns beyond the end of a row (3 nz need not be a multiple of the 64-byte row of a tile) are loaded from
+  // column 0 and never stored
+  const bool ok = blockIdx.x * B + lane < Q;
+  const size_t col = ok ? (size_t)blockIdx.x * B + lane : 0;
   const Cx<T>* in = A1 + (size_t)blockIdx.y * L * Q + col;
   Cx<T>* out = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
 #pragma unroll 1
@@ -78,8 +81,10 @@ yf_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ A2, const Cx<T>
   for (int i = slot; i < 2 * R1 * R2; i += NS) {
     Cx<T> v[R3];
     fwd_last<T, L>(sm, lane, i, v);
+    if (ok) {
 #pragma unroll
-    for (int u = 0; u < R3; ++u) out[(size_t)(i * R3 + u) * Q] = v[u];
+      for (int u = 0; u < R3; ++u) out[(size_t)(i * R3 + u) * Q] = v[u];
+    }
   }
 }
 
@@ -88,7 +93,8 @@ template <typename T, int L>
 __global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 yi_fast_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W, int Q) {
   MM_TILE_PROLOGUE
-  const size_t col = (size_t)blockIdx.x * B + lane;
+  const bool ok = blockIdx.x * B + lane < Q;
+  const size_t col = ok ? (size_t)blockIdx.x * B + lane : 0;
   const Cx<T>* in = A2 + (size_t)blockIdx.y * 2 * L * Q + col;
   Cx<T>* out = A1 + (size_t)blockIdx.y * L * Q + col;
 #pragma unroll 2
@@ -105,8 +111,10 @@ yi_fast_kernel(const Cx<T>* __restrict__ A2, Cx<T>* __restrict__ A1, const Cx<T>
   for (int bf = slot; bf < q1; bf += NS) {
     Cx<T> v[R1];
     inv_last<T, L>(sm, W, lane, bf, v);
+    if (ok) {
 #pragma unroll
-    for (int s = 0; s < R1; ++s) out[(size_t)(bf + q1 * s) * Q] = v[s];
+      for (int s = 0; s < R1; ++s) out[(size_t)(bf + q1 * s) * Q] = v[s];
+    }
   }
 }
 
@@ -119,7 +127,8 @@ __global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 xf_fast_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W,
                const uint16_t* __restrict__ pos, size_t npairs) {
   MM_TILE_PROLOGUE
-  const size_t pair = (size_t)blockIdx.x * B + lane;
+  const bool ok = (size_t)blockIdx.x * B + lane < npairs;
+  const size_t pair = ok ? (size_t)blockIdx.x * B + lane : 0;
   const Cx<T>* in = mp + pair;
 #pragma unroll 1
   for (int bf = slot; bf < q1; bf += NS) {
@@ -147,8 +156,9 @@ xf_fast_kernel(const Cx<T>* __restrict__ mp, Cx<T>* __restrict__ A1, const Cx<T>
     const int p1 = pos[k], p2 = pos[(2 * L - k) & (2 * L - 1)];
     const Cx<T> z1 = sm[p1 * B + lane], z2 = cconj(sm[p2 * B + lane]);
     const Cx<T> s = cadd(z1, z2), d = csub(z1, z2);
-    Pair2<T>::st(out + (size_t)k * rowc, mk<T>((T)0.5 * s.x, (T)0.5 * s.y),
-                 mk<T>((T)0.5 * d.y, (T)-0.5 * d.x));
+    if (ok)
+      Pair2<T>::st(out + (size_t)k * rowc, mk<T>((T)0.5 * s.x, (T)0.5 * s.y),
+                   mk<T>((T)0.5 * d.y, (T)-0.5 * d.x));
   }
 }
 
@@ -160,7 +170,8 @@ __global__ void __launch_bounds__(Tile<T, L>::NT, Tile<T, L>::min_blocks)
 xi_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>* __restrict__ W,
                const uint16_t* __restrict__ pos, size_t npairs, T scale) {
   MM_TILE_PROLOGUE
-  const size_t pair = (size_t)blockIdx.x * B + lane;
+  const bool ok = (size_t)blockIdx.x * B + lane < npairs;
+  const size_t pair = ok ? (size_t)blockIdx.x * B + lane : 0;
   const Cx<T>* in = A1 + 2 * pair;
   const size_t rowc = 2 * npairs;
   // four independent row loads in flight per thread (one at a time left this pass latency-bound: 0.26 of the
@@ -189,9 +200,11 @@ xi_fast_kernel(const Cx<T>* __restrict__ A1, Cx<T>* __restrict__ Hp, const Cx<T>
   for (int bf = slot; bf < q1; bf += NS) {
     Cx<T> v[R1];
     inv_last<T, L>(sm, W, lane, bf, v);
+    if (ok) {
 #pragma unroll
-    for (int s = 0; s < R1; ++s)
-      out[(size_t)(bf + q1 * s) * npairs] = mk<T>(scale * v[s].x, scale * v[s].y);
+      for (int s = 0; s < R1; ++s)
+        out[(size_t)(bf + q1 * s) * npairs] = mk<T>(scale * v[s].x, scale * v[s].y);
+    }
   }
 }
 
@@ -748,7 +761,7 @@ static cudaError_t launch_xf(const FastGeom& g, const FastBufs<T>& b, const T* m
   cudaError_t e = opt_in_smem(xf_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
   const size_t npairs = (size_t)g.ny * g.Q / 2;
-  xf_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
+  xf_fast_kernel<T, L><<<(unsigned)((npairs + TL::B - 1) / TL::B), TL::NT, TL::smem_bytes, st>>>(
       reinterpret_cast<const Cx<T>*>(m), b.A1, b.Wx, b.posx, npairs);
   return cudaSuccess;
 }
@@ -758,7 +771,7 @@ static cudaError_t launch_xi(const FastGeom& g, const FastBufs<T>& b, T* H, T sc
   cudaError_t e = opt_in_smem(xi_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
   const size_t npairs = (size_t)g.ny * g.Q / 2;
-  xi_fast_kernel<T, L><<<(unsigned)(npairs / TL::B), TL::NT, TL::smem_bytes, st>>>(
+  xi_fast_kernel<T, L><<<(unsigned)((npairs + TL::B - 1) / TL::B), TL::NT, TL::smem_bytes, st>>>(
       b.A1, reinterpret_cast<Cx<T>*>(H), b.Wx, b.posx, npairs, scale);
   return cudaSuccess;
 }
@@ -767,7 +780,7 @@ static cudaError_t launch_yf(const FastGeom& g, const FastBufs<T>& b, int k0, in
   using TL = Tile<T, L>;
   cudaError_t e = opt_in_smem(yf_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
-  dim3 grid(g.Q / TL::B, nk);
+  dim3 grid((g.Q + TL::B - 1) / TL::B, nk);
   yf_fast_kernel<T, L><<<grid, TL::NT, TL::smem_bytes, st>>>(
       b.A1 + (size_t)k0 * g.ny * g.Q, b.A2, b.Wy, g.Q);
   return cudaSuccess;
@@ -777,7 +790,7 @@ static cudaError_t launch_yi(const FastGeom& g, const FastBufs<T>& b, int k0, in
   using TL = Tile<T, L>;
   cudaError_t e = opt_in_smem(yi_fast_kernel<T, L>, TL::smem_bytes);
   if (e != cudaSuccess) return e;
-  dim3 grid(g.Q / TL::B, nk);
+  dim3 grid((g.Q + TL::B - 1) / TL::B, nk);
   yi_fast_kernel<T, L><<<grid, TL::NT, TL::smem_bytes, st>>>(
       b.A2, b.A1 + (size_t)k0 * g.ny * g.Q, b.Wy, g.Q);
   return cudaSuccess;

@@ -189,3 +189,40 @@ def test_persistent_box_kernels_are_race_free_over_many_calls(spec):
         bad += int(not torch.equal(out, ref))
     ctx.close()
     assert bad == 0
+
+
+@pytest.mark.parametrize("n", [(64, 1024, 18), (1024, 100, 18)])
+def test_three_stage_passes_with_a_column_tail(oracle, n):
+    """L = 1024 (three-stage strided kernels) with rows whose 3 nz complex columns (y passes) or ny 3 nz / 2 pairs
+    (x passes) do not fill the last 64-byte tile: the tail columns must be transformed too (round 1 launched
+    floor(Q / B) tiles and left them untouched: NaN / O(1) errors at 64x1024x18)."""
+    cfg = cfg_for(n)
+    P = make_problem(oracle, cfg, terms=1)
+    m64 = w.random_unit_vectors(606, n)
+    for dt in ("f32", "f64"):
+        m, mr = round_input(m64, dt)
+        ref = oracle.demag_fft(P.Nhat, cfg.Ms, mr)
+        ctx = make_ctx(cfg, dt, terms=1, path=2)
+        l2, mx = w.field_errors(ctx.demag_field(to_dev(m)).cpu().numpy(), ref)
+        ctx.close()
+        assert l2 <= TOL[dt] and mx <= 10 * TOL[dt], (n, dt, l2, mx)
+
+
+@pytest.mark.parametrize("n", [(100, 350, 18), (350, 64, 30), (400, 128, 42), (512, 100, 54), (256, 400, 70),
+                               (128, 512, 98), (1024, 64, 20), (64, 1024, 28), (1024, 1024, 18), (100, 1024, 50)])
+def test_fast_path_agrees_with_generic_passes_on_ragged_shapes(n):
+    """Mixed sides and layer counts that leave partial tiles in every strided pass and partial pencils in K3:
+    the x-first kernels against the generic z-first passes (themselves checked against the oracle), both dtypes."""
+    cfg = cfg_for(n)
+    for dt in ("f32", "f64"):
+        m, _ = round_input(w.random_unit_vectors(707, n), dt)
+        md = to_dev(m)
+        ctx = make_ctx(cfg, dt, terms=1)
+        assert ctx.path_name == "fast"
+        got = ctx.demag_field(md).cpu().numpy()
+        ctx.close()
+        ctx = make_ctx(cfg, dt, terms=1, path=1)
+        ref = ctx.demag_field(md).cpu().numpy().astype(np.float64)
+        ctx.close()
+        l2, mx = w.field_errors(got, ref)
+        assert np.isfinite(l2) and l2 <= TOL[dt], (n, dt, l2, mx)
