@@ -48,14 +48,17 @@ template <typename T, int NZ> struct ZTile {
   static constexpr int NT = 32 * (warpsA > warpsB ? warpsA : warpsB);
   static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
   static constexpr int tile_bytes = NP * PITCH * (int)sizeof(Cx<T>);
-  // one staged table row per pair (the row ky = ny of the partner of ky = 0, one pencil per plane, is read
-  // from global memory instead).  In shared memory the six components of a row are OZS apart and the rows of
+  // one staged table row per pair, plus the row ky = ny of the partner of ky = 0 (one pencil per plane).  In shared memory the six components of a row are OZS apart and the rows of
   // the pairs SLOT apart, chosen so that the three components a lane triple reads, for the neighbouring kz of
   // a warp and for both pairs, fall on different banks (OZS = 8 mod 32 words, SLOT = 4 mod 32 words in fp32;
   // OZS = 4 mod 16 double words in fp64).
   static constexpr int OZS = sizeof(T) == 4 ? OZP + ((8 - OZP % 32) + 32) % 32 : OZP + ((4 - OZP % 16) + 16) % 16;
   static constexpr int SLOT = sizeof(T) == 4 ? 6 * OZS + ((4 - 6 * OZS % 32) + 32) % 32 : 6 * OZS;
-  static constexpr int smem_bytes = tile_bytes + NPAIR * SLOT * (int)sizeof(T) + 16;
+  // NPAIR slots for the rows of the pairs + one for the row ky = ny (the partner of ky = 0, one pencil per plane)
+  // where two CTAs per SM still fit with it (not fp64 at nz = 400: that pencil then reads its row from global memory)
+  static constexpr bool NYSLOT = 2 * (tile_bytes + (NPAIR + 1) * SLOT * (int)sizeof(T) + 16 + 1024) <= 228 * 1024;
+  static constexpr int NSLOT = NPAIR + (NYSLOT ? 1 : 0);
+  static constexpr int smem_bytes = tile_bytes + NSLOT * SLOT * (int)sizeof(T) + 16;
   // resident CTAs the kernel is compiled for: what shared memory admits and what the register file admits at
   // ~80 (fp32) / ~144 (fp64) registers per thread (fp64, K1 = 32: a few hundred bytes of spills beat one CTA per SM)
   static constexpr int by_smem = (220 * 1024) / (smem_bytes + 1024);
@@ -111,7 +114,7 @@ zt_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __rest
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Cx<T>* tile = reinterpret_cast<Cx<T>*>(smem_raw);
   T* tabs = reinterpret_cast<T*>(smem_raw + Z::tile_bytes);                       // [NPAIR] x SLOT: [6] x OZS
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + Z::tile_bytes + NPAIR * SLOT * sizeof(T));
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + Z::tile_bytes + Z::NSLOT * SLOT * sizeof(T));
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int plane = blockIdx.y, i0 = blockIdx.x * NPAIR, Py = 2 * ny;
   const int npair = ny - i0 < NPAIR ? ny - i0 : NPAIR;   // pairs of this CTA that exist
@@ -130,10 +133,22 @@ zt_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __rest
   // the table rows of the pairs, element by element into the padded layout (asynchronous copies, waited for
   // before stage B)
   {
+    // (one component row per step: no index division in the copy loop, which the issue-bound pass would pay for)
     const T* rows = tab + ((size_t)(k0 + plane) * (ny + 1) + i0) * 6 * OZP;
-    for (int e = tid; e < npair * 6 * OZP; e += Z::NT) {
-      const int pp = e / (6 * OZP), r = e - pp * 6 * OZP, cc = r / OZP;
-      cp_async_elem<T>(tabs + pp * SLOT + cc * OZS + (r - cc * OZP), rows + e);
+#pragma unroll
+    for (int pp = 0; pp < NPAIR; ++pp) {
+      if (pp < npair) {
+#pragma unroll
+        for (int cc = 0; cc < 6; ++cc)
+          for (int e = tid; e < OZP; e += Z::NT)
+            cp_async_elem<T>(tabs + pp * SLOT + cc * OZS + e, rows + (pp * 6 + cc) * OZP + e);
+      }
+    }
+    if (Z::NYSLOT && i0 == 0) {   // the CTA that holds the pair (0, ny): the row ky = ny into the extra slot
+      const T* rown = tab + ((size_t)(k0 + plane) * (ny + 1) + ny) * 6 * OZP;
+#pragma unroll
+      for (int cc = 0; cc < 6; ++cc)
+        for (int e = tid; e < OZP; e += Z::NT) cp_async_elem<T>(tabs + NPAIR * SLOT + cc * OZS + e, rown + cc * OZP + e);
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
   }
@@ -185,7 +200,7 @@ zt_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __rest
     // the odd pencil of pair i is ky = Py - i: row i with the entries odd in ky (xy, yz) negated; the odd
     // pencil of pair 0 is ky = ny, whose own row is read from global memory (one pencil per plane)
     const bool nyq = odd && i == 0;
-    const T* ts = tabs + pair * SLOT;
+    const T* ts = tabs + ((Z::NYSLOT && nyq) ? NPAIR : pair) * SLOT;
     const T* tg = tab + ((size_t)(k0 + plane) * (ny + 1) + ny) * 6 * OZP;
     const T sy = (odd && i != 0) ? (T)-1 : (T)1;
     const int co = xm ? 4 : 5;   // with xy, the component that is odd along the row axis
@@ -194,10 +209,13 @@ zt_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __rest
 #pragma unroll
     for (int k2 = 0; k2 < K2; ++k2) {
       const int kz = k1 + K1 * k2;
-      const bool mir = kz > NZ;                                       // mirrored half along kz
+      // mirrored half along kz: known at compile time except for the one k2 whose block straddles kz = nz
+      const bool mir = K1 * k2 + K1 - 1 <= NZ ? false : (K1 * k2 > NZ ? true : kz > NZ);
       const int idx = mir ? Pz - kz : kz;
       T ns = ts[c * OZS + idx], na = ts[ca * OZS + idx], nb = ts[cb * OZS + idx];
-      if (nyq) { ns = __ldg(tg + c * OZP + idx); na = __ldg(tg + ca * OZP + idx); nb = __ldg(tg + cb * OZP + idx); }
+      if constexpr (!Z::NYSLOT) {
+        if (nyq) { ns = __ldg(tg + c * OZP + idx); na = __ldg(tg + ca * OZP + idx); nb = __ldg(tg + cb * OZP + idx); }
+      }
       na *= (za && mir) ? -fya : fya;
       nb *= (zb && mir) ? -fyb : fyb;
       const Cx<T> x = t[k2], xa = shfl_cx<T>(x, la), xb = shfl_cx<T>(x, lb);
