@@ -849,7 +849,7 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   cudaError_t e = cudaSuccess;
   const int nplanes = g.nx + 1;
   prof->mark(0, st);
-  e = b.two_x ? strided_tma_x_launch<T>(0, g, b, m, H, scale, st) : cudaErrorNotSupported;
+  e = strided_tma_x_launch<T>(0, g, b, m, H, scale, st);
   if (e == cudaErrorNotSupported)
     e = b.two_x ? strided2_launch<T>(0, g, b, m, H, scale, st) : launch_xf<T, 1024>(g, b, m, st);
   if (e != cudaSuccess) return e;

@@ -86,6 +86,7 @@ template <typename T>
 cudaError_t strided_tma_x_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
                                  cudaStream_t st);
 bool strided_tma_x_usable(int L, int ny, int Q, size_t real_bytes);
+bool strided_tma3_x_usable(int ny, int Q, size_t real_bytes);   // K1 at L = 1024 (xf3_tma_kernel)
 
 // Host helpers for the tables above (plan order of the fast kernels).
 int fast_pos_logical(int L, int k);   // row of frequency k < 2L in the [even half | odd half] layout

@@ -509,6 +509,73 @@ yf3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
   if (threadIdx.x == 0) bulk_wait0();
 }
 
+// K1 at L = 1024: forward x, r2c.  The input tile of m arrives by box loads one tile ahead (mapIn: m as [nx rows]
+// [ny Q reals], box {EW, R}); the Hermitian separation reads the transform tile through `pos` and stores straight
+// to global memory, 128 bytes per row and tile, as xf_fast_kernel does (an output tile of (L + 1) x 128 bytes
+// does not fit beside the two others).
+template <typename T, int L>
+__global__ void __launch_bounds__(Tma3<T, L>::NT, 1)
+xf3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W,
+               const uint16_t* __restrict__ pos, size_t npairs, int ntile) {
+  using TT = Tma3<T, L>;
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, R2 = TL::R2, R3 = TL::R3, q1 = TL::q1, B = TL::B, NS = TL::NS, R = TT::R;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Cx<T>* in = reinterpret_cast<Cx<T>*>(smem_raw);                        // [L][B], global row order
+  Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw + TT::in_bytes);         // [2L][B], swizzled
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TT::in_bytes + TT::sm_bytes);
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  auto issue = [&](int tile) {
+    mbar_expect_tx(bar, TT::in_bytes);
+#pragma unroll
+    for (int q = 0; q < L / R; ++q) tma_load_2d(in + q * R * B, &mapIn, tile * TT::EW, q * R, bar);
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if ((int)blockIdx.x < ntile) issue(blockIdx.x);
+  }
+  __syncthreads();
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+    const bool ok = (size_t)tile * B + lane < npairs;
+    const size_t pair = ok ? (size_t)tile * B + lane : 0;
+    mbar_wait(bar, it & 1);
+#pragma unroll 1
+    for (int bf = slot; bf < q1; bf += NS) {
+      Cx<T> v[R1];
+#pragma unroll
+      for (int s = 0; s < R1; ++s) v[s] = in[(bf + q1 * s) * B + lane];
+      fwd_first<T, L>(sm, W, lane, bf, v);
+    }
+    fence_async_smem();   // the reads of the input tile are performed before the next box loads overwrite it
+    __syncthreads();
+    if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
+    fwd_middle<T, L>(sm, W, lane, slot);
+    __syncthreads();
+#pragma unroll 1
+    for (int i = slot; i < 2 * R1 * R2; i += NS) {
+      Cx<T> v[R3];
+      fwd_last<T, L>(sm, lane, i, v);
+      const int g = i & 1, base = i * R3, pe = base + g, po = base - g;
+#pragma unroll
+      for (int u = 0; u < R3; ++u) sm[(((u & 1) ? po : pe) + u) * B + lane] = v[u];
+    }
+    __syncthreads();
+    Cx<T>* out = A1 + 2 * pair;
+    const size_t rowc = 2 * npairs;
+#pragma unroll 4
+    for (int k = slot; k <= L; k += NS) {
+      const int p1 = pos[k], p2 = pos[(2 * L - k) & (2 * L - 1)];
+      const Cx<T> z1 = sm[p1 * B + lane], z2 = cconj(sm[p2 * B + lane]);
+      const Cx<T> s = cadd(z1, z2), d = csub(z1, z2);
+      if (ok)
+        Vec2<T>::st(out + (size_t)k * rowc, mk<T>((T)0.5 * s.x, (T)0.5 * s.y), mk<T>((T)0.5 * d.y, (T)-0.5 * d.x));
+    }
+    __syncthreads();   // the transform tile has been read: the next tile's first stage may overwrite it
+  }
+}
+
 // ---------------------------------------------------------------- host side
 
 typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -611,6 +678,26 @@ cudaError_t launch_tma3(int which, const FastGeom& g, const FastBufs<T>& b, cuda
   return cudaErrorNotSupported;
 }
 
+// K1 at L = 1024 with its input tile by boxes
+template <typename T>
+cudaError_t launch_tma3_x(const FastGeom& g, const FastBufs<T>& b, const T* m, cudaStream_t st) {
+  constexpr int L = 1024;
+  using TT = Tma3<T, L>;
+  using TL = Tile<T, L>;
+  const size_t row_reals = (size_t)g.ny * g.Q;
+  if ((row_reals * sizeof(T)) % 32) return cudaErrorNotSupported;
+  alignas(64) CUtensorMap mapF;
+  if (!make_map_rows<T>(&mapF, m, g.nx, row_reals, 64, TT::R)) return cudaErrorNotSupported;
+  const size_t npairs = row_reals / 2;
+  const int ntile = (int)((npairs + TL::B - 1) / TL::B);
+  int grid = sm_count_tma();
+  if (grid > ntile) grid = ntile;
+  cudaError_t e = cudaFuncSetAttribute(xf3_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem2);
+  if (e != cudaSuccess) return e;
+  xf3_tma_kernel<T, L><<<grid, TT::NT, TT::smem2, st>>>(mapF, b.A1, b.Wx, b.posx, npairs, ntile);
+  return cudaSuccess;
+}
+
 // K1 / K5 by boxes: the x axis is the row axis of m, A1 and H as they lie in memory
 template <typename T, int L>
 cudaError_t launch_tma_x(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale, cudaStream_t st) {
@@ -684,12 +771,16 @@ constexpr bool tma_x_wins(int L) { return L != 350 && L != 400; }
 bool strided_tma_x_usable(int L, int ny, int Q, size_t real_bytes) {
   return tma_enabled() && encode_fn() && fast_two_stage(L) && tma_x_wins(L) && ((size_t)ny * Q * real_bytes) % 32 == 0;
 }
+bool strided_tma3_x_usable(int ny, int Q, size_t real_bytes) {   // K1 at L = 1024
+  return tma_enabled() && encode_fn() && ((size_t)ny * Q * real_bytes) % 32 == 0;
+}
 
 // which: 0 = K1 (forward x, r2c), 4 = K5 (inverse x, c2r).  cudaErrorNotSupported: the caller runs the LDG / STG kernel.
 template <typename T>
 cudaError_t strided_tma_x_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
                                  cudaStream_t st) {
   if (!tma_enabled() || !encode_fn()) return cudaErrorNotSupported;
+  if (g.nx == 1024) return which == 0 ? launch_tma3_x<T>(g, b, m, st) : cudaErrorNotSupported;
   switch (g.nx) {
 #define MM_TMA_CASE(LL) case LL: if constexpr (tma_x_wins(LL)) return launch_tma_x<T, LL>(which, g, b, m, H, scale, st); else return cudaErrorNotSupported;
     MM_PLAN2_LENGTHS(MM_TMA_CASE)

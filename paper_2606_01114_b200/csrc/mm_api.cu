@@ -424,7 +424,8 @@ const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
   if (ctx->fast) {
     const bool two_x = fast_two_stage(ctx->dnx), two_y = fast_two_stage(ctx->dny);
     switch (kind) {
-      case 0: return two_x ? (strided_tma_x_usable(ctx->dnx, ctx->dny, 3 * ctx->dnz, ctx->es) ? "xf2_tma_kernel" : "xf2_kernel") : "xf_fast_kernel";
+      case 0: return two_x ? (strided_tma_x_usable(ctx->dnx, ctx->dny, 3 * ctx->dnz, ctx->es) ? "xf2_tma_kernel" : "xf2_kernel")
+                           : (strided_tma3_x_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "xf3_tma_kernel" : "xf_fast_kernel");
       case 1: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yf2_tma_kernel" : "yf2_kernel")
                            : (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yf3_tma_kernel" : "yf_fast_kernel");
       case 2: return ctx->nzt == 256 ? "zw_fast_kernel" : (ctx->nzt > 256 ? "zt_kernel" : "zp_fast_kernel");
