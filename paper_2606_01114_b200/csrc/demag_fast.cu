@@ -862,12 +862,12 @@ cudaError_t demag_fast_launch(const FastGeom& g, const FastBufs<T>& b, const T* 
   e = k3_launch<T>(g, b, 0, nplanes, 0, st);
   if (e != cudaSuccess) return e;
   prof->mark(3, st);
-  e = b.two_y ? strided_tma_launch<T>(3, g, b, st) : cudaErrorNotSupported;
+  e = strided_tma_launch<T>(3, g, b, st);
   if (e == cudaErrorNotSupported)
     e = b.two_y ? strided2_launch<T>(3, g, b, m, H, scale, st) : launch_yi<T, 1024>(g, b, 0, nplanes, st);
   if (e != cudaSuccess) return e;
   prof->mark(4, st);
-  e = b.two_x ? strided_tma_x_launch<T>(4, g, b, m, H, scale, st) : cudaErrorNotSupported;
+  e = strided_tma_x_launch<T>(4, g, b, m, H, scale, st);
   if (e == cudaErrorNotSupported)
     e = b.two_x ? strided2_launch<T>(4, g, b, m, H, scale, st) : launch_xi<T, 1024>(g, b, H, scale, st);
   if (e != cudaSuccess) return e;

@@ -432,6 +432,17 @@ xi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
 // is transformed, and the result leaves by box stores from the transform tile.  Rows of a tile that the boxes
 // move are in global order (no XOR swizzle): the accesses of the last / first stage, whose four (fp32) or eight
 // (fp64) tasks of a warp touch rows of equal parity, swap the order of each row pair in odd slots instead.
+// shared-memory row (swizzled) of frequency k < 2L in the three-stage tile: what the host tables posx / posy hold
+// (demag_fast.cu: fast_swizzle(fast_pos_logical(k))), as arithmetic instead of a dependent table load
+template <int L> __device__ __forceinline__ int pos3(int k) {
+  using P = FastPlan<L>;
+  constexpr int l1 = ilog2c(P::R1), l2 = ilog2c(P::R2), l3 = ilog2c(P::R3);
+  const int h = k & 1, kk = k >> 1;
+  const int u1 = kk & (P::R1 - 1), u2 = (kk >> l1) & (P::R2 - 1), u3 = kk >> (l1 + l2);
+  const int row = h * L + (u1 << (l2 + l3)) + (u2 << l3) + u3;
+  return row ^ ((row >> l3) & 1);
+}
+
 template <typename T, int L> struct Tma3 {
   using TL = Tile<T, L>;
   static constexpr int R = 256;                                   // rows per box
@@ -509,6 +520,194 @@ yf3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
   if (threadIdx.x == 0) bulk_wait0();
 }
 
+// K4 at L = 1024: inverse y, truncated.  The 2L spectrum rows of a tile land in the transform tile itself by box
+// loads (global row order), in two halves with a barrier each: the first stage works in place on the even-output
+// half while the odd half is still in flight.  The L output rows leave from a separate 64 KB tile by box stores
+// that overlap the loads of the next tile, which are issued as soon as the last stage has read the transform tile.
+// Against yi_fast_kernel (LDG / STG): the loads are all in flight at once instead of 16 per thread in four
+// rounds (`long_scoreboard` was 45 % of its stall samples, profiles/r02_l1024.md).
+template <typename T, int L>
+__global__ void __launch_bounds__(Tma3<T, L>::NT, 1)
+yi3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant__ CUtensorMap mapOut,
+               const Cx<T>* __restrict__ W, int colblocks, int ntile) {
+  using TT = Tma3<T, L>;
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, R2 = TL::R2, R3 = TL::R3, q1 = TL::q1, B = TL::B, NS = TL::NS, R = TT::R;
+  static_assert((R1 * R2) % NS == 0 && NS % 2 == 0, "a thread's first-stage tasks keep the parity of its slot and split evenly over the halves");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw);                        // [2L][B]: global order on arrival, then swizzled
+  Cx<T>* outb = reinterpret_cast<Cx<T>*>(smem_raw + TT::sm_bytes);       // [L][B]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + TT::sm_bytes + TT::in_bytes);   // even half, odd half
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B, sp = slot & 1;
+  auto issue = [&](int tile) {
+    const int cb = tile % colblocks, plane = tile / colblocks;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      mbar_expect_tx(bars + h, TT::in_bytes);
+#pragma unroll
+      for (int q = 0; q < L / R; ++q)
+        tma_load_2d(sm + (h * L + q * R) * B, &mapIn, cb * TT::EW, plane * 2 * L + h * L + q * R, bars + h);
+    }
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(bars, 1);
+    mbar_init(bars + 1, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if ((int)blockIdx.x < ntile) issue(blockIdx.x);
+  }
+  __syncthreads();
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+    const int cb = tile % colblocks, plane = tile / colblocks;
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+      mbar_wait(bars + h, it & 1);
+#pragma unroll 1
+      for (int i = h * R1 * R2 + slot; i < (h + 1) * R1 * R2; i += NS) {
+        // rows i R3 + u in global order; odd slots read each row pair in swapped order (both bank halves busy)
+        Cx<T> v[R3];
+        const Cx<T>* r = sm + (size_t)i * R3 * B + lane;
+#pragma unroll
+        for (int u = 0; u < R3; u += 2) {
+          const Cx<T> a = r[(u + sp) * B], b = r[(u + 1 - sp) * B];
+          v[u] = sp ? b : a;
+          v[u + 1] = sp ? a : b;
+        }
+        inv_first<T, L>(sm, lane, i, v);   // in place: the task's own eight rows, now swizzled
+      }
+    }
+    if (threadIdx.x == 0) bulk_wait_read0();   // the previous tile's stores have read the output tile
+    __syncthreads();
+    inv_middle<T, L>(sm, W, lane, slot);
+    __syncthreads();
+#pragma unroll 1
+    for (int bf = slot; bf < q1; bf += NS) {
+      Cx<T> v[R1];
+      inv_last<T, L>(sm, W, lane, bf, v);
+#pragma unroll
+      for (int s = 0; s < R1; ++s) outb[(bf + q1 * s) * B + lane] = v[s];
+    }
+    fence_async_smem();   // reads of the transform tile performed before the next loads; output tile visible to the stores
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      if (tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
+#pragma unroll
+      for (int q = 0; q < L / R; ++q) tma_store_2d(&mapOut, cb * TT::EW, plane * L + q * R, outb + q * R * B);
+      bulk_commit();
+    }
+  }
+  if (threadIdx.x == 0) bulk_wait0();
+}
+
+// K5 at L = 1024: inverse x, c2r, truncated.  The spectrum rows k <= L of a tile (128 bytes each: A[k], B[k] side by
+// side) arrive by box loads in two halves through one 64 KB landing buffer: the rows of even k (513 of them; a
+// tensor map over every second row of A1) are scattered into the even-output half of the transform tile as
+// Z[k] = A + i B and Z[2L - k] = conj A + i conj B, and the first two stages run on that half while the rows of
+// odd k land; the second half likewise overlaps the loads of the next tile's first half.  The L output rows go
+// straight to global memory (no room for an output tile).  Against xi_fast_kernel: 0.42 -> see profiles/r02_l1024.md.
+template <typename T, int L> struct Tma3X {
+  using TL = Tile<T, L>;
+  static constexpr int land_bytes = ((L / 2 + 1) * 128 + 127) / 128 * 128;   // rows of even k: L / 2 + 1
+  static constexpr int smem5 = land_bytes + 2 * L * 64 + 64;
+};
+
+// inverse middle stage of the tasks [lo, hi) (strided3.cuh: inv_middle runs all 2 R1 q2 of them)
+template <typename T, int L>
+__device__ __forceinline__ void inv_middle_range(Cx<T>* sm, const Cx<T>* __restrict__ W, int lane, int slot, int lo, int hi) {
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, R2 = TL::R2, q1 = TL::q1, q2 = TL::q2, B = TL::B, NS = TL::NS;
+#pragma unroll 1
+  for (int i = lo + slot; i < hi; i += NS) {
+    const int t2 = i % q2, hu = i / q2;
+    const int b0 = hu * q1 + t2, b1 = b0 ^ 1;
+    Cx<T> v[R2];
+#pragma unroll
+    for (int u = 0; u < R2; ++u) v[u] = sm[(((u & 1) ? b1 : b0) + q2 * u) * B + lane];
+#pragma unroll
+    for (int u = 1; u < R2; ++u) v[u] = cmulc(v[u], __ldg(W + 2 * R1 * t2 * u));
+    Dft<T, R2, true>::run(v);
+#pragma unroll
+    for (int s2 = 0; s2 < R2; ++s2) sm[(((s2 & 1) ? b1 : b0) + q2 * s2) * B + lane] = v[s2];
+  }
+}
+
+template <typename T, int L>
+__global__ void __launch_bounds__(Tma3<T, L>::NT, 1)
+xi3_tma_kernel(const __grid_constant__ CUtensorMap mapEven, const __grid_constant__ CUtensorMap mapEvenLast,
+               const __grid_constant__ CUtensorMap mapOdd, Cx<T>* __restrict__ Hp, const Cx<T>* __restrict__ W,
+               size_t npairs, T scale, int ntile) {
+  using TT = Tma3<T, L>;
+  using TX = Tma3X<T, L>;
+  using TL = Tile<T, L>;
+  constexpr int R1 = TL::R1, R2 = TL::R2, R3 = TL::R3, q1 = TL::q1, q2 = TL::q2, B = TL::B, NS = TL::NS, R = TT::R;
+  constexpr int H = L / 2;   // rows per half (+ the row k = L in the even half)
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Cx<T>* land = reinterpret_cast<Cx<T>*>(smem_raw);                      // [H + 1][2 B]
+  Cx<T>* sm = reinterpret_cast<Cx<T>*>(smem_raw + TX::land_bytes);       // [2L][B], swizzled
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + TX::land_bytes + TT::sm_bytes);
+  const int lane = threadIdx.x % B, slot = threadIdx.x / B;
+  auto issue = [&](int tile, int odd) {
+    mbar_expect_tx(bar, (H + (odd ? 0 : 1)) * 128);
+#pragma unroll
+    for (int q = 0; q < H / R; ++q) tma_load_2d(land + q * R * 2 * B, odd ? &mapOdd : &mapEven, tile * 2 * TT::EW, q * R, bar);
+    if (!odd) tma_load_2d(land + H * 2 * B, &mapEvenLast, tile * 2 * TT::EW, H, bar);
+  };
+  // rows j of the landing buffer hold k = 2 j + odd: Z[k] and its mirror Z[2L - k] into the transform tile
+  auto scatter = [&](int odd) {
+#pragma unroll 2
+    for (int j = slot; j < H + (odd ? 0 : 1); j += NS) {
+      const int k = 2 * j + odd;
+      Cx<T> a, b;
+      Vec2<T>::ld(land + (size_t)j * 2 * B + 2 * lane, a, b);
+      sm[pos3<L>(k) * B + lane] = mk<T>(a.x - b.y, a.y + b.x);
+      if (k != 0 && k != L) sm[pos3<L>(2 * L - k) * B + lane] = mk<T>(a.x + b.y, b.x - a.y);
+    }
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if ((int)blockIdx.x < ntile) issue(blockIdx.x, 0);
+  }
+  __syncthreads();
+  for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
+    const bool ok = (size_t)tile * B + lane < npairs;
+    const size_t pair = ok ? (size_t)tile * B + lane : 0;
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+      mbar_wait(bar, h);   // two phases per tile: even rows (parity 0), odd rows (parity 1)
+      scatter(h);
+      fence_async_smem();   // the landing buffer has been read before the next loads overwrite it
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        if (h == 0) issue(tile, 1);
+        else if (tile + (int)gridDim.x < ntile) issue(tile + gridDim.x, 0);
+      }
+#pragma unroll 1
+      for (int i = h * R1 * R2 + slot; i < (h + 1) * R1 * R2; i += NS) {
+        Cx<T> v[R3];
+        const int g = i & 1, base = i * R3, pe = base + g, po = base - g;
+#pragma unroll
+        for (int u = 0; u < R3; ++u) v[u] = sm[(((u & 1) ? po : pe) + u) * B + lane];
+        inv_first<T, L>(sm, lane, i, v);
+      }
+      __syncthreads();
+      inv_middle_range<T, L>(sm, W, lane, slot, h * R1 * q2, (h + 1) * R1 * q2);
+    }
+    __syncthreads();
+    Cx<T>* out = Hp + pair;
+#pragma unroll 1
+    for (int bf = slot; bf < q1; bf += NS) {
+      Cx<T> v[R1];
+      inv_last<T, L>(sm, W, lane, bf, v);
+      if (ok) {
+#pragma unroll
+        for (int s2 = 0; s2 < R1; ++s2) out[(size_t)(bf + q1 * s2) * npairs] = mk<T>(scale * v[s2].x, scale * v[s2].y);
+      }
+    }
+    __syncthreads();   // the transform tile has been read: the next tile's scatter may overwrite it
+  }
+}
+
 // K1 at L = 1024: forward x, r2c.  The input tile of m arrives by box loads one tile ahead (mapIn: m as [nx rows]
 // [ny Q reals], box {EW, R}); the Hermitian separation reads the transform tile through `pos` and stores straight
 // to global memory, 128 bytes per row and tile, as xf_fast_kernel does (an output tile of (L + 1) x 128 bytes
@@ -516,7 +715,7 @@ yf3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
 template <typename T, int L>
 __global__ void __launch_bounds__(Tma3<T, L>::NT, 1)
 xf3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, Cx<T>* __restrict__ A1, const Cx<T>* __restrict__ W,
-               const uint16_t* __restrict__ pos, size_t npairs, int ntile) {
+               size_t npairs, int ntile) {
   using TT = Tma3<T, L>;
   using TL = Tile<T, L>;
   constexpr int R1 = TL::R1, R2 = TL::R2, R3 = TL::R3, q1 = TL::q1, B = TL::B, NS = TL::NS, R = TT::R;
@@ -566,7 +765,7 @@ xf3_tma_kernel(const __grid_constant__ CUtensorMap mapIn, Cx<T>* __restrict__ A1
     const size_t rowc = 2 * npairs;
 #pragma unroll 4
     for (int k = slot; k <= L; k += NS) {
-      const int p1 = pos[k], p2 = pos[(2 * L - k) & (2 * L - 1)];
+      const int p1 = pos3<L>(k), p2 = pos3<L>((2 * L - k) & (2 * L - 1));
       const Cx<T> z1 = sm[p1 * B + lane], z2 = cconj(sm[p2 * B + lane]);
       const Cx<T> s = cadd(z1, z2), d = csub(z1, z2);
       if (ok)
@@ -655,7 +854,7 @@ cudaError_t launch_tma(int which, const FastGeom& g, const FastBufs<T>& b, cudaS
   return cudaSuccess;
 }
 
-// L = 1024 (three-stage plan): which = 1 (K2).  Persistent, one CTA per SM.
+// L = 1024 (three-stage plan): which = 1 (K2), 3 (K4).  Persistent, one CTA per SM.
 template <typename T>
 cudaError_t launch_tma3(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st) {
   constexpr int L = 1024;
@@ -673,9 +872,49 @@ cudaError_t launch_tma3(int which, const FastGeom& g, const FastBufs<T>& b, cuda
   if (which == 1) {
     if ((e = cudaFuncSetAttribute(yf3_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem2)) != cudaSuccess) return e;
     yf3_tma_kernel<T, L><<<grid, TT::NT, TT::smem2, st>>>(mapA1, mapA2, b.Wy, colblocks, ntile);
-    return cudaSuccess;
+  } else {
+    if ((e = cudaFuncSetAttribute(yi3_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem2)) != cudaSuccess) return e;
+    yi3_tma_kernel<T, L><<<grid, TT::NT, TT::smem2, st>>>(mapA2, mapA1, b.Wy, colblocks, ntile);
   }
-  return cudaErrorNotSupported;
+  return cudaSuccess;
+}
+
+// [rows][row_reals] reals with a row pitch of its own (every second row of an array); box {box_bytes, R rows}
+template <typename T> bool make_map_pitch(CUtensorMap* map, const void* base, size_t rows, size_t row_reals, size_t pitch_reals,
+                                          int box_bytes, int R) {
+  EncodeFn fn = encode_fn();
+  if (!fn) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)row_reals, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)pitch_reals * sizeof(T)};
+  const cuuint32_t box[2] = {(cuuint32_t)(box_bytes / sizeof(T)), (cuuint32_t)R}, estr[2] = {1, 1};
+  return fn(map, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2,
+            const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// K5 at L = 1024: the rows of even and of odd k of A1 as two tensors
+template <typename T>
+cudaError_t launch_tma3_xi(const FastGeom& g, const FastBufs<T>& b, T* H, T scale, cudaStream_t st) {
+  constexpr int L = 1024;
+  using TT = Tma3<T, L>;
+  using TX = Tma3X<T, L>;
+  using TL = Tile<T, L>;
+  const size_t row_reals = (size_t)g.ny * g.Q;        // reals of one x row of H; a row of A1 holds twice as many
+  if ((row_reals * sizeof(T)) % 32) return cudaErrorNotSupported;
+  const T* a1 = reinterpret_cast<const T*>(b.A1);
+  alignas(64) CUtensorMap mapE, mapEl, mapO;
+  if (!make_map_pitch<T>(&mapE, a1, L / 2 + 1, 2 * row_reals, 4 * row_reals, 128, TT::R) ||
+      !make_map_pitch<T>(&mapEl, a1, L / 2 + 1, 2 * row_reals, 4 * row_reals, 128, 1) ||
+      !make_map_pitch<T>(&mapO, a1 + 2 * row_reals, L / 2, 2 * row_reals, 4 * row_reals, 128, TT::R))
+    return cudaErrorNotSupported;
+  const size_t npairs = row_reals / 2;
+  const int ntile = (int)((npairs + TL::B - 1) / TL::B);
+  int grid = sm_count_tma();
+  if (grid > ntile) grid = ntile;
+  cudaError_t e = cudaFuncSetAttribute(xi3_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TX::smem5);
+  if (e != cudaSuccess) return e;
+  xi3_tma_kernel<T, L><<<grid, TT::NT, TX::smem5, st>>>(mapE, mapEl, mapO, reinterpret_cast<Cx<T>*>(H), b.Wx, npairs, scale, ntile);
+  return cudaSuccess;
 }
 
 // K1 at L = 1024 with its input tile by boxes
@@ -694,7 +933,7 @@ cudaError_t launch_tma3_x(const FastGeom& g, const FastBufs<T>& b, const T* m, c
   if (grid > ntile) grid = ntile;
   cudaError_t e = cudaFuncSetAttribute(xf3_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem2);
   if (e != cudaSuccess) return e;
-  xf3_tma_kernel<T, L><<<grid, TT::NT, TT::smem2, st>>>(mapF, b.A1, b.Wx, b.posx, npairs, ntile);
+  xf3_tma_kernel<T, L><<<grid, TT::NT, TT::smem2, st>>>(mapF, b.A1, b.Wx, npairs, ntile);
   return cudaSuccess;
 }
 
@@ -780,7 +1019,7 @@ template <typename T>
 cudaError_t strided_tma_x_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,
                                  cudaStream_t st) {
   if (!tma_enabled() || !encode_fn()) return cudaErrorNotSupported;
-  if (g.nx == 1024) return which == 0 ? launch_tma3_x<T>(g, b, m, st) : cudaErrorNotSupported;
+  if (g.nx == 1024) return which == 0 ? launch_tma3_x<T>(g, b, m, st) : launch_tma3_xi<T>(g, b, H, scale, st);
   switch (g.nx) {
 #define MM_TMA_CASE(LL) case LL: if constexpr (tma_x_wins(LL)) return launch_tma_x<T, LL>(which, g, b, m, H, scale, st); else return cudaErrorNotSupported;
     MM_PLAN2_LENGTHS(MM_TMA_CASE)

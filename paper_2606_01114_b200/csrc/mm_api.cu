@@ -429,8 +429,10 @@ const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
       case 1: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yf2_tma_kernel" : "yf2_kernel")
                            : (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yf3_tma_kernel" : "yf_fast_kernel");
       case 2: return ctx->nzt == 256 ? "zw_fast_kernel" : (ctx->nzt > 256 ? "zt_kernel" : "zp_fast_kernel");
-      case 3: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) && ctx->dny != 1024 ? "yi2_tma_kernel" : "yi2_kernel") : "yi_fast_kernel";
-      default: return two_x ? (strided_tma_x_usable(ctx->dnx, ctx->dny, 3 * ctx->dnz, ctx->es) ? "xi2_tma_kernel" : "xi2_kernel") : "xi_fast_kernel";
+      case 3: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yi2_tma_kernel" : "yi2_kernel")
+                           : (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yi3_tma_kernel" : "yi_fast_kernel");
+      default: return two_x ? (strided_tma_x_usable(ctx->dnx, ctx->dny, 3 * ctx->dnz, ctx->es) ? "xi2_tma_kernel" : "xi2_kernel")
+                            : (strided_tma3_x_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "xi3_tma_kernel" : "xi_fast_kernel");
     }
   }
   static const char* const mixed[5] = {"xf_mixed_kernel", "yf_mixed_kernel", "zp_mixed_kernel", "yi_mixed_kernel",
