@@ -347,7 +347,12 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T s3, T s4, T 
 // xm != 0 (MASK variant only): the rows of a plane are kx, not ky (slab layout, demag_slab.cuh).
 // MASK: the mesh has nzd < 8 G layers (any period Pz >= 2 nzd - 1 gives the same linear convolution, reading
 // Q27): pencils in HBM hold 3 nzd values, the samples z >= nzd read as zero and only 3 nzd values go back.
-template <typename T, int G, int WARPS, int MINB, bool MASK>
+// CONTIG (only without MASK): the rows of a plane lie in natural ky order (two-stage y pass), so the NPW/2 even
+// pencils of a task (ky = i0 ..) are one contiguous run of A2, the odd ones (ky = Py - i0 - NPW/2 + 1 .. Py - i0)
+// another, and their table rows a third: three bulk copies in and two out per task instead of one per pencil
+// (NPW = 4, 8: nz = 64, 32, whose 1.5 KB / 768 B pencils made the pass wait on copy issue: 0.56 / 0.31 of the roofline
+// against 0.70 at nz = 128).  Odd pencils are kept in ascending row order: pencil pw at slot loc(pw).
+template <typename T, int G, int WARPS, int MINB, bool MASK, bool CONTIG = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
                const uint16_t* __restrict__ posy, int ny, int kx0, int ntask, int nzd, int xm) {
@@ -389,10 +394,32 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     const int ky = (p & 1) ? (i == 0 ? ny : Py - i) : i;
     return A2 + ((size_t)plane * Py + posy[ky]) * qd;
   };
+  // slot of pencil p (pair p >> 1, odd = p & 1) within a stage
+  auto loc = [&](int p) -> int {
+    if constexpr (CONTIG) return (p & 1) ? NPW - 1 - (p >> 1) : (p >> 1);
+    else return p;
+  };
+  // CONTIG: the runs of a task as (slot, first row, rows); pair i0 = 0 has ky = ny, not Py, as its odd pencil
+  auto for_runs = [&](int task, auto&& f) {
+    const int pair0 = task * (NPW / 2), plane = pair0 / ny, i0 = pair0 - plane * ny;
+    const size_t row0 = (size_t)plane * Py;
+    f(0, row0 + i0, NPW / 2);
+    if (i0 != 0) f(NPW / 2, row0 + Py - i0 - (NPW / 2 - 1), NPW / 2);
+    else {
+      if (NPW / 2 > 1) f(NPW / 2, row0 + Py - (NPW / 2 - 1), NPW / 2 - 1);
+      f(NPW - 1, row0 + ny, 1);
+    }
+  };
   auto issue = [&](int task, int stage) {
     mbar_expect_tx(bars + stage, NPW * pbytes);
-    for (int p = 0; p < NPW; ++p)
-      bulk_load(pbase + (stage * NPW + p) * Q, pencil_ptr(task, p), pbytes, bars + stage);
+    if constexpr (CONTIG) {
+      for_runs(task, [&](int slot0, size_t row, int rows) {
+        bulk_load(pbase + (stage * NPW + slot0) * Q, A2 + row * Q, rows * pbytes, bars + stage);
+      });
+    } else {
+      for (int p = 0; p < NPW; ++p)
+        bulk_load(pbase + (stage * NPW + p) * Q, pencil_ptr(task, p), pbytes, bars + stage);
+    }
   };
   // table rows of a task: ky = i for mirror pair i; the pair i = 0 (always the first of its
   // task) is (ky = 0, ky = ny) and needs the row ky = ny as well, in the extra slot
@@ -401,8 +428,12 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     const int plane = pair0 / ny, i0 = pair0 - plane * ny;
     const T* rows = tab + ((size_t)(kx0 + plane) * (ny + 1)) * 6 * C::OZP;
     mbar_expect_tx(bars + 2, (NPW / 2 + (i0 == 0 ? 1 : 0)) * C::table_bytes);
-    for (int pp = 0; pp < NPW / 2; ++pp)
-      bulk_load(tbase + pp * 6 * C::OZP, rows + (size_t)(i0 + pp) * 6 * C::OZP, C::table_bytes, bars + 2);
+    if constexpr (CONTIG) {   // the rows ky = i0 .. i0 + NPW/2 - 1 are one run of the table
+      bulk_load(tbase, rows + (size_t)i0 * 6 * C::OZP, (NPW / 2) * C::table_bytes, bars + 2);
+    } else {
+      for (int pp = 0; pp < NPW / 2; ++pp)
+        bulk_load(tbase + pp * 6 * C::OZP, rows + (size_t)(i0 + pp) * 6 * C::OZP, C::table_bytes, bars + 2);
+    }
     if (i0 == 0)
       bulk_load(tbase + (NPW / 2) * 6 * C::OZP, rows + (size_t)ny * 6 * C::OZP, C::table_bytes, bars + 2);
   };
@@ -420,7 +451,7 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     }
     __syncwarp();
     mbar_wait(bars + stage, (it >> 1) & 1);
-    Cx<T>* pen = pbase + (stage * NPW + pw) * Q;
+    Cx<T>* pen = pbase + (stage * NPW + loc(pw)) * Q;
     Cx<T> X[3][16];
     {
       Cx<T> a[3][8];
@@ -461,8 +492,14 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     fence_async_smem();
     __syncwarp();
     if (lane == 0) {
-      for (int p = 0; p < NPW; ++p)
-        bulk_store(pencil_ptr(task, p), pbase + (stage * NPW + p) * Q, pbytes);
+      if constexpr (CONTIG) {
+        for_runs(task, [&](int slot0, size_t row, int rows) {
+          bulk_store(A2 + row * Q, pbase + (stage * NPW + slot0) * Q, rows * pbytes);
+        });
+      } else {
+        for (int p = 0; p < NPW; ++p)
+          bulk_store(pencil_ptr(task, p), pbase + (stage * NPW + p) * Q, pbytes);
+      }
       bulk_commit();
     }
   }
@@ -726,16 +763,18 @@ zw_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
 // z: the warp-per-pencil kernels hold nzt = 64, 128 or 256 layers and take any 16 <= nz <= nzt (at most four
 // times the layers: K3 is a third of the work) whose pencils are multiples of 16 bytes (bulk copies); above
 // 256 layers the tile pass of demag_ztile.cu with a plan of its own.
-int fast_z_transform(int nz, size_t real_bytes) {
-  if (nz >= 16 && nz <= 256 && ((size_t)3 * nz * 2 * real_bytes) % 16 == 0) return nz <= 64 ? 64 : (nz <= 128 ? 128 : 256);
+int fast_z_transform(int nz, size_t real_bytes, int ny) {
+  if (nz >= 16 && nz <= 256 && ((size_t)3 * nz * 2 * real_bytes) % 16 == 0)
+    return (nz <= 32 && ny % 4 == 0) ? 32 : (nz <= 64 ? 64 : (nz <= 128 ? 128 : 256));
   return ztile_supported(nz) ? nz : 0;
 }
 // x, y: a two-stage plan (plan2.cuh) or the three-stage L = 1024 kernels.  K1 / K5 move the real arrays as
-// complex pairs; the nzt = 64 kernel walks two mirror pairs of ky per task.
+// complex pairs.
 bool fast_supported(int nx, int ny, int nz, size_t real_bytes) {
   auto okxy = [](int n) { return fast_two_stage(n) || n == 1024; };
-  const int nzt = fast_z_transform(nz, real_bytes);
-  return okxy(nx) && okxy(ny) && nzt != 0 && ((size_t)ny * 3 * nz) % 2 == 0 && !(nzt == 64 && ny % 2);
+  const int nzt = fast_z_transform(nz, real_bytes, ny);
+  // the nzt = 64 / 32 kernels walk two / four mirror pairs of ky per task (nzt = 32 only where ny is a multiple of 4)
+  return okxy(nx) && okxy(ny) && nzt != 0 && ((size_t)ny * 3 * nz) % 2 == 0 && !(nzt <= 64 && ny % 2);
 }
 
 template <typename K> static cudaError_t opt_in_smem(K kernel, int bytes) {
@@ -803,7 +842,11 @@ static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, in
   int grid = sm_count() * MINB;
   if (grid * WARPS > ntask) grid = (ntask + WARPS - 1) / WARPS;
   cudaError_t e;
-  if (g.nz == C::nz && !xm) {
+  if (g.nz == C::nz && !xm && b.two_y && C::NPW > 2) {   // rows in natural ky order: one copy per run of pencils
+    if ((e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB, false, true>, C::smem_bytes)) != cudaSuccess) return e;
+    zp_fast_kernel<T, G, WARPS, MINB, false, true><<<grid, WARPS * 32, C::smem_bytes, st>>>(
+        b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz, 0);
+  } else if (g.nz == C::nz && !xm) {
     if ((e = opt_in_smem(zp_fast_kernel<T, G, WARPS, MINB, false>, C::smem_bytes)) != cudaSuccess) return e;
     zp_fast_kernel<T, G, WARPS, MINB, false><<<grid, WARPS * 32, C::smem_bytes, st>>>(
         b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz, 0);
@@ -838,6 +881,7 @@ cudaError_t k3_launch(const FastGeom& g, const FastBufs<T>& b, int k0, int nk, i
   if (g.nzt == 256) return launch_zw<T>(g, b, k0, nk, xm, st);
   if (g.nzt == 128) return launch_zp<T, 16>(g, b, k0, nk, xm, st);
   if (g.nzt == 64) return launch_zp<T, 8>(g, b, k0, nk, xm, st);
+  if (g.nzt == 32) return launch_zp<T, 4>(g, b, k0, nk, xm, st);
   return ztile_launch<T>(g, b, k0, nk, xm, st);
 }
 template cudaError_t k3_launch<float>(const FastGeom&, const FastBufs<float>&, int, int, int, cudaStream_t);

@@ -19,10 +19,10 @@ struct FastGeom {
 
 // true if the fast kernels cover this mesh (otherwise the generic path of demag_passes.cu runs)
 bool fast_supported(int nx, int ny, int nz, size_t real_bytes);
-// nzt of the K3 kernel that serves nz (0: none): 64, 128, 256 for the warp-per-pencil kernels of demag_fast.cu,
+// nzt of the K3 kernel that serves nz (0: none): 32 (ny a multiple of 4), 64, 128, 256 for the warp-per-pencil kernels of demag_fast.cu,
 // which take any nz up to their capacity with the missing layers read as zero (the period 2 nzt >= 2 nz - 1
 // gives the same linear convolution, reading Q27), or nz itself for the tile pass of demag_ztile.cu.
-int fast_z_transform(int nz, size_t real_bytes);
+int fast_z_transform(int nz, size_t real_bytes, int ny);
 
 template <typename T> struct FastBufs {
   const Cx<T>* Wx;        // Wx[q] = exp(-2 pi i q / Px), q < Px
@@ -80,7 +80,7 @@ void fast2_plan(int L, int* K1, int* K2);        // P = 2L = K1 K2 (plan2.cuh; 0
 // set: the caller then runs the LDG / STG kernels of demag_fast2.cu.
 template <typename T>
 cudaError_t strided_tma_launch(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st);
-bool strided_tma_usable(int L, int Q, size_t real_bytes);   // the box kernels will run for this length / row / precision
+bool strided_tma_usable(int L, int Q, size_t real_bytes, int which);   // the box kernel of pass `which` will run for this length / row / precision
 // K1 / K5 the same way; which: 0 = K1, 4 = K5 (m, H, scale as for strided2_launch).
 template <typename T>
 cudaError_t strided_tma_x_launch(int which, const FastGeom& g, const FastBufs<T>& b, const T* m, T* H, T scale,

@@ -83,10 +83,13 @@ template <typename T, int L> struct TmaTile {
 
 // ---------------------------------------------------------------- K2: forward y
 // mapIn: A1 as [(nx + 1) ny rows][2 Q reals], box {EW, R}; mapOut: A2 as [(nx + 1) Py rows][2 Q reals].
-template <typename T, int L>
+// STG: rows that do not start on a 32-byte sector (fp32 with nz = 2 mod 4): box stores would be partial-sector
+// writes, so the output goes to global memory straight from the registers (outp, Q) as in yf2_kernel; the loads,
+// which are what the LDG / STG kernel waits for, still come by boxes one tile ahead.
+template <typename T, int L, bool STG>
 __global__ void __launch_bounds__(TmaTile<T, L>::NT, TmaTile<T, L>::mb2)
 yf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant__ CUtensorMap mapOut,
-               const Cx<T>* __restrict__ Wt, int colblocks, int ntile) {
+               const Cx<T>* __restrict__ Wt, int colblocks, int ntile, Cx<T>* __restrict__ outp, int Q) {
   using TT = TmaTile<T, L>;
   using TL = Tile2<T, L>;
   constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B, R = TT::R;
@@ -119,7 +122,7 @@ yf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
       for (int s = 0; s < A; ++s) v[s] = in[(slot + K2 * s) * B + lane];
     }
     // the previous tile's stores must have read the exchange / output buffer before it is overwritten
-    if (threadIdx.x == 0) bulk_wait_read0();
+    if (!STG && threadIdx.x == 0) bulk_wait_read0();
     fence_async_smem();   // the reads above are performed before the next box loads (async proxy) may overwrite the tile
     __syncthreads();   // every thread holds its inputs: the input buffer is free, and so is the output buffer
     if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
@@ -130,29 +133,38 @@ yf2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
       Cx<T> t[K2];
       if (slot < K1) fwdB<T, L>(ex, lane, k1, t);
       __syncthreads();   // the exchange tile has been read: it becomes the output tile, rows in natural order
-      if (slot < K1) {
+      if constexpr (STG) {
+        const int colq = cb * B + lane;
+        if (slot < K1 && colq < Q) {
+          Cx<T>* out = outp + (size_t)plane * 2 * L * Q + colq;
+#pragma unroll
+          for (int k2 = 0; k2 < K2; ++k2) out[(size_t)(k1 + K1 * k2) * Q] = t[k2];
+        }
+      } else if (slot < K1) {
 #pragma unroll
         for (int k2 = 0; k2 < K2; ++k2) ex[(k1 + K1 * k2) * B + lane] = t[k2];
       }
     }
-    fence_async_smem();
-    __syncthreads();
-    if (threadIdx.x == 0) {
+    if constexpr (!STG) {
+      fence_async_smem();
+      __syncthreads();
+      if (threadIdx.x == 0) {
 #pragma unroll
-      for (int q = 0; q < 2 * L / R; ++q)
-        tma_store_2d(&mapOut, cb * TT::EW, plane * 2 * L + q * R, ex + q * R * B);
-      bulk_commit();
+        for (int q = 0; q < 2 * L / R; ++q)
+          tma_store_2d(&mapOut, cb * TT::EW, plane * 2 * L + q * R, ex + q * R * B);
+        bulk_commit();
+      }
     }
   }
-  if (threadIdx.x == 0) bulk_wait0();
+  if (!STG && threadIdx.x == 0) bulk_wait0();
 }
 
 // ---------------------------------------------------------------- K4: inverse y, truncated
 // mapIn: A2 as [(nx + 1) Py rows][2 Q reals]; mapOut: A1 as [(nx + 1) ny rows][2 Q reals].
-template <typename T, int L>
+template <typename T, int L, bool STG>
 __global__ void __launch_bounds__(TmaTile<T, L>::NT, TmaTile<T, L>::mb4)
 yi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant__ CUtensorMap mapOut,
-               const Cx<T>* __restrict__ Wt, int colblocks, int ntile) {
+               const Cx<T>* __restrict__ Wt, int colblocks, int ntile, Cx<T>* __restrict__ outp, int Q) {
   using TT = TmaTile<T, L>;
   using TL = Tile2<T, L>;
   constexpr int K1 = TL::K1, K2 = TL::K2, A = TL::A, B = TL::B, R = TT::R;
@@ -212,23 +224,32 @@ yi2_tma_kernel(const __grid_constant__ CUtensorMap mapIn, const __grid_constant_
       rot_inv_add<T, K1>(v, o, std::make_integer_sequence<int, A>{});
     }
     // the previous tile's stores must have read the output buffer before it is overwritten
-    if (threadIdx.x == 0) bulk_wait_read0();
+    if (!STG && threadIdx.x == 0) bulk_wait_read0();
     fence_async_smem();   // reads of the exchange tile performed before the async proxy overwrites it
     __syncthreads();   // the exchange tile has been read: the loads of the next tile may land in it
     if (threadIdx.x == 0 && tile + (int)gridDim.x < ntile) issue(tile + gridDim.x);
-    if (slot < K2) {
+    if constexpr (STG) {
+      const int colq = cb * B + lane;
+      if (slot < K2 && colq < Q) {
+        Cx<T>* out = outp + (size_t)plane * L * Q + colq;
 #pragma unroll
-      for (int s = 0; s < A; ++s) outb[(slot + K2 * s) * B + lane] = v[s];
-    }
-    fence_async_smem();
-    __syncthreads();
-    if (threadIdx.x == 0) {
+        for (int s = 0; s < A; ++s) out[(size_t)(slot + K2 * s) * Q] = v[s];
+      }
+    } else {
+      if (slot < K2) {
 #pragma unroll
-      for (int q = 0; q < L / R; ++q) tma_store_2d(&mapOut, cb * TT::EW, plane * L + q * R, outb + q * R * B);
-      bulk_commit();
+        for (int s = 0; s < A; ++s) outb[(slot + K2 * s) * B + lane] = v[s];
+      }
+      fence_async_smem();
+      __syncthreads();
+      if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 0; q < L / R; ++q) tma_store_2d(&mapOut, cb * TT::EW, plane * L + q * R, outb + q * R * B);
+        bulk_commit();
+      }
     }
   }
-  if (threadIdx.x == 0) bulk_wait0();
+  if (!STG && threadIdx.x == 0) bulk_wait0();
 }
 
 // ---------------------------------------------------------------- K1: forward x, r2c
@@ -822,36 +843,49 @@ int sm_count_tma() {
   return sms;
 }
 
+template <typename T, int L, bool STG>
+cudaError_t launch_tma_y(int which, const FastGeom& g, const FastBufs<T>& b, const CUtensorMap& mapA1, const CUtensorMap& mapA2,
+                         cudaStream_t st) {
+  using TT = TmaTile<T, L>;
+  using TL = Tile2<T, L>;
+  const int colblocks = (g.Q + TL::B - 1) / TL::B, ntile = colblocks * (g.nx + 1);
+  cudaError_t e;
+  int per_sm = 1;   // persistent grid = what is resident at once (registers and shared memory)
+  if (which == 1) {
+    if ((e = cudaFuncSetAttribute(yf2_tma_kernel<T, L, STG>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem2)) != cudaSuccess) return e;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, yf2_tma_kernel<T, L, STG>, TT::NT, TT::smem2) != cudaSuccess || per_sm < 1) per_sm = 1;
+    int grid = per_sm * sm_count_tma();
+    if (grid > ntile) grid = ntile;
+    yf2_tma_kernel<T, L, STG><<<grid, TT::NT, TT::smem2, st>>>(mapA1, mapA2, b.T2y, colblocks, ntile, b.A2, g.Q);
+  } else {
+    if ((e = cudaFuncSetAttribute(yi2_tma_kernel<T, L, STG>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem4)) != cudaSuccess) return e;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, yi2_tma_kernel<T, L, STG>, TT::NT, TT::smem4) != cudaSuccess || per_sm < 1) per_sm = 1;
+    int grid = per_sm * sm_count_tma();
+    if (grid > ntile) grid = ntile;
+    yi2_tma_kernel<T, L, STG><<<grid, TT::NT, TT::smem4, st>>>(mapA2, mapA1, b.T2y, colblocks, ntile, b.A1, g.Q);
+  }
+  return cudaSuccess;
+}
+
 template <typename T, int L>
 cudaError_t launch_tma(int which, const FastGeom& g, const FastBufs<T>& b, cudaStream_t st) {
   using TT = TmaTile<T, L>;
-  using TL = Tile2<T, L>;
   alignas(64) CUtensorMap mapA1, mapA2;
-  // rows must start on a 32-byte sector: with rows 16 bytes off (fp32, nz = 2 mod 4) the box stores turn into
-  // partial-sector writes and the pass runs 1.5-2.4 x slower than the LDG / STG kernel (350^3 fp32: K2 0.70 ->
-  // 1.02 ms with two, 1.71 ms with three resident CTAs; profiles/r02_tma_strided.md)
-  if (((size_t)g.Q * 2 * sizeof(T)) % 32) return cudaErrorNotSupported;
   if (!make_map<T>(&mapA1, b.A1, (size_t)(g.nx + 1) * g.ny, g.Q, TT::R) ||
       !make_map<T>(&mapA2, b.A2, (size_t)(g.nx + 1) * g.Py, g.Q, TT::R))
     return cudaErrorNotSupported;
-  const int colblocks = (g.Q + TL::B - 1) / TL::B, ntile = colblocks * (g.nx + 1);
-  cudaError_t e;
-  if (which == 1) {
-    if ((e = cudaFuncSetAttribute(yf2_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem2)) != cudaSuccess) return e;
-    int per_sm = 1;   // persistent grid = what is resident at once (registers and shared memory)
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, yf2_tma_kernel<T, L>, TT::NT, TT::smem2) != cudaSuccess || per_sm < 1) per_sm = 1;
-    int grid = per_sm * sm_count_tma();
-    if (grid > ntile) grid = ntile;
-    yf2_tma_kernel<T, L><<<grid, TT::NT, TT::smem2, st>>>(mapA1, mapA2, b.T2y, colblocks, ntile);
-  } else {
-    if ((e = cudaFuncSetAttribute(yi2_tma_kernel<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, TT::smem4)) != cudaSuccess) return e;
-    int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, yi2_tma_kernel<T, L>, TT::NT, TT::smem4) != cudaSuccess || per_sm < 1) per_sm = 1;
-    int grid = per_sm * sm_count_tma();
-    if (grid > ntile) grid = ntile;
-    yi2_tma_kernel<T, L><<<grid, TT::NT, TT::smem4, st>>>(mapA2, mapA1, b.T2y, colblocks, ntile);
+  // rows must start on a 32-byte sector for box STORES: with rows 16 bytes off (fp32, nz = 2 mod 4) they turn into
+  // partial-sector writes and the pass runs 1.5-2.4 x slower than the LDG / STG kernel (350^3 fp32: K2 0.70 ->
+  // 1.02 ms with two, 1.71 ms with three resident CTAs; profiles/r02_tma_strided.md).
+  if (((size_t)g.Q * 2 * sizeof(T)) % 32) {
+    // measured (fp32): K4 at 512x512x90 0.399 -> 0.323 ms, but K2 (twice the stores) 0.400 -> 0.657 ms, and at L = 350
+    // both lose (K2 0.70 -> 1.07, K4 0.65 -> 0.94 ms): only K4 of the power-of-two lengths takes this variant
+    if constexpr ((L & (L - 1)) == 0) {
+      if (which == 3) return launch_tma_y<T, L, true>(which, g, b, mapA1, mapA2, st);
+    }
+    return cudaErrorNotSupported;
   }
-  return cudaSuccess;
+  return launch_tma_y<T, L, false>(which, g, b, mapA1, mapA2, st);
 }
 
 // L = 1024 (three-stage plan): which = 1 (K2), 3 (K4).  Persistent, one CTA per SM.
@@ -982,8 +1016,12 @@ bool tma_enabled() {
 }
 
 // true when strided_tma_launch will run the box kernels for this transform length, row length and precision
-bool strided_tma_usable(int L, int Q, size_t real_bytes) {
-  return tma_enabled() && encode_fn() && (fast_two_stage(L) || L == 1024) && ((size_t)Q * 2 * real_bytes) % 32 == 0;
+// which: 1 = K2, 3 = K4
+bool strided_tma_usable(int L, int Q, size_t real_bytes, int which) {
+  if (!tma_enabled() || !encode_fn()) return false;
+  const bool aligned = ((size_t)Q * 2 * real_bytes) % 32 == 0;
+  if (fast_two_stage(L)) return aligned || (which == 3 && (L & (L - 1)) == 0);   // see launch_tma
+  return L == 1024 && aligned;
 }
 
 // which: 1 = K2 (forward y), 3 = K4 (inverse y).  cudaErrorNotSupported: the caller runs the LDG / STG kernel.

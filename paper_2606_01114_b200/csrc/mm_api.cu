@@ -117,7 +117,7 @@ static bool embed_mesh(const mm_ctx* c, int* ex, int* ey, int* ez) {
   int z = 0;
   const int zc[] = {c->nz, c->nz + 1, 16, 350, 400};
   for (int v : zc)
-    if (!z && v >= c->nz && fast_z_transform(v, c->es)) z = v;
+    if (!z && v >= c->nz && fast_z_transform(v, c->es, 4)) z = v;
   if (!x || !y || !z || !fast_supported(x, y, z, c->es)) return false;
   const double r = (double)x * y * z / ((double)c->nx * c->ny * c->nz);
   // fp64 with nz' = 256 runs the wide-pencil K3 at 0.34 of the roofline: a smaller margin
@@ -134,7 +134,7 @@ static void plan_layout(mm_ctx* c) {
   c->fast = c->path_pref != 1 && c->path_pref != 3 && fast_supported(c->dnx, c->dny, c->dnz, c->es);
   // x-first kernels: the z transform may be longer than 2 nz (any period >= 2 nz - 1 yields the same linear
   // convolution, reading Q27); the table and the z twiddles follow the transform
-  c->nzt = c->fast ? fast_z_transform(c->dnz, c->es) : c->dnz;
+  c->nzt = c->fast ? fast_z_transform(c->dnz, c->es, c->dny) : c->dnz;
   g.Px = padded(c->dnx); g.Py = padded(c->dny); g.Pz = padded(c->nzt);
   g.Kz = g.Pz == 1 ? 1 : g.Pz / 2 + 1;
   g.px = make_plan(c->dnx); g.py = make_plan(c->dny); g.pz = make_plan(c->dnz);
@@ -426,11 +426,11 @@ const char* mm_ctx_kernel_name(const mm_ctx* ctx, int kind) {
     switch (kind) {
       case 0: return two_x ? (strided_tma_x_usable(ctx->dnx, ctx->dny, 3 * ctx->dnz, ctx->es) ? "xf2_tma_kernel" : "xf2_kernel")
                            : (strided_tma3_x_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "xf3_tma_kernel" : "xf_fast_kernel");
-      case 1: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yf2_tma_kernel" : "yf2_kernel")
-                           : (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yf3_tma_kernel" : "yf_fast_kernel");
+      case 1: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es, 1) ? "yf2_tma_kernel" : "yf2_kernel")
+                           : (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es, 1) ? "yf3_tma_kernel" : "yf_fast_kernel");
       case 2: return ctx->nzt == 256 ? "zw_fast_kernel" : (ctx->nzt > 256 ? "zt_kernel" : "zp_fast_kernel");
-      case 3: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yi2_tma_kernel" : "yi2_kernel")
-                           : (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "yi3_tma_kernel" : "yi_fast_kernel");
+      case 3: return two_y ? (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es, 3) ? "yi2_tma_kernel" : "yi2_kernel")
+                           : (strided_tma_usable(ctx->dny, 3 * ctx->dnz, ctx->es, 3) ? "yi3_tma_kernel" : "yi_fast_kernel");
       default: return two_x ? (strided_tma_x_usable(ctx->dnx, ctx->dny, 3 * ctx->dnz, ctx->es) ? "xi2_tma_kernel" : "xi2_kernel")
                             : (strided_tma3_x_usable(ctx->dny, 3 * ctx->dnz, ctx->es) ? "xi3_tma_kernel" : "xi_fast_kernel");
     }
