@@ -226,19 +226,26 @@ template <typename T, int G> struct ZpCfg {
   static constexpr int TWS = sizeof(T) == 4 ? 1 : G;
   static constexpr int tw_bytes = sizeof(T) == 4 ? 0 : 16 * G * (int)sizeof(Cx<T>);
   static constexpr int pencil_bytes = Q * (int)sizeof(Cx<T>);
+  // Pencil pitch in shared memory.  With G < 16 a half warp (fp32) holds 16 / G pencils whose lanes touch the same
+  // relative positions; Q = 24 G is a multiple of 16 complex values, so dense pencils would share their banks (G = 8:
+  // 43 % of the wavefronts were conflicts and the pass ran at 92 % L1/shared throughput, profiles/r02_k3_thin.md).
+  // A pitch of Q + G shifts the pencils of a half warp by G banks: with each lane taking the first-stage outputs
+  // k1 = t + G i every access pattern of the kernel then covers all 16 banks once.
+  static constexpr int PQ = Q + (G < 16 ? G : 0);
+  static constexpr int slot_bytes = PQ * (int)sizeof(Cx<T>);
   static constexpr int table_bytes = 6 * OZP * (int)sizeof(T);  // one (kx, ky) row, 16 B multiple
   // per warp: two stages of NPW pencils + the table rows of the NPW / 2 mirror pairs + one slot
   // for the row ky = ny (the partner of ky = 0, the only pair that does not share its row)
-  static constexpr int warp_bytes = 2 * NPW * pencil_bytes + (NPW / 2 + 1) * table_bytes;
+  static constexpr int warp_bytes = 2 * NPW * slot_bytes + (NPW / 2 + 1) * table_bytes;
   static constexpr int hdr_for(int warps) { return (3 * warps * 8 + 127) / 128 * 128; }  // mbarriers
   static constexpr int smem_for(int warps) { return hdr_for(warps) + warps * warp_bytes + tw_bytes; }
   static constexpr int smem_bytes = smem_for(WARPS);
   static_assert(XB <= Q, "exchange buffer must fit in the pencil it aliases");
-  static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0, "bulk copies need 16 B multiples");
+  static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0 && slot_bytes % 16 == 0, "bulk copies need 16 B multiples");
 };
 
 // Forward z transform of one component of one pencil.  a[j] = sample z = t + G j (j < 8; the
-// samples j >= 8 are the zero padding).  X[i G + v] = spectrum at kz = NSUB t + i + 16 v.
+// samples j >= 8 are the zero padding).  X[i G + v] = spectrum at kz = t + G i + 16 v.
 template <typename T, int G>
 __device__ __forceinline__ void zp_forward(const Cx<T>* a, Cx<T>* xb, const Cx<T>* tw, int t,
                                            Cx<T>* X) {
@@ -268,7 +275,7 @@ __device__ __forceinline__ void zp_forward(const Cx<T>* a, Cx<T>* xb, const Cx<T
   for (int i = 0; i < C::NSUB; ++i) {
     Cx<T> b[G];
 #pragma unroll
-    for (int tp = 0; tp < G; ++tp) b[tp] = xb[(C::NSUB * t + i) * C::PITCH + tp];
+    for (int tp = 0; tp < G; ++tp) b[tp] = xb[(t + G * i) * C::PITCH + tp];
     Dft<T, G, false>::run(b);
 #pragma unroll
     for (int v = 0; v < G; ++v) X[i * G + v] = b[v];
@@ -288,7 +295,7 @@ __device__ __forceinline__ void zp_inverse(Cx<T>* r, Cx<T>* xb, const Cx<T>* tw,
     for (int v = 0; v < G; ++v) b[v] = X[i * G + v];
     Dft<T, G, true>::run(b);
 #pragma unroll
-    for (int tp = 0; tp < G; ++tp) xb[(C::NSUB * t + i) * C::PITCH + tp] = b[tp];
+    for (int tp = 0; tp < G; ++tp) xb[(t + G * i) * C::PITCH + tp] = b[tp];
   }
   __syncwarp();
   Cx<T> e[8], o[8];
@@ -321,7 +328,7 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T s3, T s4, T 
   using C = ZpCfg<T, G>;
 #pragma unroll
   for (int f = 0; f < 16; ++f) {
-    const int kz = C::NSUB * t + (f / G) + 16 * (f % G);
+    const int kz = t + G * (f / G) + 16 * (f % G);
     // kz > nz (the mirrored half, where N_xz and N_yz change sign) is known at compile time
     // except for the one block of frequencies that straddles kz = nz
     bool mir;
@@ -347,11 +354,8 @@ __device__ __forceinline__ void zp_multiply(const T* trow, int t, T s3, T s4, T 
 // xm != 0 (MASK variant only): the rows of a plane are kx, not ky (slab layout, demag_slab.cuh).
 // MASK: the mesh has nzd < 8 G layers (any period Pz >= 2 nzd - 1 gives the same linear convolution, reading
 // Q27): pencils in HBM hold 3 nzd values, the samples z >= nzd read as zero and only 3 nzd values go back.
-// CONTIG (only without MASK): the rows of a plane lie in natural ky order (two-stage y pass), so the NPW/2 even
-// pencils of a task (ky = i0 ..) are one contiguous run of A2, the odd ones (ky = Py - i0 - NPW/2 + 1 .. Py - i0)
-// another, and their table rows a third: three bulk copies in and two out per task instead of one per pencil
-// (NPW = 4, 8: nz = 64, 32, whose 1.5 KB / 768 B pencils made the pass wait on copy issue: 0.56 / 0.31 of the roofline
-// against 0.70 at nz = 128).  Odd pencils are kept in ascending row order: pencil pw at slot loc(pw).
+// CONTIG (only without MASK): the rows of a plane lie in natural ky order (two-stage y pass), so the table rows of
+// the NPW/2 mirror pairs of a task are one contiguous run: one bulk copy instead of NPW/2.
 template <typename T, int G, int WARPS, int MINB, bool MASK, bool CONTIG = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* __restrict__ Wz,
@@ -365,7 +369,7 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 3 * warp;  // stage 0, stage 1, table
   unsigned char* wraw = smem_raw + C::hdr_for(WARPS) + (size_t)warp * C::warp_bytes;
   Cx<T>* pbase = reinterpret_cast<Cx<T>*>(wraw);
-  T* tbase = reinterpret_cast<T*>(wraw + 2 * NPW * C::pencil_bytes);
+  T* tbase = reinterpret_cast<T*>(wraw + 2 * NPW * C::slot_bytes);
   const int t = lane % G, pw = lane / G;
   const int Py = 2 * ny;
   if (threadIdx.x == 0) {
@@ -394,32 +398,10 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     const int ky = (p & 1) ? (i == 0 ? ny : Py - i) : i;
     return A2 + ((size_t)plane * Py + posy[ky]) * qd;
   };
-  // slot of pencil p (pair p >> 1, odd = p & 1) within a stage
-  auto loc = [&](int p) -> int {
-    if constexpr (CONTIG) return (p & 1) ? NPW - 1 - (p >> 1) : (p >> 1);
-    else return p;
-  };
-  // CONTIG: the runs of a task as (slot, first row, rows); pair i0 = 0 has ky = ny, not Py, as its odd pencil
-  auto for_runs = [&](int task, auto&& f) {
-    const int pair0 = task * (NPW / 2), plane = pair0 / ny, i0 = pair0 - plane * ny;
-    const size_t row0 = (size_t)plane * Py;
-    f(0, row0 + i0, NPW / 2);
-    if (i0 != 0) f(NPW / 2, row0 + Py - i0 - (NPW / 2 - 1), NPW / 2);
-    else {
-      if (NPW / 2 > 1) f(NPW / 2, row0 + Py - (NPW / 2 - 1), NPW / 2 - 1);
-      f(NPW - 1, row0 + ny, 1);
-    }
-  };
   auto issue = [&](int task, int stage) {
     mbar_expect_tx(bars + stage, NPW * pbytes);
-    if constexpr (CONTIG) {
-      for_runs(task, [&](int slot0, size_t row, int rows) {
-        bulk_load(pbase + (stage * NPW + slot0) * Q, A2 + row * Q, rows * pbytes, bars + stage);
-      });
-    } else {
-      for (int p = 0; p < NPW; ++p)
-        bulk_load(pbase + (stage * NPW + p) * Q, pencil_ptr(task, p), pbytes, bars + stage);
-    }
+    for (int p = 0; p < NPW; ++p)
+      bulk_load(pbase + (stage * NPW + p) * C::PQ, pencil_ptr(task, p), pbytes, bars + stage);
   };
   // table rows of a task: ky = i for mirror pair i; the pair i = 0 (always the first of its
   // task) is (ky = 0, ky = ny) and needs the row ky = ny as well, in the extra slot
@@ -451,7 +433,7 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     }
     __syncwarp();
     mbar_wait(bars + stage, (it >> 1) & 1);
-    Cx<T>* pen = pbase + (stage * NPW + loc(pw)) * Q;
+    Cx<T>* pen = pbase + (stage * NPW + pw) * C::PQ;
     Cx<T> X[3][16];
     {
       Cx<T> a[3][8];
@@ -492,14 +474,8 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
     fence_async_smem();
     __syncwarp();
     if (lane == 0) {
-      if constexpr (CONTIG) {
-        for_runs(task, [&](int slot0, size_t row, int rows) {
-          bulk_store(A2 + row * Q, pbase + (stage * NPW + slot0) * Q, rows * pbytes);
-        });
-      } else {
-        for (int p = 0; p < NPW; ++p)
-          bulk_store(pencil_ptr(task, p), pbase + (stage * NPW + p) * Q, pbytes);
-      }
+      for (int p = 0; p < NPW; ++p)
+        bulk_store(pencil_ptr(task, p), pbase + (stage * NPW + p) * C::PQ, pbytes);
       bulk_commit();
     }
   }
