@@ -169,7 +169,8 @@ def test_tma_box_kernels_bit_identical_to_ldg_kernels(tmp_path):
     assert n_tma >= 4 * (len(specs) - 2) + 2
 
 
-@pytest.mark.parametrize("spec", ["128,64,64,f64", "64,128,64,f64", "256,128,32,f32"])
+@pytest.mark.parametrize("spec", ["128,64,64,f64", "64,128,64,f64", "256,128,32,f32", "1024,64,16,f64", "64,1024,16,f32",
+                                  "1024,1024,16,f32"])
 def test_persistent_box_kernels_are_race_free_over_many_calls(spec):
     """The persistent TMA kernels prefetch the next tile into a buffer the threads have just read.  Without a
     proxy fence before the barrier the box load was seen to overwrite a row ahead of its read about once in
@@ -184,7 +185,7 @@ def test_persistent_box_kernels_are_race_free_over_many_calls(spec):
     ref = ctx.demag_field(md).clone()
     out = torch.empty_like(md)
     bad = 0
-    for _ in range(600):
+    for _ in range(600 if n[0] * n[1] < 1e6 else 150):
         ctx.demag_field(md, out)
         bad += int(not torch.equal(out, ref))
     ctx.close()
