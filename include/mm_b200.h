@@ -236,6 +236,34 @@ mm_status mm_ctx_path(const mm_ctx *ctx, int *path);
  * to rounding (different transform order). */
 mm_status mm_ctx_set_slabs(mm_ctx *ctx, int ranks);
 
+/* mm_demag_field for callers that cannot provide (or allocate) the scratch of the convolution at call time:
+ * code inside a CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same operation, same
+ * kernels and bit-identical result as mm_demag_field (PAPER.md:45 eq. 4, :47, :53), but the two padded spectra
+ * A1, A2 live in ONE file-scope `static __device__` array of the library of
+ * MM_STATIC_SCRATCH_BYTES bytes instead of the context's scratch workspace.  Every GPU that loads the library
+ * holds that array until the process exits.
+ *  - m, H: DEVICE pointers as for mm_demag_field, still passed by the caller.  The context must be set up as
+ *    usual (mm_ctx_set_workspace, mm_set_material, mm_demag_init: the Fourier-space tensor and the twiddle
+ *    tables in the persistent workspace are inputs of the call); the context's scratch workspace is not touched.
+ *  - Limit: the spectra of the mesh must fit (mm_static_scratch_info reports capacity and need; 64^3 in fp32
+ *    needs 19.2 MB); otherwise MM_ERR_WORKSPACE with the two numbers in mm_last_error.  Contexts with per-cell
+ *    Ms, an enclosing (embedded) mesh or the slab emulation need more than the spectra: MM_ERR_NOT_IMPLEMENTED.
+ *  - Allocates nothing: no cudaMalloc / cudaFree / allocating library routine on this call's path.  The
+ *    array's device address is looked up once per device (cudaGetSymbolAddress, which loads the module on
+ *    that device); do that outside a capture by calling mm_static_scratch_info once per device at set-up,
+ *    with that device current.  The call itself looks it up too if that has not happened.
+ *  - Shared state: ALL contexts and all calls on a device share the one array, which keeps the contents of the
+ *    last call.  Nothing in it has to start at zero (the forward passes write every element the later passes
+ *    read), so nothing is cleared.  Two calls that overlap on the GPU (different streams, or a graph replay
+ *    beside a direct call) RACE on it and both results are garbage; calls on one stream are ordered and safe.
+ *  - Asynchronous on the context's stream, capturable, like mm_demag_field. */
+#define MM_STATIC_SCRATCH_BYTES (32u << 20)
+mm_status mm_demag_field_static(mm_ctx *ctx, const void *m, void *H);
+/* capacity := MM_STATIC_SCRATCH_BYTES; needed := bytes mm_demag_field_static uses for this context (0 where it
+ * answers MM_ERR_NOT_IMPLEMENTED; left alone if ctx is NULL).  Either output may be NULL.  Also the set-up
+ * step: resolves the static array's address for the CURRENT device.  Allocates nothing. */
+mm_status mm_static_scratch_info(const mm_ctx *ctx, size_t *capacity, size_t *needed);
+
 /* Last error text of this context (or of the last failed mm_ctx_create if ctx is NULL).
  * Not thread-safe. */
 const char *mm_last_error(const mm_ctx *ctx);

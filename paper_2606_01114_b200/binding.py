@@ -73,6 +73,8 @@ def load_library():
         "mm_minimize_step": [vp, vp],
         "mm_minimize_state": [vp, C.POINTER(C.c_ulonglong), C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i32)],
         "mm_minimize": [vp, vp, i32, i32, C.POINTER(C.c_ulonglong), C.POINTER(i32)],
+        "mm_demag_field_static": [vp, vp, vp],
+        "mm_static_scratch_info": [vp, C.POINTER(sz), C.POINTER(sz)],
         "mm_demag_field_host": [vp, vp, vp],
         "mm_heff_host": [vp, vp, vp],
         "mm_llg_rhs_host": [vp, vp, vp],
@@ -243,6 +245,17 @@ class Context:
 
     def demag_field(self, m, out=None):
         return self._field("mm_demag_field", m, out)
+
+    def demag_field_static(self, m, out=None):
+        """mm_demag_field with the spectra in the library's static device array (no allocation in the library;
+        pass `out` to allocate nothing here either).  Calls that overlap on the GPU race on that array."""
+        return self._field("mm_demag_field_static", m, out)
+
+    def static_scratch_info(self):
+        """(capacity, needed) in bytes; also resolves the static array's address on the current device."""
+        cap, need = C.c_size_t(0), C.c_size_t(0)
+        self._call("mm_static_scratch_info", C.byref(cap), C.byref(need))
+        return cap.value, need.value
 
     def exchange_field(self, m, out=None):
         return self._field("mm_exchange_field", m, out)

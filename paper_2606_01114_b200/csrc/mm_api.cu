@@ -1070,6 +1070,99 @@ mm_status mm_minimize(mm_ctx* ctx, void* m_inout, int max_iter, int check_every,
   return s;
 }
 
+// ---- mm_demag_field_static: the convolution with its spectra in a static device array (no allocation)
+
+}  // extern "C"
+
+// The spectra A1, A2 of mm_demag_field_static.  One copy per GPU that loads this module, held until exit.
+// In host code `g_static_scratch` is only a handle for cudaGetSymbolAddress, never a device address.
+static __device__ __align__(256) unsigned char g_static_scratch[MM_STATIC_SCRATCH_BYTES];
+
+constexpr int kMaxStaticDevices = 64;
+static unsigned char* g_static_ptr[kMaxStaticDevices] = {nullptr};   // device address of the array, per device ordinal
+
+// device address of g_static_scratch on the current device, looked up once per device
+static cudaError_t static_scratch_ptr(unsigned char** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxStaticDevices) return cudaErrorInvalidDevice;
+  unsigned char* p = __atomic_load_n(&g_static_ptr[dev], __ATOMIC_ACQUIRE);
+  if (!p) {
+    void* q = nullptr;
+    e = cudaGetSymbolAddress(&q, g_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!q || ((uintptr_t)q & 255)) return cudaErrorInvalidSymbol;
+    p = static_cast<unsigned char*>(q);
+    __atomic_store_n(&g_static_ptr[dev], p, __ATOMIC_RELEASE);   // every thread finds the same address
+  }
+  *out = p;
+  return cudaSuccess;
+}
+
+// bytes of the two spectra (they sit first in the scratch carve-up: off_a1 = 0), or 0 where the path needs more
+static size_t static_need(const mm_ctx* c) {
+  if (c->ms_cells || c->embed || c->slabs) return 0;
+  return c->off_hd;
+}
+
+template <typename T> static mm_status demag_static_t(mm_ctx* c, unsigned char* sp, const void* m, void* H) {
+  Cx<T>* A1 = reinterpret_cast<Cx<T>*>(sp + c->off_a1);
+  Cx<T>* A2 = reinterpret_cast<Cx<T>*>(sp + c->off_a2);
+  cudaError_t e;
+  if (c->mixed) {
+    const MixedPlans pl{c->geom.px, c->geom.py, c->geom.pz};
+    MixedBufs<T> b = mixed_bufs_of<T>(c);
+    b.A1 = A1; b.A2 = A2;
+    e = demag_mixed_launch<T>(c->fgeom, pl, b, static_cast<const T*>(m), static_cast<T*>(H), (T)(-c->Ms), c->stream,
+                              &c->launches, &c->prof);
+  } else if (c->fast) {
+    FastBufs<T> b = fast_bufs_of<T>(c);
+    b.A1 = A1; b.A2 = A2;
+    e = demag_fast_launch<T>(c->fgeom, b, static_cast<const T*>(m), static_cast<T*>(H), (T)(-c->Ms), c->stream,
+                             &c->launches, &c->prof);
+  } else {
+    DemagBufs<T> b = bufs_of<T>(c);
+    b.A1 = A1; b.A2 = A2;
+    e = demag_field_launch<T>(c->geom, b, static_cast<const T*>(m), static_cast<T*>(H), (T)(-c->Ms), c->stream,
+                              &c->launches, &c->prof);
+  }
+  return e == cudaSuccess ? MM_OK : cuda_fail(c, "mm_demag_field_static launch", e);
+}
+
+extern "C" {
+
+mm_status mm_static_scratch_info(const mm_ctx* ctx, size_t* capacity, size_t* needed) {
+  if (capacity) *capacity = MM_STATIC_SCRATCH_BYTES;
+  if (ctx && needed) *needed = static_need(ctx);
+  unsigned char* sp = nullptr;
+  const cudaError_t e = static_scratch_ptr(&sp);
+  if (e == cudaSuccess) return MM_OK;
+  if (ctx) return cuda_fail(const_cast<mm_ctx*>(ctx), "mm_static_scratch_info: cudaGetSymbolAddress", e);
+  snprintf(g_create_error, sizeof g_create_error, "mm_static_scratch_info: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+  return MM_ERR_CUDA;
+}
+
+mm_status mm_demag_field_static(mm_ctx* ctx, const void* m, void* H) {
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  mm_status s;
+  if ((s = check_ptr(ctx, "mm_demag_field_static", m, H)) != MM_OK) return s;
+  if (m == H) return fail(ctx, MM_ERR_INVALID_ARG, "mm_demag_field_static: H must not alias m");
+  if ((s = need_ready(ctx, "mm_demag_field_static", true)) != MM_OK) return s;
+  const size_t need = static_need(ctx);
+  if (need == 0)
+    return fail(ctx, MM_ERR_NOT_IMPLEMENTED,
+                "mm_demag_field_static: per-cell Ms, embedded meshes and slabs need more than the spectra; use mm_demag_field");
+  if (need > (size_t)MM_STATIC_SCRATCH_BYTES)
+    return fail(ctx, MM_ERR_WORKSPACE,
+                "mm_demag_field_static: the spectra of this mesh need %zu bytes, the static array holds %zu; use mm_demag_field",
+                need, (size_t)MM_STATIC_SCRATCH_BYTES);
+  unsigned char* sp = nullptr;
+  const cudaError_t e = static_scratch_ptr(&sp);
+  if (e != cudaSuccess) return cuda_fail(ctx, "mm_demag_field_static: cudaGetSymbolAddress", e);
+  return ctx->dtype == MM_F32 ? demag_static_t<float>(ctx, sp, m, H) : demag_static_t<double>(ctx, sp, m, H);
+}
+
 // ---- host-buffer variants: H2D, device path, D2H, synchronise
 
 static mm_status host_call(mm_ctx* ctx, const char* fn, int which, const void* in_host, void* out_host,
