@@ -182,6 +182,16 @@ mm_status mm_demag_field_host(mm_ctx *ctx, const void *m_host, void *H_host);
 mm_status mm_heff_host(mm_ctx *ctx, const void *m_host, void *H_host);
 mm_status mm_llg_rhs_host(mm_ctx *ctx, const void *m_host, void *dmdt_host);
 mm_status mm_rk_step_host(mm_ctx *ctx, void *m_inout_host, double dt);
+/* count INDEPENDENT evaluations of mm_llg_rhs on host buffers (a parameter sweep, an ensemble): result i equals
+ * mm_llg_rhs_host(m_host[i], dmdt_host[i]) bit for bit.  m_host, dmdt_host: HOST arrays of count HOST pointers to
+ * [nx][ny][nz][3] buffers; an input may repeat, an output that repeats keeps the last result written to it (results
+ * leave in order), outputs must not alias inputs.  Pipelined: the
+ * upload of state i + 1 and the download of result i - 1 run on two copy streams of the library beside the kernels
+ * of state i (PCIe is full duplex), through two staging slots per direction in scratch (the second pair is the RK4
+ * stage buffers: do not run it while a captured mm_rk_steps graph is replaying).  The copies overlap only for
+ * PINNED host memory; pageable buffers work but serialise.  Creates two streams and six events on first use (no
+ * device memory).  Synchronises all three streams before returning; count = 0 is a no-op. */
+mm_status mm_llg_rhs_host_batch(mm_ctx *ctx, const void *const *m_host, void *const *dmdt_host, int count);
 
 /* ------------------------------------------------------------------------------------------
  * Diagnostics and experiments.  Not part of the method's boundary: bench.py, the

@@ -79,6 +79,7 @@ def load_library():
         "mm_heff_host": [vp, vp, vp],
         "mm_llg_rhs_host": [vp, vp, vp],
         "mm_rk_step_host": [vp, vp, dbl],
+        "mm_llg_rhs_host_batch": [vp, C.POINTER(vp), C.POINTER(vp), i32],
         "mm_ctx_launch_count": [vp, C.POINTER(C.c_ulonglong)],
         "mm_ctx_set_tiles": [vp, i32, i32, i32],
         "mm_ctx_set_path": [vp, i32],
@@ -345,6 +346,24 @@ class Context:
 
     def llg_rhs_host(self, m_host, out_host=None):
         return self._host("mm_llg_rhs_host", m_host, out_host)
+
+    def llg_rhs_host_batch(self, m_hosts, out_hosts):
+        """Independent evaluations on lists of host buffers, copies pipelined beside the kernels (pinned memory)."""
+        want = np.float32 if self.dtype == torch.float32 else np.float64
+        arrs = []
+        for lst in (m_hosts, out_hosts):
+            a = [x if isinstance(x, np.ndarray) else x.numpy() for x in lst]
+            for x in a:
+                if x.dtype != want or not x.flags.c_contiguous or x.shape != self.n + (3,):
+                    raise ValueError("host buffers must be C-contiguous, context dtype, [nx,ny,nz,3]")
+            arrs.append(a)
+        if len(arrs[0]) != len(arrs[1]):
+            raise ValueError("as many outputs as inputs")
+        k = len(arrs[0])
+        pin = (C.c_void_p * max(k, 1))(*[x.ctypes.data for x in arrs[0]])
+        pout = (C.c_void_p * max(k, 1))(*[x.ctypes.data for x in arrs[1]])
+        self._call("mm_llg_rhs_host_batch", pin, pout, k)
+        return out_hosts
 
     def rk_step_host(self, m_host, dt):
         a = m_host if isinstance(m_host, np.ndarray) else m_host.numpy()

@@ -75,6 +75,9 @@ struct mm_ctx {
   double rk_graph_dt = 0;
   int rk_graph_steps = 0;
   unsigned long long rk_graph_epoch = 0, rk_graph_launches = 0;
+  // mm_llg_rhs_host_batch: copy streams and the events that order the two staging slots
+  cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
   Prof prof;
   double prof_ms[Prof::kKinds] = {0};
   unsigned long long prof_cnt[Prof::kKinds] = {0};
@@ -244,6 +247,13 @@ mm_status mm_ctx_destroy(mm_ctx* ctx) {
   if (ctx) {
     if (ctx->rk_graph) cudaGraphExecDestroy(ctx->rk_graph);
     if (ctx->rk_capture_stream) cudaStreamDestroy(ctx->rk_capture_stream);
+    if (ctx->h2d_stream) cudaStreamDestroy(ctx->h2d_stream);
+    if (ctx->d2h_stream) cudaStreamDestroy(ctx->d2h_stream);
+    for (int i = 0; i < 2; ++i) {
+      if (ctx->ev_in[i]) cudaEventDestroy(ctx->ev_in[i]);
+      if (ctx->ev_comp[i]) cudaEventDestroy(ctx->ev_comp[i]);
+      if (ctx->ev_out[i]) cudaEventDestroy(ctx->ev_out[i]);
+    }
   }
   delete ctx;
   return MM_OK;
@@ -1200,6 +1210,57 @@ mm_status mm_llg_rhs_host(mm_ctx* ctx, const void* m_host, void* dmdt_host) {
 }
 mm_status mm_rk_step_host(mm_ctx* ctx, void* m_inout_host, double dt) {
   return host_call(ctx, "mm_rk_step_host", 3, m_inout_host, m_inout_host, dt);
+}
+
+// count independent evaluations: the upload of state i + 1 and the download of result i - 1 run on copy streams
+// of their own beside the kernels of state i, two staging slots per direction (slot 1 = the RK4 stage buffers).
+mm_status mm_llg_rhs_host_batch(mm_ctx* ctx, const void* const* m_host, void* const* dmdt_host, int count) {
+  const char* fn = "mm_llg_rhs_host_batch";
+  if (!ctx) return MM_ERR_INVALID_ARG;
+  if (count < 0 || (count > 0 && (!m_host || !dmdt_host))) return fail(ctx, MM_ERR_INVALID_ARG, "%s: NULL array or negative count", fn);
+  for (int i = 0; i < count; ++i)
+    if (!m_host[i] || !dmdt_host[i]) return fail(ctx, MM_ERR_INVALID_ARG, "%s: NULL host pointer at index %d", fn, i);
+  mm_status s;
+  if ((s = need_ready(ctx, fn, (ctx->terms & MM_TERM_DEMAG) != 0)) != MM_OK) return s;
+  if (count == 0) return MM_OK;
+  cudaError_t e = cudaSuccess;
+  if (!ctx->h2d_stream) {   // streams and events hold no device memory
+    if ((e = cudaStreamCreateWithFlags(&ctx->h2d_stream, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(ctx, fn, e);
+    if ((e = cudaStreamCreateWithFlags(&ctx->d2h_stream, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(ctx, fn, e);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+      e = cudaEventCreateWithFlags(&ctx->ev_in[i], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_comp[i], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_out[i], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, fn, e);
+  }
+  const size_t n3 = (size_t)ctx->nx * ctx->ny * ctx->nz * 3 * ctx->es;
+  void* din[2] = {ctx->scr + ctx->off_sin, ctx->scr + ctx->off_msa};
+  void* dout[2] = {ctx->scr + ctx->off_sout, ctx->scr + ctx->off_msb};
+  // earlier work on the context's stream may still use the slots
+  if ((e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) return cuda_fail(ctx, fn, e);
+  for (int i = 0; i < count; ++i) {
+    const int k = i & 1;
+    if (i >= 2) e = cudaStreamWaitEvent(ctx->h2d_stream, ctx->ev_comp[k], 0);   // evaluation i - 2 has read slot k
+    if (e == cudaSuccess) e = cudaMemcpyAsync(din[k], m_host[i], n3, cudaMemcpyHostToDevice, ctx->h2d_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_in[k], ctx->h2d_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->stream, ctx->ev_in[k], 0);
+    if (e == cudaSuccess && i >= 2) e = cudaStreamWaitEvent(ctx->stream, ctx->ev_out[k], 0);   // result i - 2 has left slot k
+    if (e != cudaSuccess) break;
+    if ((s = mm_llg_rhs(ctx, din[k], dout[k])) != MM_OK) {
+      cudaStreamSynchronize(ctx->h2d_stream); cudaStreamSynchronize(ctx->stream); cudaStreamSynchronize(ctx->d2h_stream);
+      return s;
+    }
+    e = cudaEventRecord(ctx->ev_comp[k], ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->d2h_stream, ctx->ev_comp[k], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dmdt_host[i], dout[k], n3, cudaMemcpyDeviceToHost, ctx->d2h_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_out[k], ctx->d2h_stream);
+    if (e != cudaSuccess) break;
+  }
+  const cudaError_t e1 = cudaStreamSynchronize(ctx->h2d_stream), e2 = cudaStreamSynchronize(ctx->stream),
+                    e3 = cudaStreamSynchronize(ctx->d2h_stream);
+  if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
+  return e == cudaSuccess ? MM_OK : cuda_fail(ctx, fn, e);
 }
 
 }  // extern "C"

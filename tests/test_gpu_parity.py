@@ -255,6 +255,40 @@ def test_host_calls_match_device_calls(oracle):
     assert np.array_equal(m2, md.cpu().numpy())
 
 
+@pytest.mark.parametrize("dt,pinned", [("f32", True), ("f64", True), ("f32", False)])
+def test_host_batch_matches_single_host_calls_and_the_oracle(oracle, dt, pinned):
+    """mm_llg_rhs_host_batch: seven independent states through two staging slots per direction (every slot
+    reused three times, copies on their own streams) equal the one-at-a-time host call bit for bit, and
+    the oracle within the north_star tolerance; count 0 and 1; a repeated input."""
+    cfg = cfg_for((64, 64, 16), (4e-9, 3e-9, 2e-9))
+    ctx = make_ctx(cfg, dt)
+    ndt = np.float32 if dt == "f32" else np.float64
+
+    def host(a):
+        t = torch.from_numpy(np.ascontiguousarray(a))
+        return t.pin_memory() if pinned else t
+
+    ms = [host(round_input(w.random_unit_vectors(40 + i, cfg.n), dt)[0]) for i in range(6)]
+    ms.append(ms[2])                                               # an input may repeat
+    outs = [host(np.full(cfg.n + (3,), np.nan, dtype=ndt)) for _ in ms]
+    for rep in range(2):                                           # a second batch finds the slots used
+        ctx.llg_rhs_host_batch(ms, outs)
+        for m, o in zip(ms, outs):
+            assert np.array_equal(o.numpy(), ctx.llg_rhs_host(m.numpy()))
+    assert np.array_equal(outs[6].numpy(), outs[2].numpy())
+    P = make_problem(oracle, cfg)
+    ref = P.llg_rhs(ms[5].numpy().astype(np.float64))
+    l2, mx = w.field_errors(outs[5].numpy(), ref)
+    assert l2 <= TOL[dt], (l2, mx)
+    ctx.llg_rhs_host_batch([], [])
+    one = host(np.zeros(cfg.n + (3,), dtype=ndt))
+    ctx.llg_rhs_host_batch(ms[:1], [one])
+    assert np.array_equal(one.numpy(), outs[0].numpy())
+    # the device path still works on the context's stream afterwards
+    assert np.array_equal(ctx.llg_rhs(to_dev(ms[1].numpy())).cpu().numpy(), outs[1].numpy())
+    ctx.close()
+
+
 def test_error_paths_on_device():
     from paper_2606_01114_b200 import Context, MMError
     ctx = Context((8, 8, 2), (1e-9,) * 3, dtype=torch.float32)
