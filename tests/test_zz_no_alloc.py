@@ -117,3 +117,30 @@ def test_static_rejects_contexts_that_need_more_than_the_spectra():
     assert ei.value.status == MM_ERR_NOT_IMPLEMENTED
     assert ctx.static_scratch_info()[1] == 0
     ctx.close()
+
+
+def test_static_call_inside_a_cuda_graph_capture():
+    """The caller this entry point is for: a capture, where nothing may allocate.  Set-up (address look-up,
+    kernel attributes) happens before the capture; the captured call is replayed on new inputs."""
+    n, dt = (64, 64, 32), "f32"
+    ctx = make_ctx(cfg_for(n), dt, terms=1)
+    ctx.static_scratch_info()
+    md = to_dev(round_input(w.random_unit_vectors(21, n), dt)[0])
+    H = torch.zeros_like(md)
+    ctx.demag_field_static(md, out=H)                       # warm-up outside the capture
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        ctx.use_current_stream()
+        with torch.cuda.graph(g, stream=side):
+            ctx.demag_field_static(md, out=H)
+    torch.cuda.synchronize()
+    ctx.use_current_stream()
+    for seed in (22, 23):                                   # two replays in a row on fresh inputs
+        md.copy_(to_dev(round_input(w.random_unit_vectors(seed, n), dt)[0]))
+        H.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(H, ctx.demag_field(md))
+    ctx.close()
