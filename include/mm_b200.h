@@ -192,6 +192,9 @@ mm_status mm_rk_step_host(mm_ctx *ctx, void *m_inout_host, double dt);
  * PINNED host memory; pageable buffers work but serialise.  Creates two streams and six events on first use (no
  * device memory).  Synchronises all three streams before returning; count = 0 is a no-op. */
 mm_status mm_llg_rhs_host_batch(mm_ctx *ctx, const void *const *m_host, void *const *dmdt_host, int count);
+/* The same pipeline for H_demag and H_eff (results equal mm_demag_field_host / mm_heff_host bit for bit). */
+mm_status mm_demag_field_host_batch(mm_ctx *ctx, const void *const *m_host, void *const *H_host, int count);
+mm_status mm_heff_host_batch(mm_ctx *ctx, const void *const *m_host, void *const *H_host, int count);
 
 /* ------------------------------------------------------------------------------------------
  * Diagnostics and experiments.  Not part of the method's boundary: bench.py, the

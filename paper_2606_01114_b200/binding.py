@@ -80,6 +80,8 @@ def load_library():
         "mm_llg_rhs_host": [vp, vp, vp],
         "mm_rk_step_host": [vp, vp, dbl],
         "mm_llg_rhs_host_batch": [vp, C.POINTER(vp), C.POINTER(vp), i32],
+        "mm_demag_field_host_batch": [vp, C.POINTER(vp), C.POINTER(vp), i32],
+        "mm_heff_host_batch": [vp, C.POINTER(vp), C.POINTER(vp), i32],
         "mm_ctx_launch_count": [vp, C.POINTER(C.c_ulonglong)],
         "mm_ctx_set_tiles": [vp, i32, i32, i32],
         "mm_ctx_set_path": [vp, i32],
@@ -349,6 +351,15 @@ class Context:
 
     def llg_rhs_host_batch(self, m_hosts, out_hosts):
         """Independent evaluations on lists of host buffers, copies pipelined beside the kernels (pinned memory)."""
+        return self._host_batch("mm_llg_rhs_host_batch", m_hosts, out_hosts)
+
+    def demag_field_host_batch(self, m_hosts, out_hosts):
+        return self._host_batch("mm_demag_field_host_batch", m_hosts, out_hosts)
+
+    def heff_host_batch(self, m_hosts, out_hosts):
+        return self._host_batch("mm_heff_host_batch", m_hosts, out_hosts)
+
+    def _host_batch(self, name, m_hosts, out_hosts):
         want = np.float32 if self.dtype == torch.float32 else np.float64
         arrs = []
         for lst in (m_hosts, out_hosts):
@@ -362,7 +373,7 @@ class Context:
         k = len(arrs[0])
         pin = (C.c_void_p * max(k, 1))(*[x.ctypes.data for x in arrs[0]])
         pout = (C.c_void_p * max(k, 1))(*[x.ctypes.data for x in arrs[1]])
-        self._call("mm_llg_rhs_host_batch", pin, pout, k)
+        self._call(name, pin, pout, k)
         return out_hosts
 
     def rk_step_host(self, m_host, dt):

@@ -1214,14 +1214,14 @@ mm_status mm_rk_step_host(mm_ctx* ctx, void* m_inout_host, double dt) {
 
 // count independent evaluations: the upload of state i + 1 and the download of result i - 1 run on copy streams
 // of their own beside the kernels of state i, two staging slots per direction (slot 1 = the RK4 stage buffers).
-mm_status mm_llg_rhs_host_batch(mm_ctx* ctx, const void* const* m_host, void* const* dmdt_host, int count) {
-  const char* fn = "mm_llg_rhs_host_batch";
+static mm_status host_batch(mm_ctx* ctx, const char* fn, int which, const void* const* m_host, void* const* dmdt_host,
+                            int count) {
   if (!ctx) return MM_ERR_INVALID_ARG;
   if (count < 0 || (count > 0 && (!m_host || !dmdt_host))) return fail(ctx, MM_ERR_INVALID_ARG, "%s: NULL array or negative count", fn);
   for (int i = 0; i < count; ++i)
     if (!m_host[i] || !dmdt_host[i]) return fail(ctx, MM_ERR_INVALID_ARG, "%s: NULL host pointer at index %d", fn, i);
   mm_status s;
-  if ((s = need_ready(ctx, fn, (ctx->terms & MM_TERM_DEMAG) != 0)) != MM_OK) return s;
+  if ((s = need_ready(ctx, fn, which == 0 || (ctx->terms & MM_TERM_DEMAG) != 0)) != MM_OK) return s;
   if (count == 0) return MM_OK;
   cudaError_t e = cudaSuccess;
   if (!ctx->h2d_stream) {   // streams and events hold no device memory
@@ -1247,7 +1247,8 @@ mm_status mm_llg_rhs_host_batch(mm_ctx* ctx, const void* const* m_host, void* co
     if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->stream, ctx->ev_in[k], 0);
     if (e == cudaSuccess && i >= 2) e = cudaStreamWaitEvent(ctx->stream, ctx->ev_out[k], 0);   // result i - 2 has left slot k
     if (e != cudaSuccess) break;
-    if ((s = mm_llg_rhs(ctx, din[k], dout[k])) != MM_OK) {
+    s = which == 0 ? mm_demag_field(ctx, din[k], dout[k]) : which == 1 ? mm_heff(ctx, din[k], dout[k]) : mm_llg_rhs(ctx, din[k], dout[k]);
+    if (s != MM_OK) {
       cudaStreamSynchronize(ctx->h2d_stream); cudaStreamSynchronize(ctx->stream); cudaStreamSynchronize(ctx->d2h_stream);
       return s;
     }
@@ -1261,6 +1262,16 @@ mm_status mm_llg_rhs_host_batch(mm_ctx* ctx, const void* const* m_host, void* co
                     e3 = cudaStreamSynchronize(ctx->d2h_stream);
   if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
   return e == cudaSuccess ? MM_OK : cuda_fail(ctx, fn, e);
+}
+
+mm_status mm_demag_field_host_batch(mm_ctx* ctx, const void* const* m_host, void* const* H_host, int count) {
+  return host_batch(ctx, "mm_demag_field_host_batch", 0, m_host, H_host, count);
+}
+mm_status mm_heff_host_batch(mm_ctx* ctx, const void* const* m_host, void* const* H_host, int count) {
+  return host_batch(ctx, "mm_heff_host_batch", 1, m_host, H_host, count);
+}
+mm_status mm_llg_rhs_host_batch(mm_ctx* ctx, const void* const* m_host, void* const* dmdt_host, int count) {
+  return host_batch(ctx, "mm_llg_rhs_host_batch", 2, m_host, dmdt_host, count);
 }
 
 }  // extern "C"

@@ -284,6 +284,12 @@ def test_host_batch_matches_single_host_calls_and_the_oracle(oracle, dt, pinned)
     one = host(np.zeros(cfg.n + (3,), dtype=ndt))
     ctx.llg_rhs_host_batch(ms[:1], [one])
     assert np.array_equal(one.numpy(), outs[0].numpy())
+    # the same pipeline for H_demag and H_eff
+    for batch, single in ((ctx.demag_field_host_batch, ctx.demag_field_host), (ctx.heff_host_batch, ctx.heff_host)):
+        batch(ms[:3], outs[:3])
+        for m, o in zip(ms[:3], outs[:3]):
+            assert np.array_equal(o.numpy(), single(m.numpy()))
+    ctx.llg_rhs_host_batch(ms[:2], outs[:2])
     # the device path still works on the context's stream afterwards
     assert np.array_equal(ctx.llg_rhs(to_dev(ms[1].numpy())).cpu().numpy(), outs[1].numpy())
     ctx.close()
