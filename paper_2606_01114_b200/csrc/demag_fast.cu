@@ -220,7 +220,7 @@ template <typename T, int G> struct ZpCfg {
   // (fp32: 12 x 164 registers, 12 x 18.1 KB): warps of one CTA start together and stay close
   // in the 70 KB instruction stream, which three independent 4-warp CTAs did not (1.06 -> 0.93 ms
   // at config 4, profiles/r01_v3_*.md).  fp64: 6 warps (36.3 KB per warp, 255 registers).
-  static constexpr int WARPS = sizeof(T) == 4 ? 12 : 6;
+  static constexpr int WARPS = sizeof(T) == 4 ? 12 : 7;
   static constexpr int MINB = 1;
   // fp64: the 15 inter-stage roots of a lane (60 registers) live in shared memory, [u][t]
   static constexpr int TWS = sizeof(T) == 4 ? 1 : G;
@@ -234,13 +234,16 @@ template <typename T, int G> struct ZpCfg {
   static constexpr int PQ = Q + (G < 16 ? G : 0);
   static constexpr int slot_bytes = PQ * (int)sizeof(Cx<T>);
   static constexpr int table_bytes = 6 * OZP * (int)sizeof(T);  // one (kx, ky) row, 16 B multiple
-  // per warp: two stages of NPW pencils + the table rows of the NPW / 2 mirror pairs + one slot
-  // for the row ky = ny (the partner of ky = 0, the only pair that does not share its row)
-  static constexpr int warp_bytes = 2 * NPW * slot_bytes + (NPW / 2 + 1) * table_bytes;
-  static constexpr int hdr_for(int warps) { return (3 * warps * 8 + 127) / 128 * 128; }  // mbarriers
+  // per warp: two stages of NPW pencils + the table rows of the NPW / 2 mirror pairs.  The row ky = ny (the
+  // partner of ky = 0, the only pair that does not share its row) is needed by one task per plane: it lands in
+  // the pencil area of the OTHER stage, whose prefetch that task defers until its multiply is done, instead of
+  // in a slot of its own (fp64: 37.1 -> 30.8 KB per warp, 7 warps instead of 6).
+  static constexpr int warp_bytes = 2 * NPW * slot_bytes + (NPW / 2) * table_bytes;
+  static constexpr int hdr_for(int warps) { return (4 * warps * 8 + 127) / 128 * 128; }  // mbarriers
   static constexpr int smem_for(int warps) { return hdr_for(warps) + warps * warp_bytes + tw_bytes; }
   static constexpr int smem_bytes = smem_for(WARPS);
   static_assert(XB <= Q, "exchange buffer must fit in the pencil it aliases");
+  static_assert(table_bytes <= NPW * slot_bytes, "the row ky = ny must fit in a stage's pencil area");
   static_assert(table_bytes % 16 == 0 && pencil_bytes % 16 == 0 && slot_bytes % 16 == 0, "bulk copies need 16 B multiples");
 };
 
@@ -366,14 +369,14 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
   const uint32_t pbytes = MASK ? (uint32_t)(qd * sizeof(Cx<T>)) : (uint32_t)C::pencil_bytes;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 3 * warp;  // stage 0, stage 1, table
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw) + 4 * warp;  // stage 0, stage 1, table, row ky = ny
   unsigned char* wraw = smem_raw + C::hdr_for(WARPS) + (size_t)warp * C::warp_bytes;
   Cx<T>* pbase = reinterpret_cast<Cx<T>*>(wraw);
   T* tbase = reinterpret_cast<T*>(wraw + 2 * NPW * C::slot_bytes);
   const int t = lane % G, pw = lane / G;
   const int Py = 2 * ny;
   if (threadIdx.x == 0) {
-    for (int i = 0; i < 3 * WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    for (int i = 0; i < 4 * WARPS; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if constexpr (sizeof(T) == 8) {
@@ -404,32 +407,39 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
       bulk_load(pbase + (stage * NPW + p) * C::PQ, pencil_ptr(task, p), pbytes, bars + stage);
   };
   // table rows of a task: ky = i for mirror pair i; the pair i = 0 (always the first of its
-  // task) is (ky = 0, ky = ny) and needs the row ky = ny as well, in the extra slot
+  // task) is (ky = 0, ky = ny) and needs the row ky = ny as well (issue_nyq)
   auto issue_table = [&](int task) {
     const int pair0 = task * (NPW / 2);
     const int plane = pair0 / ny, i0 = pair0 - plane * ny;
     const T* rows = tab + ((size_t)(kx0 + plane) * (ny + 1)) * 6 * C::OZP;
-    mbar_expect_tx(bars + 2, (NPW / 2 + (i0 == 0 ? 1 : 0)) * C::table_bytes);
+    mbar_expect_tx(bars + 2, (NPW / 2) * C::table_bytes);
     if constexpr (CONTIG) {   // the rows ky = i0 .. i0 + NPW/2 - 1 are one run of the table
       bulk_load(tbase, rows + (size_t)i0 * 6 * C::OZP, (NPW / 2) * C::table_bytes, bars + 2);
     } else {
       for (int pp = 0; pp < NPW / 2; ++pp)
         bulk_load(tbase + pp * 6 * C::OZP, rows + (size_t)(i0 + pp) * 6 * C::OZP, C::table_bytes, bars + 2);
     }
-    if (i0 == 0)
-      bulk_load(tbase + (NPW / 2) * 6 * C::OZP, rows + (size_t)ny * 6 * C::OZP, C::table_bytes, bars + 2);
+  };
+  // the row ky = ny of a task that holds pair 0, into the pencil area of the stage the task does not use
+  auto issue_nyq = [&](int task, int other) {
+    const int plane = task * (NPW / 2) / ny;
+    const T* rows = tab + ((size_t)(kx0 + plane) * (ny + 1)) * 6 * C::OZP;
+    mbar_expect_tx(bars + 3, C::table_bytes);
+    bulk_load(pbase + other * NPW * C::PQ, rows + (size_t)ny * 6 * C::OZP, C::table_bytes, bars + 3);
   };
   if (lane == 0 && gw < ntask) { issue(gw, 0); issue_table(gw); }
-  int it = 0;
+  int it = 0, nq = 0;
   // not unrolled: the body is ~2,300 instructions and two copies of it (the compiler's choice,
   // to make `stage` a constant) overflow the instruction cache
 #pragma unroll 1
   for (int task = gw; task < ntask; task += stride, ++it) {
     const int stage = it & 1;
     const bool more = task + stride < ntask;
+    const bool has0 = (task * (NPW / 2)) % ny == 0;   // this task holds the pair (ky = 0, ky = ny)
     if (lane == 0) {
       bulk_wait_read0();  // the previous task's store has finished reading the other stage
-      if (more) issue(task + stride, stage ^ 1);
+      if (has0) issue_nyq(task, stage ^ 1);
+      else if (more) issue(task + stride, stage ^ 1);
     }
     __syncwarp();
     mbar_wait(bars + stage, (it >> 1) & 1);
@@ -455,10 +465,16 @@ zp_fast_kernel(Cx<T>* __restrict__ A2, const T* __restrict__ tab, const Cx<T>* _
       const T sy = ((pw & 1) && i != 0) ? (T)-1 : (T)1;
       const T s4 = (MASK && xm) ? sy : (T)1, s5 = (MASK && xm) ? (T)1 : sy;
       mbar_wait(bars + 2, it & 1);
-      const T* trow = tbase + (nyq ? NPW / 2 : (pw >> 1)) * 6 * C::OZP;
+      if (has0) { mbar_wait(bars + 3, nq & 1); ++nq; }
+      const T* trow = nyq ? reinterpret_cast<const T*>(pbase + (stage ^ 1) * NPW * C::PQ)
+                          : tbase + (pw >> 1) * 6 * C::OZP;
       zp_multiply<T, G>(trow, t, sy, s4, s5, X[0], X[1], X[2]);
+      if (has0) fence_async_smem();   // the row was read through the generic proxy; pencils land there next
       __syncwarp();
-      if (lane == 0 && more) issue_table(task + stride);
+      if (lane == 0 && more) {
+        issue_table(task + stride);
+        if (has0) issue(task + stride, stage ^ 1);   // the prefetch this task deferred
+      }
     }
     // ---- inverse; the truncated samples go back into the staged pencil
     {
