@@ -847,7 +847,7 @@ static cudaError_t launch_zp(const FastGeom& g, const FastBufs<T>& b, int k0, in
     zp_fast_kernel<T, G, WARPS, MINB, true><<<grid, WARPS * 32, C::smem_bytes, st>>>(
         b.A2, b.table, b.Wz, b.posy, g.ny, k0, ntask, g.nz, xm);
   }
-  return cudaSuccess;
+  return cudaPeekAtLastError();   // a K3 that did not launch must not pass for a field
 }
 
 template <typename T>
